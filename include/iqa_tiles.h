@@ -1,0 +1,137 @@
+/* =============================================================================
+ * iqa_tiles.h -- C ABI of libiqa_tiles.so: tile-wise LISI / augLISI on one B200.
+ *
+ * What the library computes (arxiv 2501.10653; "P:NN" = line NN of PAPER.md):
+ *   clamp     negative pixels are set to zero before everything else        P:27  (Sec. 2)
+ *   Eq. 1     lisi_t    = D * L_t / (max(X_t, Y_t) + C2),
+ *             L_t = sum_k |x_k + y_k| / (|x_k - y_k| + C1)
+ *   Eq. 2     auglisi_t = 1 - A_t / (X_t + Y_t + C),
+ *             A_t = sum_k |x_k + y_k| * |x_k - y_k|
+ *             X_t = sum_k x_k, Y_t = sum_k y_k over the N_T x N_T pixels of tile t
+ *   tiling    N x N image -> n = (N/N_T)^2 tiles, one value per tile
+ *             ("IQA matrix")
+ *   Eq. 3/4   tile -> whole-image aggregation of the two matrices
+ *   merge     the "entire image" of Eqs. 3-4 may be a larger tile formed by
+ *             merging g x g smaller ones
+ *
+ * Conventions (the paper states none; DESIGN.md "Boundary" and "Readings"):
+ *   * Every pointer is a DEVICE pointer owned by the caller unless the argument name ends
+ *     in `_host`.  The library allocates no device memory and keeps no state between calls.
+ *   * `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device
+ *     entry points are ASYNCHRONOUS: they validate, enqueue and return; outputs are valid
+ *     once the stream has reached that point.  x and y are never written.
+ *   * Images are fp32, row-major, contiguous: pixel (r, c) is x[r*N + c].  Tile
+ *     t = ty*(N/N_T) + tx covers rows ty*N_T.. and columns tx*N_T..; every per-tile array
+ *     is indexed by t (a row-major (N/N_T) x (N/N_T) matrix with the image's orientation).
+ *   * Clamp is v > 0 ? v : 0, so NaN, -0 and -Inf become +0 (FITS blank pixels read as
+ *     empty sky).  +Inf pixels give unspecified output.  Outputs are NOT clamped to [0,1]
+ *     (augLISI is negative when sum|x+y||x-y| exceeds sum x + sum y + C).
+ *   * D is caller-supplied; the paper never defines it.  D = C1/2 makes LISI(x, x) -> 1.
+ *   * Errors: a status code is returned, nothing is thrown or printed, and NOTHING is
+ *     enqueued when the status is not IQA_OK (validation precedes the first launch).
+ *       NULL required pointer ....................................... IQA_ERR_NULL
+ *       N <= 0, N_T <= 0, N % N_T != 0, n_tiles <= 0, g bad .. IQA_ERR_SHAPE
+ *       C1, C2 or C not finite or <= 0, D not finite ................ IQA_ERR_PARAM
+ *       x or y not 4-byte aligned ................................... IQA_ERR_ALIGN
+ *       workspace NULL / too small when iqa_workspace_bytes() > 0 ... IQA_ERR_WORKSPACE
+ *       CUDA launch / copy failure .................................. IQA_ERR_CUDA
+ *   * Any N_T that divides N is accepted.  Power-of-two N_T >= 8 with 16-byte aligned
+ *     x and y take the vectorised strip kernels; everything else takes a generic
+ *     (slower, still CUDA) kernel.  Results are deterministic: fixed reduction order,
+ *     no floating-point atomics; two calls on the same inputs are bit-identical.
+ * ============================================================================= */
+#ifndef IQA_TILES_H
+#define IQA_TILES_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    IQA_OK = 0,
+    IQA_ERR_NULL = 1,
+    IQA_ERR_SHAPE = 2,
+    IQA_ERR_PARAM = 3,
+    IQA_ERR_ALIGN = 4,
+    IQA_ERR_WORKSPACE = 5,
+    IQA_ERR_CUDA = 6
+} iqa_status;
+
+/* Static, never-freed description of a status code ("unknown status" for other values). */
+const char* iqa_status_string(int status);
+
+/* Library version, "major.minor.patch". */
+const char* iqa_version(void);
+
+/* Bytes of device workspace the *_tiles entry points need for (N, N_T): 0 when every tile
+ * is finished inside one CTA, else room for the per-piece partial sums of split tiles
+ * (16 B per piece).  Returns 0 for invalid shapes (the entry points report those). */
+size_t iqa_workspace_bytes(int N, int N_T);
+
+/* Eq. 1 per tile (clamp P:27).
+ *   x, y      [N*N]  device, read-only
+ *   lisi      [n]    device, written; n = (N/N_T)^2
+ *   workspace        device scratch of >= iqa_workspace_bytes(N, N_T) bytes (may be NULL when 0),
+ *                    contents undefined before and after */
+int iqa_lisi_tiles(const float* x, const float* y, int N, int N_T,
+                   float C1, float C2, float D,
+                   float* lisi,
+                   void* workspace, size_t workspace_bytes, void* stream);
+
+/* Eq. 2 per tile (clamp P:27).  Arguments as above. */
+int iqa_auglisi_tiles(const float* x, const float* y, int N, int N_T, float C,
+                      float* auglisi,
+                      void* workspace, size_t workspace_bytes, void* stream);
+
+/* Eq. 1 and Eq. 2 per tile from ONE read of x and y, plus the per-tile sums Eqs. 3-4 need.
+ *   lisi, auglisi        [n] each, required
+ *   sum_x, sum_y         [n] each, required: X_t, Y_t (clamped sums)
+ *   lisi_num, auglisi_num [n] each, MAY BE NULL: the raw numerators L_t and A_t */
+int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
+                    float C1, float C2, float C, float D,
+                    float* lisi, float* auglisi,
+                    float* sum_x, float* sum_y,
+                    float* lisi_num, float* auglisi_num,
+                    void* workspace, size_t workspace_bytes, void* stream);
+
+/* Eqs. 3-4: merge n_tiles per-tile values into the whole-image pair.
+ *   out2 [2] device: out2[0] = LISI, out2[1] = augLISI.  Sums are taken in double, fixed order.
+ * Eq. 3 holds no D (it is inside lisi_t), so only C2 and C are needed. */
+int iqa_aggregate(const float* lisi, const float* auglisi,
+                  const float* sum_x, const float* sum_y, int n_tiles,
+                  float C2, float C,
+                  float* out2, void* stream);
+
+/* P:66 "a larger tile formed by merging smaller ones": apply Eqs. 3-4 to every g x g block
+ * of an nt x nt tile matrix, giving the (nt/g) x (nt/g) matrices of tile size g*N_T.
+ *   in:  lisi, auglisi, sum_x, sum_y  [nt*nt]
+ *   out: lisi_out, auglisi_out, sum_x_out, sum_y_out  [(nt/g)^2]   (nt % g == 0, g >= 1)
+ * Outputs must not alias inputs. */
+int iqa_merge_tiles(const float* lisi, const float* auglisi,
+                    const float* sum_x, const float* sum_y, int nt, int g,
+                    float C2, float C,
+                    float* lisi_out, float* auglisi_out,
+                    float* sum_x_out, float* sum_y_out, void* stream);
+
+/* Bytes of DEVICE scratch iqa_fused_host needs for (N, N_T): both images, the four per-tile
+ * arrays, out2 and the kernel workspace.  0 for invalid shapes. */
+size_t iqa_host_scratch_bytes(int N, int N_T);
+
+/* The whole hot path on HOST buffers (the call a FITS-reading front end would make):
+ * copy x_host, y_host to the device, run iqa_fused_tiles + iqa_aggregate, copy the four
+ * per-tile arrays and the aggregated pair back, and SYNCHRONISE the stream before returning.
+ *   x_host, y_host        [N*N] host (pinned memory gives full PCIe rate; pageable works)
+ *   *_host outputs        [n] each / out2_host [2]; any of them may be NULL (not copied back)
+ *   dev_scratch           device buffer of >= iqa_host_scratch_bytes(N, N_T) bytes, 256-B aligned */
+int iqa_fused_host(const float* x_host, const float* y_host, int N, int N_T,
+                   float C1, float C2, float C, float D,
+                   float* lisi_host, float* auglisi_host,
+                   float* sum_x_host, float* sum_y_host, float* out2_host,
+                   void* dev_scratch, size_t dev_scratch_bytes, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IQA_TILES_H */

@@ -1,0 +1,308 @@
+"""ctypes binding over libiqa_tiles.so (include/iqa_tiles.h) -- argument marshalling only.
+
+Two layers, both without any arithmetic of the method:
+  * ``iqa_*`` functions with the C names and argument order of the header.  Pointer
+    arguments accept a torch tensor (its ``data_ptr()``), a numpy array (host entry points),
+    an int address or None; ``stream`` accepts a ``torch.cuda.Stream``, an int handle or None.
+    They return the ``iqa_status`` code.
+  * convenience wrappers (``fused_tiles``, ``lisi_tiles``, ``auglisi_tiles``, ``aggregate``,
+    ``merge_tiles``, ``pyramid``, ``fused_host``) that allocate the output tensors with torch,
+    use torch's current stream, and raise ``IqaError`` on a non-zero status.
+
+Importing this module FAILS when the library is missing and cannot be built with nvcc:
+there is no CPU fallback (the CPU oracle under ``oracle/`` is test infrastructure only and
+is never imported from here).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKSPACE, IQA_ERR_CUDA = range(7)
+
+EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
+           "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_aggregate", "iqa_merge_tiles",
+           "iqa_host_scratch_bytes", "iqa_fused_host")
+
+
+class IqaError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = int(status)
+        super().__init__(f"{where}: iqa_status {status} ({iqa_status_string(status)})")
+
+
+def _load() -> ctypes.CDLL:
+    try:
+        path = _build.build()
+    except Exception as exc:  # no nvcc and no prebuilt library
+        if not os.path.exists(_build.LIB):
+            raise ImportError(
+                "libiqa_tiles.so is not built and nvcc could not build it "
+                f"({exc}); run `python -m paper_2501_10653_b200.build`. There is no CPU fallback.") from exc
+        path = _build.LIB      # stale but present (e.g. read-only tree): use it
+    lib = ctypes.CDLL(path)
+    vp, f, i, sz = ctypes.c_void_p, ctypes.c_float, ctypes.c_int, ctypes.c_size_t
+    lib.iqa_status_string.restype = ctypes.c_char_p
+    lib.iqa_status_string.argtypes = [i]
+    lib.iqa_version.restype = ctypes.c_char_p
+    lib.iqa_version.argtypes = []
+    lib.iqa_workspace_bytes.restype = sz
+    lib.iqa_workspace_bytes.argtypes = [i, i]
+    lib.iqa_host_scratch_bytes.restype = sz
+    lib.iqa_host_scratch_bytes.argtypes = [i, i]
+    lib.iqa_lisi_tiles.restype = i
+    lib.iqa_lisi_tiles.argtypes = [vp, vp, i, i, f, f, f, vp, vp, sz, vp]
+    lib.iqa_auglisi_tiles.restype = i
+    lib.iqa_auglisi_tiles.argtypes = [vp, vp, i, i, f, vp, vp, sz, vp]
+    lib.iqa_fused_tiles.restype = i
+    lib.iqa_fused_tiles.argtypes = [vp, vp, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_aggregate.restype = i
+    lib.iqa_aggregate.argtypes = [vp, vp, vp, vp, i, f, f, vp, vp]
+    lib.iqa_merge_tiles.restype = i
+    lib.iqa_merge_tiles.argtypes = [vp, vp, vp, vp, i, i, f, f, vp, vp, vp, vp, vp]
+    lib.iqa_fused_host.restype = i
+    lib.iqa_fused_host.argtypes = [vp, vp, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, sz, vp]
+    return lib
+
+
+lib = _load()
+LIB_PATH = _build.LIB
+
+
+# ----------------------------------------------------------------------------- marshalling
+def _ptr(a):
+    """Address of a tensor / array / int / None as c_void_p-compatible value."""
+    if a is None:
+        return None
+    if isinstance(a, int):
+        return a
+    if hasattr(a, "data_ptr"):
+        return a.data_ptr()
+    if hasattr(a, "ctypes"):
+        return a.ctypes.data
+    raise TypeError(f"cannot take the address of {type(a)!r}")
+
+
+def _stream(s):
+    if s is None:
+        return None
+    if isinstance(s, int):
+        return s
+    return s.cuda_stream
+
+
+def _current_stream(device=None):
+    import torch
+    return torch.cuda.current_stream(device).cuda_stream
+
+
+# ----------------------------------------------------------------------------- C names
+def iqa_status_string(status: int) -> str:
+    return lib.iqa_status_string(int(status)).decode()
+
+
+def iqa_version() -> str:
+    return lib.iqa_version().decode()
+
+
+def iqa_workspace_bytes(N: int, N_T: int) -> int:
+    return int(lib.iqa_workspace_bytes(int(N), int(N_T)))
+
+
+def iqa_host_scratch_bytes(N: int, N_T: int) -> int:
+    return int(lib.iqa_host_scratch_bytes(int(N), int(N_T)))
+
+
+def iqa_lisi_tiles(x, y, N, N_T, C1, C2, D, lisi, workspace=None, workspace_bytes=0, stream=None) -> int:
+    return lib.iqa_lisi_tiles(_ptr(x), _ptr(y), int(N), int(N_T), C1, C2, D, _ptr(lisi),
+                              _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
+def iqa_auglisi_tiles(x, y, N, N_T, C, auglisi, workspace=None, workspace_bytes=0, stream=None) -> int:
+    return lib.iqa_auglisi_tiles(_ptr(x), _ptr(y), int(N), int(N_T), C, _ptr(auglisi),
+                                 _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
+def iqa_fused_tiles(x, y, N, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
+                    lisi_num=None, auglisi_num=None, workspace=None, workspace_bytes=0, stream=None) -> int:
+    return lib.iqa_fused_tiles(_ptr(x), _ptr(y), int(N), int(N_T), C1, C2, C, D,
+                               _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
+                               _ptr(lisi_num), _ptr(auglisi_num),
+                               _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
+def iqa_aggregate(lisi, auglisi, sum_x, sum_y, n_tiles, C2, C, out2, stream=None) -> int:
+    return lib.iqa_aggregate(_ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), int(n_tiles),
+                             C2, C, _ptr(out2), _stream(stream))
+
+
+def iqa_merge_tiles(lisi, auglisi, sum_x, sum_y, nt, g, C2, C,
+                    lisi_out, auglisi_out, sum_x_out, sum_y_out, stream=None) -> int:
+    return lib.iqa_merge_tiles(_ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), int(nt), int(g),
+                               C2, C, _ptr(lisi_out), _ptr(auglisi_out), _ptr(sum_x_out),
+                               _ptr(sum_y_out), _stream(stream))
+
+
+def iqa_fused_host(x_host, y_host, N, N_T, C1, C2, C, D, lisi_host, auglisi_host,
+                   sum_x_host, sum_y_host, out2_host, dev_scratch, dev_scratch_bytes, stream=None) -> int:
+    return lib.iqa_fused_host(_ptr(x_host), _ptr(y_host), int(N), int(N_T), C1, C2, C, D,
+                              _ptr(lisi_host), _ptr(auglisi_host), _ptr(sum_x_host), _ptr(sum_y_host),
+                              _ptr(out2_host), _ptr(dev_scratch), int(dev_scratch_bytes), _stream(stream))
+
+
+# ----------------------------------------------------------------------------- convenience
+def _check_images(x, y):
+    import torch
+    if not (isinstance(x, torch.Tensor) and isinstance(y, torch.Tensor)):
+        raise TypeError("x and y must be torch CUDA tensors")
+    if not (x.is_cuda and y.is_cuda):
+        raise ValueError("x and y must live on a CUDA device (no CPU fallback)")
+    if x.dtype != torch.float32 or y.dtype != torch.float32:
+        raise TypeError("x and y must be float32")
+    if x.dim() != 2 or x.shape[0] != x.shape[1] or x.shape != y.shape:
+        raise ValueError("x and y must be equally sized square 2-D images")
+    if not (x.is_contiguous() and y.is_contiguous()):
+        raise ValueError("x and y must be contiguous (row-major, no pitch)")
+    return int(x.shape[0])
+
+
+def make_workspace(N: int, N_T: int, device):
+    """Device scratch for the *_tiles calls (None when none is needed)."""
+    import torch
+    nbytes = iqa_workspace_bytes(N, N_T)
+    if nbytes == 0:
+        return None, 0
+    return torch.empty(nbytes, dtype=torch.uint8, device=device), nbytes
+
+
+def fused_tiles(x, y, N_T, C1, C2, C, D, numerators: bool = False, workspace=None) -> dict:
+    """Eqs. 1-2 per tile from one read of x and y.  Returns dict of (nt, nt) float32 CUDA
+    tensors: lisi, auglisi, X, Y (+ L, A when ``numerators``)."""
+    import torch
+    N = _check_images(x, y)
+    if N_T <= 0 or N % N_T:
+        raise IqaError(IQA_ERR_SHAPE, "fused_tiles")
+    nt = N // N_T
+    names = ["lisi", "auglisi", "X", "Y"] + (["L", "A"] if numerators else [])
+    out = {k: torch.empty((nt, nt), dtype=torch.float32, device=x.device) for k in names}
+    if workspace is None:
+        workspace, _ = make_workspace(N, N_T, x.device)
+    wsb = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    rc = iqa_fused_tiles(x, y, N, N_T, C1, C2, C, D, out["lisi"], out["auglisi"], out["X"], out["Y"],
+                         out.get("L"), out.get("A"), workspace, wsb, _current_stream(x.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_fused_tiles")
+    return out
+
+
+def lisi_tiles(x, y, N_T, C1, C2, D, workspace=None):
+    import torch
+    N = _check_images(x, y)
+    if N_T <= 0 or N % N_T:
+        raise IqaError(IQA_ERR_SHAPE, "lisi_tiles")
+    nt = N // N_T
+    out = torch.empty((nt, nt), dtype=torch.float32, device=x.device)
+    if workspace is None:
+        workspace, _ = make_workspace(N, N_T, x.device)
+    wsb = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    rc = iqa_lisi_tiles(x, y, N, N_T, C1, C2, D, out, workspace, wsb, _current_stream(x.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_lisi_tiles")
+    return out
+
+
+def auglisi_tiles(x, y, N_T, C, workspace=None):
+    import torch
+    N = _check_images(x, y)
+    if N_T <= 0 or N % N_T:
+        raise IqaError(IQA_ERR_SHAPE, "auglisi_tiles")
+    nt = N // N_T
+    out = torch.empty((nt, nt), dtype=torch.float32, device=x.device)
+    if workspace is None:
+        workspace, _ = make_workspace(N, N_T, x.device)
+    wsb = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    rc = iqa_auglisi_tiles(x, y, N, N_T, C, out, workspace, wsb, _current_stream(x.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_auglisi_tiles")
+    return out
+
+
+def aggregate(lisi, auglisi, X, Y, C2, C, out2=None):
+    """Eqs. 3-4 over all given tiles -> float32 CUDA tensor [LISI, augLISI]."""
+    import torch
+    n = lisi.numel()
+    if out2 is None:
+        out2 = torch.empty(2, dtype=torch.float32, device=lisi.device)
+    rc = iqa_aggregate(lisi, auglisi, X, Y, n, C2, C, out2, _current_stream(lisi.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_aggregate")
+    return out2
+
+
+def merge_tiles(lisi, auglisi, X, Y, g, C2, C) -> dict:
+    """Eqs. 3-4 on every g x g block of the (nt, nt) matrices -> (nt/g, nt/g) matrices."""
+    import torch
+    nt = int(lisi.shape[0])
+    if g <= 0 or nt % g:
+        raise IqaError(IQA_ERR_SHAPE, "merge_tiles")
+    no = nt // g
+    out = {k: torch.empty((no, no), dtype=torch.float32, device=lisi.device)
+           for k in ("lisi", "auglisi", "X", "Y")}
+    rc = iqa_merge_tiles(lisi, auglisi, X, Y, nt, g, C2, C, out["lisi"], out["auglisi"], out["X"],
+                         out["Y"], _current_stream(lisi.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_merge_tiles")
+    return out
+
+
+def pyramid(tiles: dict, C2, C) -> list:
+    """All levels N_T, 2 N_T, 4 N_T, ... up to the coarsest the tile count allows (factor-2 merges)."""
+    levels = [tiles]
+    cur = tiles
+    while cur["lisi"].shape[0] % 2 == 0 and cur["lisi"].shape[0] > 1:
+        cur = merge_tiles(cur["lisi"], cur["auglisi"], cur["X"], cur["Y"], 2, C2, C)
+        levels.append(cur)
+    return levels
+
+
+class HostRunner:
+    """Reusable state for ``iqa_fused_host``: the device scratch and pinned result buffers."""
+
+    def __init__(self, N: int, N_T: int, device="cuda:0"):
+        import torch
+        self.N, self.N_T = int(N), int(N_T)
+        self.nt = self.N // self.N_T
+        self.device = torch.device(device)
+        self.scratch_bytes = iqa_host_scratch_bytes(N, N_T)
+        if self.scratch_bytes == 0:
+            raise IqaError(IQA_ERR_SHAPE, "HostRunner")
+        self.scratch = torch.empty(self.scratch_bytes, dtype=torch.uint8, device=self.device)
+        mk = lambda *s: torch.empty(*s, dtype=torch.float32).pin_memory()
+        self.out = {k: mk(self.nt, self.nt) for k in ("lisi", "auglisi", "X", "Y")}
+        self.out2 = mk(2)
+
+    @property
+    def h2d_bytes(self) -> int:
+        return 2 * 4 * self.N * self.N
+
+    @property
+    def d2h_bytes(self) -> int:
+        return 4 * 4 * self.nt * self.nt + 8
+
+    def __call__(self, x_host, y_host, C1, C2, C, D):
+        rc = iqa_fused_host(x_host, y_host, self.N, self.N_T, C1, C2, C, D,
+                            self.out["lisi"], self.out["auglisi"], self.out["X"], self.out["Y"],
+                            self.out2, self.scratch, self.scratch_bytes, _current_stream(self.device))
+        if rc != IQA_OK:
+            raise IqaError(rc, "iqa_fused_host")
+        return self.out, self.out2
+
+
+def fused_host(x_host, y_host, N_T, C1, C2, C, D, device="cuda:0"):
+    """One-shot host call (allocates scratch each time; use HostRunner in loops)."""
+    N = int(x_host.shape[0])
+    r = HostRunner(N, N_T, device)
+    out, out2 = r(x_host, y_host, C1, C2, C, D)
+    return {k: v.clone() for k, v in out.items()}, out2.clone()

@@ -1,0 +1,135 @@
+"""CPU-only checks of the C-ABI boundary: the library builds/loads, exports every symbol
+include/iqa_tiles.h declares, and validates arguments BEFORE touching the device (so these
+calls are safe without a GPU: nothing is enqueued when the status is not IQA_OK)."""
+import ctypes
+import math
+import os
+import re
+
+import pytest
+
+from paper_2501_10653_b200 import binding as B
+
+ROOT = os.path.abspath(os.path.join(os.path.dirname(__file__), ".."))
+HEADER = os.path.join(ROOT, "include", "iqa_tiles.h")
+
+
+def _declared():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(iqa_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_library_is_in_tree_and_exports_every_declared_symbol():
+    assert os.path.dirname(B.LIB_PATH) == os.path.join(ROOT, "paper_2501_10653_b200")
+    names = _declared()
+    assert set(names) == set(B.EXPORTS), names
+    raw = ctypes.CDLL(B.LIB_PATH)
+    for n in names:
+        assert getattr(raw, n) is not None
+
+
+def test_status_strings_and_version():
+    seen = {B.iqa_status_string(s) for s in range(7)}
+    assert len(seen) == 7 and "unknown status" not in seen
+    assert B.iqa_status_string(99) == "unknown status"
+    assert re.fullmatch(r"\d+\.\d+\.\d+", B.iqa_version())
+
+
+def test_workspace_bytes():
+    # tiles of side <= 64 are always finished inside one CTA: no second pass, no workspace
+    for N, N_T in [(256, 16), (2048, 8), (2048, 64), (8192, 64), (10, 5), (192, 48)]:
+        assert B.iqa_workspace_bytes(N, N_T) == 0
+    # split tiles: 16 B per piece; strip worst case (N_T/128 or 1) x (N_T/32) pieces per tile
+    assert B.iqa_workspace_bytes(2048, 128) == 256 * 1 * 4 * 16
+    assert B.iqa_workspace_bytes(2048, 512) == 16 * 4 * 16 * 16
+    assert B.iqa_workspace_bytes(16384, 128) == 16384 * 4 * 16
+    assert B.iqa_workspace_bytes(16384, 16384) == 128 * 512 * 16
+    assert B.iqa_workspace_bytes(200, 100) == 4 * 2 * 16          # generic: ceil(100/64) pieces
+    # invalid shapes report 0 here; the entry points return the error
+    for N, N_T in [(0, 8), (100, 0), (100, 7), (-4, 2), (64, 128), ((1 << 20) + 8, 8)]:
+        assert B.iqa_workspace_bytes(N, N_T) == 0
+        assert B.iqa_host_scratch_bytes(N, N_T) == 0
+    assert B.iqa_host_scratch_bytes(256, 16) >= 2 * 256 * 256 * 4 + 4 * 256 * 4 + 8
+
+
+FAKE = 0x1000   # a non-NULL, 16-byte aligned address that is never dereferenced on the host
+
+
+def _fused(x=FAKE, y=FAKE, N=256, N_T=16, C1=1e-6, C2=1e-6, C=1e-6, D=5e-7,
+           lisi=FAKE, aug=FAKE, sx=FAKE, sy=FAKE, ws=None, wsb=0):
+    return B.iqa_fused_tiles(x, y, N, N_T, C1, C2, C, D, lisi, aug, sx, sy, None, None, ws, wsb, None)
+
+
+def test_fused_argument_validation():
+    assert _fused(x=None) == B.IQA_ERR_NULL
+    assert _fused(y=None) == B.IQA_ERR_NULL
+    assert _fused(lisi=None) == B.IQA_ERR_NULL
+    assert _fused(aug=None) == B.IQA_ERR_NULL
+    assert _fused(sx=None) == B.IQA_ERR_NULL
+    assert _fused(sy=None) == B.IQA_ERR_NULL
+    assert _fused(N=0) == B.IQA_ERR_SHAPE
+    assert _fused(N=-256) == B.IQA_ERR_SHAPE
+    assert _fused(N_T=0) == B.IQA_ERR_SHAPE
+    assert _fused(N=100, N_T=16) == B.IQA_ERR_SHAPE          # P:64 presumes N % N_T == 0
+    assert _fused(N=16, N_T=32) == B.IQA_ERR_SHAPE
+    assert _fused(N=(1 << 20) + 16, N_T=16) == B.IQA_ERR_SHAPE
+    assert _fused(N=1 << 20, N_T=1) == B.IQA_ERR_SHAPE       # 2^40 tiles do not fit an int index
+    for bad in (0.0, -1e-6, math.inf, math.nan):
+        assert _fused(C1=bad) == B.IQA_ERR_PARAM
+        assert _fused(C2=bad) == B.IQA_ERR_PARAM
+        assert _fused(C=bad) == B.IQA_ERR_PARAM
+    assert _fused(D=math.nan) == B.IQA_ERR_PARAM
+    assert _fused(D=math.inf) == B.IQA_ERR_PARAM
+    assert _fused(x=FAKE + 2) == B.IQA_ERR_ALIGN
+    assert _fused(y=FAKE + 1) == B.IQA_ERR_ALIGN
+    assert _fused(N=256, N_T=128) == B.IQA_ERR_WORKSPACE     # split tiles need the workspace
+    assert _fused(N=256, N_T=128, ws=FAKE, wsb=8) == B.IQA_ERR_WORKSPACE
+    assert _fused(N=256, N_T=128, ws=FAKE + 4, wsb=1 << 20) == B.IQA_ERR_ALIGN
+
+
+def test_standalone_and_aggregate_validation():
+    assert B.iqa_lisi_tiles(None, FAKE, 256, 16, 1e-6, 1e-6, 5e-7, FAKE) == B.IQA_ERR_NULL
+    assert B.iqa_lisi_tiles(FAKE, FAKE, 256, 16, 1e-6, 1e-6, 5e-7, None) == B.IQA_ERR_NULL
+    assert B.iqa_lisi_tiles(FAKE, FAKE, 256, 24, 1e-6, 1e-6, 5e-7, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_lisi_tiles(FAKE, FAKE, 256, 16, 0.0, 1e-6, 5e-7, FAKE) == B.IQA_ERR_PARAM
+    assert B.iqa_auglisi_tiles(FAKE, None, 256, 16, 1e-6, FAKE) == B.IQA_ERR_NULL
+    assert B.iqa_auglisi_tiles(FAKE, FAKE, 256, 16, 1e-6, None) == B.IQA_ERR_NULL
+    assert B.iqa_auglisi_tiles(FAKE, FAKE, 256, 16, -1.0, FAKE) == B.IQA_ERR_PARAM
+    assert B.iqa_auglisi_tiles(FAKE, FAKE, 255, 16, 1e-6, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_aggregate(None, FAKE, FAKE, FAKE, 4, 1e-6, 1e-6, FAKE) == B.IQA_ERR_NULL
+    assert B.iqa_aggregate(FAKE, FAKE, FAKE, FAKE, 4, 1e-6, 1e-6, None) == B.IQA_ERR_NULL
+    assert B.iqa_aggregate(FAKE, FAKE, FAKE, FAKE, 0, 1e-6, 1e-6, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_aggregate(FAKE, FAKE, FAKE, FAKE, 4, 0.0, 1e-6, FAKE) == B.IQA_ERR_PARAM
+    assert B.iqa_merge_tiles(FAKE, FAKE, FAKE, None, 8, 2, 1e-6, 1e-6, FAKE, FAKE, FAKE, FAKE) == B.IQA_ERR_NULL
+    assert B.iqa_merge_tiles(FAKE, FAKE, FAKE, FAKE, 8, 3, 1e-6, 1e-6, FAKE, FAKE, FAKE, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_merge_tiles(FAKE, FAKE, FAKE, FAKE, 8, 0, 1e-6, 1e-6, FAKE, FAKE, FAKE, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_merge_tiles(FAKE, FAKE, FAKE, FAKE, 8, 2, 1e-6, math.nan, FAKE, FAKE, FAKE, FAKE) == B.IQA_ERR_PARAM
+    assert B.iqa_fused_host(None, FAKE, 256, 16, 1e-6, 1e-6, 1e-6, 5e-7, None, None, None, None, None,
+                            FAKE, 1 << 30) == B.IQA_ERR_NULL
+    assert B.iqa_fused_host(FAKE, FAKE, 256, 16, 1e-6, 1e-6, 1e-6, 5e-7, None, None, None, None, None,
+                            0x1000, 16) == B.IQA_ERR_WORKSPACE
+    assert B.iqa_fused_host(FAKE, FAKE, 256, 16, 1e-6, 1e-6, 1e-6, 5e-7, None, None, None, None, None,
+                            0x1010, 1 << 30) == B.IQA_ERR_ALIGN
+
+
+def test_convenience_wrappers_refuse_cpu_tensors():
+    """No CPU fallback: the product path fails loudly on host tensors."""
+    torch = pytest.importorskip("torch")
+    x = torch.zeros((16, 16))
+    with pytest.raises(ValueError):
+        B.fused_tiles(x, x, 8, 1e-6, 1e-6, 1e-6, 5e-7)
+
+
+def test_product_package_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2501_10653_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", src, flags=re.M), fn
+                assert "liboracle" not in src and "iqa_oracle" not in src, fn
+    for fn in os.listdir(os.path.join(ROOT, "oracle")):
+        if fn.endswith((".py", ".cpp")):
+            src = open(os.path.join(ROOT, "oracle", fn)).read()
+            assert "paper_2501_10653_b200." not in src and "import paper_2501_10653_b200" not in src, fn

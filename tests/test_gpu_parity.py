@@ -1,0 +1,305 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by
+element, on the same seeded fp32 buffers.  SURVEY.md 8(c) P11-P12 plus the edge cases.
+
+Citations: Eq. 1, Eq. 2, clamp PAPER.md:27, Eqs. 3-4 PAPER.md:55-60.
+"""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from paper_2501_10653_b200 import synth  # noqa: E402
+
+K6 = dict(C1=1e-6, C2=1e-6, C=1e-6, D=float(np.float32(1e-6)) / 2)
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2501_10653_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def U():
+    import gpu_util
+    return gpu_util
+
+
+def _rand_pair(N, seed, frac_equal=0.2):
+    rng = np.random.default_rng(seed)
+    x = rng.normal(0.1, 1.0, (N, N)).astype(np.float32)
+    y = rng.normal(0.1, 1.0, (N, N)).astype(np.float32)
+    m = rng.random((N, N)) < frac_equal
+    y[m] = x[m]                       # equal pixels: |x-y| = 0, term (x+y)/C1
+    x[rng.random((N, N)) < 0.05] = 0.0
+    return x, y
+
+
+# ----------------------------------------------------------------------------- worked example
+def test_worked_example_4x4(B, U):
+    """tests/golden/worked_example_4x4.txt (derived from Eqs. 1-4 with exact rationals)."""
+    from fractions import Fraction as Fr
+    x = np.array([[1, 0.5, -1, 0], [0.25, 0, 0, 0], [0.75, 0.75, 2, -0.5], [0.125, 0.5, 0, 1]], np.float32)
+    y = np.array([[1, 0.25, 3, -2], [0, 0.5, 0, 0], [0.75, 0.75, 0, 0.5], [0.125, 0.5, 1, 0]], np.float32)
+    k = dict(C1=2.0 ** -20, C2=2.0 ** -20, C=2.0 ** -20, D=2.0 ** -21)
+    golden = {}
+    for ln in open(os.path.join(os.path.dirname(__file__), "golden", "worked_example_4x4.txt")):
+        if ln.startswith("tile") or ln.startswith("whole"):
+            parts = ln.split()
+            vals = {q.split("=")[0]: float(Fr(q.split("=")[1])) for q in parts if "=" in q}
+            golden[parts[1] if parts[0] == "tile" else "whole"] = vals
+    got = U.run_gpu(U.to_dev(x), U.to_dev(y), 2, k)
+    for t in range(4):
+        for nm in ("lisi", "auglisi", "X", "Y", "L", "A"):
+            exp = golden[str(t)][nm]
+            assert abs(got[nm].ravel()[t] - exp) <= 1e-6 * abs(exp) + 1e-12, (t, nm)
+    assert got["auglisi"].ravel()[2] == 1.0            # identical tile: exactly 1
+    assert got["auglisi"].ravel()[1] < -1.99           # outputs are not clamped
+    one = U.run_gpu(U.to_dev(x), U.to_dev(y), 4, k)
+    for nm in ("lisi", "auglisi", "X", "Y", "L", "A"):
+        exp = golden["whole"][nm]
+        assert abs(one[nm][0, 0] - exp) <= 1e-6 * abs(exp), nm
+    # Eqs. 3-4 on the device reproduce the whole-image values
+    o = B.fused_tiles(U.to_dev(x), U.to_dev(y), 2, **k)
+    agg = B.aggregate(o["lisi"], o["auglisi"], o["X"], o["Y"], k["C2"], k["C"]).cpu().numpy()
+    assert abs(agg[0] - golden["whole"]["lisi"]) <= 1e-6 * golden["whole"]["lisi"]
+    assert abs(agg[1] - golden["whole"]["auglisi"]) <= 1e-6
+
+
+# ----------------------------------------------------------------------------- BASELINE.json configs
+def test_config0(U):
+    cfg = synth.CONFIGS[0]
+    x, y, _ = synth.make_pair(cfg)
+    U.check_pair(x, y, cfg.N_T, U.consts(cfg), "cfg0")
+
+
+def test_config1_and_shared_noise(U):
+    cfg = synth.CONFIGS[1]
+    x, y, _ = synth.make_pair(cfg)
+    got, ref, _ = U.check_pair(x, y, cfg.N_T, U.consts(cfg), "cfg1")
+    # soft science echo (P10): the lowest augLISI tiles hold the dropped sources
+    xs, ys, _ = synth.make_pair(cfg, shared_noise=True)
+    U.check_pair(xs, ys, cfg.N_T, U.consts(cfg), "cfg1 shared noise")
+
+
+@pytest.mark.parametrize("N_T", [8, 16, 32, 64, 128, 256, 512, 1024, 2048])
+def test_config2_tile_sweep(U, N_T):
+    cfg = synth.CONFIGS[2]
+    x, y, _ = _cfg2_pair()
+    U.check_pair(x, y, N_T, U.consts(cfg), f"cfg2 N_T={N_T}", *_cfg2_dev(U))
+
+
+_CFG2 = {}
+
+
+def _cfg2_pair():
+    if "host" not in _CFG2:
+        _CFG2["host"] = synth.make_pair(synth.CONFIGS[2])
+    return _CFG2["host"]
+
+
+def _cfg2_dev(U):
+    if "dev" not in _CFG2:
+        x, y, _ = _cfg2_pair()
+        _CFG2["dev"] = (U.to_dev(x), U.to_dev(y))
+    return _CFG2["dev"]
+
+
+def test_config3_full(U, B):
+    cfg = synth.CONFIGS[3]
+    x, y, _ = synth.make_pair(cfg)
+    k = U.consts(cfg)
+    xd, yd = U.to_dev(x), U.to_dev(y)
+    got, ref, _ = U.check_pair(x, y, cfg.N_T, k, "cfg3", xd, yd)
+    # aggregate (Eqs. 3-4) against the oracle's whole-image value computed directly
+    o = B.fused_tiles(xd, yd, cfg.N_T, **k)
+    agg = B.aggregate(o["lisi"], o["auglisi"], o["X"], o["Y"], k["C2"], k["C"]).cpu().numpy()
+    exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], k["C2"], k["C"])
+    assert abs(agg[0] - exp[0]) <= 1e-5 * abs(exp[0])
+    assert abs(agg[1] - exp[1]) <= 1e-5 * abs(exp[1])
+
+
+def test_config4_full_size(U, B):
+    """N=16384, N_T=128, 1 GiB per image: noise drawn on the device, buffers copied back for the oracle."""
+    cfg = synth.CONFIGS[4]
+    k = U.consts(cfg)
+    xd, yd, _ = synth.make_pair(cfg, device="cuda")
+    x, y = xd.cpu().numpy(), yd.cpu().numpy()
+    got, ref, _ = U.check_pair(x, y, cfg.N_T, k, "cfg4", xd, yd)
+    o = B.fused_tiles(xd, yd, cfg.N_T, **k)
+    agg = B.aggregate(o["lisi"], o["auglisi"], o["X"], o["Y"], k["C2"], k["C"]).cpu().numpy()
+    exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], k["C2"], k["C"])
+    assert abs(agg[0] - exp[0]) <= 1e-5 * abs(exp[0])
+    assert abs(agg[1] - exp[1]) <= 1e-5 * abs(exp[1])
+    # whole image as ONE tile (maximum tile size; 65536 pieces through the workspace)
+    one = U.run_gpu(xd, yd, cfg.N, k)
+    whole = oracle.tiles(x, y, cfg.N, **k)
+    U.assert_parity(one, whole, k["C"], "cfg4 single tile")
+
+
+# ----------------------------------------------------------------------------- shapes and edges
+@pytest.mark.parametrize("N,N_T", [
+    (8, 8), (16, 8), (24, 8), (136, 8), (200, 8), (264, 8), (64, 64), (192, 64), (320, 64),
+    (128, 128), (384, 128), (256, 256), (768, 256), (1536, 512), (48, 16), (96, 32), (160, 32),
+    (4, 2), (12, 4), (10, 5), (9, 3), (7, 1), (36, 12), (200, 100), (130, 65), (390, 130), (5, 5)])
+def test_shapes(U, N, N_T):
+    x, y = _rand_pair(N, seed=N * 1000 + N_T)
+    U.check_pair(x, y, N_T, K6, f"N={N} N_T={N_T}")
+
+
+@pytest.mark.parametrize("N,N_T", [(256, 8), (256, 64), (512, 128), (100, 20)])
+def test_unaligned_pointers_take_generic_kernel(U, B, N, N_T):
+    x, y = _rand_pair(N, seed=7)
+    buf_x = torch.empty(N * N + 3, dtype=torch.float32, device="cuda")
+    buf_y = torch.empty(N * N + 3, dtype=torch.float32, device="cuda")
+    xd = buf_x[1:1 + N * N].view(N, N)
+    yd = buf_y[3:3 + N * N].view(N, N)
+    xd.copy_(torch.from_numpy(x))
+    yd.copy_(torch.from_numpy(y))
+    assert xd.data_ptr() % 16 != 0
+    U.check_pair(x, y, N_T, K6, "unaligned", xd, yd)
+
+
+def test_special_values(U):
+    """NaN, -0, -Inf and negatives clamp to zero (reading R3); all-zero tile gives lisi 0, auglisi 1 (R7)."""
+    N, N_T = 128, 16
+    x, y = _rand_pair(N, seed=11)
+    x[0:16, 0:16] = -1.0
+    y[0:16, 0:16] = np.nan                 # tile 0: everything clamps to zero
+    x[20, 20] = np.nan
+    y[21, 21] = -np.inf
+    x[22, 22] = -0.0
+    y[22, 22] = -0.0
+    got, ref, _ = U.check_pair(x, y, N_T, K6, "special")
+    assert got["lisi"][0, 0] == 0.0 and got["auglisi"][0, 0] == 1.0
+    assert got["X"][0, 0] == 0.0 and got["Y"][0, 0] == 0.0
+    # P7: replacing the clamped pixels by zeros changes nothing, bit for bit
+    xz = np.where(x > 0, x, 0).astype(np.float32)
+    yz = np.where(y > 0, y, 0).astype(np.float32)
+    got2 = U.run_gpu(U.to_dev(xz), U.to_dev(yz), N_T, K6)
+    for nm in got:
+        assert np.array_equal(got[nm], got2[nm]), nm
+
+
+def test_identical_images(U):
+    """P3: auglisi(x, x) = 1 exactly; lisi(x, x) = (2D/C1) X/(X+C2)."""
+    cfg = synth.CONFIGS[0]
+    x, _, _ = synth.make_pair(cfg)
+    k = U.consts(cfg)
+    got, ref, _ = U.check_pair(x, x, cfg.N_T, k, "identical")
+    assert np.all(got["auglisi"] == 1.0)
+    assert np.array_equal(got["X"], got["Y"])
+    X = ref["X"]
+    closed = X / (X + float(np.float32(cfg.C2)))
+    assert np.max(np.abs(got["lisi"] - closed) / closed) <= 1e-5
+
+
+def test_symmetry_bitwise(U):
+    """P4: swapping x and y leaves both indices bit-identical and swaps X, Y."""
+    x, y = _rand_pair(256, seed=3)
+    a = U.run_gpu(U.to_dev(x), U.to_dev(y), 32, K6)
+    b = U.run_gpu(U.to_dev(y), U.to_dev(x), 32, K6)
+    assert np.array_equal(a["lisi"], b["lisi"]) and np.array_equal(a["auglisi"], b["auglisi"])
+    assert np.array_equal(a["X"], b["Y"]) and np.array_equal(a["Y"], b["X"])
+
+
+def test_determinism_and_mapping_independence(U, monkeypatch):
+    """P12: two runs bit-identical; every mapping (rows per warp 4/8/16, generic kernel) agrees to 1e-6."""
+    cfg = synth.CONFIGS[0]
+    x, y, _ = synth.make_pair(synth.scaled(synth.CONFIGS[3], 1024))
+    xd, yd = U.to_dev(x), U.to_dev(y)
+    k = U.consts(cfg)
+    for N_T in (8, 32, 64, 128, 512):
+        base = U.run_gpu(xd, yd, N_T, k)
+        again = U.run_gpu(xd, yd, N_T, k)
+        for nm in base:
+            assert np.array_equal(base[nm], again[nm]), (N_T, nm)
+        ref = U.run_oracle(x, y, N_T, k)
+        for env, val in (("IQA_FORCE_RW", "4"), ("IQA_FORCE_RW", "16"), ("IQA_FORCE_GENERIC", "1")):
+            monkeypatch.setenv(env, val)
+            other = U.run_gpu(xd, yd, N_T, k)
+            monkeypatch.delenv(env)
+            U.assert_parity(other, ref, k["C"], f"{env}={val} N_T={N_T}")
+            for nm in base:
+                assert np.max(U.rel_err(other[nm], base[nm])) <= 2e-6, (env, val, N_T, nm)
+
+
+def test_standalone_entry_points_match_fused(U, B):
+    cfg = synth.CONFIGS[1]
+    x, y, _ = synth.make_pair(cfg)
+    xd, yd = U.to_dev(x), U.to_dev(y)
+    k = U.consts(cfg)
+    for N_T in (16, 64, 256):
+        f = B.fused_tiles(xd, yd, N_T, **k)
+        li = B.lisi_tiles(xd, yd, N_T, k["C1"], k["C2"], k["D"])
+        au = B.auglisi_tiles(xd, yd, N_T, k["C"])
+        assert torch.equal(li, f["lisi"]) and torch.equal(au, f["auglisi"])
+
+
+def test_aggregate_equals_whole_image_and_merge(U, B):
+    """P6: Eqs. 3-4 over the tiles == the index of the whole image; g x g merge == tiles at g*N_T."""
+    cfg = synth.CONFIGS[1]
+    x, y, _ = synth.make_pair(cfg)
+    xd, yd = U.to_dev(x), U.to_dev(y)
+    k = U.consts(cfg)
+    whole = oracle.tiles(x, y, cfg.N, **k)
+    for N_T in (8, 64, 256):
+        o = B.fused_tiles(xd, yd, N_T, **k)
+        agg = B.aggregate(o["lisi"], o["auglisi"], o["X"], o["Y"], k["C2"], k["C"]).cpu().numpy()
+        assert abs(agg[0] - whole["lisi"][0, 0]) <= 1e-5 * whole["lisi"][0, 0], N_T
+        assert abs(agg[1] - whole["auglisi"][0, 0]) <= 1e-5 * abs(whole["auglisi"][0, 0]), N_T
+    o = B.fused_tiles(xd, yd, 32, **k)
+    for g in (1, 2, 4, 64):
+        m = B.merge_tiles(o["lisi"], o["auglisi"], o["X"], o["Y"], g, k["C2"], k["C"])
+        ref = oracle.tiles(x, y, 32 * g, **k)
+        got = {n: m[n].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y")}
+        U.assert_parity(got, ref, k["C"], f"merge g={g}")
+    lv = B.pyramid(o, k["C2"], k["C"])
+    assert [l["lisi"].shape[0] for l in lv] == [64, 32, 16, 8, 4, 2, 1]
+
+
+def test_fused_host_entry_point(U, B):
+    cfg = synth.CONFIGS[0]
+    x, y, _ = synth.make_pair(cfg)
+    k = U.consts(cfg)
+    xp, yp = torch.from_numpy(x).pin_memory(), torch.from_numpy(y).pin_memory()
+    out, out2 = B.fused_host(xp, yp, cfg.N_T, **k)
+    ref = U.run_oracle(x, y, cfg.N_T, k)
+    got = {n: out[n].numpy().astype(np.float64) for n in out}
+    U.assert_parity(got, ref, k["C"], "fused_host")
+    exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], k["C2"], k["C"])
+    assert abs(out2[0].item() - exp[0]) <= 1e-5 * abs(exp[0])
+    assert abs(out2[1].item() - exp[1]) <= 1e-5 * abs(exp[1])
+    out_np, _ = B.fused_host(x, y, 128, **k)          # pageable numpy input, split-tile mapping
+    ref = U.run_oracle(x, y, 128, k)
+    U.assert_parity({n: out_np[n].numpy().astype(np.float64) for n in out_np}, ref, k["C"], "fused_host 128")
+
+
+def test_many_small_tiles(U):
+    """N=4096, N_T=8: 262144 tiles (16 tile segments per warp row)."""
+    x, y = _rand_pair(4096, seed=5)
+    U.check_pair(x, y, 8, K6, "many tiles")
+
+
+def test_error_codes_on_device(B):
+    N, N_T = 256, 128
+    x = torch.zeros((N, N), device="cuda")
+    n = (N // N_T) ** 2
+    o = [torch.zeros(n, device="cuda") for _ in range(4)]
+    need = B.iqa_workspace_bytes(N, N_T)
+    assert need > 0
+    rc = B.iqa_fused_tiles(x, x, N, N_T, 1e-6, 1e-6, 1e-6, 5e-7, *o, None, None, None, 0, None)
+    assert rc == B.IQA_ERR_WORKSPACE
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    rc = B.iqa_fused_tiles(x, x, N, N_T, 1e-6, 1e-6, 1e-6, 5e-7, *o, None, None, ws, need - 1, None)
+    assert rc == B.IQA_ERR_WORKSPACE
+    rc = B.iqa_fused_tiles(x, x, N, N_T, 1e-6, 1e-6, 1e-6, 5e-7, *o, None, None, ws, need, None)
+    assert rc == B.IQA_OK
+    rc = B.iqa_fused_tiles(x.data_ptr() + 2, x, N, N_T, 1e-6, 1e-6, 1e-6, 5e-7, *o, None, None, ws, need, None)
+    assert rc == B.IQA_ERR_ALIGN
+    torch.cuda.synchronize()
