@@ -1,0 +1,422 @@
+#!/usr/bin/env python
+"""bench.py -- us per image pair and achieved HBM GB/s of the tiled LISI/augLISI hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg3|cfg4] [--impl reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A STEP is one pass of the whole hot path -- iqa_fused_tiles (S1-S4) then iqa_aggregate (S5,
+Eqs. 3-4) -- over one batch of P distinct synthetic image pairs already resident in HBM.
+The batch is several times larger than the 126 MB L2, so every pair is read cold from HBM
+(said in ``config.l2``).  The step is captured once in a CUDA graph (2 P kernel launches) so
+that Python/ctypes launch overhead does not sit between 5-us kernels; ``--no-graph`` launches
+directly.  One JSON line is printed by rank 0; see DESIGN.md "Measurement" for every key.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "us_per_image_pair"
+UNIT = "us/pair"
+
+# workload name -> (BASELINE.json config index, pairs per step, pairs per e2e step)
+WORKLOADS = {"cfg1": (1, 32, 8), "cfg3": (3, 8, 2), "cfg4": (4, 16, 1), "cfg0": (0, 64, 8)}
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused strip kernel, from the
+# `ncu --set full` capture summarised under profiles/ (null until captured for that workload).
+NCU_TRAFFIC_BYTES = {}
+
+
+def algorithmic_bytes(N: int, N_T: int) -> int:
+    """SURVEY.md 8(d) / DESIGN.md: 8 B read per pixel pair + 16 B written per tile."""
+    n = (N // N_T) ** 2
+    return 8 * N * N + 16 * n
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy rate)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap",
+               0x8: "hw_slowdown", 0x10: "sync_boost", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index: int):
+        self.samples, self.mask, self.ok = [], 0, False
+        self._stop = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as exc:  # NVML missing: report that, never fake a clock
+            self.err = repr(exc)
+
+    def _once(self):
+        nv = self.nv
+        self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+        try:
+            self.mask |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+        except Exception:
+            try:
+                self.mask |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            except Exception:
+                pass
+
+    def _run(self):
+        while not self._stop.is_set():
+            self._once()
+            time.sleep(0.0005)
+
+    def __enter__(self):
+        if self.ok:
+            self.t = threading.Thread(target=self._run, daemon=True)
+            self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        if self.ok:
+            self._once()
+            self._stop.set()
+            self.t.join()
+
+    def summary(self):
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "error": self.err}
+        s = sorted(self.samples)
+        reasons = [n for b, n in self.REASONS.items() if self.mask & b and n != "gpu_idle"]
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": reasons,
+                "samples": len(s)}
+
+
+# ----------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on this box's host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import numpy as np
+    import oracle
+    from paper_2501_10653_b200 import synth
+    idx, _, _ = WORKLOADS[args.workload]
+    cfg = synth.CONFIGS[idx]
+    k = (cfg.C1, cfg.C2, cfg.C, cfg.D)
+    n_sample = 2 if cfg.N <= 2048 else 1
+    pairs = [synth.make_pair(cfg, seed=s)[:2] for s in range(n_sample)]
+    cores = oracle.max_threads()
+
+    def step():
+        for x, y in pairs:
+            t = oracle.tiles(x, y, cfg.N_T, *k)
+            oracle.aggregate(t["lisi"], t["auglisi"], t["X"], t["Y"], cfg.C2, cfg.C)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    us = dt / (args.steps * n_sample) * 1e6
+    sample = f"{n_sample} pair(s) of {cfg.name} per step, oracle tiles + aggregate, all host cores"
+    line = {"impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(cfg, n_sample, "host memory (CPU oracle)"),
+            "cpu_baseline": {"value": us, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": us, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(cfg, pairs_per_step, l2):
+    return {"workload": cfg.name, "N": cfg.N, "N_T": cfg.N_T, "tiles": (cfg.N // cfg.N_T) ** 2,
+            "pairs_per_step": pairs_per_step, "C1": cfg.C1, "C2": cfg.C2, "C": cfg.C, "D": cfg.D,
+            "l2": l2, "parallelism": "independent pairs per GPU, no collective"}
+
+
+# ----------------------------------------------------------------------------- our arm
+class Batch:
+    """P image pairs of one workload resident in HBM, their outputs, and the step that runs them."""
+
+    def __init__(self, cfg, pairs, device, seed0=0):
+        import torch
+        from paper_2501_10653_b200 import binding, synth
+        self.torch, self.B, self.cfg, self.P = torch, binding, cfg, pairs
+        nt = cfg.N // cfg.N_T
+        self.n = nt * nt
+        self.x, self.y = [], []
+        for s in range(pairs):
+            xd, yd, _ = synth.make_pair(cfg, seed=seed0 + s, device=str(device))
+            self.x.append(xd)
+            self.y.append(yd)
+        mk = lambda: torch.empty((pairs, self.n), dtype=torch.float32, device=device)
+        self.lisi, self.aug, self.sx, self.sy = mk(), mk(), mk(), mk()
+        self.out2 = torch.empty((pairs, 2), dtype=torch.float32, device=device)
+        self.ws, self.wsb = binding.make_workspace(cfg.N, cfg.N_T, device)
+        self.k = (float(cfg.C1), float(cfg.C2), float(cfg.C), float(cfg.D))
+
+    def step(self, aggregate=True):
+        B, cfg = self.B, self.cfg
+        st = self.torch.cuda.current_stream().cuda_stream
+        C1, C2, C, D = self.k
+        for i in range(self.P):
+            rc = B.iqa_fused_tiles(self.x[i], self.y[i], cfg.N, cfg.N_T, C1, C2, C, D,
+                                   self.lisi[i], self.aug[i], self.sx[i], self.sy[i], None, None,
+                                   self.ws, self.wsb, st)
+            if rc:
+                raise B.IqaError(rc, "iqa_fused_tiles")
+            if aggregate:
+                rc = B.iqa_aggregate(self.lisi[i], self.aug[i], self.sx[i], self.sy[i], self.n,
+                                     C2, C, self.out2[i], st)
+                if rc:
+                    raise B.IqaError(rc, "iqa_aggregate")
+
+    def launches_per_step(self, aggregate=True):
+        split = self.B.iqa_workspace_bytes(self.cfg.N, self.cfg.N_T) > 0
+        return self.P * ((2 if split else 1) + (1 if aggregate else 0))
+
+    def graph(self, aggregate=True):
+        torch = self.torch
+        g = torch.cuda.CUDAGraph()
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            self.step(aggregate)                      # warm-up outside capture
+        torch.cuda.current_stream().wait_stream(s)
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g):
+            self.step(aggregate)
+        return g
+
+
+def time_region(torch, fn, steps, dist=None):
+    """Barrier + synchronize, CUDA events around `steps` calls of fn on the current stream,
+    synchronize + barrier; returns elapsed ms (max over ranks when distributed)."""
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.barrier()
+        ms = float(t.item())
+    return ms
+
+
+def cpu_baseline(cfg, budget_s=8.0):
+    """The oracle as it stands on this box's host cores, on a bounded sample of the workload."""
+    import oracle
+    from paper_2501_10653_b200 import synth
+    x, y, _ = synth.make_pair(cfg, seed=0) if cfg.N <= 8192 else synth.make_pair(synth.scaled(cfg, 8192), seed=0)
+    N = x.shape[0]
+    k = (cfg.C1, cfg.C2, cfg.C, cfg.D)
+    oracle.tiles(x[:256, :256].copy(), y[:256, :256].copy(), min(cfg.N_T, 256), *k)   # load the library
+    reps, t0 = 0, time.perf_counter()
+    while True:
+        t = oracle.tiles(x, y, cfg.N_T, *k)
+        oracle.aggregate(t["lisi"], t["auglisi"], t["X"], t["Y"], cfg.C2, cfg.C)
+        reps += 1
+        dt = time.perf_counter() - t0
+        if dt >= budget_s or reps >= 200:
+            break
+    us = dt / reps * 1e6 * (cfg.N / N) ** 2      # scaled by pixel count when the sample is a smaller canvas
+    sample = (f"{reps} repetition(s) of one {N}x{N} pair of the {cfg.name} recipe (N_T={cfg.N_T}), "
+              f"oracle tiles + aggregate" + ("" if N == cfg.N else f", time scaled by ({cfg.N}/{N})^2"))
+    return {"value": us, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample}
+
+
+def run_e2e(torch, binding, cfg, pairs, steps, warmup, device, dist):
+    """Same metric through iqa_fused_host: pinned host buffers in, H2D + kernels + D2H + sync per pair."""
+    from paper_2501_10653_b200 import synth
+    host = []
+    for s in range(pairs):
+        if cfg.N <= 8192:
+            x, y, _ = synth.make_pair(cfg, seed=100 + s)
+            host.append((torch.from_numpy(x).pin_memory(), torch.from_numpy(y).pin_memory()))
+        else:   # 1 GiB images: draw on the device, keep pinned copies
+            xd, yd, _ = synth.make_pair(cfg, seed=100 + s, device=str(device))
+            host.append((xd.cpu().pin_memory(), yd.cpu().pin_memory()))
+            del xd, yd
+    runner = binding.HostRunner(cfg.N, cfg.N_T, device)
+    k = (float(cfg.C1), float(cfg.C2), float(cfg.C), float(cfg.D))
+
+    def step():
+        for xh, yh in host:
+            runner(xh, yh, *k)
+
+    for _ in range(max(1, warmup)):
+        step()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        step()                      # every call ends in cudaStreamSynchronize inside the library
+    torch.cuda.synchronize()
+    dt_ms = (time.perf_counter() - t0) * 1e3
+    if dist is not None:
+        t = torch.tensor([dt_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt_ms = float(t.item())
+    world = 1 if dist is None else dist.get_world_size()
+    return {"value": dt_ms * 1e3 / (steps * pairs * world), "unit": UNIT,
+            "h2d_bytes_per_step": pairs * runner.h2d_bytes, "d2h_bytes_per_step": pairs * runner.d2h_bytes,
+            "pairs_per_step": pairs, "gb_per_s_h2d": pairs * runner.h2d_bytes * steps / (dt_ms * 1e-3) / 1e9,
+            "launches_per_step": pairs * 2, "host_memory": "pinned"}
+
+
+def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, use_graph, rank):
+    """Device-resident timing of one workload.  Returns dict with step time and kernel-only time."""
+    batch = Batch(cfg, pairs, device, seed0=1000 * rank)
+    if use_graph:
+        g_full, g_kernel = batch.graph(True), batch.graph(False)
+        full, kern = g_full.replay, g_kernel.replay
+    else:
+        full, kern = (lambda: batch.step(True)), (lambda: batch.step(False))
+    for _ in range(warmup):
+        full()
+    with ClockSampler(torch.cuda.current_device()) as clk:
+        ms = time_region(torch, full, steps, dist)
+    for _ in range(warmup):
+        kern()
+    ms_kernel = time_region(torch, kern, steps, dist)
+    # warm (L2-resident when the pair fits): the same pair back to back, as the paper's 10 runs
+    one = Batch.__new__(Batch)
+    one.__dict__.update(batch.__dict__)
+    one.P = 1
+    one_fn = one.graph(False).replay if use_graph else (lambda: one.step(False))
+    for _ in range(max(3, warmup)):
+        one_fn()
+    ms_warm = time_region(torch, one_fn, max(steps, 20), dist) / max(steps, 20)
+    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "us_warm_same_pair": ms_warm * 1e3,
+            "clocks": clk.summary()}
+
+
+def run_ours(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    from paper_2501_10653_b200 import binding, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as td
+        td.init_process_group("nccl", device_id=device)
+        dist = td
+
+    idx, pairs, pairs_e2e = WORKLOADS[args.workload]
+    if args.pairs:
+        pairs = args.pairs
+    cfg = synth.CONFIGS[idx]
+    use_graph = not args.no_graph
+    K, W = args.steps, args.warmup
+
+    m = measure_workload(torch, binding, cfg, pairs, K, W, device, dist, use_graph, rank)
+    total_pairs = K * pairs * world
+    us_per_pair = m["ms"] * 1e3 / total_pairs
+    us_kernel = m["ms_kernel"] * 1e3 / (K * pairs)          # per launch of the fused kernel (max over ranks)
+    us_warm, clocks = m["us_warm_same_pair"], m["clocks"]
+    alg = algorithmic_bytes(cfg.N, cfg.N_T)
+    peak, peak_src = measured_peak()
+    achieved = alg / (us_kernel * 1e-6) / 1e9
+    split = binding.iqa_workspace_bytes(cfg.N, cfg.N_T) > 0
+    del m
+    torch.cuda.empty_cache()
+
+    e2e = run_e2e(torch, binding, cfg, pairs_e2e, max(2, min(K, 10)), min(W, 2), device, dist)
+
+    also = {}
+    if args.workload == "cfg1" and not args.no_also and world == 1:
+        # the north-star bar (>= 75 % of HBM peak) is quoted at N >= 8192: measure config [3] beside the headline
+        c3, p3, k3 = synth.CONFIGS[3], 4, max(3, min(K, 10))
+        m3 = measure_workload(torch, binding, c3, p3, k3, max(3, W), device, None, use_graph, rank)
+        us3 = m3["ms_kernel"] * 1e3 / (k3 * p3)
+        gbs3 = algorithmic_bytes(c3.N, c3.N_T) / (us3 * 1e-6) / 1e9
+        also[c3.name] = {"us_per_pair_step": m3["ms"] * 1e3 / (k3 * p3), "us_fused_kernel": us3,
+                         "achieved_GBps": gbs3, "frac_of_measured_peak": gbs3 / peak,
+                         "frac_of_nominal_8000": gbs3 / 8000.0, "pairs_per_step": p3, "clocks": m3["clocks"]}
+        del m3
+        torch.cuda.empty_cache()
+
+    cpu = cpu_baseline(cfg) if rank == 0 and world == 1 else None
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": us_per_pair, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": (us_per_pair * pairs * world) / 1e3, "higher_is_better": False, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_config(cfg, pairs, f"inputs {pairs * 8 * cfg.N * cfg.N / 2**20:.0f} MiB per step > 126 MB L2: "
+                                      "every pair is read cold from HBM; no explicit flush"),
+            "pairs_per_s": 1e6 / us_per_pair,
+            "launch": "cuda graph of the step" if use_graph else "direct launches through ctypes",
+            "gpu_launches": K * world * (pairs * ((2 if split else 1) + 1)),
+            "kernels": ["iqa::strip_kernel<3,RW> (fused S1-S4)"] + (["iqa::finalise_*_kernel"] if split else [])
+                       + ["iqa::aggregate_kernel (S5)"],
+            "roofline": {"bound": "hbm", "kernel": "iqa::strip_kernel<fused>", "achieved": achieved, "peak": peak,
+                         "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+                         "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
+                         "us_per_launch": us_kernel, "frac_of_nominal_8000": achieved / 8000.0},
+            "us_warm_same_pair": us_warm,
+            "e2e": e2e,
+            "clocks": clocks,
+            "paper_context": {"note": "H100 kernel-only medians at N=2048, N_T=64 (PAPER.md:31); context, not the target",
+                              "h100_split_lisi_us": 101.0, "h100_split_auglisi_us": 91.0},
+        }
+        if cpu is not None:
+            line["cpu_baseline"] = cpu
+        if also:
+            line["also"] = also
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg1", choices=sorted(WORKLOADS))
+    ap.add_argument("--pairs", type=int, default=0, help="pairs per step (default per workload)")
+    ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the extra N=8192 measurement")
+    args = ap.parse_args()
+    args.warmup = max(3, args.warmup)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -15,6 +15,8 @@ import ctypes
 import os
 import subprocess
 
+os.environ.setdefault("OMP_WAIT_POLICY", "passive")   # idle OpenMP threads sleep instead of spinning
+
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -51,8 +53,31 @@ def _load():
     return _lib
 
 
+def _cpu_budget() -> int:
+    """CPUs this process may actually use: scheduler affinity capped by the cgroup CPU quota.
+    (OpenMP's own default ignores the quota; oversubscribed spinning threads are very slow.)"""
+    n = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    for path in ("/sys/fs/cgroup/cpu.max", "/sys/fs/cgroup/cpu/cpu.cfs_quota_us"):
+        try:
+            with open(path) as f:
+                parts = f.read().split()
+            if path.endswith("cpu.max"):
+                if parts[0] != "max":
+                    n = min(n, max(1, int(int(parts[0]) / int(parts[1]))))
+            else:
+                quota = int(parts[0])
+                if quota > 0:
+                    with open("/sys/fs/cgroup/cpu/cpu.cfs_period_us") as g:
+                        n = min(n, max(1, quota // int(g.read().split()[0])))
+            break
+        except (OSError, ValueError, IndexError):
+            continue
+    return max(1, n)
+
+
 def max_threads() -> int:
-    return int(_load().iqa_oracle_max_threads())
+    """Threads the oracle uses by default: min(OpenMP default, usable CPUs)."""
+    return max(1, min(int(_load().iqa_oracle_max_threads()), _cpu_budget()))
 
 
 def _f32c(a) -> np.ndarray:
@@ -88,7 +113,7 @@ def tiles(x, y, N_T: int, C1, C2, C, D, threads: int = 0) -> dict:
         x.ctypes.data_as(fp), y.ctypes.data_as(fp), N, N_T,
         float(np.float32(C1)), float(np.float32(C2)), float(np.float32(C)), float(np.float32(D)),
         _dptr(out["lisi"]), _dptr(out["auglisi"]), _dptr(out["X"]), _dptr(out["Y"]),
-        _dptr(out["L"]), _dptr(out["A"]), int(threads))
+        _dptr(out["L"]), _dptr(out["A"]), int(threads) if threads > 0 else max_threads())
     if rc != 0:
         raise RuntimeError(f"iqa_oracle_tiles failed with code {rc}")
     return out

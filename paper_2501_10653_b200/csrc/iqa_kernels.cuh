@@ -96,9 +96,13 @@ __device__ __forceinline__ void finalise_tile(const TileParams& p, int t, float4
 // flight together).  Requires: N_T a power of two >= max(8, RW), N % N_T == 0, x and y
 // 16-byte aligned (N % 4 == 0 follows).  Ragged right/bottom edges (N % 128, N % (8*RW))
 // are handled by idle lanes / warps: they contribute exact zeros.
+// MIN_CTAS is the register budget handed to ptxas (65536 / (256 * MIN_CTAS) registers per
+// thread): with the default "maximise occupancy" heuristic ptxas sinks each load next to its
+// use and keeps only 2-4 of them in flight; with MIN_CTAS = 2 it hoists all 2*RW loads of a
+// lane above the arithmetic (checked in SASS), which is what keeps HBM busy.
 // -----------------------------------------------------------------------------
-template <int MODE, int RW>
-__global__ void __launch_bounds__(kCtaThreads)
+template <int MODE, int RW, int MIN_CTAS = 2>
+__global__ void __launch_bounds__(kCtaThreads, MIN_CTAS)
 strip_kernel(const TileParams p) {
     constexpr int RB = kWarpsPerCta * RW;      // rows per unit
     __shared__ float4 part[kWarpsPerCta][16];  // per warp: <= 16 tile segments (N_T = 8)
@@ -114,8 +118,9 @@ strip_kernel(const TileParams p) {
     float aL[4] = {0.f, 0.f, 0.f, 0.f}, aA[4] = {0.f, 0.f, 0.f, 0.f};
     float aX[4] = {0.f, 0.f, 0.f, 0.f}, aY[4] = {0.f, 0.f, 0.f, 0.f};
 
-    if (col < N && row0 < N) {
-        const size_t off = (size_t)row0 * (size_t)N + (size_t)col;
+    if (row0 < N) {                            // warp-uniform: the whole warp is inside or outside
+        const bool in_cols = col < N;          // ragged right edge: idle lanes contribute exact zeros
+        const size_t off = (size_t)row0 * (size_t)N + (size_t)(in_cols ? col : 0);
         const float* px = p.x + off;
         const float* py = p.y + off;
         const float C1 = p.C1;
@@ -124,10 +129,12 @@ strip_kernel(const TileParams p) {
             float4 vx[4], vy[4];
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                vx[k] = ldg_stream(px + (size_t)(i + k) * (size_t)N);
-                vy[k] = ldg_stream(py + (size_t)(i + k) * (size_t)N);
+                vx[k] = vy[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (in_cols) {
+                    vx[k] = ldg_stream(px + (size_t)(i + k) * (size_t)N);
+                    vy[k] = ldg_stream(py + (size_t)(i + k) * (size_t)N);
+                }
             }
-            __syncwarp();   // scheduling fence: keeps all 8 loads in flight ahead of the arithmetic
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 pixel_terms<MODE>(vx[k].x, vy[k].x, C1, aL[0], aA[0], aX[0], aY[0]);
