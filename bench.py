@@ -4,12 +4,13 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg3|cfg4] [--impl reference]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
-A STEP is one pass of the whole hot path -- iqa_fused_tiles (S1-S4) then iqa_aggregate (S5,
-Eqs. 3-4) -- over one batch of P distinct synthetic image pairs already resident in HBM.
-The batch is several times larger than the 126 MB L2, so every pair is read cold from HBM
-(said in ``config.l2``).  The step is captured once in a CUDA graph (2 P kernel launches) so
-that Python/ctypes launch overhead does not sit between 5-us kernels; ``--no-graph`` launches
-directly.  One JSON line is printed by rank 0; see DESIGN.md "Measurement" for every key.
+A STEP is one pass of the whole hot path -- S1-S4 (clamp, per-pixel terms, per-tile sums,
+Eqs. 1-2) and S5 (Eqs. 3-4 per pair) -- over one batch of P distinct synthetic image pairs
+already resident in HBM, through ONE call of iqa_fused_batch (one persistent stream kernel
+over all pairs, a finalise pass for split tiles, one aggregate launch).  The batch is several
+times larger than the 126 MB L2, so every pair is read cold from HBM (said in ``config.l2``).
+The step is captured once in a CUDA graph; ``--no-graph`` launches through ctypes each step.
+One JSON line is printed by rank 0; see DESIGN.md "Measurement" for every key.
 """
 from __future__ import annotations
 
@@ -153,7 +154,8 @@ def workload_config(cfg, pairs_per_step, l2):
 
 # ----------------------------------------------------------------------------- our arm
 class Batch:
-    """P image pairs of one workload resident in HBM, their outputs, and the step that runs them."""
+    """P image pairs of one workload resident in HBM, their outputs, and the step that runs them:
+    ONE iqa_fused_batch call (S1-S4 for all pairs in one persistent kernel, then Eqs. 3-4 per pair)."""
 
     def __init__(self, cfg, pairs, device, seed0=0):
         import torch
@@ -169,40 +171,53 @@ class Batch:
         mk = lambda: torch.empty((pairs, self.n), dtype=torch.float32, device=device)
         self.lisi, self.aug, self.sx, self.sy = mk(), mk(), mk(), mk()
         self.out2 = torch.empty((pairs, 2), dtype=torch.float32, device=device)
-        self.ws, self.wsb = binding.make_workspace(cfg.N, cfg.N_T, device)
+        self.wsb = binding.iqa_batch_workspace_bytes(pairs, cfg.N, cfg.N_T)
+        self.ws = torch.empty(self.wsb, dtype=torch.uint8, device=device) if self.wsb else None
         self.k = (float(cfg.C1), float(cfg.C2), float(cfg.C), float(cfg.D))
+        self.xt, _ = binding._ptr_table(self.x)          # host tables of device pointers, built once
+        self.yt, _ = binding._ptr_table(self.y)
+        self.ws1, self.wsb1 = binding.make_workspace(cfg.N, cfg.N_T, device)
 
     def step(self, aggregate=True):
         B, cfg = self.B, self.cfg
         st = self.torch.cuda.current_stream().cuda_stream
         C1, C2, C, D = self.k
-        for i in range(self.P):
-            rc = B.iqa_fused_tiles(self.x[i], self.y[i], cfg.N, cfg.N_T, C1, C2, C, D,
-                                   self.lisi[i], self.aug[i], self.sx[i], self.sy[i], None, None,
-                                   self.ws, self.wsb, st)
+        rc = B.iqa_fused_batch(self.xt, self.yt, self.P, cfg.N, cfg.N_T, C1, C2, C, D,
+                               self.lisi, self.aug, self.sx, self.sy, None, None,
+                               self.out2 if aggregate else None, self.ws, self.wsb, st)
+        if rc:
+            raise B.IqaError(rc, "iqa_fused_batch")
+
+    def step_single(self, i=0, aggregate=True):
+        """The per-pair entry points on pair i: iqa_fused_tiles then iqa_aggregate (2-3 launches)."""
+        B, cfg = self.B, self.cfg
+        st = self.torch.cuda.current_stream().cuda_stream
+        C1, C2, C, D = self.k
+        rc = B.iqa_fused_tiles(self.x[i], self.y[i], cfg.N, cfg.N_T, C1, C2, C, D,
+                               self.lisi[i], self.aug[i], self.sx[i], self.sy[i], None, None,
+                               self.ws1, self.wsb1, st)
+        if rc:
+            raise B.IqaError(rc, "iqa_fused_tiles")
+        if aggregate:
+            rc = B.iqa_aggregate(self.lisi[i], self.aug[i], self.sx[i], self.sy[i], self.n, C2, C, self.out2[i], st)
             if rc:
-                raise B.IqaError(rc, "iqa_fused_tiles")
-            if aggregate:
-                rc = B.iqa_aggregate(self.lisi[i], self.aug[i], self.sx[i], self.sy[i], self.n,
-                                     C2, C, self.out2[i], st)
-                if rc:
-                    raise B.IqaError(rc, "iqa_aggregate")
+                raise B.IqaError(rc, "iqa_aggregate")
 
     def launches_per_step(self, aggregate=True):
-        split = self.B.iqa_workspace_bytes(self.cfg.N, self.cfg.N_T) > 0
-        return self.P * ((2 if split else 1) + (1 if aggregate else 0))
+        split = self.wsb > 0
+        return -(-self.P // 32) + (1 if split else 0) + (1 if aggregate else 0)
 
-    def graph(self, aggregate=True):
+    def graph(self, fn):
         torch = self.torch
         g = torch.cuda.CUDAGraph()
         s = torch.cuda.Stream()
         s.wait_stream(torch.cuda.current_stream())
         with torch.cuda.stream(s):
-            self.step(aggregate)                      # warm-up outside capture
+            fn()                                      # warm-up outside capture
         torch.cuda.current_stream().wait_stream(s)
         torch.cuda.synchronize()
         with torch.cuda.graph(g):
-            self.step(aggregate)
+            fn()
         return g
 
 
@@ -286,17 +301,16 @@ def run_e2e(torch, binding, cfg, pairs, steps, warmup, device, dist):
     return {"value": dt_ms * 1e3 / (steps * pairs * world), "unit": UNIT,
             "h2d_bytes_per_step": pairs * runner.h2d_bytes, "d2h_bytes_per_step": pairs * runner.d2h_bytes,
             "pairs_per_step": pairs, "gb_per_s_h2d": pairs * runner.h2d_bytes * steps / (dt_ms * 1e-3) / 1e9,
-            "launches_per_step": pairs * 2, "host_memory": "pinned"}
+            "launches_per_step": pairs * (3 if binding.iqa_workspace_bytes(cfg.N, cfg.N_T) else 2), "host_memory": "pinned"}
 
 
 def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, use_graph, rank):
     """Device-resident timing of one workload.  Returns dict with step time and kernel-only time."""
     batch = Batch(cfg, pairs, device, seed0=1000 * rank)
+    full, kern = (lambda: batch.step(True)), (lambda: batch.step(False))
+    single = lambda: batch.step_single(0, True)
     if use_graph:
-        g_full, g_kernel = batch.graph(True), batch.graph(False)
-        full, kern = g_full.replay, g_kernel.replay
-    else:
-        full, kern = (lambda: batch.step(True)), (lambda: batch.step(False))
+        full, kern, single = batch.graph(full).replay, batch.graph(kern).replay, batch.graph(single).replay
     for _ in range(warmup):
         full()
     with ClockSampler(torch.cuda.current_device()) as clk:
@@ -304,15 +318,13 @@ def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, us
     for _ in range(warmup):
         kern()
     ms_kernel = time_region(torch, kern, steps, dist)
-    # warm (L2-resident when the pair fits): the same pair back to back, as the paper's 10 runs
-    one = Batch.__new__(Batch)
-    one.__dict__.update(batch.__dict__)
-    one.P = 1
-    one_fn = one.graph(False).replay if use_graph else (lambda: one.step(False))
+    # latency of ONE pair through the per-pair entry points, same pair back to back (warm: L2-resident
+    # when the pair fits) -- the quantity the paper's 10-run median measures
+    reps = max(steps, 20)
     for _ in range(max(3, warmup)):
-        one_fn()
-    ms_warm = time_region(torch, one_fn, max(steps, 20), dist) / max(steps, 20)
-    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "us_warm_same_pair": ms_warm * 1e3,
+        single()
+    ms_single = time_region(torch, single, reps, dist) / reps
+    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "us_single_pair_warm": ms_single * 1e3,
             "clocks": clk.summary()}
 
 
@@ -343,12 +355,14 @@ def run_ours(args):
     m = measure_workload(torch, binding, cfg, pairs, K, W, device, dist, use_graph, rank)
     total_pairs = K * pairs * world
     us_per_pair = m["ms"] * 1e3 / total_pairs
-    us_kernel = m["ms_kernel"] * 1e3 / (K * pairs)          # per launch of the fused kernel (max over ranks)
-    us_warm, clocks = m["us_warm_same_pair"], m["clocks"]
-    alg = algorithmic_bytes(cfg.N, cfg.N_T)
+    n_stream = -(-pairs // 32)                               # launches of the stream kernel per step
+    us_launch = m["ms_kernel"] * 1e3 / (K * n_stream)       # per launch of the stream kernel (max over ranks)
+    us_single, clocks = m["us_single_pair_warm"], m["clocks"]
+    alg = algorithmic_bytes(cfg.N, cfg.N_T) * pairs / n_stream    # algorithmic bytes one launch moves
     peak, peak_src = measured_peak()
-    achieved = alg / (us_kernel * 1e-6) / 1e9
+    achieved = alg / (us_launch * 1e-6) / 1e9
     split = binding.iqa_workspace_bytes(cfg.N, cfg.N_T) > 0
+    launches = m["batch"].launches_per_step(True)
     del m
     torch.cuda.empty_cache()
 
@@ -361,7 +375,8 @@ def run_ours(args):
         m3 = measure_workload(torch, binding, c3, p3, k3, max(3, W), device, None, use_graph, rank)
         us3 = m3["ms_kernel"] * 1e3 / (k3 * p3)
         gbs3 = algorithmic_bytes(c3.N, c3.N_T) / (us3 * 1e-6) / 1e9
-        also[c3.name] = {"us_per_pair_step": m3["ms"] * 1e3 / (k3 * p3), "us_fused_kernel": us3,
+        also[c3.name] = {"us_per_pair_step": m3["ms"] * 1e3 / (k3 * p3), "us_per_pair_stream_kernel": us3,
+                         "us_single_pair_warm": m3["us_single_pair_warm"],
                          "achieved_GBps": gbs3, "frac_of_measured_peak": gbs3 / peak,
                          "frac_of_nominal_8000": gbs3 / 8000.0, "pairs_per_step": p3, "clocks": m3["clocks"]}
         del m3
@@ -377,15 +392,17 @@ def run_ours(args):
             "config": workload_config(cfg, pairs, f"inputs {pairs * 8 * cfg.N * cfg.N / 2**20:.0f} MiB per step > 126 MB L2: "
                                       "every pair is read cold from HBM; no explicit flush"),
             "pairs_per_s": 1e6 / us_per_pair,
-            "launch": "cuda graph of the step" if use_graph else "direct launches through ctypes",
-            "gpu_launches": K * world * (pairs * ((2 if split else 1) + 1)),
-            "kernels": ["iqa::strip_kernel<3,RW> (fused S1-S4)"] + (["iqa::finalise_*_kernel"] if split else [])
-                       + ["iqa::aggregate_kernel (S5)"],
-            "roofline": {"bound": "hbm", "kernel": "iqa::strip_kernel<fused>", "achieved": achieved, "peak": peak,
+            "launch": ("cuda graph of the step" if use_graph else "direct launches through ctypes")
+                      + ": one iqa_fused_batch call per step",
+            "gpu_launches": K * world * launches,
+            "kernels": ["iqa::stream_kernel<3,K,2,CTAs> (fused S1-S4, all pairs of the step)"]
+                       + (["iqa::finalise_*_kernel"] if split else []) + ["iqa::aggregate_kernel (S5, one CTA per pair)"],
+            "roofline": {"bound": "hbm", "kernel": "iqa::stream_kernel<fused>", "achieved": achieved, "peak": peak,
                          "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
                          "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
-                         "us_per_launch": us_kernel, "frac_of_nominal_8000": achieved / 8000.0},
-            "us_warm_same_pair": us_warm,
+                         "us_per_launch": us_launch, "pairs_per_launch": pairs / n_stream,
+                         "frac_of_nominal_8000": achieved / 8000.0},
+            "us_single_pair_warm": us_single,
             "e2e": e2e,
             "clocks": clocks,
             "paper_context": {"note": "H100 kernel-only medians at N=2048, N_T=64 (PAPER.md:31); context, not the target",
@@ -408,7 +425,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg1", choices=sorted(WORKLOADS))
     ap.add_argument("--pairs", type=int, default=0, help="pairs per step (default per workload)")
-    ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="launch through ctypes each step instead of replaying a CUDA graph")
     ap.add_argument("--no-also", action="store_true", help="skip the extra N=8192 measurement")
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)

@@ -16,7 +16,8 @@
  *
  * Conventions (the paper states none; DESIGN.md "Boundary" and "Readings"):
  *   * Every pointer is a DEVICE pointer owned by the caller unless the argument name ends
- *     in `_host`.  The library allocates no device memory and keeps no state between calls.
+ *     in `_host`.  The library allocates no device memory and keeps no state between calls
+ *     (beyond a per-device cache of launch geometry: SM count, resident CTAs per SM).
  *   * `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device
  *     entry points are ASYNCHRONOUS: they validate, enqueue and return; outputs are valid
  *     once the stream has reached that point.  x and y are never written.
@@ -30,14 +31,15 @@
  *   * Errors: a status code is returned, nothing is thrown or printed, and NOTHING is
  *     enqueued when the status is not IQA_OK (validation precedes the first launch).
  *       NULL required pointer ....................................... IQA_ERR_NULL
- *       N <= 0, N_T <= 0, N % N_T != 0, n_tiles <= 0, g bad .. IQA_ERR_SHAPE
+ *       N <= 0, N_T <= 0, N % N_T != 0, n_tiles <= 0,
+ *       n_pairs <= 0, g bad ......................................... IQA_ERR_SHAPE
  *       C1, C2 or C not finite or <= 0, D not finite ................ IQA_ERR_PARAM
  *       x or y not 4-byte aligned ................................... IQA_ERR_ALIGN
  *       workspace NULL / too small when iqa_workspace_bytes() > 0 ... IQA_ERR_WORKSPACE
  *       CUDA launch / copy failure .................................. IQA_ERR_CUDA
  *   * Any N_T that divides N is accepted.  Power-of-two N_T >= 8 with 16-byte aligned
- *     x and y take the vectorised strip kernels; everything else takes a generic
- *     (slower, still CUDA) kernel.  Results are deterministic: fixed reduction order,
+ *     x and y take the persistent cp.async-pipelined stream kernel; everything else takes a
+ *     generic (slower, still CUDA) kernel.  Results are deterministic: fixed reduction order,
  *     no floating-point atomics; two calls on the same inputs are bit-identical.
  * ============================================================================= */
 #ifndef IQA_TILES_H
@@ -67,7 +69,7 @@ const char* iqa_version(void);
 
 /* Bytes of device workspace the *_tiles entry points need for (N, N_T): 0 when every tile
  * is finished inside one CTA, else room for the per-piece partial sums of split tiles
- * (16 B per piece).  Returns 0 for invalid shapes (the entry points report those). */
+ * (16 B per piece of 128 x 64 pixels).  Returns 0 for invalid shapes (the entry points report those). */
 size_t iqa_workspace_bytes(int N, int N_T);
 
 /* Eq. 1 per tile (clamp P:27).
@@ -94,6 +96,28 @@ int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
                     float* lisi, float* auglisi,
                     float* sum_x, float* sum_y,
                     float* lisi_num, float* auglisi_num,
+                    void* workspace, size_t workspace_bytes, void* stream);
+
+/* Bytes of device workspace iqa_fused_batch needs: n_pairs * iqa_workspace_bytes(N, N_T). */
+size_t iqa_batch_workspace_bytes(int n_pairs, int N, int N_T);
+
+/* The whole hot path over a BATCH of image pairs of one shape (e.g. the snapshots of a time
+ * series, or the 16-pair throughput loop of BASELINE.json config [4]) in as few launches as
+ * possible: one persistent kernel streams all pairs (Eqs. 1-2 per tile, clamp fused into the
+ * load), then -- only for tiles larger than 64 -- one finalise pass, then, when out2 is given,
+ * one launch applies Eqs. 3-4 to every pair.
+ *   x_ptrs_host, y_ptrs_host  HOST arrays of n_pairs DEVICE pointers to [N*N] images; the
+ *                        arrays are read during the call only (they may be freed on return)
+ *   lisi, auglisi, sum_x, sum_y  [n_pairs * n] device, required; pair p occupies [p*n, (p+1)*n)
+ *   lisi_num, auglisi_num        [n_pairs * n] device, MAY BE NULL
+ *   out2                 [n_pairs * 2] device, MAY BE NULL: out2[2p] = LISI, out2[2p+1] = augLISI of pair p
+ *   workspace            >= iqa_batch_workspace_bytes(n_pairs, N, N_T) bytes (may be NULL when 0)
+ * n_pairs * n must stay below 2^31.  Results are bit-identical to n_pairs calls of
+ * iqa_fused_tiles + iqa_aggregate. */
+int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,
+                    int N, int N_T, float C1, float C2, float C, float D,
+                    float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                    float* lisi_num, float* auglisi_num, float* out2,
                     void* workspace, size_t workspace_bytes, void* stream);
 
 /* Eqs. 3-4: merge n_tiles per-tile values into the whole-image pair.

@@ -23,8 +23,8 @@ from . import build as _build
 IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKSPACE, IQA_ERR_CUDA = range(7)
 
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
-           "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_aggregate", "iqa_merge_tiles",
-           "iqa_host_scratch_bytes", "iqa_fused_host")
+           "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
+           "iqa_aggregate", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host")
 
 
 class IqaError(RuntimeError):
@@ -58,6 +58,10 @@ def _load() -> ctypes.CDLL:
     lib.iqa_auglisi_tiles.argtypes = [vp, vp, i, i, f, vp, vp, sz, vp]
     lib.iqa_fused_tiles.restype = i
     lib.iqa_fused_tiles.argtypes = [vp, vp, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_batch_workspace_bytes.restype = sz
+    lib.iqa_batch_workspace_bytes.argtypes = [i, i, i]
+    lib.iqa_fused_batch.restype = i
+    lib.iqa_fused_batch.argtypes = [vp, vp, i, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.iqa_aggregate.restype = i
     lib.iqa_aggregate.argtypes = [vp, vp, vp, vp, i, f, f, vp, vp]
     lib.iqa_merge_tiles.restype = i
@@ -133,6 +137,32 @@ def iqa_fused_tiles(x, y, N, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
                                _ptr(workspace), int(workspace_bytes), _stream(stream))
 
 
+def iqa_batch_workspace_bytes(n_pairs: int, N: int, N_T: int) -> int:
+    return int(lib.iqa_batch_workspace_bytes(int(n_pairs), int(N), int(N_T)))
+
+
+def _ptr_table(images):
+    """HOST array of device pointers (ctypes) from a sequence of tensors / addresses, or None."""
+    if images is None:
+        return None, 0
+    if isinstance(images, ctypes.Array):
+        return images, len(images)
+    vals = [_ptr(a) or 0 for a in images]
+    return (ctypes.c_void_p * len(vals))(*vals), len(vals)
+
+
+def iqa_fused_batch(x_ptrs_host, y_ptrs_host, n_pairs, N, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
+                    lisi_num=None, auglisi_num=None, out2=None, workspace=None, workspace_bytes=0,
+                    stream=None) -> int:
+    """x_ptrs_host / y_ptrs_host: sequences of n_pairs CUDA tensors (or addresses), or ready ctypes arrays."""
+    xt, _ = _ptr_table(x_ptrs_host)
+    yt, _ = _ptr_table(y_ptrs_host)
+    return lib.iqa_fused_batch(xt, yt, int(n_pairs), int(N), int(N_T), C1, C2, C, D,
+                               _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
+                               _ptr(lisi_num), _ptr(auglisi_num), _ptr(out2),
+                               _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
 def iqa_aggregate(lisi, auglisi, sum_x, sum_y, n_tiles, C2, C, out2, stream=None) -> int:
     return lib.iqa_aggregate(_ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), int(n_tiles),
                              C2, C, _ptr(out2), _stream(stream))
@@ -194,6 +224,33 @@ def fused_tiles(x, y, N_T, C1, C2, C, D, numerators: bool = False, workspace=Non
                          out.get("L"), out.get("A"), workspace, wsb, _current_stream(x.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_fused_tiles")
+    return out
+
+
+def fused_batch(xs, ys, N_T, C1, C2, C, D, numerators: bool = False, aggregate: bool = True) -> dict:
+    """The whole hot path over a batch of equally shaped pairs (lists of CUDA tensors).  Returns
+    (P, nt, nt) float32 CUDA tensors lisi, auglisi, X, Y (+ L, A when ``numerators``) and, when
+    ``aggregate``, ``whole`` of shape (P, 2): [LISI, augLISI] per pair (Eqs. 3-4)."""
+    import torch
+    if len(xs) != len(ys) or not xs:
+        raise IqaError(IQA_ERR_SHAPE, "fused_batch")
+    N = _check_images(xs[0], ys[0])
+    for x, y in zip(xs, ys):
+        if _check_images(x, y) != N or x.device != xs[0].device:
+            raise ValueError("all pairs of a batch must have the same shape and device")
+    if N_T <= 0 or N % N_T:
+        raise IqaError(IQA_ERR_SHAPE, "fused_batch")
+    P, nt, dev = len(xs), N // N_T, xs[0].device
+    names = ["lisi", "auglisi", "X", "Y"] + (["L", "A"] if numerators else [])
+    out = {k: torch.empty((P, nt, nt), dtype=torch.float32, device=dev) for k in names}
+    if aggregate:
+        out["whole"] = torch.empty((P, 2), dtype=torch.float32, device=dev)
+    nbytes = iqa_batch_workspace_bytes(P, N, N_T)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev) if nbytes else None
+    rc = iqa_fused_batch(xs, ys, P, N, N_T, C1, C2, C, D, out["lisi"], out["auglisi"], out["X"], out["Y"],
+                         out.get("L"), out.get("A"), out.get("whole"), ws, nbytes, _current_stream(dev))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_fused_batch")
     return out
 
 

@@ -10,6 +10,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "iqa_kernels.cuh"
+
 namespace iqa {
 
 constexpr int kAggThreads = 1024;
@@ -41,12 +43,16 @@ __device__ __forceinline__ void agg_finish(const Agg4& a, double n, double C2, d
     *aug_out = (float)((a.n4 - (n - 1.0) * C) / (a.sx + a.sy + C));      // Eq. 4
 }
 
-// One CTA of 1024 threads: thread-strided partial sums, warp butterfly, then warp order.
+// One CTA of 1024 threads per image pair (blockIdx.x = pair of the batch; arrays are
+// [n_pairs][n]): thread-strided partial sums, warp butterfly, then warp order.
 __global__ void __launch_bounds__(kAggThreads)
 aggregate_kernel(const float* __restrict__ lisi, const float* __restrict__ aug,
                  const float* __restrict__ X, const float* __restrict__ Y, int n,
                  float C2f, float Cf, float* __restrict__ out2) {
     __shared__ Agg4 part[kAggThreads / 32];
+    pdl_prologue();
+    const size_t base = (size_t)blockIdx.x * (size_t)n;
+    lisi += base; aug += base; X += base; Y += base; out2 += 2 * (size_t)blockIdx.x;
     const double C2 = (double)C2f, C = (double)Cf;
     Agg4 a = {0.0, 0.0, 0.0, 0.0};
     for (int t = threadIdx.x; t < n; t += kAggThreads)
@@ -70,6 +76,7 @@ merge_kernel(const float* __restrict__ lisi, const float* __restrict__ aug,
              float C2f, float Cf,
              float* __restrict__ lisi_o, float* __restrict__ aug_o,
              float* __restrict__ X_o, float* __restrict__ Y_o) {
+    pdl_prologue();
     const int nto = nt / g;
     const long long o = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (o >= (long long)nto * nto) return;

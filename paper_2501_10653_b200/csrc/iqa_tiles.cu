@@ -1,22 +1,27 @@
 // =============================================================================
 // iqa_tiles.cu -- the C ABI of include/iqa_tiles.h: argument validation, the N_T-dependent
-// choice of mapping, and the launches.  No torch types, no allocation, no global state.
+// choice of mapping, and the launches.  No torch types, no allocation; the only thing kept
+// between calls is a per-device cache of launch geometry (SM count, CTAs per SM).
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -shared -Xcompiler -fPIC
 // =============================================================================
 #include "../../include/iqa_tiles.h"
 
+#include <atomic>
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
+#include <utility>
 
 #include "iqa_aggregate.cuh"
 #include "iqa_kernels.cuh"
+#include "iqa_stream.cuh"
 
 namespace {
 
 using namespace iqa;
 
 constexpr int kMaxN = 1 << 20;   // 2^40 pixels; keeps every grid and tile index inside int
+constexpr int kMaxDevices = 64;
 
 bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
@@ -27,13 +32,85 @@ int env_int(const char* name, int dflt) {
     return (s && *s) ? std::atoi(s) : dflt;
 }
 
-// How (N, N_T) is mapped onto CTAs.  DESIGN.md "Mapping".
-struct Plan {
-    bool strip;        // vectorised strip kernel (else generic kernel)
-    int rw;            // rows per warp (strip): 4, 8 or 16
-    int pieces_x, pieces_y, pieces;   // pieces per tile; pieces == 1 -> finished in one CTA
-    long long grid;    // CTAs of the first pass
-};
+// ---- stream-kernel variants (rows per warp and stage K, ring depth, CTAs per SM) -----------
+// Measured on B200 (profiles/): about 64 KiB of copies in flight per SM is
+// the sweet spot; deeper rings or more CTAs lose DRAM locality, fewer warps lose latency hiding.
+//   variant 0  K=2, depth 2, 4 CTAs/SM  (stage = 16 rows, 36 KiB smem/CTA)   default
+//   variant 1  K=4, depth 2, 3 CTAs/SM  (stage = 32 rows, 68 KiB smem/CTA)   N_T <= 16: fewer, larger reductions
+//   variant 2  K=8, depth 2, 1 CTA/SM   (stage = 64 rows, 132 KiB smem/CTA)  debug / mapping-independence tests
+constexpr int kNumVariants = 3;
+struct VariantInfo { int K, depth, min_ctas; };
+constexpr VariantInfo kVariants[kNumVariants] = {{2, 2, 4}, {4, 2, 3}, {8, 2, 1}};
+
+using StreamFn = void (*)(const BatchParams);
+
+template <int MODE>
+StreamFn stream_fn(int variant) {
+    switch (variant) {
+        case 1: return stream_kernel<MODE, 4, 2, 3>;
+        case 2: return stream_kernel<MODE, 8, 2, 1>;
+        default: return stream_kernel<MODE, 2, 2, 4>;
+    }
+}
+StreamFn stream_fn(int mode, int variant) {
+    switch (mode) {
+        case kModeLisi: return stream_fn<kModeLisi>(variant);
+        case kModeAug: return stream_fn<kModeAug>(variant);
+        default: return stream_fn<kModeFused>(variant);
+    }
+}
+size_t stream_smem(int variant) {
+    switch (variant) {
+        case 1: return stream_smem_bytes<4, 2>();
+        case 2: return stream_smem_bytes<8, 2>();
+        default: return stream_smem_bytes<2, 2>();
+    }
+}
+
+// Per-device launch geometry, filled on first use (benign race: every thread computes the same values).
+struct Geometry { std::atomic<int> ready{0}; int sms; int ctas[3][kNumVariants]; };
+Geometry g_geo[kMaxDevices];
+
+const Geometry* geometry() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
+    Geometry& g = g_geo[dev];
+    if (g.ready.load(std::memory_order_acquire)) return &g;
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return nullptr;
+    for (int m = 0; m < 3; ++m)
+        for (int v = 0; v < kNumVariants; ++v) {
+            StreamFn fn = stream_fn(m + 1, v);
+            const size_t smem = stream_smem(v);
+            if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return nullptr;
+            int occ = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kCtaThreads, smem) != cudaSuccess || occ <= 0) return nullptr;
+            g.ctas[m][v] = occ < kVariants[v].min_ctas ? occ : kVariants[v].min_ctas;
+        }
+    g.sms = sms;
+    g.ready.store(1, std::memory_order_release);
+    return &g;
+}
+
+// Launch with the programmatic-stream-serialisation attribute (PDL): the kernel may become
+// resident while the previous kernel of the stream drains; every kernel of this library
+// starts with griddepcontrol.wait, so nothing is read or written before that kernel is done.
+template <typename... KArgs, typename... Args>
+cudaError_t launch(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st,
+                   Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    static const bool no_pdl = env_int("IQA_NO_PDL", 0) != 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = no_pdl ? 0 : 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
 
 int status_of_shape(int N, int N_T) {
     if (N <= 0 || N_T <= 0 || N > kMaxN || N_T > N || N % N_T != 0) return IQA_ERR_SHAPE;
@@ -42,123 +119,168 @@ int status_of_shape(int N, int N_T) {
     return IQA_OK;
 }
 
-// Rows per warp for the strip kernel.  A tile of side <= 64 must sit inside one unit
-// (8*rw >= N_T) so that the common cases need no second pass; rw never exceeds N_T.
-int choose_rw(int N, int N_T) {
-    int rw = 8;
-    const int forced = env_int("IQA_FORCE_RW", 0);          // debug knob (tests: mapping independence)
-    if (forced == 4 || forced == 8 || forced == 16) rw = forced;
-    if (rw > N_T) rw = N_T >= 8 ? 8 : 4;
-    if (N_T <= 64 && 8 * rw < N_T) rw = N_T / 8;
-    (void)N;
-    return rw;
-}
+// How (N, N_T) is mapped onto CTAs.  DESIGN.md "Mapping".
+struct Plan {
+    bool stream;       // persistent stream kernel (else generic kernel)
+    int variant;       // stream: index into kVariants
+    int item_rows;     // stream: R
+    int pieces_x, pieces_y, pieces;   // pieces per tile; pieces == 1 -> finished inside one CTA
+};
 
-Plan make_plan(int N, int N_T, bool aligned16) {
+constexpr int kSplitItemRows = 64;   // tiles of side >= 128: items of 128 x 64, pieces to the workspace
+
+Plan make_plan(int N_T, bool aligned16) {
     Plan pl{};
-    const long long nt = N / N_T;
-    pl.strip = is_pow2(N_T) && N_T >= 8 && aligned16 && !env_int("IQA_FORCE_GENERIC", 0);
-    if (pl.strip) {
-        pl.rw = choose_rw(N, N_T);
-        const int rb = kWarpsPerCta * pl.rw;
-        pl.pieces_x = N_T > kUnitCols ? N_T / kUnitCols : 1;
-        pl.pieces_y = N_T > rb ? N_T / rb : 1;
-        pl.pieces = pl.pieces_x * pl.pieces_y;
-        const long long ux = (N + kUnitCols - 1) / kUnitCols, uy = (N + rb - 1) / rb;
-        pl.grid = ux * uy;
+    pl.stream = is_pow2(N_T) && N_T >= 8 && aligned16 && !env_int("IQA_FORCE_GENERIC", 0);
+    if (pl.stream) {
+        pl.variant = N_T <= 16 ? 1 : 0;
+        const int forced = env_int("IQA_FORCE_VARIANT", -1);     // debug knob (tests: mapping independence)
+        if (forced >= 0 && forced < kNumVariants) pl.variant = forced;
+        const int rs = kWarpsPerCta * kVariants[pl.variant].K;   // stage height
+        if (N_T <= 64) {
+            pl.item_rows = N_T > rs ? N_T : rs;                  // whole tiles inside one item
+            pl.pieces_x = pl.pieces_y = 1;
+        } else {
+            pl.item_rows = kSplitItemRows;
+            pl.pieces_x = N_T / kUnitCols;
+            pl.pieces_y = N_T / kSplitItemRows;
+        }
     } else {
-        pl.rw = 0;
         pl.pieces_x = 1;
         pl.pieces_y = (N_T + kGenericRows - 1) / kGenericRows;
-        pl.pieces = pl.pieces_y;
-        pl.grid = nt * nt * pl.pieces;
     }
+    pl.pieces = pl.pieces_x * pl.pieces_y;
     return pl;
 }
 
-size_t workspace_bytes_for(int N, int N_T) {
-    if (N_T <= 64) return 0;                                  // every path finishes tiles in one CTA
+// Pieces per tile in the worst case over the mappings a call may take (stream or generic).
+size_t max_pieces(int N_T) {
+    if (N_T <= 64) return 1;                                      // every path finishes tiles inside one CTA
+    size_t pieces = (size_t)(N_T + kGenericRows - 1) / kGenericRows;
+    if (is_pow2(N_T)) {
+        const size_t s = (size_t)(N_T / kUnitCols) * (size_t)(N_T / kSplitItemRows);
+        if (s > pieces) pieces = s;
+    }
+    return pieces;
+}
+
+size_t workspace_bytes_for(int n_pairs, int N, int N_T) {
+    const size_t pieces = max_pieces(N_T);
+    if (pieces <= 1) return 0;
     const size_t n = (size_t)(N / N_T) * (size_t)(N / N_T);
-    size_t pieces = (size_t)(N_T + kGenericRows - 1) / kGenericRows;       // generic path
-    if (is_pow2(N_T)) {                                       // strip path, worst case rw = 4
-        const size_t px = N_T > kUnitCols ? N_T / kUnitCols : 1;
-        const size_t py = N_T / 32;
-        if (px * py > pieces) pieces = px * py;
-    }
-    return n * pieces * sizeof(float4);
+    return (size_t)n_pairs * n * pieces * sizeof(float4);
 }
 
-template <int MODE>
-void launch_strip(const TileParams& p, int rw, unsigned grid, cudaStream_t st) {
-    switch (rw) {
-        case 4: strip_kernel<MODE, 4><<<grid, kCtaThreads, 0, st>>>(p); break;
-        case 16: strip_kernel<MODE, 16><<<grid, kCtaThreads, 0, st>>>(p); break;
-        default: strip_kernel<MODE, 8><<<grid, kCtaThreads, 0, st>>>(p); break;
+struct Outputs {
+    float *lisi, *auglisi, *sum_x, *sum_y, *lisi_num, *aug_num;   // [n_pairs * n] each (or nullptr)
+    Outputs offset(size_t k) const {
+        auto o = [k](float* p) { return p ? p + k : nullptr; };
+        return {o(lisi), o(auglisi), o(sum_x), o(sum_y), o(lisi_num), o(aug_num)};
     }
-}
+};
 
-void launch_generic(int mode, const GenericParams& g, unsigned grid, cudaStream_t st) {
-    switch (mode) {
-        case kModeLisi: generic_kernel<kModeLisi><<<grid, kCtaThreads, 0, st>>>(g); break;
-        case kModeAug: generic_kernel<kModeAug><<<grid, kCtaThreads, 0, st>>>(g); break;
-        default: generic_kernel<kModeFused><<<grid, kCtaThreads, 0, st>>>(g); break;
-    }
-}
-
-// Shared body of the three *_tiles entry points.
-int run_tiles(int mode, const float* x, const float* y, int N, int N_T,
-              float C1, float C2, float C, float D,
-              float* lisi, float* auglisi, float* sum_x, float* sum_y,
-              float* lisi_num, float* aug_num,
+// Shared body of every *_tiles / *_batch entry point: validation, then the launches.
+// xs, ys: HOST arrays of n_pairs device pointers.  out2 (nullable): Eqs. 3-4 per pair.
+int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pairs, int N, int N_T,
+              float C1, float C2, float C, float D, Outputs out, float* out2,
               void* workspace, size_t workspace_bytes, void* stream) {
-    if (!x || !y) return IQA_ERR_NULL;
-    if ((mode & kModeLisi) && !lisi) return IQA_ERR_NULL;
-    if ((mode & kModeAug) && !auglisi) return IQA_ERR_NULL;
-    if (mode == kModeFused && (!sum_x || !sum_y)) return IQA_ERR_NULL;
+    if (!xs || !ys) return IQA_ERR_NULL;
+    if (n_pairs <= 0) return IQA_ERR_SHAPE;
+    for (int i = 0; i < n_pairs; ++i)
+        if (!xs[i] || !ys[i]) return IQA_ERR_NULL;
+    if ((mode & kModeLisi) && !out.lisi) return IQA_ERR_NULL;
+    if ((mode & kModeAug) && !out.auglisi) return IQA_ERR_NULL;
+    if (mode == kModeFused && (!out.sum_x || !out.sum_y)) return IQA_ERR_NULL;
     if (const int s = status_of_shape(N, N_T)) return s;
-    if ((mode & kModeLisi) && (!pos_finite(C1) || !pos_finite(C2) || !std::isfinite(D)))
-        return IQA_ERR_PARAM;
+    const int nt = N / N_T;
+    const long long n = (long long)nt * nt;
+    if (n * n_pairs > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    if ((mode & kModeLisi) && (!pos_finite(C1) || !pos_finite(C2) || !std::isfinite(D))) return IQA_ERR_PARAM;
     if ((mode & kModeAug) && !pos_finite(C)) return IQA_ERR_PARAM;
-    if (((uintptr_t)x | (uintptr_t)y) & 3u) return IQA_ERR_ALIGN;
-    const size_t need = workspace_bytes_for(N, N_T);
+    if (out2 && (!pos_finite(C2) || !pos_finite(C))) return IQA_ERR_PARAM;
+    uintptr_t bits = 0;
+    for (int i = 0; i < n_pairs; ++i) bits |= (uintptr_t)xs[i] | (uintptr_t)ys[i];
+    if (bits & 3u) return IQA_ERR_ALIGN;
+    const size_t need = workspace_bytes_for(n_pairs, N, N_T);
     if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
     if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
 
-    const bool aligned16 = ((((uintptr_t)x | (uintptr_t)y) & 15u) == 0) && (N % 4 == 0);
-    const Plan pl = make_plan(N, N_T, aligned16);
-    if (pl.grid > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    const bool aligned16 = ((bits & 15u) == 0) && (N % 4 == 0);
+    const Plan pl = make_plan(N_T, aligned16);
     cudaStream_t st = (cudaStream_t)stream;
+    float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
+    out.lisi = (mode & kModeLisi) ? out.lisi : nullptr;
+    out.auglisi = (mode & kModeAug) ? out.auglisi : nullptr;
+    out.lisi_num = (mode & kModeLisi) ? out.lisi_num : nullptr;
+    out.aug_num = (mode & kModeAug) ? out.aug_num : nullptr;
 
-    TileParams p{};
-    p.x = x; p.y = y; p.N = N; p.nt = N / N_T;
-    p.log2_nt = is_pow2(N_T) ? ilog2(N_T) : 0;
-    p.units_x = (N + kUnitCols - 1) / kUnitCols;
-    p.C1 = C1; p.C2 = C2; p.C = C; p.D = D;
-    p.lisi = (mode & kModeLisi) ? lisi : nullptr;
-    p.auglisi = (mode & kModeAug) ? auglisi : nullptr;
-    p.sum_x = sum_x; p.sum_y = sum_y;
-    p.lisi_num = (mode & kModeLisi) ? lisi_num : nullptr;
-    p.aug_num = (mode & kModeAug) ? aug_num : nullptr;
-    p.pieces_x = pl.pieces_x; p.pieces_y = pl.pieces_y;
-    p.ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
-
-    if (pl.strip) {
-        switch (mode) {
-            case kModeLisi: launch_strip<kModeLisi>(p, pl.rw, (unsigned)pl.grid, st); break;
-            case kModeAug: launch_strip<kModeAug>(p, pl.rw, (unsigned)pl.grid, st); break;
-            default: launch_strip<kModeFused>(p, pl.rw, (unsigned)pl.grid, st); break;
+    if (pl.stream) {
+        const Geometry* geo = geometry();
+        if (!geo) return IQA_ERR_CUDA;
+        const int units_x = (N + kUnitCols - 1) / kUnitCols;
+        const int units_y = (N + pl.item_rows - 1) / pl.item_rows;
+        const long long items_per_pair = (long long)units_x * units_y;
+        if (items_per_pair * kMaxBatch > 0x7fffffffLL) return IQA_ERR_SHAPE;
+        StreamFn fn = stream_fn(mode, pl.variant);
+        for (int first = 0; first < n_pairs; first += kMaxBatch) {
+            const int np = n_pairs - first < kMaxBatch ? n_pairs - first : kMaxBatch;
+            BatchParams p{};
+            for (int i = 0; i < np; ++i) { p.x[i] = xs[first + i]; p.y[i] = ys[first + i]; }
+            p.n_pairs = np; p.N = N; p.log2_nt = ilog2(N_T); p.nt = nt; p.n_tiles = (int)n;
+            p.units_x = units_x; p.units_y = units_y; p.item_rows = pl.item_rows;
+            p.n_items = (int)(items_per_pair * np);
+            p.C1 = C1; p.C2 = C2; p.C = C; p.D = D;
+            const Outputs o = out.offset((size_t)first * (size_t)n);
+            p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
+            p.lisi_num = o.lisi_num; p.aug_num = o.aug_num;
+            p.ws = ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr;
+            p.pieces_x = pl.pieces_x; p.pieces_y = pl.pieces_y;
+            const long long resident = (long long)geo->sms * geo->ctas[mode - 1][pl.variant];
+            const unsigned grid = (unsigned)(p.n_items < resident ? p.n_items : resident);
+            if (launch(fn, grid, kCtaThreads, stream_smem(pl.variant), st, p) != cudaSuccess) return IQA_ERR_CUDA;
         }
     } else {
-        GenericParams g{};
-        g.tp = p; g.N_T = N_T; g.pieces = pl.pieces;
-        launch_generic(mode, g, (unsigned)pl.grid, st);
+        const long long grid = n * pl.pieces;
+        if (grid > 0x7fffffffLL) return IQA_ERR_SHAPE;
+        for (int i = 0; i < n_pairs; ++i) {
+            GenericParams g{};
+            TileParams& p = g.tp;
+            p.x = xs[i]; p.y = ys[i]; p.N = N; p.nt = nt;
+            p.C1 = C1; p.C2 = C2; p.C = C; p.D = D;
+            const Outputs o = out.offset((size_t)i * (size_t)n);
+            p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
+            p.lisi_num = o.lisi_num; p.aug_num = o.aug_num;
+            p.ws = ws ? ws + (size_t)i * (size_t)n * pl.pieces : nullptr;
+            g.N_T = N_T; g.pieces = pl.pieces;
+            cudaError_t e;
+            switch (mode) {
+                case kModeLisi: e = launch(generic_kernel<kModeLisi>, (unsigned)grid, kCtaThreads, 0, st, g); break;
+                case kModeAug: e = launch(generic_kernel<kModeAug>, (unsigned)grid, kCtaThreads, 0, st, g); break;
+                default: e = launch(generic_kernel<kModeFused>, (unsigned)grid, kCtaThreads, 0, st, g); break;
+            }
+            if (e != cudaSuccess) return IQA_ERR_CUDA;
+        }
     }
-    if (pl.pieces > 1) {
-        const int n = p.nt * p.nt;
-        if (pl.pieces <= 32 && n >= 64)
-            finalise_small_kernel<<<(n + kCtaThreads - 1) / kCtaThreads, kCtaThreads, 0, st>>>(p, pl.pieces, n);
+    if (pl.pieces > 1) {                       // second pass over all tiles of the batch, fixed order
+        TileParams p{};
+        p.C1 = C1; p.C2 = C2; p.C = C; p.D = D;
+        p.lisi = out.lisi; p.auglisi = out.auglisi; p.sum_x = out.sum_x; p.sum_y = out.sum_y;
+        p.lisi_num = out.lisi_num; p.aug_num = out.aug_num;
+        p.ws = ws;
+        const int total = (int)(n * n_pairs);
+        cudaError_t e;
+        if (pl.pieces <= 32 && total >= 64)
+            e = launch(finalise_small_kernel, (unsigned)((total + kCtaThreads - 1) / kCtaThreads), kCtaThreads, 0, st,
+                       p, pl.pieces, total);
         else
-            finalise_kernel<<<n, kCtaThreads, 0, st>>>(p, pl.pieces);
+            e = launch(finalise_kernel, (unsigned)total, kCtaThreads, 0, st, p, pl.pieces);
+        if (e != cudaSuccess) return IQA_ERR_CUDA;
+    }
+    if (out2) {                                // Eqs. 3-4 per pair
+        if (launch(aggregate_kernel, (unsigned)n_pairs, kAggThreads, 0, st,
+                   (const float*)out.lisi, (const float*)out.auglisi, (const float*)out.sum_x,
+                   (const float*)out.sum_y, (int)n, C2, C, out2) != cudaSuccess)
+            return IQA_ERR_CUDA;
     }
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }
@@ -173,33 +295,38 @@ const char* iqa_status_string(int status) {
     switch (status) {
         case IQA_OK: return "ok";
         case IQA_ERR_NULL: return "required pointer is NULL";
-        case IQA_ERR_SHAPE: return "bad shape: need 0 < N_T <= N <= 2^20, N % N_T == 0, tile count < 2^31";
+        case IQA_ERR_SHAPE: return "bad shape: need 0 < N_T <= N <= 2^20, N % N_T == 0, n_pairs >= 1, tile count < 2^31";
         case IQA_ERR_PARAM: return "bad constant: C1, C2, C must be finite and > 0, D finite";
         case IQA_ERR_ALIGN: return "pointer alignment: images 4-byte, workspace 16-byte";
-        case IQA_ERR_WORKSPACE: return "workspace missing or smaller than iqa_workspace_bytes(N, N_T)";
+        case IQA_ERR_WORKSPACE: return "workspace missing or smaller than iqa_workspace_bytes / iqa_batch_workspace_bytes";
         case IQA_ERR_CUDA: return "CUDA launch or copy failed";
         default: return "unknown status";
     }
 }
 
-const char* iqa_version(void) { return "0.1.0"; }
+const char* iqa_version(void) { return "0.2.0"; }
 
 size_t iqa_workspace_bytes(int N, int N_T) {
     if (status_of_shape(N, N_T) != IQA_OK) return 0;
-    return workspace_bytes_for(N, N_T);
+    return workspace_bytes_for(1, N, N_T);
+}
+
+size_t iqa_batch_workspace_bytes(int n_pairs, int N, int N_T) {
+    if (n_pairs <= 0 || status_of_shape(N, N_T) != IQA_OK) return 0;
+    return workspace_bytes_for(n_pairs, N, N_T);
 }
 
 int iqa_lisi_tiles(const float* x, const float* y, int N, int N_T,
                    float C1, float C2, float D, float* lisi,
                    void* workspace, size_t workspace_bytes, void* stream) {
-    return run_tiles(kModeLisi, x, y, N, N_T, C1, C2, 1.0f, D, lisi, nullptr, nullptr, nullptr,
-                     nullptr, nullptr, workspace, workspace_bytes, stream);
+    const Outputs o{lisi, nullptr, nullptr, nullptr, nullptr, nullptr};
+    return run_batch(kModeLisi, &x, &y, 1, N, N_T, C1, C2, 1.0f, D, o, nullptr, workspace, workspace_bytes, stream);
 }
 
 int iqa_auglisi_tiles(const float* x, const float* y, int N, int N_T, float C,
                       float* auglisi, void* workspace, size_t workspace_bytes, void* stream) {
-    return run_tiles(kModeAug, x, y, N, N_T, 1.0f, 1.0f, C, 0.0f, nullptr, auglisi, nullptr, nullptr,
-                     nullptr, nullptr, workspace, workspace_bytes, stream);
+    const Outputs o{nullptr, auglisi, nullptr, nullptr, nullptr, nullptr};
+    return run_batch(kModeAug, &x, &y, 1, N, N_T, 1.0f, 1.0f, C, 0.0f, o, nullptr, workspace, workspace_bytes, stream);
 }
 
 int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
@@ -207,8 +334,18 @@ int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
                     float* lisi, float* auglisi, float* sum_x, float* sum_y,
                     float* lisi_num, float* auglisi_num,
                     void* workspace, size_t workspace_bytes, void* stream) {
-    return run_tiles(kModeFused, x, y, N, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
-                     lisi_num, auglisi_num, workspace, workspace_bytes, stream);
+    const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
+    return run_batch(kModeFused, &x, &y, 1, N, N_T, C1, C2, C, D, o, nullptr, workspace, workspace_bytes, stream);
+}
+
+int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,
+                    int N, int N_T, float C1, float C2, float C, float D,
+                    float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                    float* lisi_num, float* auglisi_num, float* out2,
+                    void* workspace, size_t workspace_bytes, void* stream) {
+    const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
+    return run_batch(kModeFused, x_ptrs_host, y_ptrs_host, n_pairs, N, N_T, C1, C2, C, D, o, out2,
+                     workspace, workspace_bytes, stream);
 }
 
 int iqa_aggregate(const float* lisi, const float* auglisi,
@@ -217,8 +354,9 @@ int iqa_aggregate(const float* lisi, const float* auglisi,
     if (!lisi || !auglisi || !sum_x || !sum_y || !out2) return IQA_ERR_NULL;
     if (n_tiles <= 0) return IQA_ERR_SHAPE;
     if (!pos_finite(C2) || !pos_finite(C)) return IQA_ERR_PARAM;
-    aggregate_kernel<<<1, kAggThreads, 0, (cudaStream_t)stream>>>(lisi, auglisi, sum_x, sum_y,
-                                                                  n_tiles, C2, C, out2);
+    if (launch(aggregate_kernel, 1u, kAggThreads, 0, (cudaStream_t)stream, lisi, auglisi, sum_x, sum_y,
+               n_tiles, C2, C, out2) != cudaSuccess)
+        return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }
 
@@ -234,8 +372,9 @@ int iqa_merge_tiles(const float* lisi, const float* auglisi,
     if (!pos_finite(C2) || !pos_finite(C)) return IQA_ERR_PARAM;
     const long long n_out = (long long)(nt / g) * (nt / g);
     const unsigned grid = (unsigned)((n_out + 7) / 8);
-    merge_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(lisi, auglisi, sum_x, sum_y, nt, g, C2, C,
-                                                         lisi_out, auglisi_out, sum_x_out, sum_y_out);
+    if (launch(merge_kernel, grid, 256u, 0, (cudaStream_t)stream, lisi, auglisi, sum_x, sum_y, nt, g, C2, C,
+               lisi_out, auglisi_out, sum_x_out, sum_y_out) != cudaSuccess)
+        return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }
 
@@ -244,7 +383,7 @@ size_t iqa_host_scratch_bytes(int N, int N_T) {
     const size_t img = align_up((size_t)N * (size_t)N * sizeof(float), 256);
     const size_t n = (size_t)(N / N_T) * (size_t)(N / N_T);
     const size_t per_tile = align_up(n * sizeof(float), 256);
-    return 2 * img + 4 * per_tile + 256 + align_up(workspace_bytes_for(N, N_T), 256);
+    return 2 * img + 4 * per_tile + 256 + align_up(workspace_bytes_for(1, N, N_T), 256);
 }
 
 int iqa_fused_host(const float* x_host, const float* y_host, int N, int N_T,
@@ -272,14 +411,14 @@ int iqa_fused_host(const float* x_host, const float* y_host, int N, int N_T,
     float* d_sy = (float*)(base + 2 * img + 3 * per_tile);
     float* d_out2 = (float*)(base + 2 * img + 4 * per_tile);
     void* ws = base + 2 * img + 4 * per_tile + 256;
-    const size_t ws_bytes = workspace_bytes_for(N, N_T);
+    const size_t ws_bytes = workspace_bytes_for(1, N, N_T);
 
     if (cudaMemcpyAsync(xd, x_host, img_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return IQA_ERR_CUDA;
     if (cudaMemcpyAsync(yd, y_host, img_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return IQA_ERR_CUDA;
-    int rc = iqa_fused_tiles(xd, yd, N, N_T, C1, C2, C, D, d_lisi, d_aug, d_sx, d_sy, nullptr, nullptr,
-                             ws_bytes ? ws : nullptr, ws_bytes, stream);
-    if (rc != IQA_OK) return rc;
-    rc = iqa_aggregate(d_lisi, d_aug, d_sx, d_sy, (int)n, C2, C, d_out2, stream);
+    const float* xs[1] = {xd};
+    const float* ys[1] = {yd};
+    const int rc = iqa_fused_batch(xs, ys, 1, N, N_T, C1, C2, C, D, d_lisi, d_aug, d_sx, d_sy, nullptr, nullptr,
+                                   d_out2, ws_bytes ? ws : nullptr, ws_bytes, stream);
     if (rc != IQA_OK) return rc;
     const size_t nb = n * sizeof(float);
     cudaError_t e = cudaSuccess;

@@ -40,11 +40,14 @@ def test_workspace_bytes():
     # tiles of side <= 64 are always finished inside one CTA: no second pass, no workspace
     for N, N_T in [(256, 16), (2048, 8), (2048, 64), (8192, 64), (10, 5), (192, 48)]:
         assert B.iqa_workspace_bytes(N, N_T) == 0
-    # split tiles: 16 B per piece; strip worst case (N_T/128 or 1) x (N_T/32) pieces per tile
-    assert B.iqa_workspace_bytes(2048, 128) == 256 * 1 * 4 * 16
-    assert B.iqa_workspace_bytes(2048, 512) == 16 * 4 * 16 * 16
-    assert B.iqa_workspace_bytes(16384, 128) == 16384 * 4 * 16
-    assert B.iqa_workspace_bytes(16384, 16384) == 128 * 512 * 16
+    # split tiles: 16 B per piece of 128 x 64 pixels -> (N_T/128) x (N_T/64) pieces per tile
+    assert B.iqa_workspace_bytes(2048, 128) == 256 * 1 * 2 * 16
+    assert B.iqa_workspace_bytes(2048, 512) == 16 * 4 * 8 * 16
+    assert B.iqa_workspace_bytes(16384, 128) == 16384 * 2 * 16
+    assert B.iqa_workspace_bytes(16384, 16384) == 128 * 256 * 16
+    assert B.iqa_batch_workspace_bytes(16, 16384, 128) == 16 * 16384 * 2 * 16
+    assert B.iqa_batch_workspace_bytes(5, 2048, 64) == 0
+    assert B.iqa_batch_workspace_bytes(0, 2048, 128) == 0
     assert B.iqa_workspace_bytes(200, 100) == 4 * 2 * 16          # generic: ceil(100/64) pieces
     # invalid shapes report 0 here; the entry points return the error
     for N, N_T in [(0, 8), (100, 0), (100, 7), (-4, 2), (64, 128), ((1 << 20) + 8, 8)]:
@@ -111,6 +114,30 @@ def test_standalone_and_aggregate_validation():
                             0x1000, 16) == B.IQA_ERR_WORKSPACE
     assert B.iqa_fused_host(FAKE, FAKE, 256, 16, 1e-6, 1e-6, 1e-6, 5e-7, None, None, None, None, None,
                             0x1010, 1 << 30) == B.IQA_ERR_ALIGN
+
+
+def test_batch_validation():
+    tbl = (ctypes.c_void_p * 3)(FAKE, FAKE, FAKE)
+    bad = (ctypes.c_void_p * 3)(FAKE, 0, FAKE)
+    odd = (ctypes.c_void_p * 3)(FAKE, FAKE + 2, FAKE)
+
+    def call(xs=tbl, ys=tbl, P=3, N=256, N_T=16, C=1e-6, lisi=FAKE, out2=None, ws=None, wsb=0):
+        return B.iqa_fused_batch(xs, ys, P, N, N_T, 1e-6, 1e-6, C, 5e-7, lisi, FAKE, FAKE, FAKE,
+                                 None, None, out2, ws, wsb, None)
+
+    assert call(xs=None) == B.IQA_ERR_NULL
+    assert call(ys=bad) == B.IQA_ERR_NULL                   # a NULL entry in the pointer table
+    assert call(lisi=None) == B.IQA_ERR_NULL
+    assert call(P=0) == B.IQA_ERR_SHAPE
+    assert call(P=-1) == B.IQA_ERR_SHAPE
+    assert call(N=100) == B.IQA_ERR_SHAPE
+    assert call(N=1 << 20, N_T=32, P=3) == B.IQA_ERR_SHAPE  # 3 * 2^30 tiles do not fit an int index
+    assert call(C=0.0) == B.IQA_ERR_PARAM
+    assert call(xs=odd) == B.IQA_ERR_ALIGN
+    assert call(N_T=128) == B.IQA_ERR_WORKSPACE
+    need = B.iqa_batch_workspace_bytes(3, 256, 128)
+    assert need == 3 * B.iqa_workspace_bytes(256, 128) > 0
+    assert call(N_T=128, ws=FAKE, wsb=need - 1) == B.IQA_ERR_WORKSPACE
 
 
 def test_convenience_wrappers_refuse_cpu_tensors():

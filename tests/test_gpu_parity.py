@@ -209,7 +209,7 @@ def test_symmetry_bitwise(U):
 
 
 def test_determinism_and_mapping_independence(U, monkeypatch):
-    """P12: two runs bit-identical; every mapping (rows per warp 4/8/16, generic kernel) agrees to 1e-6."""
+    """P12: two runs bit-identical; every mapping (stream variants 0/1/2, generic kernel) agrees to 2e-6."""
     cfg = synth.CONFIGS[0]
     x, y, _ = synth.make_pair(synth.scaled(synth.CONFIGS[3], 1024))
     xd, yd = U.to_dev(x), U.to_dev(y)
@@ -220,7 +220,8 @@ def test_determinism_and_mapping_independence(U, monkeypatch):
         for nm in base:
             assert np.array_equal(base[nm], again[nm]), (N_T, nm)
         ref = U.run_oracle(x, y, N_T, k)
-        for env, val in (("IQA_FORCE_RW", "4"), ("IQA_FORCE_RW", "16"), ("IQA_FORCE_GENERIC", "1")):
+        for env, val in (("IQA_FORCE_VARIANT", "0"), ("IQA_FORCE_VARIANT", "1"), ("IQA_FORCE_VARIANT", "2"),
+                         ("IQA_FORCE_GENERIC", "1"), ("IQA_NO_PDL", "1")):
             monkeypatch.setenv(env, val)
             other = U.run_gpu(xd, yd, N_T, k)
             monkeypatch.delenv(env)
@@ -239,6 +240,50 @@ def test_standalone_entry_points_match_fused(U, B):
         li = B.lisi_tiles(xd, yd, N_T, k["C1"], k["C2"], k["D"])
         au = B.auglisi_tiles(xd, yd, N_T, k["C"])
         assert torch.equal(li, f["lisi"]) and torch.equal(au, f["auglisi"])
+
+
+@pytest.mark.parametrize("N,N_T,P", [(256, 16, 5), (2048, 64, 3), (1024, 8, 2), (1024, 256, 3), (392, 8, 4),
+                                     (200, 100, 2), (512, 128, 40)])
+def test_fused_batch_matches_per_pair_calls_and_oracle(U, B, N, N_T, P):
+    """iqa_fused_batch == P calls of iqa_fused_tiles + iqa_aggregate, bit for bit, and == the oracle."""
+    cfg = synth.scaled(synth.CONFIGS[3], N, N_T)
+    k = U.consts(cfg)
+    hosts = [synth.make_pair(cfg, seed=s)[:2] for s in range(min(P, 6))]
+    hosts = [hosts[i % len(hosts)] for i in range(P)]
+    xs = [U.to_dev(h[0]) for h in hosts]
+    ys = [U.to_dev(h[1]) for h in hosts]
+    out = B.fused_batch(xs, ys, N_T, numerators=True, **k)
+    torch.cuda.synchronize()
+    nt = N // N_T
+    assert out["lisi"].shape == (P, nt, nt) and out["whole"].shape == (P, 2)
+    for i in range(P):
+        one = B.fused_tiles(xs[i], ys[i], N_T, numerators=True, **k)
+        agg = B.aggregate(one["lisi"], one["auglisi"], one["X"], one["Y"], k["C2"], k["C"])
+        for nm in one:
+            assert torch.equal(one[nm], out[nm][i]), (i, nm)
+        assert torch.equal(agg, out["whole"][i]), i
+    for i in range(min(P, 6)):
+        ref = U.run_oracle(hosts[i][0], hosts[i][1], N_T, k)
+        got = {nm: out[nm][i].cpu().numpy().astype(np.float64) for nm in ("lisi", "auglisi", "X", "Y", "L", "A")}
+        U.assert_parity(got, ref, k["C"], f"batch pair {i}")
+        exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], k["C2"], k["C"])
+        w = out["whole"][i].cpu().numpy()
+        assert abs(w[0] - exp[0]) <= 1e-5 * abs(exp[0]) and abs(w[1] - exp[1]) <= 1e-5 * abs(exp[1])
+
+
+def test_fused_batch_unaligned_pair_takes_generic_kernel(U, B):
+    N, N_T, P = 128, 16, 3
+    hosts = [_rand_pair(N, seed=20 + s) for s in range(P)]
+    buf = torch.empty(N * N + 3, dtype=torch.float32, device="cuda")
+    x1 = buf[1:1 + N * N].view(N, N)
+    x1.copy_(torch.from_numpy(hosts[1][0]))
+    xs = [U.to_dev(hosts[0][0]), x1, U.to_dev(hosts[2][0])]
+    ys = [U.to_dev(h[1]) for h in hosts]
+    out = B.fused_batch(xs, ys, N_T, numerators=True, **K6)
+    for i in range(P):
+        ref = U.run_oracle(hosts[i][0], hosts[i][1], N_T, K6)
+        got = {nm: out[nm][i].cpu().numpy().astype(np.float64) for nm in ("lisi", "auglisi", "X", "Y", "L", "A")}
+        U.assert_parity(got, ref, K6["C"], f"unaligned batch pair {i}")
 
 
 def test_aggregate_equals_whole_image_and_merge(U, B):
