@@ -235,10 +235,9 @@ def time_region(torch, fn, steps, dist=None):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
     if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        from paper_2501_10653_b200 import shard
+        ms = shard.max_over_ranks(ms, dist, "cuda")
         dist.barrier()
-        ms = float(t.item())
     return ms
 
 
@@ -294,9 +293,8 @@ def run_e2e(torch, binding, cfg, pairs, steps, warmup, device, dist):
     torch.cuda.synchronize()
     dt_ms = (time.perf_counter() - t0) * 1e3
     if dist is not None:
-        t = torch.tensor([dt_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dt_ms = float(t.item())
+        from paper_2501_10653_b200 import shard
+        dt_ms = shard.max_over_ranks(dt_ms, dist, "cuda")
     world = 1 if dist is None else dist.get_world_size()
     return {"value": dt_ms * 1e3 / (steps * pairs * world), "unit": UNIT,
             "h2d_bytes_per_step": pairs * runner.h2d_bytes, "d2h_bytes_per_step": pairs * runner.d2h_bytes,
@@ -306,7 +304,9 @@ def run_e2e(torch, binding, cfg, pairs, steps, warmup, device, dist):
 
 def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, use_graph, rank):
     """Device-resident timing of one workload.  Returns dict with step time and kernel-only time."""
-    batch = Batch(cfg, pairs, device, seed0=1000 * rank)
+    from paper_2501_10653_b200 import shard
+    world = 1 if dist is None else dist.get_world_size()
+    batch = Batch(cfg, pairs, device, seed0=shard.weak_seeds(pairs, rank, world)[0])   # weak scaling: own pairs per rank
     full, kern = (lambda: batch.step(True)), (lambda: batch.step(False))
     single = lambda: batch.step_single(0, True)
     if use_graph:

@@ -90,18 +90,28 @@ constexpr size_t stream_smem_bytes() {
     return (size_t)DEPTH * 2 * (kWarpsPerCta * K) * kUnitCols * sizeof(float) + 2 * kWarpsPerCta * 16 * sizeof(float4);
 }
 
-// Walks the (item, stage) sequence of one CTA; the issue side runs DEPTH-1 stages ahead of the consume side.
-struct StageCursor {
-    int q;        // item
-    int s;        // stage inside the item
+// Position of one CTA in its item sequence b, b+G, b+2G, ... kept as (pair, uy, ux) and advanced
+// by the decoded stride (no integer division in the loop).
+struct ItemCursor {
     int pair, uy, ux;
-    __device__ __forceinline__ void decode(const BatchParams& p, int items_per_pair) {
-        pair = q / items_per_pair;
-        const int rem = q - pair * items_per_pair;
-        uy = rem / p.units_x;
-        ux = rem - uy * p.units_x;
+    __device__ __forceinline__ void advance(const ItemCursor& d, int units_x, int units_y) {
+        ux += d.ux;
+        const int cx = ux >= units_x;
+        ux -= cx ? units_x : 0;
+        uy += d.uy + cx;
+        const int cy = uy >= units_y;
+        uy -= cy ? units_y : 0;
+        pair += d.pair + cy;
     }
 };
+__device__ __forceinline__ ItemCursor decode_item(int q, int units_x, int units_y) {
+    ItemCursor c;
+    const int t = q / units_x;
+    c.ux = q - t * units_x;
+    c.pair = t / units_y;
+    c.uy = t - c.pair * units_y;
+    return c;
+}
 
 template <int MODE, int K, int DEPTH, int MIN_CTAS>
 __global__ void __launch_bounds__(kCtaThreads, MIN_CTAS)
@@ -109,10 +119,11 @@ stream_kernel(const __grid_constant__ BatchParams p) {
     constexpr int RS = kWarpsPerCta * K;                    // rows per stage
     constexpr int kImgFloats = RS * kUnitCols;              // one image block of a stage
     constexpr int kStageFloats = 2 * kImgFloats;
+    constexpr uint32_t kStageBytes = kStageFloats * 4u;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* ring = reinterpret_cast<float*>(smem_raw);
     float4 (*part)[kWarpsPerCta][16] =
-        reinterpret_cast<float4 (*)[kWarpsPerCta][16]>(smem_raw + (size_t)DEPTH * kStageFloats * sizeof(float));
+        reinterpret_cast<float4 (*)[kWarpsPerCta][16]>(smem_raw + (size_t)DEPTH * kStageBytes);
 
     pdl_prologue();
     const int lane = threadIdx.x & 31;
@@ -120,38 +131,56 @@ stream_kernel(const __grid_constant__ BatchParams p) {
     const int N = p.N;
     const int R = p.item_rows;
     const int stages_per_item = R / RS;
-    const int items_per_pair = p.units_x * p.units_y;
+    const int units_x = p.units_x, units_y = p.units_y;
     const uint64_t pol = policy_evict_first();
     // this thread's slot inside a stage (the same for the copy and for the read)
     const int my_off = (w * K) * kUnitCols + lane * 4;
     const uint32_t ring_u32 = smem_u32(ring) + (uint32_t)my_off * 4u;
+    const ItemCursor stride = decode_item((int)gridDim.x, units_x, units_y);
+    const size_t stage_step = (size_t)RS * (size_t)N;      // elements between two stages of an item
 
-    // ---- issue side ---------------------------------------------------------------------
-    StageCursor a;
-    a.q = blockIdx.x; a.s = 0;
-    if (a.q < p.n_items) a.decode(p, items_per_pair);
+    // ---- issue side: runs DEPTH-1 stages ahead of the consume side ---------------------------
+    ItemCursor a = decode_item((int)blockIdx.x, units_x, units_y);
+    int a_s = 0;                    // stage inside the item
+    uint32_t a_dst = ring_u32;      // shared address of this thread's slot in the stage being filled
     int a_slot = 0;
+    const float* ax = nullptr;      // this thread's first pixel of the stage, in x and in y
+    const float* ay = nullptr;
+    bool a_inside = false;          // item entirely inside the image: no predicates, no zero fill
     auto issue = [&]() {
-        if (a.q < p.n_items) {
-            const int col = a.ux * kUnitCols + lane * 4;
-            const int row = a.uy * R + a.s * RS + w * K;
-            const bool in_cols = col < N;
-            const float* px = p.x[a.pair];
-            const float* py = p.y[a.pair];
-            const uint32_t dst = ring_u32 + (uint32_t)a_slot * (kStageFloats * 4u);
+        if (a.pair < p.n_pairs) {
+            if (a_s == 0) {         // new item: base pointers and the inside test
+                const int col = a.ux * kUnitCols + lane * 4;
+                const int row = a.uy * R + w * K;
+                a_inside = (a.ux + 1) * kUnitCols <= N && (a.uy + 1) * R <= N;       // CTA-uniform
+                const size_t off = a_inside ? (size_t)row * (size_t)N + (size_t)col : 0;
+                ax = p.x[a.pair] + off;
+                ay = p.y[a.pair] + off;
+            }
+            if (a_inside) {
 #pragma unroll
-            for (int k = 0; k < K; ++k) {
-                const bool ok = in_cols && (row + k < N);
-                const size_t off = ok ? (size_t)(row + k) * (size_t)N + (size_t)col : 0;
-                cp_async16(dst + k * (kUnitCols * 4u), px + off, ok ? 16u : 0u, pol);
-                cp_async16(dst + (kImgFloats + k * kUnitCols) * 4u, py + off, ok ? 16u : 0u, pol);
+                for (int k = 0; k < K; ++k) {
+                    cp_async16(a_dst + k * (kUnitCols * 4u), ax + (size_t)k * (size_t)N, 16u, pol);
+                    cp_async16(a_dst + (kImgFloats + k * kUnitCols) * 4u, ay + (size_t)k * (size_t)N, 16u, pol);
+                }
+                ax += stage_step;
+                ay += stage_step;
+            } else {                // ragged right / bottom edge: rows and columns outside are zero-filled
+                const int col = a.ux * kUnitCols + lane * 4;
+                const int row = a.uy * R + a_s * RS + w * K;
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+                    const bool ok = col < N && row + k < N;
+                    const size_t off = ok ? (size_t)(row + k) * (size_t)N + (size_t)col : 0;
+                    cp_async16(a_dst + k * (kUnitCols * 4u), ax + off, ok ? 16u : 0u, pol);
+                    cp_async16(a_dst + (kImgFloats + k * kUnitCols) * 4u, ay + off, ok ? 16u : 0u, pol);
+                }
             }
-            if (++a.s == stages_per_item) {
-                a.s = 0;
-                a.q += gridDim.x;
-                if (a.q < p.n_items) a.decode(p, items_per_pair);
+            if (++a_s == stages_per_item) {
+                a_s = 0;
+                a.advance(stride, units_x, units_y);
             }
-            a_slot = (a_slot + 1 == DEPTH) ? 0 : a_slot + 1;
+            if (++a_slot == DEPTH) { a_slot = 0; a_dst = ring_u32; } else { a_dst += kStageBytes; }
         }
         cp_async_commit();                                  // always: keeps the group count uniform
     };
@@ -165,20 +194,21 @@ stream_kernel(const __grid_constant__ BatchParams p) {
     const int log2_tpw = 5 - log2_g;                              // tile segments per warp row
     const int wpt = min(kWarpsPerCta, (1 << log2_nt) / K);        // warps per tile row of the item
     const int n_ty = kWarpsPerCta / wpt;                          // tile rows per item (> 1 only when N_T < 8*K)
+    const float* c_src = ring + my_off;                           // this thread's slot in the stage being consumed
     int c_slot = 0;
     int buf = 0;
-    for (int q = blockIdx.x; q < p.n_items; q += gridDim.x, buf ^= 1) {
+    for (ItemCursor c = decode_item((int)blockIdx.x, units_x, units_y); c.pair < p.n_pairs;
+         c.advance(stride, units_x, units_y), buf ^= 1) {
         float aL[4] = {0.f, 0.f, 0.f, 0.f}, aA[4] = {0.f, 0.f, 0.f, 0.f};
         float aX[4] = {0.f, 0.f, 0.f, 0.f}, aY[4] = {0.f, 0.f, 0.f, 0.f};
         for (int s = 0; s < stages_per_item; ++s) {
             issue();                                              // stage (now + DEPTH - 1)
             cp_async_wait<DEPTH - 1>();                           // the oldest stage of this thread has landed
-            const float* sx = ring + (size_t)c_slot * kStageFloats + my_off;
             float4 vx[K], vy[K];
 #pragma unroll
             for (int k = 0; k < K; ++k) {
-                vx[k] = *reinterpret_cast<const float4*>(sx + k * kUnitCols);
-                vy[k] = *reinterpret_cast<const float4*>(sx + kImgFloats + k * kUnitCols);
+                vx[k] = *reinterpret_cast<const float4*>(c_src + k * kUnitCols);
+                vy[k] = *reinterpret_cast<const float4*>(c_src + kImgFloats + k * kUnitCols);
             }
 #pragma unroll
             for (int k = 0; k < K; ++k) {
@@ -187,13 +217,10 @@ stream_kernel(const __grid_constant__ BatchParams p) {
                 pixel_terms<MODE>(vx[k].z, vy[k].z, C1, aL[2], aA[2], aX[2], aY[2]);
                 pixel_terms<MODE>(vx[k].w, vy[k].w, C1, aL[3], aA[3], aX[3], aY[3]);
             }
-            c_slot = (c_slot + 1 == DEPTH) ? 0 : c_slot + 1;
+            if (++c_slot == DEPTH) { c_slot = 0; c_src = ring + my_off; } else { c_src += kStageFloats; }
         }
 
-        const int pair = q / items_per_pair;
-        const int rem = q - pair * items_per_pair;
-        const int uy = rem / p.units_x;
-        const int ux = rem - uy * p.units_x;
+        const int pair = c.pair, uy = c.uy, ux = c.ux;
         // lane: 4 columns -> 1
         float4 v;
         v.x = (aL[0] + aL[1]) + (aL[2] + aL[3]);

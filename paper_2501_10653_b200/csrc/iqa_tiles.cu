@@ -33,23 +33,25 @@ int env_int(const char* name, int dflt) {
 }
 
 // ---- stream-kernel variants (rows per warp and stage K, ring depth, CTAs per SM) -----------
-// Measured on B200 (profiles/): about 64 KiB of copies in flight per SM is
-// the sweet spot; deeper rings or more CTAs lose DRAM locality, fewer warps lose latency hiding.
-//   variant 0  K=2, depth 2, 4 CTAs/SM  (stage = 16 rows, 36 KiB smem/CTA)   default
-//   variant 1  K=4, depth 2, 3 CTAs/SM  (stage = 32 rows, 68 KiB smem/CTA)   N_T <= 16: fewer, larger reductions
-//   variant 2  K=8, depth 2, 1 CTA/SM   (stage = 64 rows, 132 KiB smem/CTA)  debug / mapping-independence tests
+// Measured on B200 (profiles/r01*_variants.md): 48-64 KiB of copies in
+// flight per SM is the sweet spot; deeper rings or more CTAs lose DRAM locality (down to
+// 6.1-6.4 TB/s), fewer warps lose latency hiding.  Variants 0 and 1 are within 1 % of each other.
+//   variant 0  K=4, depth 2, 2 CTAs/SM  (stage = 32 rows, 68 KiB smem/CTA, 64 KiB in flight per SM)  default
+//   variant 1  K=2, depth 2, 3 CTAs/SM  (stage = 16 rows, 36 KiB smem/CTA, 48 KiB in flight per SM)
+//   variant 2  K=8, depth 2, 1 CTA/SM   (stage = 64 rows, 132 KiB smem/CTA)  mapping-independence tests only
+// IQA_FORCE_VARIANT=v selects one (debug / tuning knob); all agree to ~1e-7 relative.
 constexpr int kNumVariants = 3;
 struct VariantInfo { int K, depth, min_ctas; };
-constexpr VariantInfo kVariants[kNumVariants] = {{2, 2, 4}, {4, 2, 3}, {8, 2, 1}};
+constexpr VariantInfo kVariants[kNumVariants] = {{4, 2, 2}, {2, 2, 3}, {8, 2, 1}};
 
 using StreamFn = void (*)(const BatchParams);
 
 template <int MODE>
 StreamFn stream_fn(int variant) {
     switch (variant) {
-        case 1: return stream_kernel<MODE, 4, 2, 3>;
+        case 1: return stream_kernel<MODE, 2, 2, 3>;
         case 2: return stream_kernel<MODE, 8, 2, 1>;
-        default: return stream_kernel<MODE, 2, 2, 4>;
+        default: return stream_kernel<MODE, 4, 2, 2>;
     }
 }
 StreamFn stream_fn(int mode, int variant) {
@@ -61,9 +63,9 @@ StreamFn stream_fn(int mode, int variant) {
 }
 size_t stream_smem(int variant) {
     switch (variant) {
-        case 1: return stream_smem_bytes<4, 2>();
+        case 1: return stream_smem_bytes<2, 2>();
         case 2: return stream_smem_bytes<8, 2>();
-        default: return stream_smem_bytes<2, 2>();
+        default: return stream_smem_bytes<4, 2>();
     }
 }
 
@@ -133,7 +135,7 @@ Plan make_plan(int N_T, bool aligned16) {
     Plan pl{};
     pl.stream = is_pow2(N_T) && N_T >= 8 && aligned16 && !env_int("IQA_FORCE_GENERIC", 0);
     if (pl.stream) {
-        pl.variant = N_T <= 16 ? 1 : 0;
+        pl.variant = 0;
         const int forced = env_int("IQA_FORCE_VARIANT", -1);     // debug knob (tests: mapping independence)
         if (forced >= 0 && forced < kNumVariants) pl.variant = forced;
         const int rs = kWarpsPerCta * kVariants[pl.variant].K;   // stage height

@@ -1,0 +1,82 @@
+"""world_size-2 gloo tests (CPU) of the multi-GPU host logic: pairs shard over ranks with no
+data-path collective; timing is the max over ranks."""
+import os
+import socket
+
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from paper_2501_10653_b200 import shard  # noqa: E402
+
+
+def test_pair_range_partitions_the_job():
+    for total in (0, 1, 2, 7, 16, 33):
+        for world in (1, 2, 3, 8):
+            got = [i for r in range(world) for i in shard.pair_range(total, r, world)]
+            assert got == list(range(total))
+            sizes = [len(shard.pair_range(total, r, world)) for r in range(world)]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        shard.pair_range(4, 2, 2)
+
+
+def test_weak_seeds_are_disjoint():
+    seen = set()
+    for r in range(8):
+        s = shard.weak_seeds(32, r, 8, seed0=100)
+        assert len(s) == 32 and not seen.intersection(s)
+        seen.update(s)
+    assert seen == set(range(100, 100 + 256))
+
+
+def test_single_process_is_identity():
+    assert shard.max_over_ranks(3.5) == 3.5
+    j = shard.job_throughput(32, 0.16)
+    assert j["world"] == 1 and j["units"] == 32 and abs(j["us_per_unit"] - 5.0) < 1e-12
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, q):
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        dist.barrier()
+        local_ms = 1.0 + rank                                  # rank 1 is the slow one
+        j = shard.job_throughput(16, local_ms, dist)
+        mine = list(shard.pair_range(5, rank, world))
+        whole = torch.tensor([[float(i), float(10 * i)] for i in shard.weak_seeds(2, rank, world)])
+        allw = shard.gather_whole(whole, dist)
+        dist.barrier()
+        q.put((rank, j, mine, allw.tolist()))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_ranks_gloo():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    (r0, j0, m0, w0), (r1, j1, m1, w1) = res
+    assert (r0, r1) == (0, 1)
+    assert j0 == j1                                            # every rank sees the same job numbers
+    assert j0["world"] == 2 and j0["ms"] == 2.0 and j0["units"] == 32     # max over ranks, all ranks' units
+    assert abs(j0["us_per_unit"] - 62.5) < 1e-9
+    assert m0 == [0, 1, 2] and m1 == [3, 4]                    # disjoint, ordered, complete
+    assert w0 == w1 == [[0.0, 0.0], [1.0, 10.0], [2.0, 20.0], [3.0, 30.0]]
