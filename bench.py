@@ -31,9 +31,10 @@ UNIT = "us/pair"
 # workload name -> (BASELINE.json config index, pairs per step, pairs per e2e step)
 WORKLOADS = {"cfg1": (1, 32, 8), "cfg3": (3, 8, 2), "cfg4": (4, 16, 1), "cfg0": (0, 64, 8)}
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused strip kernel, from the
-# `ncu --set full` capture summarised under profiles/ (null until captured for that workload).
-NCU_TRAFFIC_BYTES = {}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused stream kernel at the default pairs
+# per step, from the `ncu --set full` captures summarised under profiles/r01e_ncu_full_*_stream.md
+# (null when not captured for that workload; algorithmic bytes: cfg1 1.07427e9, cfg3 4.29706e9).
+NCU_TRAFFIC_BYTES = {"cfg1": 1.073763e9 + 4.388e6, "cfg3": 4.295033e9 + 5.502e6}
 
 
 def algorithmic_bytes(N: int, N_T: int) -> int:
@@ -203,6 +204,23 @@ class Batch:
             if rc:
                 raise B.IqaError(rc, "iqa_aggregate")
 
+    def step_entry(self, kind):
+        """Every pair of the batch through ONE per-pair entry point (kind: fused | lisi | auglisi),
+        so each call reads its pair cold from HBM."""
+        B, cfg = self.B, self.cfg
+        st = self.torch.cuda.current_stream().cuda_stream
+        C1, C2, C, D = self.k
+        for i in range(self.P):
+            if kind == "fused":
+                rc = B.iqa_fused_tiles(self.x[i], self.y[i], cfg.N, cfg.N_T, C1, C2, C, D, self.lisi[i], self.aug[i],
+                                       self.sx[i], self.sy[i], None, None, self.ws1, self.wsb1, st)
+            elif kind == "lisi":
+                rc = B.iqa_lisi_tiles(self.x[i], self.y[i], cfg.N, cfg.N_T, C1, C2, D, self.lisi[i], self.ws1, self.wsb1, st)
+            else:
+                rc = B.iqa_auglisi_tiles(self.x[i], self.y[i], cfg.N, cfg.N_T, C, self.aug[i], self.ws1, self.wsb1, st)
+            if rc:
+                raise B.IqaError(rc, "iqa_%s_tiles" % kind)
+
     def launches_per_step(self, aggregate=True):
         split = self.wsb > 0
         return -(-self.P // 32) + (1 if split else 0) + (1 if aggregate else 0)
@@ -302,15 +320,22 @@ def run_e2e(torch, binding, cfg, pairs, steps, warmup, device, dist):
             "launches_per_step": pairs * (3 if binding.iqa_workspace_bytes(cfg.N, cfg.N_T) else 2), "host_memory": "pinned"}
 
 
-def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, use_graph, rank):
+def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, use_graph, rank, latency=True):
     """Device-resident timing of one workload.  Returns dict with step time and kernel-only time."""
     from paper_2501_10653_b200 import shard
     world = 1 if dist is None else dist.get_world_size()
     batch = Batch(cfg, pairs, device, seed0=shard.weak_seeds(pairs, rank, world)[0])   # weak scaling: own pairs per rank
     full, kern = (lambda: batch.step(True)), (lambda: batch.step(False))
-    single = lambda: batch.step_single(0, True)
+    # latency of ONE pair through the per-pair entry points (iqa_fused_tiles + iqa_aggregate), L calls back
+    # to back: the same pair (warm: L2-resident when it fits -- what the paper's 10-run median measures,
+    # P:31) and rotating over the batch's distinct pairs (cold: every call reads HBM)
+    L = 16
+    single_warm = lambda: [batch.step_single(0, True) for _ in range(L)]
+    single_cold = lambda: [batch.step_single(i % pairs, True) for i in range(L)]
     if use_graph:
-        full, kern, single = batch.graph(full).replay, batch.graph(kern).replay, batch.graph(single).replay
+        full, kern = batch.graph(full).replay, batch.graph(kern).replay
+        if latency:
+            single_warm, single_cold = batch.graph(single_warm).replay, batch.graph(single_cold).replay
     for _ in range(warmup):
         full()
     with ClockSampler(torch.cuda.current_device()) as clk:
@@ -318,14 +343,53 @@ def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, us
     for _ in range(warmup):
         kern()
     ms_kernel = time_region(torch, kern, steps, dist)
-    # latency of ONE pair through the per-pair entry points, same pair back to back (warm: L2-resident
-    # when the pair fits) -- the quantity the paper's 10-run median measures
-    reps = max(steps, 20)
-    for _ in range(max(3, warmup)):
-        single()
-    ms_single = time_region(torch, single, reps, dist) / reps
-    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "us_single_pair_warm": ms_single * 1e3,
-            "clocks": clk.summary()}
+    reps = max(3, min(steps, 20))
+    lat = [] if latency else [None, None]
+    for fn in ((single_warm, single_cold) if latency else ()):
+        for _ in range(max(3, warmup)):
+            fn()
+        lat.append(time_region(torch, fn, reps, dist) / (reps * L))
+    ms_single, ms_single_cold = lat
+    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "us_single_pair_warm": None if ms_single is None else ms_single * 1e3,
+            "us_single_pair_cold": None if ms_single_cold is None else ms_single_cold * 1e3, "clocks": clk.summary()}
+
+
+def measure_entry_points(torch, cfg, pairs, steps, warmup, device, use_graph):
+    """us per pair of the three per-pair entry points (BJ metric: fused headline + the two standalone
+    ones), each over `pairs` distinct pairs so every call reads cold from HBM."""
+    batch = Batch(cfg, pairs, device)
+    out = {}
+    for kind in ("fused", "lisi", "auglisi"):
+        fn = (lambda k=kind: batch.step_entry(k))
+        if use_graph:
+            fn = batch.graph(fn).replay
+        for _ in range(warmup):
+            fn()
+        ms = time_region(torch, fn, steps)
+        us = ms * 1e3 / (steps * pairs)
+        out["iqa_%s_tiles" % kind] = {"us_per_pair": us, "GBps": algorithmic_bytes(cfg.N, cfg.N_T) / (us * 1e-6) / 1e9}
+    del batch
+    torch.cuda.empty_cache()
+    return out
+
+
+def measure_sweep(torch, binding, base_cfg, pairs, steps, warmup, device, use_graph):
+    """BASELINE.json config [2]: one generator, N_T in sweep_N_T; batch of `pairs` pairs per step."""
+    from dataclasses import replace
+    rows = {}
+    for N_T in base_cfg.sweep_N_T:
+        cfg = replace(base_cfg, N_T=N_T, name=f"{base_cfg.name}_T{N_T}")
+        m = measure_workload(torch, binding, cfg, pairs, steps, warmup, device, None, use_graph, 0)
+        us_step = m["ms"] * 1e3 / (steps * pairs)
+        us_kern = m["ms_kernel"] * 1e3 / (steps * pairs)
+        rows[str(N_T)] = {"tiles": (cfg.N // N_T) ** 2, "us_per_pair_step": us_step, "us_per_pair_tiles_only": us_kern,
+                          "GBps_tiles_only": algorithmic_bytes(cfg.N, N_T) / (us_kern * 1e-6) / 1e9,
+                          "us_single_pair_warm": m["us_single_pair_warm"],
+                          "us_single_pair_cold": m["us_single_pair_cold"],
+                          "split_tiles": binding.iqa_workspace_bytes(cfg.N, N_T) > 0}
+        del m
+        torch.cuda.empty_cache()
+    return rows
 
 
 def run_ours(args):
@@ -352,12 +416,12 @@ def run_ours(args):
     use_graph = not args.no_graph
     K, W = args.steps, args.warmup
 
-    m = measure_workload(torch, binding, cfg, pairs, K, W, device, dist, use_graph, rank)
+    m = measure_workload(torch, binding, cfg, pairs, K, W, device, dist, use_graph, rank, latency=not args.no_latency)
     total_pairs = K * pairs * world
     us_per_pair = m["ms"] * 1e3 / total_pairs
     n_stream = -(-pairs // 32)                               # launches of the stream kernel per step
     us_launch = m["ms_kernel"] * 1e3 / (K * n_stream)       # per launch of the stream kernel (max over ranks)
-    us_single, clocks = m["us_single_pair_warm"], m["clocks"]
+    us_single, us_single_cold, clocks = m["us_single_pair_warm"], m["us_single_pair_cold"], m["clocks"]
     alg = algorithmic_bytes(cfg.N, cfg.N_T) * pairs / n_stream    # algorithmic bytes one launch moves
     peak, peak_src = measured_peak()
     achieved = alg / (us_launch * 1e-6) / 1e9
@@ -377,10 +441,17 @@ def run_ours(args):
         gbs3 = algorithmic_bytes(c3.N, c3.N_T) / (us3 * 1e-6) / 1e9
         also[c3.name] = {"us_per_pair_step": m3["ms"] * 1e3 / (k3 * p3), "us_per_pair_stream_kernel": us3,
                          "us_single_pair_warm": m3["us_single_pair_warm"],
+                         "us_single_pair_cold": m3["us_single_pair_cold"],
                          "achieved_GBps": gbs3, "frac_of_measured_peak": gbs3 / peak,
                          "frac_of_nominal_8000": gbs3 / 8000.0, "pairs_per_step": p3, "clocks": m3["clocks"]}
         del m3
         torch.cuda.empty_cache()
+
+    if args.entry_points and world == 1:
+        also["entry_points_cold"] = measure_entry_points(torch, cfg, pairs, max(3, min(K, 20)), max(3, W), device, use_graph)
+    if args.sweep and world == 1:
+        also["cfg2_sweep"] = measure_sweep(torch, binding, synth.CONFIGS[2], 32, max(3, min(K, 20)), max(3, W),
+                                           device, use_graph)
 
     cpu = cpu_baseline(cfg) if rank == 0 and world == 1 else None
 
@@ -398,11 +469,12 @@ def run_ours(args):
             "kernels": ["iqa::stream_kernel<3,K,2,CTAs> (fused S1-S4, all pairs of the step)"]
                        + (["iqa::finalise_*_kernel"] if split else []) + ["iqa::aggregate_kernel (S5, one CTA per pair)"],
             "roofline": {"bound": "hbm", "kernel": "iqa::stream_kernel<fused>", "achieved": achieved, "peak": peak,
-                         "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+                         "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if not args.pairs else None,
                          "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
                          "us_per_launch": us_launch, "pairs_per_launch": pairs / n_stream,
                          "frac_of_nominal_8000": achieved / 8000.0},
             "us_single_pair_warm": us_single,
+            "us_single_pair_cold": us_single_cold,
             "e2e": e2e,
             "clocks": clocks,
             "paper_context": {"note": "H100 kernel-only medians at N=2048, N_T=64 (PAPER.md:31); context, not the target",
@@ -420,13 +492,18 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg1", choices=sorted(WORKLOADS))
     ap.add_argument("--pairs", type=int, default=0, help="pairs per step (default per workload)")
     ap.add_argument("--no-graph", action="store_true", help="launch through ctypes each step instead of replaying a CUDA graph")
     ap.add_argument("--no-also", action="store_true", help="skip the extra N=8192 measurement")
+    ap.add_argument("--no-latency", action="store_true",
+                    help="skip the single-pair latency loops (keeps the launch list short under ncu)")
+    ap.add_argument("--sweep", action="store_true", help="also time BASELINE.json config [2] (N=2048, N_T = 8..512)")
+    ap.add_argument("--entry-points", action="store_true",
+                    help="also time iqa_fused_tiles / iqa_lisi_tiles / iqa_auglisi_tiles per pair, cold")
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)
     if args.impl == "reference":

@@ -8,13 +8,20 @@
 //   with SX = sum_t X_t, SY = sum_t Y_t and n the number of merged tiles.
 // =============================================================================
 #pragma once
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
+#include <stdint.h>
 
 #include "iqa_kernels.cuh"
 
 namespace iqa {
 
-constexpr int kAggThreads = 1024;
+constexpr int kAggThreads = 256;
+constexpr int kAggCluster = 8;      // CTAs per image pair for large tile counts (portable cluster size)
+constexpr int kAggClusterMinTiles = 8192;   // below this one CTA is faster (measured: the cluster barriers cost ~0.5 us)
+
+// Cluster size used for n tiles: a function of n only, so the order of additions stays fixed.
+inline int agg_cluster_size(long long n) { return n >= kAggClusterMinTiles ? kAggCluster : 1; }
 
 struct Agg4 { double n3, n4, sx, sy; };
 
@@ -43,28 +50,81 @@ __device__ __forceinline__ void agg_finish(const Agg4& a, double n, double C2, d
     *aug_out = (float)((a.n4 - (n - 1.0) * C) / (a.sx + a.sy + C));      // Eq. 4
 }
 
-// One CTA of 1024 threads per image pair (blockIdx.x = pair of the batch; arrays are
-// [n_pairs][n]): thread-strided partial sums, warp butterfly, then warp order.
+// One thread-block CLUSTER of agg_cluster_size(n) CTAs per image pair (arrays are [n_pairs][n]; cluster
+// c = pair c).  A pair's arrays are at most a few MiB out of L2, so the loop is bound by load
+// latency and by the fp32 -> fp64 conversions of one SM: the cluster spreads a pair over
+// kAggCluster SMs, every thread takes 128-bit loads when the arrays allow it and issues
+// kAggUnroll of them before the first double is added.  CTA r of the cluster owns the contiguous
+// element range [r * per, (r + 1) * per); its partial (thread-strided, warp butterfly, warp
+// order) goes to its own shared memory, and after a cluster barrier CTA 0 adds the kAggCluster
+// partials in rank order through distributed shared memory and applies Eqs. 3-4.  The order
+// of every addition is fixed by (n, thread, rank): results are bit-reproducible.
+constexpr int kAggUnroll = 4;
+
 __global__ void __launch_bounds__(kAggThreads)
 aggregate_kernel(const float* __restrict__ lisi, const float* __restrict__ aug,
                  const float* __restrict__ X, const float* __restrict__ Y, int n,
                  float C2f, float Cf, float* __restrict__ out2) {
+    namespace cg = cooperative_groups;
     __shared__ Agg4 part[kAggThreads / 32];
+    __shared__ Agg4 cta_part;
+    cg::cluster_group cluster = cg::this_cluster();
     pdl_prologue();
-    const size_t base = (size_t)blockIdx.x * (size_t)n;
-    lisi += base; aug += base; X += base; Y += base; out2 += 2 * (size_t)blockIdx.x;
+    const int rank = (int)cluster.block_rank();
+    const int csize = (int)cluster.num_blocks();              // launch attribute: agg_cluster_size(n)
+    const size_t pair = blockIdx.x / csize;
+    const size_t base = pair * (size_t)n;
+    lisi += base; aug += base; X += base; Y += base; out2 += 2 * pair;
     const double C2 = (double)C2f, C = (double)Cf;
     Agg4 a = {0.0, 0.0, 0.0, 0.0};
-    for (int t = threadIdx.x; t < n; t += kAggThreads)
+    // this CTA's element range; a multiple of 4 long so the 128-bit groups never straddle ranks
+    const int per = ((n + 4 * csize - 1) / (4 * csize)) * 4;
+    const int e0 = min(n, rank * per), e1 = min(n, e0 + per);
+    const bool vec = ((((uintptr_t)lisi | (uintptr_t)aug | (uintptr_t)X | (uintptr_t)Y) & 15u) == 0);
+    const int g0 = e0 >> 2;                                   // first float4 group of the range
+    const int g1 = vec ? (e1 >> 2) : g0;                      // one past the last whole group
+    const float4* l4 = reinterpret_cast<const float4*>(lisi);
+    const float4* a4 = reinterpret_cast<const float4*>(aug);
+    const float4* x4 = reinterpret_cast<const float4*>(X);
+    const float4* y4 = reinterpret_cast<const float4*>(Y);
+    for (int i0 = g0 + threadIdx.x; i0 < g1; i0 += kAggThreads * kAggUnroll) {
+        float4 vl[kAggUnroll], va[kAggUnroll], vx[kAggUnroll], vy[kAggUnroll];
+#pragma unroll
+        for (int u = 0; u < kAggUnroll; ++u) {
+            const int i = i0 + u * kAggThreads;
+            if (i < g1) { vl[u] = __ldg(l4 + i); va[u] = __ldg(a4 + i); vx[u] = __ldg(x4 + i); vy[u] = __ldg(y4 + i); }
+        }
+#pragma unroll
+        for (int u = 0; u < kAggUnroll; ++u) {
+            if (i0 + u * kAggThreads < g1) {
+                agg_add(a, vl[u].x, va[u].x, vx[u].x, vy[u].x, C2, C);
+                agg_add(a, vl[u].y, va[u].y, vx[u].y, vy[u].y, C2, C);
+                agg_add(a, vl[u].z, va[u].z, vx[u].z, vy[u].z, C2, C);
+                agg_add(a, vl[u].w, va[u].w, vx[u].w, vy[u].w, C2, C);
+            }
+        }
+    }
+    for (int t = (vec ? 4 * g1 : e0) + threadIdx.x; t < e1; t += kAggThreads)     // scalar rest of the range
         agg_add(a, lisi[t], aug[t], X[t], Y[t], C2, C);
     a = agg_warp_sum(a);
     if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = a;
     __syncthreads();
     if (threadIdx.x < 32) {
-        Agg4 b = part[threadIdx.x];          // kAggThreads / 32 == 32 entries
+        Agg4 b = {0.0, 0.0, 0.0, 0.0};
+        if (threadIdx.x < kAggThreads / 32) b = part[threadIdx.x];
         b = agg_warp_sum(b);
-        if (threadIdx.x == 0) agg_finish(b, (double)n, C2, C, out2, out2 + 1);
+        if (threadIdx.x == 0) cta_part = b;
     }
+    cluster.sync();                                           // every CTA's partial is in its shared memory
+    if (rank == 0 && threadIdx.x == 0) {
+        Agg4 s = cta_part;
+        for (int r = 1; r < csize; ++r) {
+            const Agg4* q = cluster.map_shared_rank(&cta_part, r);
+            s.n3 += q->n3; s.n4 += q->n4; s.sx += q->sx; s.sy += q->sy;
+        }
+        agg_finish(s, (double)n, C2, C, out2, out2 + 1);
+    }
+    cluster.sync();                                           // nobody exits while CTA 0 reads its shared memory
 }
 
 // P:66 merge: one warp per output tile; lanes stride over the g*g input tiles (row-major

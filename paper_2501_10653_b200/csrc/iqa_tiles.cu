@@ -98,20 +98,36 @@ const Geometry* geometry() {
 // resident while the previous kernel of the stream drains; every kernel of this library
 // starts with griddepcontrol.wait, so nothing is read or written before that kernel is done.
 template <typename... KArgs, typename... Args>
-cudaError_t launch(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st,
-                   Args&&... args) {
+cudaError_t launch_cluster(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st,
+                           unsigned cluster, Args&&... args) {
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(block);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute attr[2];
+    unsigned na = 0;
     static const bool no_pdl = env_int("IQA_NO_PDL", 0) != 0;
+    if (!no_pdl) {
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    if (cluster > 0) {                        // thread-block cluster of `cluster` CTAs along x
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = cluster;
+        attr[na].val.clusterDim.y = 1;
+        attr[na].val.clusterDim.z = 1;
+        ++na;
+    }
     cfg.attrs = attr;
-    cfg.numAttrs = no_pdl ? 0 : 1;
+    cfg.numAttrs = na;
     return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+template <typename... KArgs, typename... Args>
+cudaError_t launch(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st,
+                   Args&&... args) {
+    return launch_cluster(kernel, grid, block, smem, st, 0u, std::forward<Args>(args)...);
 }
 
 int status_of_shape(int N, int N_T) {
@@ -279,7 +295,8 @@ int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pa
         if (e != cudaSuccess) return IQA_ERR_CUDA;
     }
     if (out2) {                                // Eqs. 3-4 per pair
-        if (launch(aggregate_kernel, (unsigned)n_pairs, kAggThreads, 0, st,
+        const unsigned cs = (unsigned)agg_cluster_size(n);
+        if (launch_cluster(aggregate_kernel, (unsigned)n_pairs * cs, kAggThreads, 0, st, cs,
                    (const float*)out.lisi, (const float*)out.auglisi, (const float*)out.sum_x,
                    (const float*)out.sum_y, (int)n, C2, C, out2) != cudaSuccess)
             return IQA_ERR_CUDA;
@@ -356,7 +373,8 @@ int iqa_aggregate(const float* lisi, const float* auglisi,
     if (!lisi || !auglisi || !sum_x || !sum_y || !out2) return IQA_ERR_NULL;
     if (n_tiles <= 0) return IQA_ERR_SHAPE;
     if (!pos_finite(C2) || !pos_finite(C)) return IQA_ERR_PARAM;
-    if (launch(aggregate_kernel, 1u, kAggThreads, 0, (cudaStream_t)stream, lisi, auglisi, sum_x, sum_y,
+    const unsigned cs = (unsigned)agg_cluster_size(n_tiles);
+    if (launch_cluster(aggregate_kernel, cs, kAggThreads, 0, (cudaStream_t)stream, cs, lisi, auglisi, sum_x, sum_y,
                n_tiles, C2, C, out2) != cudaSuccess)
         return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
