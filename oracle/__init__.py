@@ -133,3 +133,6 @@ def aggregate(lisi, auglisi, X, Y, C2, C) -> tuple[float, float]:
     if rc != 0:
         raise RuntimeError(f"iqa_oracle_aggregate failed with code {rc}")
     return float(out2[0]), float(out2[1])
+
+
+from .series import below_threshold, bottom_k, comparison_indices, series  # noqa: E402  (time series, candidates)

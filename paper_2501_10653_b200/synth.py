@@ -26,6 +26,12 @@ configs prescribe.  The recipe (also in DESIGN.md, "Input recipe"):
                   image does not depend on N_T.  With ``device="cuda"`` the noise is drawn by
                   a seeded torch CUDA generator instead (same recipe, different realisation;
                   the finished buffers are the source of truth for both sides).
+  time series     ``make_series``: M snapshots of one field ("on-and-off emission
+                  behaviour ... between observations of the same section of the sky").  The sources
+                  the config's change rule selects are the transients; snapshot 0 shows all of them
+                  in their x state (MS1), and in every later snapshot each transient is, with
+                  probability 1/2, in its y state (absent / scaled) instead; fixed sources never
+                  change; every snapshot has fresh noise.
 """
 from __future__ import annotations
 
@@ -34,11 +40,13 @@ from dataclasses import dataclass, field, replace
 
 import numpy as np
 
-_STREAMS = {"pos": 1, "flux": 2, "ext": 3, "select": 4, "noise_x": 5, "noise_y": 6}
+_STREAMS = {"pos": 1, "flux": 2, "ext": 3, "select": 4, "noise_x": 5, "noise_y": 6, "series": 7}
+_NOISE_SNAPSHOT0 = 100         # snapshot j of a series draws its noise from stream 100 + j
 
 
-def _rng(seed: int, stream: str) -> np.random.Generator:
-    return np.random.Generator(np.random.Philox(key=[int(seed), _STREAMS[stream]]))
+def _rng(seed: int, stream) -> np.random.Generator:
+    sid = _STREAMS[stream] if isinstance(stream, str) else int(stream)
+    return np.random.Generator(np.random.Philox(key=[int(seed), sid]))
 
 
 @dataclass(frozen=True)
@@ -226,3 +234,41 @@ def make_pair(cfg: SkyConfig, seed: int | None = None, device: str | None = None
         yt.add_(torch.randn(yt.shape, generator=gy, device=dev, dtype=torch.float32),
                 alpha=cfg.noise_sigma)
     return xt, yt, meta
+
+
+def make_series(cfg: SkyConfig, n_images: int, seed: int | None = None, device: str | None = None):
+    """A time series of ``n_images`` snapshots of the config's sky (recipe in the module docstring).
+    Host (default): list of C-contiguous float32 numpy arrays; ``device="cuda"``: list of torch CUDA
+    tensors (sky rendered on the host, noise drawn on the device).  Returns (images, meta);
+    ``meta["state_y"][j, i]`` tells whether changed source i is in its y state in snapshot j."""
+    if n_images < 2:
+        raise ValueError("a series needs at least two images")
+    seed = cfg.seed if seed is None else seed
+    src = _draw_sources(cfg, seed)
+    amp_x, amp_y = _select_changes(cfg, src, seed)
+    same = amp_x == amp_y
+    changed = np.nonzero(~same)[0]
+    base = np.zeros((cfg.N, cfg.N), dtype=np.float32)
+    _render(base, src, amp_x, np.nonzero(same)[0])
+    state_y = _rng(seed, "series").random((n_images, changed.size)) < 0.5
+    state_y[0] = False                                  # snapshot 0: every transient in its x state
+    images = []
+    if device is not None:
+        import torch
+        dev = torch.device(device)
+    for j in range(n_images):
+        amps = amp_x.copy()
+        amps[changed[state_y[j]]] = amp_y[changed[state_y[j]]]
+        img = base.copy()
+        _render(img, src, amps, changed)
+        if device is None:
+            _add_noise_host(img, cfg.noise_sigma, _rng(seed, _NOISE_SNAPSHOT0 + j))
+            images.append(img)
+        else:
+            g = torch.Generator(device=dev).manual_seed(1000003 * seed + 17 * j + 5)
+            t = torch.from_numpy(img).to(dev)
+            t.add_(torch.randn(t.shape, generator=g, device=dev, dtype=torch.float32), alpha=cfg.noise_sigma)
+            images.append(t)
+    meta = {"cfg": cfg, "seed": seed, "sources": dict(src, amp_x=amp_x, amp_y=amp_y),
+            "changed": changed, "state_y": state_y}
+    return images, meta
