@@ -38,7 +38,7 @@
  *       workspace NULL / too small when iqa_workspace_bytes() > 0 ... IQA_ERR_WORKSPACE
  *       CUDA launch / copy failure .................................. IQA_ERR_CUDA
  *   * Any N_T that divides N is accepted.  Power-of-two N_T >= 8 with 16-byte aligned
- *     x and y take the persistent cp.async-pipelined stream kernel; everything else takes a
+ *     x and y (and N % 4 == 0) take the persistent TMA-fed kernel; everything else takes a
  *     generic (slower, still CUDA) kernel.  Results are deterministic: fixed reduction order,
  *     no floating-point atomics; two calls on the same inputs are bit-identical.
  * ============================================================================= */
@@ -119,6 +119,40 @@ int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_
                     float* lisi, float* auglisi, float* sum_x, float* sum_y,
                     float* lisi_num, float* auglisi_num, float* out2,
                     void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- time series ---------------------------------------------------------
+ * "Transients typically exhibit on-and-off emission behaviour, causing intensity variations
+ * between observations of the same section of the sky, while fixed sources remain unchanged"
+ * (P:39); "the rest of the image remains largely stable with slight variations over time".
+ * A series of n_images snapshots I_0 .. I_{n_images-1} of one field gives K = n_images - 1
+ * comparisons, each of them exactly the pair computation above (clamp P:27, Eqs. 1-2 per tile,
+ * Eqs. 3-4 for the whole image):
+ *   IQA_SERIES_REFERENCE    comparison k is (x, y) = (I_0, I_{k+1})
+ *   IQA_SERIES_CONSECUTIVE  comparison k is (x, y) = (I_k, I_{k+1})
+ * For 16-byte aligned images and a power-of-two N_T >= 8 one persistent TMA-fed kernel keeps the
+ * x block of every comparison in shared memory, so each image is read from HBM ONCE:
+ * 4 (K+1)/K bytes per pixel and comparison instead of the 8 of K independent pair calls.  Other
+ * shapes are computed pair by pair (same results, 8 bytes). */
+#define IQA_SERIES_REFERENCE 0
+#define IQA_SERIES_CONSECUTIVE 1
+
+/* Bytes of device workspace iqa_series_tiles needs: (n_images - 1) * iqa_workspace_bytes(N, N_T). */
+size_t iqa_series_workspace_bytes(int n_images, int N, int N_T);
+
+/*   img_ptrs_host        HOST array of n_images DEVICE pointers to [N*N] images (read during the call only)
+ *   mode                 IQA_SERIES_REFERENCE or IQA_SERIES_CONSECUTIVE (anything else: IQA_ERR_SHAPE)
+ *   lisi, auglisi, sum_x, sum_y  [K * n] device, required; comparison k occupies [k*n, (k+1)*n);
+ *                        sum_x holds the tile sums of the comparison's x image, sum_y of its y image
+ *   lisi_num, auglisi_num        [K * n] device, MAY BE NULL
+ *   out2                 [K * 2] device, MAY BE NULL: Eqs. 3-4 per comparison (LISI, augLISI)
+ *   workspace            >= iqa_series_workspace_bytes(n_images, N, N_T) bytes (may be NULL when 0)
+ * n_images >= 2; K * n must stay below 2^31.  Results agree with K calls of iqa_fused_tiles +
+ * iqa_aggregate to fp32 rounding of the same sums (bit-identical when the same kernel serves both). */
+int iqa_series_tiles(const float* const* img_ptrs_host, int n_images, int mode,
+                     int N, int N_T, float C1, float C2, float C, float D,
+                     float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                     float* lisi_num, float* auglisi_num, float* out2,
+                     void* workspace, size_t workspace_bytes, void* stream);
 
 /* Eqs. 3-4: merge n_tiles per-tile values into the whole-image pair.
  *   out2 [2] device: out2[0] = LISI, out2[1] = augLISI.  Sums are taken in double, fixed order.

@@ -24,7 +24,11 @@ IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKS
 
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
+           "iqa_series_workspace_bytes", "iqa_series_tiles",
            "iqa_aggregate", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host")
+
+IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
+SERIES_MODES = {"reference": IQA_SERIES_REFERENCE, "consecutive": IQA_SERIES_CONSECUTIVE}
 
 
 class IqaError(RuntimeError):
@@ -62,6 +66,10 @@ def _load() -> ctypes.CDLL:
     lib.iqa_batch_workspace_bytes.argtypes = [i, i, i]
     lib.iqa_fused_batch.restype = i
     lib.iqa_fused_batch.argtypes = [vp, vp, i, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_series_workspace_bytes.restype = sz
+    lib.iqa_series_workspace_bytes.argtypes = [i, i, i]
+    lib.iqa_series_tiles.restype = i
+    lib.iqa_series_tiles.argtypes = [vp, i, i, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.iqa_aggregate.restype = i
     lib.iqa_aggregate.argtypes = [vp, vp, vp, vp, i, f, f, vp, vp]
     lib.iqa_merge_tiles.restype = i
@@ -163,6 +171,21 @@ def iqa_fused_batch(x_ptrs_host, y_ptrs_host, n_pairs, N, N_T, C1, C2, C, D, lis
                                _ptr(workspace), int(workspace_bytes), _stream(stream))
 
 
+def iqa_series_workspace_bytes(n_images: int, N: int, N_T: int) -> int:
+    return int(lib.iqa_series_workspace_bytes(int(n_images), int(N), int(N_T)))
+
+
+def iqa_series_tiles(img_ptrs_host, n_images, mode, N, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
+                     lisi_num=None, auglisi_num=None, out2=None, workspace=None, workspace_bytes=0,
+                     stream=None) -> int:
+    """img_ptrs_host: sequence of n_images CUDA tensors (or addresses), or a ready ctypes array."""
+    it, _ = _ptr_table(img_ptrs_host)
+    return lib.iqa_series_tiles(it, int(n_images), int(mode), int(N), int(N_T), C1, C2, C, D,
+                                _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
+                                _ptr(lisi_num), _ptr(auglisi_num), _ptr(out2),
+                                _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
 def iqa_aggregate(lisi, auglisi, sum_x, sum_y, n_tiles, C2, C, out2, stream=None) -> int:
     return lib.iqa_aggregate(_ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), int(n_tiles),
                              C2, C, _ptr(out2), _stream(stream))
@@ -251,6 +274,36 @@ def fused_batch(xs, ys, N_T, C1, C2, C, D, numerators: bool = False, aggregate: 
                          out.get("L"), out.get("A"), out.get("whole"), ws, nbytes, _current_stream(dev))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_fused_batch")
+    return out
+
+
+def series_tiles(images, mode, N_T, C1, C2, C, D, numerators: bool = False, aggregate: bool = True) -> dict:
+    """Time series: K = len(images) - 1 comparisons, ``mode`` "reference"
+    (I_0 vs I_k+1) or "consecutive" (I_k vs I_k+1).  Returns (K, nt, nt) float32 CUDA tensors lisi,
+    auglisi, X, Y (+ L, A when ``numerators``) and, when ``aggregate``, ``whole`` (K, 2)."""
+    import torch
+    if mode not in SERIES_MODES:
+        raise ValueError(f"mode must be one of {tuple(SERIES_MODES)}")
+    if len(images) < 2:
+        raise IqaError(IQA_ERR_SHAPE, "series_tiles")
+    N = _check_images(images[0], images[1])
+    for im in images:
+        if _check_images(images[0], im) != N or im.device != images[0].device:
+            raise ValueError("all images of a series must have the same shape and device")
+    if N_T <= 0 or N % N_T:
+        raise IqaError(IQA_ERR_SHAPE, "series_tiles")
+    K, nt, dev = len(images) - 1, N // N_T, images[0].device
+    names = ["lisi", "auglisi", "X", "Y"] + (["L", "A"] if numerators else [])
+    out = {k: torch.empty((K, nt, nt), dtype=torch.float32, device=dev) for k in names}
+    if aggregate:
+        out["whole"] = torch.empty((K, 2), dtype=torch.float32, device=dev)
+    nbytes = iqa_series_workspace_bytes(len(images), N, N_T)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev) if nbytes else None
+    rc = iqa_series_tiles(images, len(images), SERIES_MODES[mode], N, N_T, C1, C2, C, D,
+                          out["lisi"], out["auglisi"], out["X"], out["Y"], out.get("L"), out.get("A"),
+                          out.get("whole"), ws, nbytes, _current_stream(dev))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_series_tiles")
     return out
 
 

@@ -17,7 +17,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "iqa_tiles.cu")]
 HEADERS = [os.path.join(CSRC, "iqa_kernels.cuh"), os.path.join(CSRC, "iqa_aggregate.cuh"),
-           os.path.join(CSRC, "iqa_stream.cuh"),
+           os.path.join(CSRC, "iqa_stream.cuh"), os.path.join(CSRC, "iqa_tma.cuh"),
            os.path.join(_ROOT, "include", "iqa_tiles.h")]
 LIB = os.path.join(_HERE, "libiqa_tiles.so")
 

@@ -15,6 +15,7 @@
 #include "iqa_aggregate.cuh"
 #include "iqa_kernels.cuh"
 #include "iqa_stream.cuh"
+#include "iqa_tma.cuh"
 
 namespace {
 
@@ -39,8 +40,10 @@ int env_int(const char* name, int dflt) {
 //   variant 0  K=4, depth 2, 2 CTAs/SM  (stage = 32 rows, 68 KiB smem/CTA, 64 KiB in flight per SM)  default
 //   variant 1  K=2, depth 2, 3 CTAs/SM  (stage = 16 rows, 36 KiB smem/CTA, 48 KiB in flight per SM)
 //   variant 2  K=8, depth 2, 1 CTA/SM   (stage = 64 rows, 132 KiB smem/CTA)  mapping-independence tests only
+//   variant 3  the TMA-fed kernel of iqa_tma.cuh (boxes of 128 x 32, mbarrier ring, packed fp32 pairs)  default
 // IQA_FORCE_VARIANT=v selects one (debug / tuning knob); all agree to ~1e-7 relative.
-constexpr int kNumVariants = 3;
+constexpr int kVariantTma = 3;
+constexpr int kNumVariants = 3;      // cp.async variants (the TMA kernel has its own geometry entry)
 struct VariantInfo { int K, depth, min_ctas; };
 constexpr VariantInfo kVariants[kNumVariants] = {{4, 2, 2}, {2, 2, 3}, {8, 2, 1}};
 
@@ -69,8 +72,54 @@ size_t stream_smem(int variant) {
     }
 }
 
+using TmaFn = void (*)(const TmaParams);
+
+// The standalone LISI / augLISI entry points only exist for pairs; the series modes are fused.
+TmaFn tma_fn(int mode, int series) {
+    if (series == kPairs) {
+        switch (mode) {
+            case kModeLisi: return tma_kernel<kModeLisi, kPairs>;
+            case kModeAug: return tma_kernel<kModeAug, kPairs>;
+            default: return tma_kernel<kModeFused, kPairs>;
+        }
+    }
+    if (mode != kModeFused) return nullptr;
+    return series == kReference ? tma_kernel<kModeFused, kReference> : tma_kernel<kModeFused, kConsecutive>;
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda).
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+    static const EncodeTiledFn fn = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            f = nullptr;
+        return (EncodeTiledFn)f;
+    }();
+    return fn;
+}
+
+// Tensor map of one N x N fp32 row-major image: boxes of 128 columns x 32 rows, no swizzle (a box
+// lands as [32][128] floats), out-of-bounds elements read as zero.  Needs a 16-byte aligned base
+// and N % 4 == 0 (row pitch a multiple of 16 bytes).
+bool encode_image_map(CUtensorMap* map, const float* img, int N) {
+    const EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return false;
+    const cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)N};
+    const cuuint64_t strides[1] = {(cuuint64_t)N * sizeof(float)};
+    const cuuint32_t box[2] = {(cuuint32_t)kUnitCols, (cuuint32_t)kBoxRows};
+    const cuuint32_t estr[2] = {1u, 1u};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2u, const_cast<float*>(img), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // Per-device launch geometry, filled on first use (benign race: every thread computes the same values).
-struct Geometry { std::atomic<int> ready{0}; int sms; int ctas[3][kNumVariants]; };
+struct Geometry { std::atomic<int> ready{0}; int sms; int ctas[3][kNumVariants]; int tma_ctas; };
 Geometry g_geo[kMaxDevices];
 
 const Geometry* geometry() {
@@ -88,6 +137,17 @@ const Geometry* geometry() {
             int occ = 0;
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kCtaThreads, smem) != cudaSuccess || occ <= 0) return nullptr;
             g.ctas[m][v] = occ < kVariants[v].min_ctas ? occ : kVariants[v].min_ctas;
+        }
+    g.tma_ctas = 0;
+    for (int m = 1; m <= 3; ++m)
+        for (int ser = 0; ser < 3; ++ser) {
+            TmaFn fn = tma_fn(m, ser);
+            if (!fn) continue;
+            if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tma_smem_bytes()) != cudaSuccess) return nullptr;
+            int occ = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kTmaThreads, tma_smem_bytes()) != cudaSuccess || occ <= 0) return nullptr;
+            occ = occ < 2 ? occ : 2;
+            g.tma_ctas = g.tma_ctas == 0 || occ < g.tma_ctas ? occ : g.tma_ctas;
         }
     g.sms = sms;
     g.ready.store(1, std::memory_order_release);
@@ -138,23 +198,29 @@ int status_of_shape(int N, int N_T) {
 }
 
 // How (N, N_T) is mapped onto CTAs.  DESIGN.md "Mapping".
+enum PlanKind { kPlanGeneric = 0, kPlanStream = 1, kPlanTma = 2 };
 struct Plan {
-    bool stream;       // persistent stream kernel (else generic kernel)
+    PlanKind kind;     // generic kernel / cp.async stream kernel / TMA kernel
     int variant;       // stream: index into kVariants
-    int item_rows;     // stream: R
+    int item_rows;     // stream, tma: R
     int pieces_x, pieces_y, pieces;   // pieces per tile; pieces == 1 -> finished inside one CTA
 };
 
 constexpr int kSplitItemRows = 64;   // tiles of side >= 128: items of 128 x 64, pieces to the workspace
 
-Plan make_plan(int N_T, bool aligned16) {
+// first_image: one image of the call (the TMA path is taken only when its tensor map encodes).
+Plan make_plan(int N, int N_T, bool aligned16, const float* first_image) {
     Plan pl{};
-    pl.stream = is_pow2(N_T) && N_T >= 8 && aligned16 && !env_int("IQA_FORCE_GENERIC", 0);
-    if (pl.stream) {
-        pl.variant = 0;
+    const bool fast = is_pow2(N_T) && N_T >= 8 && aligned16 && !env_int("IQA_FORCE_GENERIC", 0);
+    pl.kind = fast ? kPlanTma : kPlanGeneric;
+    if (fast) {
         const int forced = env_int("IQA_FORCE_VARIANT", -1);     // debug knob (tests: mapping independence)
-        if (forced >= 0 && forced < kNumVariants) pl.variant = forced;
-        const int rs = kWarpsPerCta * kVariants[pl.variant].K;   // stage height
+        if (forced >= 0 && forced < kNumVariants) { pl.kind = kPlanStream; pl.variant = forced; }
+        if (pl.kind == kPlanTma) {
+            CUtensorMap probe;
+            if (!encode_image_map(&probe, first_image, N)) { pl.kind = kPlanStream; pl.variant = 0; }
+        }
+        const int rs = pl.kind == kPlanTma ? kBoxRows : kWarpsPerCta * kVariants[pl.variant].K;   // stage height
         if (N_T <= 64) {
             pl.item_rows = N_T > rs ? N_T : rs;                  // whole tiles inside one item
             pl.pieces_x = pl.pieces_y = 1;
@@ -171,7 +237,7 @@ Plan make_plan(int N_T, bool aligned16) {
     return pl;
 }
 
-// Pieces per tile in the worst case over the mappings a call may take (stream or generic).
+// Pieces per tile in the worst case over the mappings a call may take (tma, stream or generic).
 size_t max_pieces(int N_T) {
     if (N_T <= 64) return 1;                                      // every path finishes tiles inside one CTA
     size_t pieces = (size_t)(N_T + kGenericRows - 1) / kGenericRows;
@@ -190,49 +256,71 @@ size_t workspace_bytes_for(int n_pairs, int N, int N_T) {
 }
 
 struct Outputs {
-    float *lisi, *auglisi, *sum_x, *sum_y, *lisi_num, *aug_num;   // [n_pairs * n] each (or nullptr)
+    float *lisi, *auglisi, *sum_x, *sum_y, *lisi_num, *aug_num;   // [n_comparisons * n] each (or nullptr)
     Outputs offset(size_t k) const {
         auto o = [k](float* p) { return p ? p + k : nullptr; };
         return {o(lisi), o(auglisi), o(sum_x), o(sum_y), o(lisi_num), o(aug_num)};
     }
+    Outputs for_mode(int mode) const {
+        return {(mode & kModeLisi) ? lisi : nullptr, (mode & kModeAug) ? auglisi : nullptr, sum_x, sum_y,
+                (mode & kModeLisi) ? lisi_num : nullptr, (mode & kModeAug) ? aug_num : nullptr};
+    }
 };
 
-// Shared body of every *_tiles / *_batch entry point: validation, then the launches.
-// xs, ys: HOST arrays of n_pairs device pointers.  out2 (nullable): Eqs. 3-4 per pair.
-int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pairs, int N, int N_T,
-              float C1, float C2, float C, float D, Outputs out, float* out2,
-              void* workspace, size_t workspace_bytes, void* stream) {
-    if (!xs || !ys) return IQA_ERR_NULL;
-    if (n_pairs <= 0) return IQA_ERR_SHAPE;
-    for (int i = 0; i < n_pairs; ++i)
-        if (!xs[i] || !ys[i]) return IQA_ERR_NULL;
-    if ((mode & kModeLisi) && !out.lisi) return IQA_ERR_NULL;
-    if ((mode & kModeAug) && !out.auglisi) return IQA_ERR_NULL;
-    if (mode == kModeFused && (!out.sum_x || !out.sum_y)) return IQA_ERR_NULL;
-    if (const int s = status_of_shape(N, N_T)) return s;
+struct Consts { float C1, C2, C, D; };
+
+// The TMA kernel over n_groups groups of M images (imgs[g * M + i], HOST array of device pointers);
+// `out` and `ws` point at the first comparison of the first group.  n_groups * M may exceed
+// kMaxImages (several launches); M itself may not.
+int launch_tma(int mode, int series, const float* const* imgs, int n_groups, int M, int N, int N_T, const Consts& k,
+               const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st) {
+    const Geometry* geo = geometry();
+    TmaFn fn = tma_fn(mode, series);
+    if (!geo || !fn || geo->tma_ctas <= 0 || M < 2 || M > kMaxImages) return IQA_ERR_CUDA;
     const int nt = N / N_T;
     const long long n = (long long)nt * nt;
-    if (n * n_pairs > 0x7fffffffLL) return IQA_ERR_SHAPE;
-    if ((mode & kModeLisi) && (!pos_finite(C1) || !pos_finite(C2) || !std::isfinite(D))) return IQA_ERR_PARAM;
-    if ((mode & kModeAug) && !pos_finite(C)) return IQA_ERR_PARAM;
-    if (out2 && (!pos_finite(C2) || !pos_finite(C))) return IQA_ERR_PARAM;
-    uintptr_t bits = 0;
-    for (int i = 0; i < n_pairs; ++i) bits |= (uintptr_t)xs[i] | (uintptr_t)ys[i];
-    if (bits & 3u) return IQA_ERR_ALIGN;
-    const size_t need = workspace_bytes_for(n_pairs, N, N_T);
-    if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
-    if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
+    const int units_x = (N + kUnitCols - 1) / kUnitCols;
+    const int units_y = (N + pl.item_rows - 1) / pl.item_rows;
+    const long long items_per_group = (long long)units_x * units_y;
+    const int groups_per_launch = kMaxImages / M;
+    if (items_per_group * groups_per_launch > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    for (int first = 0; first < n_groups; first += groups_per_launch) {
+        const int ng = n_groups - first < groups_per_launch ? n_groups - first : groups_per_launch;
+        TmaParams p{};
+        for (int i = 0; i < ng * M; ++i)
+            if (!encode_image_map(&p.maps[i], imgs[(size_t)first * M + i], N)) return IQA_ERR_CUDA;
+        p.n_groups = ng; p.M = M; p.N = N; p.log2_nt = ilog2(N_T); p.nt = nt; p.n_tiles = (int)n;
+        p.units_x = units_x; p.units_y = units_y; p.S = pl.item_rows / kBoxRows;
+        p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
+        const size_t cmp0 = (size_t)first * (size_t)(M - 1);
+        const Outputs o = out.offset(cmp0 * (size_t)n);
+        p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
+        p.lisi_num = o.lisi_num; p.aug_num = o.aug_num;
+        p.ws = ws ? ws + cmp0 * (size_t)n * pl.pieces : nullptr;
+        p.pieces_x = pl.pieces_x; p.pieces_y = pl.pieces_y;
+        const long long n_items = items_per_group * ng;
+        const long long resident = (long long)geo->sms * geo->tma_ctas;
+        const unsigned grid = (unsigned)(n_items < resident ? n_items : resident);
+        if (launch(fn, grid, kTmaThreads, tma_smem_bytes(), st, p) != cudaSuccess) return IQA_ERR_CUDA;
+    }
+    return IQA_OK;
+}
 
-    const bool aligned16 = ((bits & 15u) == 0) && (N % 4 == 0);
-    const Plan pl = make_plan(N_T, aligned16);
-    cudaStream_t st = (cudaStream_t)stream;
-    float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
-    out.lisi = (mode & kModeLisi) ? out.lisi : nullptr;
-    out.auglisi = (mode & kModeAug) ? out.auglisi : nullptr;
-    out.lisi_num = (mode & kModeLisi) ? out.lisi_num : nullptr;
-    out.aug_num = (mode & kModeAug) ? out.aug_num : nullptr;
-
-    if (pl.stream) {
+// S1-S4 for n_pairs pairs (xs[i], ys[i]) with the plan's kernel; `out` / `ws` point at pair 0.
+int launch_pairs(int mode, const float* const* xs, const float* const* ys, int n_pairs, int N, int N_T,
+                 const Consts& k, const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st) {
+    const int nt = N / N_T;
+    const long long n = (long long)nt * nt;
+    if (pl.kind == kPlanTma) {
+        const float* imgs[kMaxImages];
+        for (int first = 0; first < n_pairs; first += kMaxImages / 2) {
+            const int np = n_pairs - first < kMaxImages / 2 ? n_pairs - first : kMaxImages / 2;
+            for (int i = 0; i < np; ++i) { imgs[2 * i] = xs[first + i]; imgs[2 * i + 1] = ys[first + i]; }
+            const int rc = launch_tma(mode, kPairs, imgs, np, 2, N, N_T, k, out.offset((size_t)first * (size_t)n),
+                                      ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st);
+            if (rc != IQA_OK) return rc;
+        }
+    } else if (pl.kind == kPlanStream) {
         const Geometry* geo = geometry();
         if (!geo) return IQA_ERR_CUDA;
         const int units_x = (N + kUnitCols - 1) / kUnitCols;
@@ -247,7 +335,7 @@ int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pa
             p.n_pairs = np; p.N = N; p.log2_nt = ilog2(N_T); p.nt = nt; p.n_tiles = (int)n;
             p.units_x = units_x; p.units_y = units_y; p.item_rows = pl.item_rows;
             p.n_items = (int)(items_per_pair * np);
-            p.C1 = C1; p.C2 = C2; p.C = C; p.D = D;
+            p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
             const Outputs o = out.offset((size_t)first * (size_t)n);
             p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
             p.lisi_num = o.lisi_num; p.aug_num = o.aug_num;
@@ -264,7 +352,7 @@ int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pa
             GenericParams g{};
             TileParams& p = g.tp;
             p.x = xs[i]; p.y = ys[i]; p.N = N; p.nt = nt;
-            p.C1 = C1; p.C2 = C2; p.C = C; p.D = D;
+            p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
             const Outputs o = out.offset((size_t)i * (size_t)n);
             p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
             p.lisi_num = o.lisi_num; p.aug_num = o.aug_num;
@@ -279,13 +367,19 @@ int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pa
             if (e != cudaSuccess) return IQA_ERR_CUDA;
         }
     }
+    return IQA_OK;
+}
+
+// After S1-S4 of n_cmp comparisons: the second pass of split tiles, then Eqs. 3-4 per comparison.
+int finish_comparisons(const Outputs& out, float* out2, int n_cmp, long long n, const Consts& k, float4* ws,
+                       const Plan& pl, cudaStream_t st) {
     if (pl.pieces > 1) {                       // second pass over all tiles of the batch, fixed order
         TileParams p{};
-        p.C1 = C1; p.C2 = C2; p.C = C; p.D = D;
+        p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
         p.lisi = out.lisi; p.auglisi = out.auglisi; p.sum_x = out.sum_x; p.sum_y = out.sum_y;
         p.lisi_num = out.lisi_num; p.aug_num = out.aug_num;
         p.ws = ws;
-        const int total = (int)(n * n_pairs);
+        const int total = (int)(n * n_cmp);
         cudaError_t e;
         if (pl.pieces <= 32 && total >= 64)
             e = launch(finalise_small_kernel, (unsigned)((total + kCtaThreads - 1) / kCtaThreads), kCtaThreads, 0, st,
@@ -294,14 +388,112 @@ int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pa
             e = launch(finalise_kernel, (unsigned)total, kCtaThreads, 0, st, p, pl.pieces);
         if (e != cudaSuccess) return IQA_ERR_CUDA;
     }
-    if (out2) {                                // Eqs. 3-4 per pair
+    if (out2) {                                // Eqs. 3-4 per comparison
         const unsigned cs = (unsigned)agg_cluster_size(n);
-        if (launch_cluster(aggregate_kernel, (unsigned)n_pairs * cs, kAggThreads, 0, st, cs,
+        if (launch_cluster(aggregate_kernel, (unsigned)n_cmp * cs, kAggThreads, 0, st, cs,
                    (const float*)out.lisi, (const float*)out.auglisi, (const float*)out.sum_x,
-                   (const float*)out.sum_y, (int)n, C2, C, out2) != cudaSuccess)
+                   (const float*)out.sum_y, (int)n, k.C2, k.C, out2) != cudaSuccess)
             return IQA_ERR_CUDA;
     }
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+}
+
+// Validation shared by the batch and the series entry points (everything but the image lists).
+int validate_common(int mode, int n_cmp, int N, int N_T, float C1, float C2, float C, float D, const Outputs& out,
+                    const float* out2) {
+    if (n_cmp <= 0) return IQA_ERR_SHAPE;
+    if ((mode & kModeLisi) && !out.lisi) return IQA_ERR_NULL;
+    if ((mode & kModeAug) && !out.auglisi) return IQA_ERR_NULL;
+    if (mode == kModeFused && (!out.sum_x || !out.sum_y)) return IQA_ERR_NULL;
+    if (const int s = status_of_shape(N, N_T)) return s;
+    const long long nt = N / N_T;
+    if (nt * nt * n_cmp > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    if ((mode & kModeLisi) && (!pos_finite(C1) || !pos_finite(C2) || !std::isfinite(D))) return IQA_ERR_PARAM;
+    if ((mode & kModeAug) && !pos_finite(C)) return IQA_ERR_PARAM;
+    if (out2 && (!pos_finite(C2) || !pos_finite(C))) return IQA_ERR_PARAM;
+    return IQA_OK;
+}
+
+// Shared body of every *_tiles / *_batch entry point: validation, then the launches.
+// xs, ys: HOST arrays of n_pairs device pointers.  out2 (nullable): Eqs. 3-4 per pair.
+int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pairs, int N, int N_T,
+              float C1, float C2, float C, float D, Outputs out, float* out2,
+              void* workspace, size_t workspace_bytes, void* stream) {
+    if (!xs || !ys) return IQA_ERR_NULL;
+    if (n_pairs <= 0) return IQA_ERR_SHAPE;
+    for (int i = 0; i < n_pairs; ++i)
+        if (!xs[i] || !ys[i]) return IQA_ERR_NULL;
+    if (const int s = validate_common(mode, n_pairs, N, N_T, C1, C2, C, D, out, out2)) return s;
+    uintptr_t bits = 0;
+    for (int i = 0; i < n_pairs; ++i) bits |= (uintptr_t)xs[i] | (uintptr_t)ys[i];
+    if (bits & 3u) return IQA_ERR_ALIGN;
+    const size_t need = workspace_bytes_for(n_pairs, N, N_T);
+    if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
+    if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
+
+    const bool aligned16 = ((bits & 15u) == 0) && (N % 4 == 0);
+    const Plan pl = make_plan(N, N_T, aligned16, xs[0]);
+    cudaStream_t st = (cudaStream_t)stream;
+    float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
+    out = out.for_mode(mode);
+    const Consts k{C1, C2, C, D};
+    if (const int rc = launch_pairs(mode, xs, ys, n_pairs, N, N_T, k, out, ws, pl, st)) return rc;
+    const long long n = (long long)(N / N_T) * (N / N_T);
+    return finish_comparisons(out, out2, n_pairs, n, k, ws, pl, st);
+}
+
+// Time series: imgs = HOST array of n_images device pointers; K = n_images - 1
+// comparisons, (I_0, I_k+1) or (I_k, I_k+1).  Aligned power-of-two shapes take the TMA kernel, which
+// keeps the x box of every comparison in shared memory (each image is read from HBM once);
+// everything else is computed pair by pair with the kernels of the pair entry points.
+int run_series(const float* const* imgs, int n_images, int series, int N, int N_T,
+               float C1, float C2, float C, float D, Outputs out, float* out2,
+               void* workspace, size_t workspace_bytes, void* stream) {
+    if (!imgs) return IQA_ERR_NULL;
+    if (n_images < 2 || (series != kReference && series != kConsecutive)) return IQA_ERR_SHAPE;
+    for (int i = 0; i < n_images; ++i)
+        if (!imgs[i]) return IQA_ERR_NULL;
+    const int K = n_images - 1;
+    if (const int s = validate_common(kModeFused, K, N, N_T, C1, C2, C, D, out, out2)) return s;
+    uintptr_t bits = 0;
+    for (int i = 0; i < n_images; ++i) bits |= (uintptr_t)imgs[i];
+    if (bits & 3u) return IQA_ERR_ALIGN;
+    const size_t need = workspace_bytes_for(K, N, N_T);
+    if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
+    if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
+
+    const bool aligned16 = ((bits & 15u) == 0) && (N % 4 == 0);
+    const Plan pl = make_plan(N, N_T, aligned16, imgs[0]);
+    cudaStream_t st = (cudaStream_t)stream;
+    float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
+    const Consts k{C1, C2, C, D};
+    const long long n = (long long)(N / N_T) * (N / N_T);
+    if (pl.kind == kPlanTma) {
+        // chunks of at most kMaxImages images; consecutive chunks share one image
+        const float* chunk[kMaxImages];
+        for (int first = 0; first < K; first += kMaxImages - 1) {       // first = first comparison of the chunk
+            const int kc = K - first < kMaxImages - 1 ? K - first : kMaxImages - 1;
+            chunk[0] = series == kReference ? imgs[0] : imgs[first];
+            for (int i = 0; i < kc; ++i) chunk[1 + i] = imgs[first + 1 + i];
+            const int rc = launch_tma(kModeFused, series, chunk, 1, kc + 1, N, N_T, k, out.offset((size_t)first * (size_t)n),
+                                      ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st);
+            if (rc != IQA_OK) return rc;
+        }
+    } else {
+        const float* xs[kMaxBatch];
+        const float* ys[kMaxBatch];
+        for (int first = 0; first < K; first += kMaxBatch) {
+            const int kc = K - first < kMaxBatch ? K - first : kMaxBatch;
+            for (int i = 0; i < kc; ++i) {
+                xs[i] = series == kReference ? imgs[0] : imgs[first + i];
+                ys[i] = imgs[first + i + 1];
+            }
+            const int rc = launch_pairs(kModeFused, xs, ys, kc, N, N_T, k, out.offset((size_t)first * (size_t)n),
+                                        ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st);
+            if (rc != IQA_OK) return rc;
+        }
+    }
+    return finish_comparisons(out, out2, K, n, k, ws, pl, st);
 }
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -323,7 +515,7 @@ const char* iqa_status_string(int status) {
     }
 }
 
-const char* iqa_version(void) { return "0.2.0"; }
+const char* iqa_version(void) { return "0.3.0"; }
 
 size_t iqa_workspace_bytes(int N, int N_T) {
     if (status_of_shape(N, N_T) != IQA_OK) return 0;
@@ -365,6 +557,22 @@ int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_
     const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
     return run_batch(kModeFused, x_ptrs_host, y_ptrs_host, n_pairs, N, N_T, C1, C2, C, D, o, out2,
                      workspace, workspace_bytes, stream);
+}
+
+size_t iqa_series_workspace_bytes(int n_images, int N, int N_T) {
+    if (n_images < 2 || status_of_shape(N, N_T) != IQA_OK) return 0;
+    return workspace_bytes_for(n_images - 1, N, N_T);
+}
+
+int iqa_series_tiles(const float* const* img_ptrs_host, int n_images, int mode,
+                     int N, int N_T, float C1, float C2, float C, float D,
+                     float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                     float* lisi_num, float* auglisi_num, float* out2,
+                     void* workspace, size_t workspace_bytes, void* stream) {
+    const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
+    const int series = mode == IQA_SERIES_REFERENCE ? kReference : mode == IQA_SERIES_CONSECUTIVE ? kConsecutive : -1;
+    return run_series(img_ptrs_host, n_images, series, N, N_T, C1, C2, C, D, o, out2,
+                      workspace, workspace_bytes, stream);
 }
 
 int iqa_aggregate(const float* lisi, const float* auglisi,
