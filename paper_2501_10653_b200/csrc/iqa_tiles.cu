@@ -40,10 +40,10 @@ int env_int(const char* name, int dflt) {
 //   variant 0  K=4, depth 2, 2 CTAs/SM  (stage = 32 rows, 68 KiB smem/CTA, 64 KiB in flight per SM)  default
 //   variant 1  K=2, depth 2, 3 CTAs/SM  (stage = 16 rows, 36 KiB smem/CTA, 48 KiB in flight per SM)
 //   variant 2  K=8, depth 2, 1 CTA/SM   (stage = 64 rows, 132 KiB smem/CTA)  mapping-independence tests only
-//   variant 3  the TMA-fed kernel of iqa_tma.cuh (boxes of 128 x 32, mbarrier ring, packed fp32 pairs)  default
-// IQA_FORCE_VARIANT=v selects one (debug / tuning knob); all agree to ~1e-7 relative.
-constexpr int kVariantTma = 3;
-constexpr int kNumVariants = 3;      // cp.async variants (the TMA kernel has its own geometry entry)
+// The default path is the TMA-fed kernel of iqa_tma.cuh (kTmaConfigs below); the cp.async variants stay as the
+// fallback when a tensor map cannot be encoded and for the mapping-independence tests.
+// IQA_FORCE_VARIANT=v selects one of them (debug / tuning knob); all kernels agree to ~1e-7 relative.
+constexpr int kNumVariants = 3;
 struct VariantInfo { int K, depth, min_ctas; };
 constexpr VariantInfo kVariants[kNumVariants] = {{4, 2, 2}, {2, 2, 3}, {8, 2, 1}};
 
@@ -74,18 +74,38 @@ size_t stream_smem(int variant) {
 
 using TmaFn = void (*)(const TmaParams);
 
+// TMA kernel configurations: {box slots per CTA, rows per warp and box}.  Measured on B200
+// (profiles/r01f_tma_configs.md): pairs are HBM-bound and want FEW bytes in flight (config 1: two
+// 16 KiB boxes in flight per CTA while two are consumed; six boxes lose 3-6 % to DRAM locality, as
+// the cp.async variants did); the series modes keep S + 1 boxes alive and want the deeper ring of
+// config 0.  IQA_TMA_CONFIG=c forces one (tuning knob).
+struct TmaConfig { int boxes, rpw; };
+constexpr int kNumTmaConfigs = 5;
+constexpr TmaConfig kTmaConfigs[kNumTmaConfigs] = {{6, 4}, {4, 4}, {8, 2}, {6, 2}, {4, 2}};
+
+template <int MODE, int SERIES>
+TmaFn tma_fn_cfg(int cfg) {
+    switch (cfg) {
+        case 1: return tma_kernel<MODE, SERIES, 4, 4>;
+        case 2: return tma_kernel<MODE, SERIES, 8, 2>;
+        case 3: return tma_kernel<MODE, SERIES, 6, 2>;
+        case 4: return tma_kernel<MODE, SERIES, 4, 2>;
+        default: return tma_kernel<MODE, SERIES, 6, 4>;
+    }
+}
 // The standalone LISI / augLISI entry points only exist for pairs; the series modes are fused.
-TmaFn tma_fn(int mode, int series) {
+TmaFn tma_fn(int mode, int series, int cfg) {
     if (series == kPairs) {
         switch (mode) {
-            case kModeLisi: return tma_kernel<kModeLisi, kPairs>;
-            case kModeAug: return tma_kernel<kModeAug, kPairs>;
-            default: return tma_kernel<kModeFused, kPairs>;
+            case kModeLisi: return tma_fn_cfg<kModeLisi, kPairs>(cfg);
+            case kModeAug: return tma_fn_cfg<kModeAug, kPairs>(cfg);
+            default: return tma_fn_cfg<kModeFused, kPairs>(cfg);
         }
     }
     if (mode != kModeFused) return nullptr;
-    return series == kReference ? tma_kernel<kModeFused, kReference> : tma_kernel<kModeFused, kConsecutive>;
+    return series == kReference ? tma_fn_cfg<kModeFused, kReference>(cfg) : tma_fn_cfg<kModeFused, kConsecutive>(cfg);
 }
+size_t tma_smem(int cfg) { return tma_smem_bytes(kTmaConfigs[cfg].boxes, kTmaConfigs[cfg].rpw); }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda).
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -103,15 +123,15 @@ EncodeTiledFn encode_tiled_fn() {
     return fn;
 }
 
-// Tensor map of one N x N fp32 row-major image: boxes of 128 columns x 32 rows, no swizzle (a box
-// lands as [32][128] floats), out-of-bounds elements read as zero.  Needs a 16-byte aligned base
+// Tensor map of one N x N fp32 row-major image: boxes of 128 columns x box_rows rows, no swizzle (a box
+// lands as [box_rows][128] floats), out-of-bounds elements read as zero.  Needs a 16-byte aligned base
 // and N % 4 == 0 (row pitch a multiple of 16 bytes).
-bool encode_image_map(CUtensorMap* map, const float* img, int N) {
+bool encode_image_map(CUtensorMap* map, const float* img, int N, int box_rows) {
     const EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return false;
     const cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)N};
     const cuuint64_t strides[1] = {(cuuint64_t)N * sizeof(float)};
-    const cuuint32_t box[2] = {(cuuint32_t)kUnitCols, (cuuint32_t)kBoxRows};
+    const cuuint32_t box[2] = {(cuuint32_t)kUnitCols, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1u, 1u};
     return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2u, const_cast<float*>(img), dims, strides, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
@@ -119,7 +139,7 @@ bool encode_image_map(CUtensorMap* map, const float* img, int N) {
 }
 
 // Per-device launch geometry, filled on first use (benign race: every thread computes the same values).
-struct Geometry { std::atomic<int> ready{0}; int sms; int ctas[3][kNumVariants]; int tma_ctas; };
+struct Geometry { std::atomic<int> ready{0}; int sms; int ctas[3][kNumVariants]; int tma_ctas[kNumTmaConfigs]; };
 Geometry g_geo[kMaxDevices];
 
 const Geometry* geometry() {
@@ -138,17 +158,19 @@ const Geometry* geometry() {
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kCtaThreads, smem) != cudaSuccess || occ <= 0) return nullptr;
             g.ctas[m][v] = occ < kVariants[v].min_ctas ? occ : kVariants[v].min_ctas;
         }
-    g.tma_ctas = 0;
-    for (int m = 1; m <= 3; ++m)
-        for (int ser = 0; ser < 3; ++ser) {
-            TmaFn fn = tma_fn(m, ser);
-            if (!fn) continue;
-            if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tma_smem_bytes()) != cudaSuccess) return nullptr;
-            int occ = 0;
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kTmaThreads, tma_smem_bytes()) != cudaSuccess || occ <= 0) return nullptr;
-            occ = occ < 2 ? occ : 2;
-            g.tma_ctas = g.tma_ctas == 0 || occ < g.tma_ctas ? occ : g.tma_ctas;
-        }
+    for (int c = 0; c < kNumTmaConfigs; ++c) {
+        g.tma_ctas[c] = 0;
+        for (int m = 1; m <= 3; ++m)
+            for (int ser = 0; ser < 3; ++ser) {
+                TmaFn fn = tma_fn(m, ser, c);
+                if (!fn) continue;
+                if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tma_smem(c)) != cudaSuccess) return nullptr;
+                int occ = 0;
+                if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kTmaThreads, tma_smem(c)) != cudaSuccess || occ <= 0) return nullptr;
+                occ = occ < 2 ? occ : 2;
+                g.tma_ctas[c] = g.tma_ctas[c] == 0 || occ < g.tma_ctas[c] ? occ : g.tma_ctas[c];
+            }
+    }
     g.sms = sms;
     g.ready.store(1, std::memory_order_release);
     return &g;
@@ -202,6 +224,7 @@ enum PlanKind { kPlanGeneric = 0, kPlanStream = 1, kPlanTma = 2 };
 struct Plan {
     PlanKind kind;     // generic kernel / cp.async stream kernel / TMA kernel
     int variant;       // stream: index into kVariants
+    int tma_cfg;       // tma: index into kTmaConfigs
     int item_rows;     // stream, tma: R
     int pieces_x, pieces_y, pieces;   // pieces per tile; pieces == 1 -> finished inside one CTA
 };
@@ -209,7 +232,7 @@ struct Plan {
 constexpr int kSplitItemRows = 64;   // tiles of side >= 128: items of 128 x 64, pieces to the workspace
 
 // first_image: one image of the call (the TMA path is taken only when its tensor map encodes).
-Plan make_plan(int N, int N_T, bool aligned16, const float* first_image) {
+Plan make_plan(int N, int N_T, bool aligned16, const float* first_image, bool series) {
     Plan pl{};
     const bool fast = is_pow2(N_T) && N_T >= 8 && aligned16 && !env_int("IQA_FORCE_GENERIC", 0);
     pl.kind = fast ? kPlanTma : kPlanGeneric;
@@ -217,10 +240,16 @@ Plan make_plan(int N, int N_T, bool aligned16, const float* first_image) {
         const int forced = env_int("IQA_FORCE_VARIANT", -1);     // debug knob (tests: mapping independence)
         if (forced >= 0 && forced < kNumVariants) { pl.kind = kPlanStream; pl.variant = forced; }
         if (pl.kind == kPlanTma) {
+            const int dflt = series ? 0 : 1;
+            const int c = env_int("IQA_TMA_CONFIG", dflt);
+            pl.tma_cfg = c >= 0 && c < kNumTmaConfigs ? c : dflt;
+            // the series modes keep S + 1 boxes alive (S = 64 / box rows for N_T >= 64): small rings fall back
+            if (series && kTmaConfigs[pl.tma_cfg].boxes < 64 / (kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw) + 2) pl.tma_cfg = 0;
             CUtensorMap probe;
-            if (!encode_image_map(&probe, first_image, N)) { pl.kind = kPlanStream; pl.variant = 0; }
+            if (!encode_image_map(&probe, first_image, N, kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw)) { pl.kind = kPlanStream; pl.variant = 0; }
         }
-        const int rs = pl.kind == kPlanTma ? kBoxRows : kWarpsPerCta * kVariants[pl.variant].K;   // stage height
+        const int rs = pl.kind == kPlanTma ? kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw
+                                           : kWarpsPerCta * kVariants[pl.variant].K;   // stage height
         if (N_T <= 64) {
             pl.item_rows = N_T > rs ? N_T : rs;                  // whole tiles inside one item
             pl.pieces_x = pl.pieces_y = 1;
@@ -275,8 +304,9 @@ struct Consts { float C1, C2, C, D; };
 int launch_tma(int mode, int series, const float* const* imgs, int n_groups, int M, int N, int N_T, const Consts& k,
                const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st) {
     const Geometry* geo = geometry();
-    TmaFn fn = tma_fn(mode, series);
-    if (!geo || !fn || geo->tma_ctas <= 0 || M < 2 || M > kMaxImages) return IQA_ERR_CUDA;
+    TmaFn fn = tma_fn(mode, series, pl.tma_cfg);
+    const int box_rows = kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw;
+    if (!geo || !fn || geo->tma_ctas[pl.tma_cfg] <= 0 || M < 2 || M > kMaxImages) return IQA_ERR_CUDA;
     const int nt = N / N_T;
     const long long n = (long long)nt * nt;
     const int units_x = (N + kUnitCols - 1) / kUnitCols;
@@ -288,9 +318,9 @@ int launch_tma(int mode, int series, const float* const* imgs, int n_groups, int
         const int ng = n_groups - first < groups_per_launch ? n_groups - first : groups_per_launch;
         TmaParams p{};
         for (int i = 0; i < ng * M; ++i)
-            if (!encode_image_map(&p.maps[i], imgs[(size_t)first * M + i], N)) return IQA_ERR_CUDA;
+            if (!encode_image_map(&p.maps[i], imgs[(size_t)first * M + i], N, box_rows)) return IQA_ERR_CUDA;
         p.n_groups = ng; p.M = M; p.N = N; p.log2_nt = ilog2(N_T); p.nt = nt; p.n_tiles = (int)n;
-        p.units_x = units_x; p.units_y = units_y; p.S = pl.item_rows / kBoxRows;
+        p.units_x = units_x; p.units_y = units_y; p.S = pl.item_rows / box_rows;
         p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
         const size_t cmp0 = (size_t)first * (size_t)(M - 1);
         const Outputs o = out.offset(cmp0 * (size_t)n);
@@ -299,9 +329,9 @@ int launch_tma(int mode, int series, const float* const* imgs, int n_groups, int
         p.ws = ws ? ws + cmp0 * (size_t)n * pl.pieces : nullptr;
         p.pieces_x = pl.pieces_x; p.pieces_y = pl.pieces_y;
         const long long n_items = items_per_group * ng;
-        const long long resident = (long long)geo->sms * geo->tma_ctas;
+        const long long resident = (long long)geo->sms * geo->tma_ctas[pl.tma_cfg];
         const unsigned grid = (unsigned)(n_items < resident ? n_items : resident);
-        if (launch(fn, grid, kTmaThreads, tma_smem_bytes(), st, p) != cudaSuccess) return IQA_ERR_CUDA;
+        if (launch(fn, grid, kTmaThreads, tma_smem(pl.tma_cfg), st, p) != cudaSuccess) return IQA_ERR_CUDA;
     }
     return IQA_OK;
 }
@@ -432,7 +462,7 @@ int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pa
     if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
 
     const bool aligned16 = ((bits & 15u) == 0) && (N % 4 == 0);
-    const Plan pl = make_plan(N, N_T, aligned16, xs[0]);
+    const Plan pl = make_plan(N, N_T, aligned16, xs[0], false);
     cudaStream_t st = (cudaStream_t)stream;
     float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
     out = out.for_mode(mode);
@@ -463,7 +493,7 @@ int run_series(const float* const* imgs, int n_images, int series, int N, int N_
     if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
 
     const bool aligned16 = ((bits & 15u) == 0) && (N % 4 == 0);
-    const Plan pl = make_plan(N, N_T, aligned16, imgs[0]);
+    const Plan pl = make_plan(N, N_T, aligned16, imgs[0], true);
     cudaStream_t st = (cudaStream_t)stream;
     float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
     const Consts k{C1, C2, C, D};

@@ -37,9 +37,11 @@
 //                           snapshots stream through a ring of kNumBoxes - S boxes
 //   consume   warp w owns rows 4w..4w+3 of a box, lane l the columns 4l..4l+3: conflict-free
 //             LDS.128, 16 fp32 accumulators per lane
-//   reduce    per item and comparison exactly as iqa_stream.cuh: lane -> segmented warp
-//             butterfly -> shared-memory combine of the warps of a tile (fixed order) -> Eq. 1 /
-//             Eq. 2, or the piece's partial sums to the workspace (tiles larger than an item)
+//   reduce    per item and comparison: lane -> warp (segmented reduce-scatter butterfly) ->
+//             part[buf][warp][segment] in shared memory, handed through an mbarrier to a tenth
+//             FINALISER warp, which combines the warps of a tile in warp order and applies Eq. 1 /
+//             Eq. 2 (or writes the piece's partial sums to the workspace: tiles larger than an
+//             item).  The consumer warps never meet at a CTA barrier.
 // No floating-point atomics: results are bit-reproducible and do not depend on the grid size.
 // =============================================================================
 #pragma once
@@ -53,13 +55,12 @@
 namespace iqa {
 
 constexpr int kMaxImages = 64;                 // tensor maps per launch (kernel parameter space: 8 KiB)
-constexpr int kBoxRows = 32;                   // 8 consumer warps x 4 rows
-constexpr int kRowsPerWarp = kBoxRows / kWarpsPerCta;
-constexpr int kBoxFloats = kBoxRows * kUnitCols;
-constexpr uint32_t kBoxBytes = kBoxFloats * 4u;
-constexpr int kNumBoxes = 6;                   // 96 KiB of boxes per CTA, 2 CTAs per SM
-constexpr int kTmaThreads = kCtaThreads + 32;  // + the producer warp
-constexpr int kConsumerBarrier = 1;            // named barrier of the 256 consumer threads
+// Box geometry and ring size are template parameters of the kernel:
+//   RPW  rows per consumer warp and box (box = 8 RPW rows x 128 columns: 16 KiB for RPW = 4)
+//   NB   box slots per CTA (NB boxes of shared memory; 2 CTAs per SM)
+constexpr int kMaxBoxSlots = 12;
+constexpr int kTmaThreads = kCtaThreads + 64;  // + the producer warp + the finaliser warp
+constexpr int kPartBufs = 4;                   // per-warp partial sums in flight between consumers and finaliser
 
 enum : int { kPairs = 0, kReference = 1, kConsecutive = 2 };
 
@@ -73,7 +74,7 @@ struct TmaParams {
     int n_tiles;         // nt * nt
     int units_x;         // items across: ceil(N / 128)
     int units_y;         // items down:   ceil(N / R)
-    int S;               // boxes (stages) per item and image: R = 32 S
+    int S;               // boxes (stages) per item and image: R = S * box rows
     float C1, C2, C, D;
     float* lisi;         // [n_groups * (M-1) * n_tiles] or nullptr; comparison c = g (M-1) + k
     float* auglisi;
@@ -85,9 +86,9 @@ struct TmaParams {
     int pieces_x, pieces_y;
 };
 
-constexpr size_t tma_smem_bytes() {
-    return 1024 /* alignment slack */ + (size_t)kNumBoxes * kBoxBytes + 2 * kWarpsPerCta * 16 * sizeof(float4) +
-           2 * kNumBoxes * sizeof(uint64_t);
+constexpr size_t tma_smem_bytes(int NB, int RPW) {
+    return 1024 /* alignment slack */ + (size_t)NB * (kWarpsPerCta * RPW * kUnitCols * 4) +
+           kPartBufs * kWarpsPerCta * 16 * sizeof(float4) + (2 * NB + 2 * kPartBufs) * sizeof(uint64_t);
 }
 
 // ---- mbarrier / TMA primitives (PTX ISA: mbarrier, cp.async.bulk.tensor) --------------------
@@ -106,20 +107,18 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "{\n"
         ".reg .pred p;\n"
         "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra DONE_%=;\n"
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
+        "}\n" ::"r"(bar), "r"(parity), "r"(0x989680u) /* suspend-time hint: sleep in hardware, not in a spin */
+        : "memory");
 }
 // One box: 128 columns x 32 rows of the image described by `map`, top-left (col, row), -> dst.
 __device__ __forceinline__ void tma_load_box(uint32_t dst, const CUtensorMap* map, int col, int row, uint32_t bar) {
     asm volatile(
         "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
         ::"r"(dst), "l"(map), "r"(col), "r"(row), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void consumer_barrier() {
-    asm volatile("bar.sync %0, %1;" ::"n"(kConsumerBarrier), "n"(kCtaThreads) : "memory");
 }
 
 // ---- packed fp32 pairs ---------------------------------------------------------------------
@@ -184,8 +183,8 @@ __device__ __forceinline__ void pixel_terms2(float x0, float x1, float y0, float
     aY = add2(aY, yc);
 }
 
-// One box pair (x box, y box) -> this thread's 4 rows x 4 columns into the accumulators.
-template <int MODE>
+// One box pair (x box, y box) -> this thread's RPW rows x 4 columns into the accumulators.
+template <int MODE, int kRowsPerWarp>
 __device__ __forceinline__ void consume_boxes(const float* xs, const float* ys, float C1, Acc16& a) {
     float4 vx[kRowsPerWarp], vy[kRowsPerWarp];
 #pragma unroll
@@ -210,40 +209,52 @@ struct RingPos {
     }
 };
 
-// Per item and comparison: lane -> warp (segmented butterfly) -> CTA (shared memory, warp
-// order) -> Eq. 1 / Eq. 2 or the workspace.  Called by the 256 consumer threads.
-template <int MODE>
-__device__ __forceinline__ void reduce_item(const TmaParams& p, const Acc16& a, float4 (*part)[16],
-                                            int cmp, int uy, int ux, int lane, int w) {
+// Consumer side of the per-item reduction: lane (4 columns -> 1) -> warp.  The g = min(32, N_T/4)
+// lanes of a tile row are combined with a reduce-scatter butterfly: at the first two levels every
+// lane gives away half of what it holds (4 -> 2 -> 1 values), so a segment of 16 lanes costs 5
+// shuffles + 5 adds instead of the 16 + 16 of an all-reduce.  Afterwards lane (seg << log2_g) + c'
+// holds component c of segment seg (c' = bit-reversed c: L at +0, X at +1, A at +2, Y at +3; for
+// g = 2: lane +0 holds (L, A), lane +1 holds (X, Y)) and stores it into part[w][seg].
+__device__ __forceinline__ void warp_partials(const Acc16& a, float4* part_w /* part[w] */, int log2_g, int lane) {
+    float lo, hi;
+    unpack2(add2(a.L[0], a.L[1]), lo, hi); const float vL = lo + hi;          // (c0 + c2) + (c1 + c3)
+    const float vA = (a.A[0] + a.A[2]) + (a.A[1] + a.A[3]);
+    unpack2(add2(a.X[0], a.X[1]), lo, hi); const float vX = lo + hi;
+    unpack2(add2(a.Y[0], a.Y[1]), lo, hi); const float vY = lo + hi;
+    const bool b0 = lane & 1, b1 = lane & 2;
+    // level 1 (xor 1): even lanes keep (L, A), odd lanes keep (X, Y)
+    float k0 = b0 ? vX : vL, k1 = b0 ? vY : vA;
+    k0 += __shfl_xor_sync(0xffffffffu, b0 ? vL : vX, 1);
+    k1 += __shfl_xor_sync(0xffffffffu, b0 ? vA : vY, 1);
+    float* dst = reinterpret_cast<float*>(part_w + (lane >> log2_g));
+    if (log2_g == 1) {                                     // N_T = 8: two lanes per segment
+        *reinterpret_cast<float2*>(dst + (b0 ? 2 : 0)) = make_float2(k0, k1);   // (L, A) or (X, Y)
+        return;
+    }
+    // level 2 (xor 2): lanes with bit 1 clear keep the first value, the others the second
+    float k = b1 ? k1 : k0;
+    k += __shfl_xor_sync(0xffffffffu, b1 ? k0 : k1, 2);
+    for (int o = 4; o < (1 << log2_g); o <<= 1) k += __shfl_xor_sync(0xffffffffu, k, o);
+    if ((lane & ((1 << log2_g) - 1)) < 4) dst[(b0 ? 2 : 0) + (b1 ? 1 : 0)] = k;   // float4 order (L, A, X, Y)
+}
+
+// Finaliser side: combine the warps of every tile of the item in warp order, then Eq. 1 / Eq. 2
+// (or the piece's partial sums to the workspace).  Executed by one warp; lanes take tiles.
+template <int kRowsPerWarp>
+__device__ __forceinline__ void finalise_item(const TmaParams& p, const float4 (*part)[16], int cmp, int uy, int ux,
+                                              int lane) {
+    constexpr int kBoxRows = kWarpsPerCta * kRowsPerWarp;
     const int log2_nt = p.log2_nt;
     const int log2_g = min(log2_nt - 2, 5);                       // g = min(32, N_T / 4) lanes per tile row
     const int log2_tpw = 5 - log2_g;                              // tile segments per warp row
     const int wpt = min(kWarpsPerCta, (1 << log2_nt) / kRowsPerWarp);   // warps per tile row-band of a box
-    const int n_ty = kWarpsPerCta / wpt;                          // tile rows per item (> 1 only when N_T < 32)
+    const int n_ty = kWarpsPerCta / wpt;                          // tile rows per item (> 1 only when N_T < box rows)
     const int R = p.S * kBoxRows;
-    // lane: 4 columns -> 1   ((c0 + c2) + (c1 + c3))
-    float4 v;
-    float lo, hi;
-    unpack2(add2(a.L[0], a.L[1]), lo, hi); v.x = lo + hi;
-    v.y = (a.A[0] + a.A[2]) + (a.A[1] + a.A[3]);
-    unpack2(add2(a.X[0], a.X[1]), lo, hi); v.z = lo + hi;
-    unpack2(add2(a.Y[0], a.Y[1]), lo, hi); v.w = lo + hi;
-    // warp: segmented butterfly over the g lanes that share a tile row
-    for (int o = (1 << log2_g) >> 1; o > 0; o >>= 1) {
-        if (MODE & kModeLisi) v.x += __shfl_xor_sync(0xffffffffu, v.x, o);
-        if (MODE & kModeAug) v.y += __shfl_xor_sync(0xffffffffu, v.y, o);
-        v.z += __shfl_xor_sync(0xffffffffu, v.z, o);
-        v.w += __shfl_xor_sync(0xffffffffu, v.w, o);
-    }
-    if ((lane & ((1 << log2_g) - 1)) == 0) part[w][lane >> log2_g] = v;
-    consumer_barrier();      // part[] of this buffer complete; the other buffer is rewritten only after the next barrier
-
-    const int t = threadIdx.x;
-    if (t < (n_ty << log2_tpw)) {
+    for (int t = lane; t < (n_ty << log2_tpw); t += 32) {
         const int jy = t >> log2_tpw;
         const int jx = t & ((1 << log2_tpw) - 1);
         const int c0 = ux * kUnitCols + (jx << log2_nt);          // jx == 0 when N_T >= 128
-        const int r0 = uy * R + (jy << log2_nt);                  // jy == 0 unless N_T < 32
+        const int r0 = uy * R + (jy << log2_nt);                  // jy == 0 unless N_T < box rows
         if (c0 < p.N && r0 < p.N) {
             float4 s = part[jy * wpt][jx];
             for (int k = 1; k < wpt; ++k) {
@@ -262,24 +273,33 @@ __device__ __forceinline__ void reduce_item(const TmaParams& p, const Acc16& a, 
     }
 }
 
-template <int MODE, int SERIES>
+template <int MODE, int SERIES, int kNumBoxes, int kRowsPerWarp>
 __global__ void __launch_bounds__(kTmaThreads, 2)
 tma_kernel(const __grid_constant__ TmaParams p) {
+    constexpr int kBoxRows = kWarpsPerCta * kRowsPerWarp;
+    constexpr int kBoxFloats = kBoxRows * kUnitCols;
+    constexpr uint32_t kBoxBytes = kBoxFloats * 4u;
     extern __shared__ unsigned char smem_dyn[];
     // 1 KiB-aligned start of the boxes (pointer arithmetic on smem_dyn keeps the shared address space)
     unsigned char* base = smem_dyn + ((1024u - (smem_addr(smem_dyn) & 1023u)) & 1023u);
     float* boxes = reinterpret_cast<float*>(base);
-    float4 (*part)[kWarpsPerCta][16] =
-        reinterpret_cast<float4 (*)[kWarpsPerCta][16]>(base + (size_t)kNumBoxes * kBoxBytes);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(base + (size_t)kNumBoxes * kBoxBytes + 2 * kWarpsPerCta * 16 * sizeof(float4));
+    constexpr size_t kPartOff = (size_t)kNumBoxes * kBoxBytes;
+    constexpr size_t kBarOff = kPartOff + kPartBufs * kWarpsPerCta * 16 * sizeof(float4);
+    float4 (*part)[kWarpsPerCta][16] = reinterpret_cast<float4 (*)[kWarpsPerCta][16]>(base + kPartOff);
     const uint32_t boxes_u32 = smem_addr(boxes);
-    const uint32_t full_u32 = smem_addr(bars);                    // full[slot]  at full_u32  + 8 slot
+    const uint32_t full_u32 = smem_addr(base + kBarOff);          // full[slot]  at full_u32  + 8 slot
     const uint32_t empty_u32 = full_u32 + 8u * kNumBoxes;         // empty[slot] at empty_u32 + 8 slot
+    const uint32_t pfull_u32 = empty_u32 + 8u * kNumBoxes;        // part_full[buf]: 8 consumer warps -> finaliser
+    const uint32_t pempty_u32 = pfull_u32 + 8u * kPartBufs;       // part_empty[buf]: finaliser -> consumers
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < kNumBoxes; ++i) {
             mbar_init(full_u32 + 8u * i, 1u);                     // the producer's expect_tx arrival
             mbar_init(empty_u32 + 8u * i, (uint32_t)kWarpsPerCta); // one arrival per consumer warp
+        }
+        for (int i = 0; i < kPartBufs; ++i) {
+            mbar_init(pfull_u32 + 8u * i, (uint32_t)kWarpsPerCta);
+            mbar_init(pempty_u32 + 8u * i, 1u);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -324,20 +344,46 @@ tma_kernel(const __grid_constant__ TmaParams p) {
         return;
     }
 
+    if (w == kWarpsPerCta + 1) {
+        // ================= finaliser warp: per item and comparison, warps -> tiles -> Eqs. 1-2 =================
+        int buf = 0;
+        uint32_t phase = 0u;
+        for (ItemCursor c = decode_item((int)blockIdx.x, units_x, units_y); c.pair < p.n_groups;
+             c.advance(stride, units_x, units_y)) {
+            for (int j = 1; j < M; ++j) {
+                mbar_wait(pfull_u32 + 8u * buf, phase);           // the eight warps' partial sums are in part[buf]
+                finalise_item<kRowsPerWarp>(p, part[buf], c.pair * (M - 1) + (j - 1), c.uy, c.ux, lane);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(pempty_u32 + 8u * buf);
+                if (++buf == kPartBufs) { buf = 0; phase ^= 1u; }
+            }
+        }
+        return;
+    }
+
     // ================= consumer warps =================
     const float C1 = p.C1;
-    const int my_off = (w * kRowsPerWarp) * kUnitCols + lane * 4;   // this thread's 4 x 4 patch inside a box
+    const int log2_g = min(p.log2_nt - 2, 5);
+    const int my_off = (w * kRowsPerWarp) * kUnitCols + lane * 4;   // this thread's RPW x 4 patch inside a box
     const float* my_boxes = boxes + my_off;
     auto wait_full = [&](int slot, uint32_t phase) { mbar_wait(full_u32 + 8u * slot, phase); };
     auto release = [&](int slot) {                                  // after __syncwarp(): every lane has read the box
         if (lane == 0) mbar_arrive(empty_u32 + 8u * slot);
+    };
+    int buf = 0;
+    uint32_t part_phase = 0u;
+    auto hand_over = [&](const Acc16& acc) {                        // this warp's partial sums -> finaliser warp
+        mbar_wait(pempty_u32 + 8u * buf, part_phase ^ 1u);          // part[buf] of kPartBufs reductions ago has been read
+        warp_partials(acc, part[buf][w], log2_g, lane);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(pfull_u32 + 8u * buf);
+        if (++buf == kPartBufs) { buf = 0; part_phase ^= 1u; }
     };
     RingPos cy{ring_first, ring_first, kNumBoxes - ring_first, 0u};
     RingPos cx = cy;                                                // kConsecutive: trails cy by S boxes
     if (SERIES == kConsecutive)
         for (int s = 0; s < S; ++s) cy.advance();
     uint32_t ref_phase = 0u;
-    int buf = 0;
     Acc16 acc;
     for (ItemCursor c = decode_item((int)blockIdx.x, units_x, units_y); c.pair < p.n_groups;
          c.advance(stride, units_x, units_y)) {
@@ -348,13 +394,12 @@ tma_kernel(const __grid_constant__ TmaParams p) {
                 const int ys = cy.slot; const uint32_t yp = cy.phase; cy.advance();
                 wait_full(xs, xp);
                 wait_full(ys, yp);
-                consume_boxes<MODE>(my_boxes + xs * kBoxFloats, my_boxes + ys * kBoxFloats, C1, acc);
+                consume_boxes<MODE, kRowsPerWarp>(my_boxes + xs * kBoxFloats, my_boxes + ys * kBoxFloats, C1, acc);
                 __syncwarp();
                 release(xs);
                 release(ys);
             }
-            reduce_item<MODE>(p, acc, part[buf], c.pair, c.uy, c.ux, lane, w);
-            buf ^= 1;
+            hand_over(acc);
         } else {
             for (int j = 1; j < M; ++j) {
                 acc.clear();
@@ -362,7 +407,7 @@ tma_kernel(const __grid_constant__ TmaParams p) {
                     const int xs = SERIES == kReference ? s : cx.slot;
                     if (j == 1) wait_full(xs, SERIES == kReference ? ref_phase : cx.phase);
                     wait_full(cy.slot, cy.phase);
-                    consume_boxes<MODE>(my_boxes + xs * kBoxFloats, my_boxes + cy.slot * kBoxFloats, C1, acc);
+                    consume_boxes<MODE, kRowsPerWarp>(my_boxes + xs * kBoxFloats, my_boxes + cy.slot * kBoxFloats, C1, acc);
                     __syncwarp();
                     if (SERIES == kReference) {
                         release(cy.slot);
@@ -374,8 +419,7 @@ tma_kernel(const __grid_constant__ TmaParams p) {
                     }
                     cy.advance();
                 }
-                reduce_item<MODE>(p, acc, part[buf], c.pair * (M - 1) + (j - 1), c.uy, c.ux, lane, w);
-                buf ^= 1;
+                hand_over(acc);
             }
             if (SERIES == kReference) ref_phase ^= 1u;
             if (SERIES == kConsecutive)
