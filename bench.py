@@ -6,7 +6,7 @@
 
 A STEP is one pass of the whole hot path -- S1-S4 (clamp, per-pixel terms, per-tile sums,
 Eqs. 1-2) and S5 (Eqs. 3-4 per pair) -- over one batch of P distinct synthetic image pairs
-already resident in HBM, through ONE call of iqa_fused_batch (one persistent stream kernel
+already resident in HBM, through ONE call of iqa_fused_batch (one persistent TMA-fed kernel
 over all pairs, a finalise pass for split tiles, one aggregate launch).  The batch is several
 times larger than the 126 MB L2, so every pair is read cold from HBM (said in ``config.l2``).
 The step is captured once in a CUDA graph; ``--no-graph`` launches through ctypes each step.
@@ -31,10 +31,10 @@ UNIT = "us/pair"
 # workload name -> (BASELINE.json config index, pairs per step, pairs per e2e step)
 WORKLOADS = {"cfg1": (1, 32, 8), "cfg3": (3, 8, 2), "cfg4": (4, 16, 1), "cfg0": (0, 64, 8)}
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused stream kernel at the default pairs
-# per step, from the `ncu --set full` captures summarised under profiles/r01e_ncu_full_*_stream.md
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused TMA kernel at the default pairs
+# per step, from the `ncu --set full` captures summarised under profiles/r01f_ncu_full_*_tma.md
 # (null when not captured for that workload; algorithmic bytes: cfg1 1.07427e9, cfg3 4.29706e9).
-NCU_TRAFFIC_BYTES = {"cfg1": 1.073763e9 + 4.388e6, "cfg3": 4.295033e9 + 5.502e6}
+NCU_TRAFFIC_BYTES = {"cfg1": None, "cfg3": None}
 
 
 def algorithmic_bytes(N: int, N_T: int) -> int:
@@ -392,6 +392,68 @@ def measure_sweep(torch, binding, base_cfg, pairs, steps, warmup, device, use_gr
     return rows
 
 
+def series_bytes(N: int, N_T: int, M: int) -> int:
+    """Algorithmic bytes of one iqa_series_tiles call: every image read once + 16 B per tile and comparison."""
+    return 4 * N * N * M + 16 * (N // N_T) ** 2 * (M - 1)
+
+
+def measure_series(torch, binding, cfg, M, steps, warmup, device, use_graph):
+    """Time-series modes: M snapshots of the workload's sky resident in HBM, one
+    iqa_series_tiles call per step (K = M - 1 comparisons, Eqs. 1-4 each)."""
+    from paper_2501_10653_b200 import synth
+    imgs, _ = synth.make_series(cfg, M, device=str(device))
+    K, n = M - 1, (cfg.N // cfg.N_T) ** 2
+    outs = [torch.empty((K, n), dtype=torch.float32, device=device) for _ in range(4)]
+    out2 = torch.empty((K, 2), dtype=torch.float32, device=device)
+    wsb = binding.iqa_series_workspace_bytes(M, cfg.N, cfg.N_T)
+    ws = torch.empty(wsb, dtype=torch.uint8, device=device) if wsb else None
+    table, _ = binding._ptr_table(imgs)
+    k = (float(cfg.C1), float(cfg.C2), float(cfg.C), float(cfg.D))
+    res = {}
+    for name, mode in binding.SERIES_MODES.items():
+        def step():
+            rc = binding.iqa_series_tiles(table, M, mode, cfg.N, cfg.N_T, *k, *outs, None, None, out2, ws, wsb,
+                                          torch.cuda.current_stream().cuda_stream)
+            if rc:
+                raise binding.IqaError(rc, "iqa_series_tiles")
+        fn = step
+        if use_graph:
+            g = torch.cuda.CUDAGraph()
+            step()
+            torch.cuda.synchronize()
+            with torch.cuda.graph(g):
+                step()
+            fn = g.replay
+        for _ in range(warmup):
+            fn()
+        us = time_region(torch, fn, steps) * 1e3 / steps
+        res[name] = {"us_per_comparison": us / K, "us_per_call": us,
+                     "hbm_GBps": series_bytes(cfg.N, cfg.N_T, M) / (us * 1e-6) / 1e9,
+                     "pairwise_equivalent_GBps": K * algorithmic_bytes(cfg.N, cfg.N_T) / (us * 1e-6) / 1e9,
+                     "bytes_per_pixel_and_comparison": 4.0 * M / K}
+    res.update({"images": M, "comparisons": K, "N": cfg.N, "N_T": cfg.N_T,
+                "l2": f"{M * 4 * cfg.N * cfg.N / 2**20:.0f} MiB of snapshots per call"})
+    del imgs, outs
+    torch.cuda.empty_cache()
+    return res
+
+
+def measure_read_ceiling():
+    """Read-only HBM ceiling of this GPU (build step 5): the standalone probe
+    paper_2501_10653_b200/csrc/hbm_read_ceiling.cu streams 2 GiB through TMA rings with no arithmetic,
+    over box shapes / ring depths / CTAs per SM, and prints the best rate."""
+    import subprocess
+    from paper_2501_10653_b200 import build
+    exe = build.build_read_ceiling()
+    out = subprocess.run([exe], capture_output=True, text=True, timeout=300).stdout
+    best = [ln for ln in out.splitlines() if ln.startswith("best")]
+    if not best:
+        return {"GBps": None, "error": out[-300:]}
+    f = best[0].split()
+    return {"GBps": float(f[1]) * 1e3, "pattern": " ".join(f[3:]),
+            "what": "hbm_read_ceiling: TMA loads into shared-memory rings, nothing computed, best of the sweep"}
+
+
 def run_ours(args):
     import torch
     if not torch.cuda.is_available():
@@ -439,7 +501,7 @@ def run_ours(args):
         m3 = measure_workload(torch, binding, c3, p3, k3, max(3, W), device, None, use_graph, rank)
         us3 = m3["ms_kernel"] * 1e3 / (k3 * p3)
         gbs3 = algorithmic_bytes(c3.N, c3.N_T) / (us3 * 1e-6) / 1e9
-        also[c3.name] = {"us_per_pair_step": m3["ms"] * 1e3 / (k3 * p3), "us_per_pair_stream_kernel": us3,
+        also[c3.name] = {"us_per_pair_step": m3["ms"] * 1e3 / (k3 * p3), "us_per_pair_tiles_kernel": us3,
                          "us_single_pair_warm": m3["us_single_pair_warm"],
                          "us_single_pair_cold": m3["us_single_pair_cold"],
                          "achieved_GBps": gbs3, "frac_of_measured_peak": gbs3 / peak,
@@ -447,6 +509,12 @@ def run_ours(args):
         del m3
         torch.cuda.empty_cache()
 
+    if world == 1 and not args.no_also:
+        # read-only ceiling of the kernel's own access pattern, and the time-series modes at N = 8192
+        also["read_ceiling"] = measure_read_ceiling()
+        cs = synth.CONFIGS[3] if args.workload in ("cfg1", "cfg3") else cfg
+        also[f"series_{cs.name}_M{args.series_images}"] = measure_series(
+            torch, binding, cs, args.series_images, max(3, min(K, 10)), 3, device, use_graph)
     if args.entry_points and world == 1:
         also["entry_points_cold"] = measure_entry_points(torch, cfg, pairs, max(3, min(K, 20)), max(3, W), device, use_graph)
     if args.sweep and world == 1:
@@ -466,9 +534,9 @@ def run_ours(args):
             "launch": ("cuda graph of the step" if use_graph else "direct launches through ctypes")
                       + ": one iqa_fused_batch call per step",
             "gpu_launches": K * world * launches,
-            "kernels": ["iqa::stream_kernel<3,K,2,CTAs> (fused S1-S4, all pairs of the step)"]
+            "kernels": ["iqa::tma_kernel<3,0,NB,RPW> (fused S1-S4, all pairs of the step)"]
                        + (["iqa::finalise_*_kernel"] if split else []) + ["iqa::aggregate_kernel (S5, one CTA per pair)"],
-            "roofline": {"bound": "hbm", "kernel": "iqa::stream_kernel<fused>", "achieved": achieved, "peak": peak,
+            "roofline": {"bound": "hbm", "kernel": "iqa::tma_kernel<fused, pairs>", "achieved": achieved, "peak": peak,
                          "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if not args.pairs else None,
                          "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
                          "us_per_launch": us_launch, "pairs_per_launch": pairs / n_stream,
@@ -480,6 +548,9 @@ def run_ours(args):
             "paper_context": {"note": "H100 kernel-only medians at N=2048, N_T=64 (PAPER.md:31); context, not the target",
                               "h100_split_lisi_us": 101.0, "h100_split_auglisi_us": 91.0},
         }
+        if also.get("read_ceiling", {}).get("GBps"):
+            line["roofline"]["read_ceiling_GBps"] = also["read_ceiling"]["GBps"]
+            line["roofline"]["frac_of_read_ceiling"] = achieved / also["read_ceiling"]["GBps"]
         if cpu is not None:
             line["cpu_baseline"] = cpu
         if also:
@@ -501,6 +572,7 @@ def main():
     ap.add_argument("--no-also", action="store_true", help="skip the extra N=8192 measurement")
     ap.add_argument("--no-latency", action="store_true",
                     help="skip the single-pair latency loops (keeps the launch list short under ncu)")
+    ap.add_argument("--series-images", type=int, default=9, help="snapshots of the time-series measurement in `also`")
     ap.add_argument("--sweep", action="store_true", help="also time BASELINE.json config [2] (N=2048, N_T = 8..512)")
     ap.add_argument("--entry-points", action="store_true",
                     help="also time iqa_fused_tiles / iqa_lisi_tiles / iqa_auglisi_tiles per pair, cold")

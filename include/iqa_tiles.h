@@ -162,6 +162,27 @@ int iqa_aggregate(const float* lisi, const float* auglisi,
                   float C2, float C,
                   float* out2, void* stream);
 
+/* ---- candidate extraction ------------------------------------------------
+ * The finder's output: which tiles changed.  The paper gives no decision rule -- it shows the
+ * matrices (Fig. 3) and says augLISI localises "transients to tiles with fewer false positives"
+ * -- so the rule is the plainest one, applied to any of the per-tile matrices (lisi or
+ * auglisi; low = dissimilar).  `values` holds n_maps matrices of n_tiles values each
+ * ([n_maps][n_tiles]: a batch of pairs or the comparisons of a series); values are compared as
+ * the fp32 numbers they are, -0 == +0; results are exact and deterministic.
+ *
+ * iqa_tiles_below: tiles with value < threshold, ascending tile index.
+ *   indices [n_maps * capacity]  first min(count, capacity) tile indices of each matrix (rest untouched)
+ *   counts  [n_maps]             number of tiles below the threshold (may exceed capacity)
+ *   threshold NaN -> IQA_ERR_PARAM; capacity may be 0 (count only; indices may then be NULL). */
+int iqa_tiles_below(const float* values, int n_tiles, int n_maps, float threshold,
+                    int* indices, int capacity, int* counts, void* stream);
+
+/* iqa_tiles_bottom_k: the k tiles of lowest value of each matrix, ascending by (value, tile index).
+ *   indices [n_maps * k], vals [n_maps * k] (MAY BE NULL: the values of those tiles)
+ *   1 <= k <= 1024; when k > n_tiles the entries beyond n_tiles are index -1 / value +Inf. */
+int iqa_tiles_bottom_k(const float* values, int n_tiles, int n_maps, int k,
+                       int* indices, float* vals, void* stream);
+
 /* P:66 "a larger tile formed by merging smaller ones": apply Eqs. 3-4 to every g x g block
  * of an nt x nt tile matrix, giving the (nt/g) x (nt/g) matrices of tile size g*N_T.
  *   in:  lisi, auglisi, sum_x, sum_y  [nt*nt]

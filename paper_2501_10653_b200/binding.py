@@ -24,7 +24,7 @@ IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKS
 
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
-           "iqa_series_workspace_bytes", "iqa_series_tiles",
+           "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
            "iqa_aggregate", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
@@ -70,6 +70,10 @@ def _load() -> ctypes.CDLL:
     lib.iqa_series_workspace_bytes.argtypes = [i, i, i]
     lib.iqa_series_tiles.restype = i
     lib.iqa_series_tiles.argtypes = [vp, i, i, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_tiles_below.restype = i
+    lib.iqa_tiles_below.argtypes = [vp, i, i, f, vp, i, vp, vp]
+    lib.iqa_tiles_bottom_k.restype = i
+    lib.iqa_tiles_bottom_k.argtypes = [vp, i, i, i, vp, vp, vp]
     lib.iqa_aggregate.restype = i
     lib.iqa_aggregate.argtypes = [vp, vp, vp, vp, i, f, f, vp, vp]
     lib.iqa_merge_tiles.restype = i
@@ -184,6 +188,16 @@ def iqa_series_tiles(img_ptrs_host, n_images, mode, N, N_T, C1, C2, C, D, lisi, 
                                 _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
                                 _ptr(lisi_num), _ptr(auglisi_num), _ptr(out2),
                                 _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
+def iqa_tiles_below(values, n_tiles, n_maps, threshold, indices, capacity, counts, stream=None) -> int:
+    return lib.iqa_tiles_below(_ptr(values), int(n_tiles), int(n_maps), threshold, _ptr(indices), int(capacity),
+                               _ptr(counts), _stream(stream))
+
+
+def iqa_tiles_bottom_k(values, n_tiles, n_maps, k, indices, vals=None, stream=None) -> int:
+    return lib.iqa_tiles_bottom_k(_ptr(values), int(n_tiles), int(n_maps), int(k), _ptr(indices), _ptr(vals),
+                                  _stream(stream))
 
 
 def iqa_aggregate(lisi, auglisi, sum_x, sum_y, n_tiles, C2, C, out2, stream=None) -> int:
@@ -305,6 +319,45 @@ def series_tiles(images, mode, N_T, C1, C2, C, D, numerators: bool = False, aggr
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_series_tiles")
     return out
+
+
+def _check_maps(values):
+    import torch
+    if not (isinstance(values, torch.Tensor) and values.is_cuda and values.dtype == torch.float32
+            and values.is_contiguous()):
+        raise TypeError("values must be a contiguous float32 CUDA tensor (no CPU fallback)")
+    if values.dim() == 2:                       # one (nt, nt) matrix
+        return 1, values.numel()
+    if values.dim() == 3:                       # (n_maps, nt, nt)
+        return int(values.shape[0]), int(values.shape[1] * values.shape[2])
+    raise ValueError("values must be (nt, nt) or (n_maps, nt, nt)")
+
+
+def tiles_below(values, threshold, capacity=None):
+    """Candidate tiles with value < threshold.  Returns (indices, counts): int32 CUDA
+    tensors (n_maps, capacity) -- the first ``counts[m]`` entries of row m are valid, ascending -- and (n_maps,)."""
+    import torch
+    n_maps, n = _check_maps(values)
+    capacity = n if capacity is None else int(capacity)
+    idx = torch.full((n_maps, capacity), -1, dtype=torch.int32, device=values.device)
+    cnt = torch.empty(n_maps, dtype=torch.int32, device=values.device)
+    rc = iqa_tiles_below(values, n, n_maps, float(threshold), idx, capacity, cnt, _current_stream(values.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_tiles_below")
+    return idx, cnt
+
+
+def tiles_bottom_k(values, k):
+    """The k tiles of lowest value per matrix, ascending by (value, index).  Returns (indices int32
+    (n_maps, k), vals float32 (n_maps, k)) CUDA tensors."""
+    import torch
+    n_maps, n = _check_maps(values)
+    idx = torch.empty((n_maps, k), dtype=torch.int32, device=values.device)
+    val = torch.empty((n_maps, k), dtype=torch.float32, device=values.device)
+    rc = iqa_tiles_bottom_k(values, n, n_maps, k, idx, val, _current_stream(values.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_tiles_bottom_k")
+    return idx, val
 
 
 def lisi_tiles(x, y, N_T, C1, C2, D, workspace=None):

@@ -17,7 +17,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "iqa_tiles.cu")]
 HEADERS = [os.path.join(CSRC, "iqa_kernels.cuh"), os.path.join(CSRC, "iqa_aggregate.cuh"),
-           os.path.join(CSRC, "iqa_stream.cuh"), os.path.join(CSRC, "iqa_tma.cuh"),
+           os.path.join(CSRC, "iqa_stream.cuh"), os.path.join(CSRC, "iqa_tma.cuh"), os.path.join(CSRC, "iqa_candidates.cuh"),
            os.path.join(_ROOT, "include", "iqa_tiles.h")]
 LIB = os.path.join(_HERE, "libiqa_tiles.so")
 
@@ -49,6 +49,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
         print(" ".join(cmd), file=sys.stderr)
     subprocess.run(cmd, check=True)
     return LIB
+
+
+CEILING_SRC = os.path.join(CSRC, "hbm_read_ceiling.cu")
+CEILING_EXE = os.path.join(_HERE, "hbm_read_ceiling")
+
+
+def build_read_ceiling(force: bool = False) -> str:
+    """Compile the standalone read-only HBM ceiling probe (csrc/hbm_read_ceiling.cu). Returns its path."""
+    if not force and os.path.exists(CEILING_EXE) and os.path.getmtime(CEILING_EXE) >= os.path.getmtime(CEILING_SRC):
+        return CEILING_EXE
+    subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17",
+                    "-o", CEILING_EXE, CEILING_SRC], check=True)
+    return CEILING_EXE
 
 
 if __name__ == "__main__":

@@ -13,6 +13,7 @@
 #include <utility>
 
 #include "iqa_aggregate.cuh"
+#include "iqa_candidates.cuh"
 #include "iqa_kernels.cuh"
 #include "iqa_stream.cuh"
 #include "iqa_tma.cuh"
@@ -614,6 +615,27 @@ int iqa_aggregate(const float* lisi, const float* auglisi,
     const unsigned cs = (unsigned)agg_cluster_size(n_tiles);
     if (launch_cluster(aggregate_kernel, cs, kAggThreads, 0, (cudaStream_t)stream, cs, lisi, auglisi, sum_x, sum_y,
                n_tiles, C2, C, out2) != cudaSuccess)
+        return IQA_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+}
+
+int iqa_tiles_below(const float* values, int n_tiles, int n_maps, float threshold,
+                    int* indices, int capacity, int* counts, void* stream) {
+    if (!values || !counts || (capacity > 0 && !indices)) return IQA_ERR_NULL;
+    if (n_tiles <= 0 || n_maps <= 0 || capacity < 0) return IQA_ERR_SHAPE;
+    if (threshold != threshold) return IQA_ERR_PARAM;
+    if (launch(below_kernel, (unsigned)n_maps, kCandThreads, 0, (cudaStream_t)stream, values, n_tiles, threshold,
+               indices, capacity, counts) != cudaSuccess)
+        return IQA_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+}
+
+int iqa_tiles_bottom_k(const float* values, int n_tiles, int n_maps, int k,
+                       int* indices, float* vals, void* stream) {
+    if (!values || !indices) return IQA_ERR_NULL;
+    if (n_tiles <= 0 || n_maps <= 0 || k <= 0 || k > kMaxBottomK) return IQA_ERR_SHAPE;
+    if (launch(bottom_k_kernel, (unsigned)n_maps, kCandThreads, 0, (cudaStream_t)stream, values, n_tiles, k,
+               indices, vals) != cudaSuccess)
         return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }

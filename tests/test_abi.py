@@ -140,6 +140,40 @@ def test_batch_validation():
     assert call(N_T=128, ws=FAKE, wsb=need - 1) == B.IQA_ERR_WORKSPACE
 
 
+def test_series_and_candidate_validation():
+    """Error paths of iqa_series_tiles / iqa_tiles_below / iqa_tiles_bottom_k: nothing is enqueued."""
+    tbl = (ctypes.c_void_p * 3)(FAKE, FAKE, FAKE)
+    bad = (ctypes.c_void_p * 3)(FAKE, 0, FAKE)
+    odd = (ctypes.c_void_p * 3)(FAKE, FAKE + 2, FAKE)
+
+    def call(imgs=tbl, M=3, mode=B.IQA_SERIES_REFERENCE, N=256, N_T=16, C=1e-6, lisi=FAKE, ws=None, wsb=0):
+        return B.iqa_series_tiles(imgs, M, mode, N, N_T, 1e-6, 1e-6, C, 5e-7, lisi, FAKE, FAKE, FAKE,
+                                  None, None, None, ws, wsb, None)
+
+    assert call(imgs=None) == B.IQA_ERR_NULL
+    assert call(imgs=bad) == B.IQA_ERR_NULL
+    assert call(lisi=None) == B.IQA_ERR_NULL
+    assert call(M=1) == B.IQA_ERR_SHAPE
+    assert call(mode=2) == B.IQA_ERR_SHAPE
+    assert call(N=100) == B.IQA_ERR_SHAPE
+    assert call(C=0.0) == B.IQA_ERR_PARAM
+    assert call(imgs=odd) == B.IQA_ERR_ALIGN
+    assert call(N_T=128) == B.IQA_ERR_WORKSPACE
+    assert B.iqa_series_workspace_bytes(3, 256, 128) == 2 * B.iqa_workspace_bytes(256, 128) > 0
+    assert B.iqa_series_workspace_bytes(3, 256, 16) == 0 and B.iqa_series_workspace_bytes(1, 256, 128) == 0
+    assert B.iqa_tiles_bottom_k(None, 16, 1, 4, FAKE) == B.IQA_ERR_NULL
+    assert B.iqa_tiles_bottom_k(FAKE, 16, 1, 4, None) == B.IQA_ERR_NULL
+    assert B.iqa_tiles_bottom_k(FAKE, 16, 1, 0, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_tiles_bottom_k(FAKE, 16, 1, 1025, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_tiles_bottom_k(FAKE, 0, 1, 4, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_tiles_below(None, 16, 1, 0.5, FAKE, 16, FAKE) == B.IQA_ERR_NULL
+    assert B.iqa_tiles_below(FAKE, 16, 1, 0.5, FAKE, 16, None) == B.IQA_ERR_NULL
+    assert B.iqa_tiles_below(FAKE, 16, 1, 0.5, None, 16, FAKE) == B.IQA_ERR_NULL
+    assert B.iqa_tiles_below(FAKE, 16, 0, 0.5, FAKE, 16, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_tiles_below(FAKE, 16, 1, 0.5, FAKE, -1, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_tiles_below(FAKE, 16, 1, math.nan, FAKE, 16, FAKE) == B.IQA_ERR_PARAM
+
+
 def test_convenience_wrappers_refuse_cpu_tensors():
     """No CPU fallback: the product path fails loudly on host tensors."""
     torch = pytest.importorskip("torch")

@@ -1,0 +1,113 @@
+"""-m gpu parity tests of candidate extraction (iqa_tiles_below, iqa_tiles_bottom_k)
+against oracle/series.py: index work, so the bar is BIT-EXACT indices and values.
+
+Inputs are seeded and never come from the CUDA path: random fp32 matrices with many ties, and the
+ORACLE's augLISI / LISI matrices (cast to fp32) of BASELINE.json skies.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2501_10653_b200 import binding
+    return binding
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def _check_bottom_k(B, maps, k):
+    import torch
+    import oracle
+    idx, val = B.tiles_bottom_k(_dev(maps), k)
+    torch.cuda.synchronize()
+    idx, val = idx.cpu().numpy(), val.cpu().numpy()
+    for m in range(maps.shape[0]):
+        ei, ev = oracle.bottom_k(maps[m], k)
+        kk = ei.size
+        assert np.array_equal(idx[m, :kk], ei), (m, k)
+        assert np.array_equal(val[m, :kk], ev), (m, k)
+        assert np.all(idx[m, kk:] == -1) and np.all(np.isposinf(val[m, kk:]))
+
+
+def _check_below(B, maps, thr, capacity=None):
+    import torch
+    import oracle
+    idx, cnt = B.tiles_below(_dev(maps), thr, capacity)
+    torch.cuda.synchronize()
+    idx, cnt = idx.cpu().numpy(), cnt.cpu().numpy()
+    cap = idx.shape[1]
+    for m in range(maps.shape[0]):
+        e = oracle.below_threshold(maps[m], thr)
+        assert cnt[m] == e.size, (m, thr)
+        w = min(cap, e.size)
+        assert np.array_equal(idx[m, :w], e[:w])
+        assert np.all(idx[m, w:] == -1)          # untouched entries keep the wrapper's fill
+
+
+@pytest.mark.parametrize("nt,n_maps,k", [(4, 1, 3), (16, 3, 16), (16, 2, 256), (32, 4, 1), (64, 2, 100),
+                                         (128, 2, 1024), (256, 1, 777), (5, 2, 64), (33, 3, 1000)])
+def test_bottom_k_random_with_ties(B, nt, n_maps, k):
+    rng = np.random.default_rng(nt * 1000 + k)
+    maps = np.round(rng.random((n_maps, nt, nt)), 2).astype(np.float32)      # two decimals: many ties
+    maps[0].ravel()[:: 7] = -0.0
+    maps[-1].ravel()[1:: 5] = 0.0
+    maps[0].ravel()[3] = -1.5
+    _check_bottom_k(B, maps, k)
+
+
+def test_bottom_k_all_equal_and_sorted_inputs(B):
+    maps = np.stack([np.full((16, 16), 0.25, np.float32),
+                     np.arange(256, dtype=np.float32).reshape(16, 16),
+                     np.arange(256, dtype=np.float32)[::-1].reshape(16, 16).copy(),
+                     -np.arange(256, dtype=np.float32).reshape(16, 16)])
+    for k in (1, 5, 255, 256, 300):
+        _check_bottom_k(B, maps, k)
+
+
+@pytest.mark.parametrize("thr", [-1.0, 0.0, 0.25, 0.5, 0.99, 2.0])
+def test_below_threshold_random(B, thr):
+    rng = np.random.default_rng(3)
+    maps = np.round(rng.random((3, 40, 40)), 2).astype(np.float32)
+    maps[1].ravel()[::9] = -0.0
+    _check_below(B, maps, thr)
+    _check_below(B, maps, thr, capacity=10)
+    _check_below(B, maps, thr, capacity=0)
+
+
+def test_candidates_on_oracle_matrices_of_config1(B):
+    """The matrices of BASELINE.json config [1] (computed by the ORACLE, cast to fp32) and of the N_T = 8
+    sweep point (65 536 tiles): bottom-k and thresholds as a finder would use them."""
+    import oracle
+    from paper_2501_10653_b200 import synth
+    cfg = synth.CONFIGS[1]
+    x, y, _ = synth.make_pair(cfg)
+    for N_T in (64, 8):
+        t = oracle.tiles(x, y, N_T, cfg.C1, cfg.C2, cfg.C, cfg.D)
+        maps = np.stack([t["auglisi"], t["lisi"]]).astype(np.float32)
+        for k in (5, 64, 1024):
+            _check_bottom_k(B, maps, k)
+        for thr in (float(np.quantile(maps[0], 0.01)), 0.999, 1.0):
+            _check_below(B, maps, thr)
+
+
+def test_candidate_error_codes(B):
+    import torch
+    v = torch.zeros((4, 4), dtype=torch.float32, device="cuda")
+    i = torch.zeros(16, dtype=torch.int32, device="cuda")
+    c = torch.zeros(1, dtype=torch.int32, device="cuda")
+    assert B.iqa_tiles_bottom_k(v, 16, 1, 4, i) == B.IQA_OK
+    assert B.iqa_tiles_bottom_k(v, 16, 1, 0, i) == B.IQA_ERR_SHAPE
+    assert B.iqa_tiles_bottom_k(v, 16, 1, 1025, i) == B.IQA_ERR_SHAPE
+    assert B.iqa_tiles_bottom_k(None, 16, 1, 4, i) == B.IQA_ERR_NULL
+    assert B.iqa_tiles_below(v, 16, 1, 0.5, i, 16, c) == B.IQA_OK
+    assert B.iqa_tiles_below(v, 16, 1, float("nan"), i, 16, c) == B.IQA_ERR_PARAM
+    assert B.iqa_tiles_below(v, 16, 1, 0.5, None, 16, c) == B.IQA_ERR_NULL
+    assert B.iqa_tiles_below(v, 16, 1, 0.5, None, 0, c) == B.IQA_OK
+    assert B.iqa_tiles_below(v, 0, 1, 0.5, i, 16, c) == B.IQA_ERR_SHAPE
+    torch.cuda.synchronize()
