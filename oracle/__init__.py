@@ -45,6 +45,10 @@ def _load():
         lib.iqa_oracle_tiles.argtypes = [fp, fp, ctypes.c_long, ctypes.c_long,
                                          ctypes.c_double, ctypes.c_double, ctypes.c_double,
                                          ctypes.c_double, dp, dp, dp, dp, dp, dp, ctypes.c_int]
+        lib.iqa_oracle_tiles_2d.restype = ctypes.c_int
+        lib.iqa_oracle_tiles_2d.argtypes = [fp, fp, ctypes.c_long, ctypes.c_long, ctypes.c_long, ctypes.c_long,
+                                            ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                            ctypes.c_double, dp, dp, dp, dp, dp, dp, ctypes.c_int]
         lib.iqa_oracle_aggregate.restype = ctypes.c_int
         lib.iqa_oracle_aggregate.argtypes = [dp, dp, dp, dp, ctypes.c_long,
                                              ctypes.c_double, ctypes.c_double, dp]
@@ -116,6 +120,38 @@ def tiles(x, y, N_T: int, C1, C2, C, D, threads: int = 0) -> dict:
         _dptr(out["L"]), _dptr(out["A"]), int(threads) if threads > 0 else max_threads())
     if rc != 0:
         raise RuntimeError(f"iqa_oracle_tiles failed with code {rc}")
+    return out
+
+
+def tiles_2d(x, y, N_T: int, C1, C2, C, D, threads: int = 0) -> dict:
+    """Per-tile Eq. 1 / Eq. 2 of two H x W fp32 images with EDGE TILES (reading R18):
+    the tile grid is ceil(H/N_T) x ceil(W/N_T), cells over the border hold only the pixels that exist.
+    x, y: 2-D float32 arrays whose rows are contiguous; a row stride (pitch) larger than W is allowed
+    (e.g. a column slice of a wider array) and is passed through, not copied away.
+    Returns (nty, ntx) float64 arrays: lisi, auglisi, X, Y, L, A."""
+    def prep(a):
+        a = np.asarray(a)
+        if a.dtype != np.float32 or a.ndim != 2:
+            raise ValueError("need 2-D float32 arrays")
+        if a.strides[1] != 4 or a.strides[0] % 4 or a.strides[0] < 4 * a.shape[1]:
+            a = np.ascontiguousarray(a)
+        return a
+    x, y = prep(x), prep(y)
+    if x.shape != y.shape:
+        raise ValueError("x and y must have the same shape")
+    H, W = x.shape
+    if N_T <= 0:
+        raise ValueError("N_T must be positive")
+    nty, ntx = -(-H // N_T), -(-W // N_T)
+    out = {k: np.empty((nty, ntx), dtype=np.float64) for k in ("lisi", "auglisi", "X", "Y", "L", "A")}
+    fp = ctypes.POINTER(ctypes.c_float)
+    rc = _load().iqa_oracle_tiles_2d(
+        ctypes.cast(x.ctypes.data, fp), ctypes.cast(y.ctypes.data, fp), H, W, x.strides[0] // 4, y.strides[0] // 4, N_T,
+        float(np.float32(C1)), float(np.float32(C2)), float(np.float32(C)), float(np.float32(D)),
+        _dptr(out["lisi"]), _dptr(out["auglisi"]), _dptr(out["X"]), _dptr(out["Y"]),
+        _dptr(out["L"]), _dptr(out["A"]), int(threads) if threads > 0 else max_threads())
+    if rc != 0:
+        raise RuntimeError(f"iqa_oracle_tiles_2d failed with code {rc}")
     return out
 
 
