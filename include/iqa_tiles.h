@@ -98,6 +98,26 @@ int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
                     float* lisi_num, float* auglisi_num,
                     void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- general images -------------------------------------------------------
+ * The paper's images are square and N is a multiple of N_T.  This entry point drops
+ * both: an H x W image with a row pitch (elements between rows; a sub-window of a larger array, a
+ * padded FITS plane) is cut into cells of N_T x N_T starting at (0, 0); a cell that sticks out over
+ * the right / bottom border is an EDGE TILE and holds only the pixels that exist ("N" in Eqs. 1-2
+ * is the pixel count of the region compared).  That equals zero-padding both images to a multiple
+ * of N_T, because after the clamp a zero pixel pair adds nothing to any of the four sums.
+ *   x, y            pixel (r, c) is x[r * pitch_x + c] / y[r * pitch_y + c]; pitch >= W
+ *   outputs         [nty * ntx], nty = ceil(H / N_T), ntx = ceil(W / N_T), t = ty * ntx + tx
+ *   workspace       >= iqa_workspace_bytes_2d(H, W, N_T) bytes (may be NULL when 0)
+ * Eqs. 3-4 over the result: iqa_aggregate with n_tiles = nty * ntx.  16-byte aligned bases, pitches
+ * that are multiples of 4 and a power-of-two N_T >= 8 take the TMA kernel (the TMA unit zero-fills
+ * what lies outside the image); everything else takes the generic kernel. */
+size_t iqa_workspace_bytes_2d(int H, int W, int N_T);
+int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long pitch_x, long long pitch_y, int N_T,
+                       float C1, float C2, float C, float D,
+                       float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                       float* lisi_num, float* auglisi_num,
+                       void* workspace, size_t workspace_bytes, void* stream);
+
 /* Bytes of device workspace iqa_fused_batch needs: n_pairs * iqa_workspace_bytes(N, N_T). */
 size_t iqa_batch_workspace_bytes(int n_pairs, int N, int N_T);
 

@@ -24,7 +24,7 @@ IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKS
 
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
-           "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
+           "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
            "iqa_aggregate", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
@@ -70,6 +70,11 @@ def _load() -> ctypes.CDLL:
     lib.iqa_series_workspace_bytes.argtypes = [i, i, i]
     lib.iqa_series_tiles.restype = i
     lib.iqa_series_tiles.argtypes = [vp, i, i, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_workspace_bytes_2d.restype = sz
+    lib.iqa_workspace_bytes_2d.argtypes = [i, i, i]
+    lib.iqa_fused_tiles_2d.restype = i
+    lib.iqa_fused_tiles_2d.argtypes = [vp, vp, i, i, ctypes.c_longlong, ctypes.c_longlong, i, f, f, f, f,
+                                       vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.iqa_tiles_below.restype = i
     lib.iqa_tiles_below.argtypes = [vp, i, i, f, vp, i, vp, vp]
     lib.iqa_tiles_bottom_k.restype = i
@@ -173,6 +178,18 @@ def iqa_fused_batch(x_ptrs_host, y_ptrs_host, n_pairs, N, N_T, C1, C2, C, D, lis
                                _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
                                _ptr(lisi_num), _ptr(auglisi_num), _ptr(out2),
                                _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
+def iqa_workspace_bytes_2d(H: int, W: int, N_T: int) -> int:
+    return int(lib.iqa_workspace_bytes_2d(int(H), int(W), int(N_T)))
+
+
+def iqa_fused_tiles_2d(x, y, H, W, pitch_x, pitch_y, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
+                       lisi_num=None, auglisi_num=None, workspace=None, workspace_bytes=0, stream=None) -> int:
+    return lib.iqa_fused_tiles_2d(_ptr(x), _ptr(y), int(H), int(W), int(pitch_x), int(pitch_y), int(N_T),
+                                  C1, C2, C, D, _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
+                                  _ptr(lisi_num), _ptr(auglisi_num), _ptr(workspace), int(workspace_bytes),
+                                  _stream(stream))
 
 
 def iqa_series_workspace_bytes(n_images: int, N: int, N_T: int) -> int:
@@ -288,6 +305,33 @@ def fused_batch(xs, ys, N_T, C1, C2, C, D, numerators: bool = False, aggregate: 
                          out.get("L"), out.get("A"), out.get("whole"), ws, nbytes, _current_stream(dev))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_fused_batch")
+    return out
+
+
+def fused_tiles_2d(x, y, N_T, C1, C2, C, D, numerators: bool = False) -> dict:
+    """Eqs. 1-2 per tile of two H x W float32 CUDA tensors with EDGE TILES.  x and y
+    may be row-pitched views (``stride(1) == 1``, e.g. a window ``big[r0:r1, c0:c1]``); nothing is copied.
+    Returns dict of (ceil(H/N_T), ceil(W/N_T)) float32 CUDA tensors: lisi, auglisi, X, Y (+ L, A)."""
+    import torch
+    for t in (x, y):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.dim() == 2):
+            raise TypeError("x and y must be 2-D float32 CUDA tensors (no CPU fallback)")
+        if t.stride(1) != 1 or t.stride(0) < t.shape[1]:
+            raise ValueError("rows must be contiguous (stride(1) == 1) and must not overlap")
+    if x.shape != y.shape or x.device != y.device:
+        raise ValueError("x and y must have the same shape and device")
+    if N_T <= 0:
+        raise IqaError(IQA_ERR_SHAPE, "fused_tiles_2d")
+    H, W = int(x.shape[0]), int(x.shape[1])
+    nty, ntx = -(-H // N_T), -(-W // N_T)
+    names = ["lisi", "auglisi", "X", "Y"] + (["L", "A"] if numerators else [])
+    out = {k: torch.empty((nty, ntx), dtype=torch.float32, device=x.device) for k in names}
+    nbytes = iqa_workspace_bytes_2d(H, W, N_T)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=x.device) if nbytes else None
+    rc = iqa_fused_tiles_2d(x, y, H, W, x.stride(0), y.stride(0), N_T, C1, C2, C, D, out["lisi"], out["auglisi"],
+                            out["X"], out["Y"], out.get("L"), out.get("A"), ws, nbytes, _current_stream(x.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_fused_tiles_2d")
     return out
 
 

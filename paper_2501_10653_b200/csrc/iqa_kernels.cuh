@@ -27,8 +27,10 @@ enum : int { kModeLisi = 1, kModeAug = 2, kModeFused = 3 };
 struct TileParams {
     const float* __restrict__ x;
     const float* __restrict__ y;
-    int N;               // image side
-    int nt;              // tiles per side, N / N_T
+    int N;               // image width W (= side N of the square API)
+    int H;               // image height
+    long long pitch_x, pitch_y;   // elements between rows of x / y (N when contiguous)
+    int nt;              // tiles per row: ceil(W / N_T)
     float C1, C2, C, D;
     float* lisi;         // [n] or nullptr (mode without LISI)
     float* auglisi;      // [n] or nullptr
@@ -81,7 +83,7 @@ __device__ __forceinline__ void finalise_tile(const Params& p, size_t t, float4 
 }
 
 // -----------------------------------------------------------------------------
-// Generic kernel: any N_T dividing N, any 4-byte aligned pointers (the stream kernel needs a
+// Generic kernel: any N_T, any H x W with row pitches (edge tiles), any 4-byte aligned pointers (the stream kernel needs a
 // power-of-two N_T >= 8 and 16-byte alignment).  One CTA per (tile, piece), a piece being up
 // to kGenericRows rows of the tile; scalar coalesced loads, thread-strided partial sums,
 // warp butterfly, warp order.  pieces == 1: the CTA finalises its tile; otherwise the
@@ -106,16 +108,19 @@ generic_kernel(const GenericParams g) {
     const int piece = (int)(b % g.pieces);
     const int tile = (int)(b / g.pieces);
     const int ty = tile / p.nt, tx = tile % p.nt;
+    const int rows_t = min(N_T, p.H - ty * N_T);             // edge tiles hold only the pixels that exist
+    const int cols_t = min(N_T, p.N - tx * N_T);
     const int r_begin = piece * kGenericRows;
-    const int r_end = min(N_T, r_begin + kGenericRows);
-    const long long npix = (long long)(r_end - r_begin) * N_T;
-    const size_t base = ((size_t)ty * N_T + r_begin) * (size_t)p.N + (size_t)tx * N_T;
+    const int r_end = min(rows_t, r_begin + kGenericRows);
+    const long long npix = r_end > r_begin ? (long long)(r_end - r_begin) * cols_t : 0;
+    const size_t row0 = (size_t)ty * N_T + r_begin, col0 = (size_t)tx * N_T;
 
     float aL = 0.f, aA = 0.f, aX = 0.f, aY = 0.f;
     for (long long k = threadIdx.x; k < npix; k += kCtaThreads) {
-        const int r = (int)(k / N_T), c = (int)(k % N_T);
-        const size_t off = base + (size_t)r * (size_t)p.N + (size_t)c;
-        pixel_terms<MODE>(__ldg(p.x + off), __ldg(p.y + off), p.C1, aL, aA, aX, aY);
+        const int r = (int)(k / cols_t), c = (int)(k % cols_t);
+        const size_t ox = (row0 + r) * (size_t)p.pitch_x + col0 + c;
+        const size_t oy = (row0 + r) * (size_t)p.pitch_y + col0 + c;
+        pixel_terms<MODE>(__ldg(p.x + ox), __ldg(p.y + oy), p.C1, aL, aA, aX, aY);
     }
     float4 v = make_float4(aL, aA, aX, aY);
     for (int o = 16; o > 0; o >>= 1) {

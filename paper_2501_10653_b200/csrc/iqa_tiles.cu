@@ -124,14 +124,14 @@ EncodeTiledFn encode_tiled_fn() {
     return fn;
 }
 
-// Tensor map of one N x N fp32 row-major image: boxes of 128 columns x box_rows rows, no swizzle (a box
+// Tensor map of one H x W fp32 row-major image with a row pitch (in elements): boxes of 128 columns x box_rows rows, no swizzle (a box
 // lands as [box_rows][128] floats), out-of-bounds elements read as zero.  Needs a 16-byte aligned base
-// and N % 4 == 0 (row pitch a multiple of 16 bytes).
-bool encode_image_map(CUtensorMap* map, const float* img, int N, int box_rows) {
+// and pitch % 4 == 0 (row pitch a multiple of 16 bytes); W itself is free.
+bool encode_image_map(CUtensorMap* map, const float* img, int H, int W, long long pitch, int box_rows) {
     const EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return false;
-    const cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)N};
-    const cuuint64_t strides[1] = {(cuuint64_t)N * sizeof(float)};
+    const cuuint64_t dims[2] = {(cuuint64_t)W, (cuuint64_t)H};
+    const cuuint64_t strides[1] = {(cuuint64_t)pitch * sizeof(float)};
     const cuuint32_t box[2] = {(cuuint32_t)kUnitCols, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1u, 1u};
     return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2u, const_cast<float*>(img), dims, strides, box, estr,
@@ -232,14 +232,17 @@ struct Plan {
 
 constexpr int kSplitItemRows = 64;   // tiles of side >= 128: items of 128 x 64, pieces to the workspace
 
+// General image geometry of the 2-D entry point (pairs only): x has pitch_x, y has pitch_y.
+struct Geom2D { int H, W; long long pitch_x, pitch_y; };
+
 // first_image: one image of the call (the TMA path is taken only when its tensor map encodes).
-Plan make_plan(int N, int N_T, bool aligned16, const float* first_image, bool series) {
+Plan make_plan(int N, int N_T, bool aligned16, const float* first_image, bool series, const Geom2D* g2 = nullptr) {
     Plan pl{};
     const bool fast = is_pow2(N_T) && N_T >= 8 && aligned16 && !env_int("IQA_FORCE_GENERIC", 0);
     pl.kind = fast ? kPlanTma : kPlanGeneric;
     if (fast) {
         const int forced = env_int("IQA_FORCE_VARIANT", -1);     // debug knob (tests: mapping independence)
-        if (forced >= 0 && forced < kNumVariants) { pl.kind = kPlanStream; pl.variant = forced; }
+        if (forced >= 0 && forced < kNumVariants && !g2) { pl.kind = kPlanStream; pl.variant = forced; }
         if (pl.kind == kPlanTma) {
             const int dflt = series ? 0 : 1;
             const int c = env_int("IQA_TMA_CONFIG", dflt);
@@ -247,7 +250,9 @@ Plan make_plan(int N, int N_T, bool aligned16, const float* first_image, bool se
             // the series modes keep S + 1 boxes alive (S = 64 / box rows for N_T >= 64): small rings fall back
             if (series && kTmaConfigs[pl.tma_cfg].boxes < 64 / (kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw) + 2) pl.tma_cfg = 0;
             CUtensorMap probe;
-            if (!encode_image_map(&probe, first_image, N, kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw)) { pl.kind = kPlanStream; pl.variant = 0; }
+            const bool ok = g2 ? encode_image_map(&probe, first_image, g2->H, g2->W, g2->pitch_x, kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw)
+                               : encode_image_map(&probe, first_image, N, N, N, kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw);
+            if (!ok) { pl.kind = g2 ? kPlanGeneric : kPlanStream; pl.variant = 0; }
         }
         const int rs = pl.kind == kPlanTma ? kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw
                                            : kWarpsPerCta * kVariants[pl.variant].K;   // stage height
@@ -259,7 +264,8 @@ Plan make_plan(int N, int N_T, bool aligned16, const float* first_image, bool se
             pl.pieces_x = N_T / kUnitCols;
             pl.pieces_y = N_T / kSplitItemRows;
         }
-    } else {
+    }
+    if (pl.kind == kPlanGeneric) {
         pl.pieces_x = 1;
         pl.pieces_y = (N_T + kGenericRows - 1) / kGenericRows;
     }
@@ -303,15 +309,18 @@ struct Consts { float C1, C2, C, D; };
 // `out` and `ws` point at the first comparison of the first group.  n_groups * M may exceed
 // kMaxImages (several launches); M itself may not.
 int launch_tma(int mode, int series, const float* const* imgs, int n_groups, int M, int N, int N_T, const Consts& k,
-               const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st) {
+               const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st, const Geom2D* g2 = nullptr) {
     const Geometry* geo = geometry();
     TmaFn fn = tma_fn(mode, series, pl.tma_cfg);
     const int box_rows = kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw;
     if (!geo || !fn || geo->tma_ctas[pl.tma_cfg] <= 0 || M < 2 || M > kMaxImages) return IQA_ERR_CUDA;
-    const int nt = N / N_T;
-    const long long n = (long long)nt * nt;
-    const int units_x = (N + kUnitCols - 1) / kUnitCols;
-    const int units_y = (N + pl.item_rows - 1) / pl.item_rows;
+    const int H = g2 ? g2->H : N, W = g2 ? g2->W : N;
+    const int ntx = (W + N_T - 1) / N_T, nty = (H + N_T - 1) / N_T;
+    const long long n = (long long)ntx * nty;
+    // split tiles: the items cover the whole tile grid, so that every piece of an edge tile is written
+    // (boxes entirely outside the image are zero-filled by the TMA unit without touching memory)
+    const int units_x = pl.pieces > 1 ? ntx * pl.pieces_x : (W + kUnitCols - 1) / kUnitCols;
+    const int units_y = pl.pieces > 1 ? nty * pl.pieces_y : (H + pl.item_rows - 1) / pl.item_rows;
     const long long items_per_group = (long long)units_x * units_y;
     const int groups_per_launch = kMaxImages / M;
     if (items_per_group * groups_per_launch > 0x7fffffffLL) return IQA_ERR_SHAPE;
@@ -319,8 +328,10 @@ int launch_tma(int mode, int series, const float* const* imgs, int n_groups, int
         const int ng = n_groups - first < groups_per_launch ? n_groups - first : groups_per_launch;
         TmaParams p{};
         for (int i = 0; i < ng * M; ++i)
-            if (!encode_image_map(&p.maps[i], imgs[(size_t)first * M + i], N, box_rows)) return IQA_ERR_CUDA;
-        p.n_groups = ng; p.M = M; p.N = N; p.log2_nt = ilog2(N_T); p.nt = nt; p.n_tiles = (int)n;
+            if (!encode_image_map(&p.maps[i], imgs[(size_t)first * M + i], H, W,
+                                  g2 ? ((i & 1) ? g2->pitch_y : g2->pitch_x) : (long long)N, box_rows))
+                return IQA_ERR_CUDA;
+        p.n_groups = ng; p.M = M; p.W = W; p.H = H; p.log2_nt = ilog2(N_T); p.ntx = ntx; p.n_tiles = (int)n;
         p.units_x = units_x; p.units_y = units_y; p.S = pl.item_rows / box_rows;
         p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
         const size_t cmp0 = (size_t)first * (size_t)(M - 1);
@@ -339,16 +350,18 @@ int launch_tma(int mode, int series, const float* const* imgs, int n_groups, int
 
 // S1-S4 for n_pairs pairs (xs[i], ys[i]) with the plan's kernel; `out` / `ws` point at pair 0.
 int launch_pairs(int mode, const float* const* xs, const float* const* ys, int n_pairs, int N, int N_T,
-                 const Consts& k, const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st) {
-    const int nt = N / N_T;
-    const long long n = (long long)nt * nt;
+                 const Consts& k, const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st,
+                 const Geom2D* g2 = nullptr) {
+    const int H = g2 ? g2->H : N, W = g2 ? g2->W : N;
+    const int nt = (W + N_T - 1) / N_T;                       // tiles per row
+    const long long n = (long long)nt * ((H + N_T - 1) / N_T);
     if (pl.kind == kPlanTma) {
         const float* imgs[kMaxImages];
         for (int first = 0; first < n_pairs; first += kMaxImages / 2) {
             const int np = n_pairs - first < kMaxImages / 2 ? n_pairs - first : kMaxImages / 2;
             for (int i = 0; i < np; ++i) { imgs[2 * i] = xs[first + i]; imgs[2 * i + 1] = ys[first + i]; }
             const int rc = launch_tma(mode, kPairs, imgs, np, 2, N, N_T, k, out.offset((size_t)first * (size_t)n),
-                                      ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st);
+                                      ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st, g2);
             if (rc != IQA_OK) return rc;
         }
     } else if (pl.kind == kPlanStream) {
@@ -382,7 +395,8 @@ int launch_pairs(int mode, const float* const* xs, const float* const* ys, int n
         for (int i = 0; i < n_pairs; ++i) {
             GenericParams g{};
             TileParams& p = g.tp;
-            p.x = xs[i]; p.y = ys[i]; p.N = N; p.nt = nt;
+            p.x = xs[i]; p.y = ys[i]; p.N = W; p.H = H; p.nt = nt;
+            p.pitch_x = g2 ? g2->pitch_x : (long long)N; p.pitch_y = g2 ? g2->pitch_y : (long long)N;
             p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
             const Outputs o = out.offset((size_t)i * (size_t)n);
             p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
@@ -578,6 +592,41 @@ int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
                     void* workspace, size_t workspace_bytes, void* stream) {
     const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
     return run_batch(kModeFused, &x, &y, 1, N, N_T, C1, C2, C, D, o, nullptr, workspace, workspace_bytes, stream);
+}
+
+size_t iqa_workspace_bytes_2d(int H, int W, int N_T) {
+    if (H <= 0 || W <= 0 || N_T <= 0 || H > kMaxN || W > kMaxN) return 0;
+    const size_t pieces = max_pieces(N_T);
+    if (pieces <= 1) return 0;
+    const size_t n = (size_t)((H + N_T - 1) / N_T) * (size_t)((W + N_T - 1) / N_T);
+    return n * pieces * sizeof(float4);
+}
+
+int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long pitch_x, long long pitch_y, int N_T,
+                       float C1, float C2, float C, float D,
+                       float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                       float* lisi_num, float* auglisi_num,
+                       void* workspace, size_t workspace_bytes, void* stream) {
+    if (!x || !y || !lisi || !auglisi || !sum_x || !sum_y) return IQA_ERR_NULL;
+    if (H <= 0 || W <= 0 || N_T <= 0 || H > kMaxN || W > kMaxN || pitch_x < W || pitch_y < W) return IQA_ERR_SHAPE;
+    const long long ntx = (W + N_T - 1) / N_T, nty = (H + N_T - 1) / N_T;
+    if (ntx * nty > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    if (!pos_finite(C1) || !pos_finite(C2) || !pos_finite(C) || !std::isfinite(D)) return IQA_ERR_PARAM;
+    const uintptr_t bits = (uintptr_t)x | (uintptr_t)y;
+    if (bits & 3u) return IQA_ERR_ALIGN;
+    const size_t need = iqa_workspace_bytes_2d(H, W, N_T);
+    if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
+    if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
+
+    const Geom2D g2{H, W, pitch_x, pitch_y};
+    const bool aligned16 = ((bits & 15u) == 0) && (pitch_x % 4 == 0) && (pitch_y % 4 == 0);
+    const Plan pl = make_plan(W, N_T, aligned16, x, false, &g2);
+    cudaStream_t st = (cudaStream_t)stream;
+    float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
+    const Outputs out{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
+    const Consts k{C1, C2, C, D};
+    if (const int rc = launch_pairs(kModeFused, &x, &y, 1, W, N_T, k, out, ws, pl, st, &g2)) return rc;
+    return finish_comparisons(out, nullptr, 1, ntx * nty, k, ws, pl, st);
 }
 
 int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,

@@ -68,12 +68,12 @@ struct TmaParams {
     CUtensorMap maps[kMaxImages];   // image i of group g is maps[g * M + i]; box 128 x 32, OOB -> 0
     int n_groups;
     int M;               // images per group (2 for pairs)
-    int N;               // image side
+    int W, H;            // image width and height in pixels (the square API passes N, N)
     int log2_nt;         // log2(N_T), N_T a power of two >= 8
-    int nt;              // tiles per side
-    int n_tiles;         // nt * nt
-    int units_x;         // items across: ceil(N / 128)
-    int units_y;         // items down:   ceil(N / R)
+    int ntx;             // tiles per row: ceil(W / N_T)
+    int n_tiles;         // ntx * ceil(H / N_T)
+    int units_x;         // items across: ceil(W / 128), or the full tile grid when tiles are split
+    int units_y;         // items down:   ceil(H / R),   or the full tile grid when tiles are split
     int S;               // boxes (stages) per item and image: R = S * box rows
     float C1, C2, C, D;
     float* lisi;         // [n_groups * (M-1) * n_tiles] or nullptr; comparison c = g (M-1) + k
@@ -255,13 +255,15 @@ __device__ __forceinline__ void finalise_item(const TmaParams& p, const float4 (
         const int jx = t & ((1 << log2_tpw) - 1);
         const int c0 = ux * kUnitCols + (jx << log2_nt);          // jx == 0 when N_T >= 128
         const int r0 = uy * R + (jy << log2_nt);                  // jy == 0 unless N_T < box rows
-        if (c0 < p.N && r0 < p.N) {
+        // split tiles: the items cover the whole tile grid and EVERY piece is written (a piece outside the
+        // image is all zeros); otherwise tiles that start outside the image do not exist
+        if (p.ws != nullptr || (c0 < p.W && r0 < p.H)) {
             float4 s = part[jy * wpt][jx];
             for (int k = 1; k < wpt; ++k) {
                 const float4 u = part[jy * wpt + k][jx];
                 s.x += u.x; s.y += u.y; s.z += u.z; s.w += u.w;
             }
-            const size_t tile = (size_t)cmp * p.n_tiles + (size_t)(r0 >> log2_nt) * p.nt + (c0 >> log2_nt);
+            const size_t tile = (size_t)cmp * p.n_tiles + (size_t)(r0 >> log2_nt) * p.ntx + (c0 >> log2_nt);
             if (p.ws == nullptr) {
                 finalise_tile(p, tile, s);                        // S4: Eq. 1 / Eq. 2
             } else {                                              // split tile: piece -> workspace

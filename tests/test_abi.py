@@ -174,6 +174,23 @@ def test_series_and_candidate_validation():
     assert B.iqa_tiles_below(FAKE, 16, 1, math.nan, FAKE, 16, FAKE) == B.IQA_ERR_PARAM
 
 
+def test_2d_validation():
+    a = (1e-6, 1e-6, 1e-6, 5e-7)
+    o = (FAKE, FAKE, FAKE, FAKE)
+    assert B.iqa_fused_tiles_2d(None, FAKE, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_NULL
+    assert B.iqa_fused_tiles_2d(FAKE, FAKE, 64, 64, 64, 64, 8, *a, FAKE, FAKE, FAKE, None) == B.IQA_ERR_NULL
+    assert B.iqa_fused_tiles_2d(FAKE, FAKE, 64, 64, 63, 64, 8, *a, *o) == B.IQA_ERR_SHAPE      # pitch < W
+    assert B.iqa_fused_tiles_2d(FAKE, FAKE, 64, 0, 64, 64, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_fused_tiles_2d(FAKE, FAKE, 64, 64, 64, 64, 0, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_fused_tiles_2d(FAKE, FAKE, 64, 64, 64, 64, 8, 1e-6, -1.0, 1e-6, 5e-7, *o) == B.IQA_ERR_PARAM
+    assert B.iqa_fused_tiles_2d(FAKE + 2, FAKE, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_ALIGN
+    assert B.iqa_fused_tiles_2d(FAKE, FAKE, 100, 300, 300, 300, 128, *a, *o) == B.IQA_ERR_WORKSPACE
+    assert B.iqa_workspace_bytes_2d(100, 300, 128) == 1 * 3 * 2 * 16
+    assert B.iqa_workspace_bytes_2d(100, 300, 64) == 0 and B.iqa_workspace_bytes_2d(0, 300, 128) == 0
+    # the square entry points keep the paper's divisibility requirement
+    assert B.iqa_fused_tiles(FAKE, FAKE, 100, 64, *a, *o) == B.IQA_ERR_SHAPE
+
+
 def test_convenience_wrappers_refuse_cpu_tensors():
     """No CPU fallback: the product path fails loudly on host tensors."""
     torch = pytest.importorskip("torch")

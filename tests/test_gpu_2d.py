@@ -1,0 +1,119 @@
+"""-m gpu parity tests of iqa_fused_tiles_2d (H x W, row pitch, edge tiles) against
+oracle.tiles_2d, element by element on the same seeded buffers, through the C ABI.  Tolerance: that of
+the square path (tests/gpu_util.py)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2501_10653_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def U():
+    import gpu_util
+    return gpu_util
+
+
+K = dict(C1=1e-6, C2=1e-6, C=1e-6, D=5e-7)
+
+
+def _pair(H, W, seed):
+    rng = np.random.default_rng(seed)
+    x = rng.normal(0.05, 0.2, (H, W)).astype(np.float32)
+    y = rng.normal(0.05, 0.2, (H, W)).astype(np.float32)
+    m = rng.random((H, W)) < 0.3
+    y[m] = x[m]
+    return x, y
+
+
+def _window(a, pitch, off):
+    """Device copy of `a` as a window of a wider buffer: row pitch `pitch` elements, first element `off`
+    elements into the allocation (controls the alignment of the base pointer)."""
+    import torch
+    H, W = a.shape
+    buf = torch.full((H * pitch + off + 16,), float("nan"), dtype=torch.float32, device="cuda")   # NaN around the window
+    view = torch.as_strided(buf, (H, W), (pitch, 1), off)
+    view.copy_(torch.from_numpy(a))
+    return view
+
+
+def _check(B, U, x, y, xd, yd, N_T, what):
+    import torch
+    import oracle
+    got = B.fused_tiles_2d(xd, yd, N_T, K["C1"], K["C2"], K["C"], K["D"], numerators=True)
+    torch.cuda.synchronize()
+    g = {n: v.cpu().numpy().astype(np.float64) for n, v in got.items()}
+    ref = oracle.tiles_2d(x, y, N_T, **K)
+    U.assert_parity(g, ref, K["C"], what)
+    # Eqs. 3-4 over the edge-tiled matrices == the oracle's aggregate
+    agg = B.aggregate(got["lisi"], got["auglisi"], got["X"], got["Y"], K["C2"], K["C"]).cpu().numpy()
+    exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], K["C2"], K["C"])
+    assert abs(agg[0] - exp[0]) <= 1e-5 * abs(exp[0]) and abs(agg[1] - exp[1]) <= 1e-5 * abs(exp[1]) + 1e-6
+    return g
+
+
+@pytest.mark.parametrize("H,W,N_T,pitch", [
+    (100, 130, 16, 132), (257, 513, 64, 516), (64, 64, 8, 64), (300, 300, 256, 300), (1000, 40, 32, 40),
+    (513, 1027, 128, 1028), (33, 1500, 8, 1504), (700, 129, 512, 132), (2048, 2048, 64, 2048),
+    (31, 31, 32, 32), (1, 4, 8, 4), (200, 1234, 64, 1236)])
+def test_tma_path_shapes(B, U, H, W, N_T, pitch):
+    """16-byte aligned windows, pitch % 4 == 0, power-of-two N_T: the TMA kernel; W need not be a multiple of 4;
+    edge tiles right and bottom; split tiles with pieces wholly outside the image (700 x 129, N_T = 512)."""
+    x, y = _pair(H, W, H + W)
+    xd, yd = _window(x, pitch, 0), _window(y, pitch + 4, 8)          # different pitches for x and y
+    assert xd.data_ptr() % 16 == 0 and yd.data_ptr() % 16 == 0
+    _check(B, U, x, y, xd, yd, N_T, f"tma {H}x{W} N_T={N_T}")
+
+
+@pytest.mark.parametrize("H,W,N_T,pitch,off", [
+    (100, 130, 16, 131, 0), (257, 300, 64, 300, 1), (90, 70, 20, 72, 0), (300, 200, 150, 200, 0),
+    (64, 64, 7, 67, 3)])
+def test_generic_path_shapes(B, U, H, W, N_T, pitch, off):
+    """Odd pitches, unaligned bases, tile sides that are not powers of two: the generic kernel."""
+    x, y = _pair(H, W, H * 3 + W)
+    xd, yd = _window(x, pitch, off), _window(y, pitch, off + 1)
+    _check(B, U, x, y, xd, yd, N_T, f"generic {H}x{W} N_T={N_T}")
+
+
+def test_2d_equals_square_entry_point_bitwise(B, U):
+    """On a square, contiguous, divisible image the 2-D entry point runs the same kernel: bit-identical."""
+    import torch
+    x, y = _pair(512, 512, 9)
+    xd, yd = U.to_dev(x), U.to_dev(y)
+    for N_T in (16, 64, 256):
+        a = B.fused_tiles(xd, yd, N_T, K["C1"], K["C2"], K["C"], K["D"], numerators=True)
+        b = B.fused_tiles_2d(xd, yd, N_T, K["C1"], K["C2"], K["C"], K["D"], numerators=True)
+        torch.cuda.synchronize()
+        for n in a:
+            assert torch.equal(a[n], b[n]), (N_T, n)
+
+
+def test_window_of_a_config1_sky(B, U):
+    """A 1000 x 1500 window cut out of a BASELINE.json config [1] sky (row pitch 2048), N_T = 64."""
+    from paper_2501_10653_b200 import synth
+    cfg = synth.CONFIGS[1]
+    x, y, _ = synth.make_pair(cfg)
+    xd, yd = U.to_dev(x), U.to_dev(y)
+    r0, c0 = 512, 256                                          # 16-byte aligned window origin
+    _check(B, U, x[r0:r0 + 1000, c0:c0 + 1500], y[r0:r0 + 1000, c0:c0 + 1500],
+           xd[r0:r0 + 1000, c0:c0 + 1500], yd[r0:r0 + 1000, c0:c0 + 1500], 64, "cfg1 window")
+
+
+def test_2d_error_codes(B):
+    import torch
+    x = torch.zeros((64, 64), dtype=torch.float32, device="cuda")
+    o = [torch.zeros(64, dtype=torch.float32, device="cuda") for _ in range(4)]
+    a = (K["C1"], K["C2"], K["C"], K["D"])
+    assert B.iqa_fused_tiles_2d(x, x, 64, 64, 64, 64, 8, *a, *o) == B.IQA_OK
+    assert B.iqa_fused_tiles_2d(x, x, 64, 64, 63, 64, 8, *a, *o) == B.IQA_ERR_SHAPE      # pitch < W
+    assert B.iqa_fused_tiles_2d(x, x, 0, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_fused_tiles_2d(x, None, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_NULL
+    assert B.iqa_fused_tiles_2d(x, x, 64, 64, 64, 64, 8, 0.0, K["C2"], K["C"], K["D"], *o) == B.IQA_ERR_PARAM
+    assert B.iqa_fused_tiles_2d(x, x, 64, 64, 64, 64, 128, *a, *o) == B.IQA_ERR_WORKSPACE
+    assert B.iqa_workspace_bytes_2d(65, 130, 128) == 2 * 2 * 16 and B.iqa_workspace_bytes_2d(65, 130, 64) == 0
+    torch.cuda.synchronize()
