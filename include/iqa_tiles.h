@@ -182,6 +182,22 @@ int iqa_aggregate(const float* lisi, const float* auglisi,
                   float C2, float C,
                   float* out2, void* stream);
 
+/* ---- one image pair sharded over GPUs by bands of tile rows -------------------
+ * Tiles are independent, so rank r computes the tiles of its band of rows with
+ * iqa_fused_tiles_2d (a band is a contiguous range of rows: H = rows of the band, same pitch) and
+ * nothing is exchanged for the matrices.  Only the whole-image pair of Eqs. 3-4 needs the other
+ * bands: every rank reduces ITS tiles to four double sums with iqa_aggregate_partial,
+ *   sums4 = { sum_t lisi_t (max(X_t, Y_t) + C2),  sum_t auglisi_t (X_t + Y_t + C),  sum_t X_t,  sum_t Y_t },
+ * the ranks all-reduce (sum) these 32 bytes (NCCL), and iqa_aggregate_finish applies
+ *   LISI = sums4[0] / (max(sums4[2], sums4[3]) + C2),
+ *   augLISI = (sums4[1] - (n_tiles_total - 1) C) / (sums4[2] + sums4[3] + C)            (Eqs. 3-4).
+ * sums4: DEVICE double[4], 8-byte aligned. */
+int iqa_aggregate_partial(const float* lisi, const float* auglisi,
+                          const float* sum_x, const float* sum_y, int n_tiles,
+                          float C2, float C, double* sums4, void* stream);
+int iqa_aggregate_finish(const double* sums4, long long n_tiles_total, float C2, float C,
+                         float* out2, void* stream);
+
 /* ---- candidate extraction ------------------------------------------------
  * The finder's output: which tiles changed.  The paper gives no decision rule -- it shows the
  * matrices (Fig. 3) and says augLISI localises "transients to tiles with fewer false positives"

@@ -25,7 +25,7 @@ IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKS
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
            "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
-           "iqa_aggregate", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host")
+           "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
 SERIES_MODES = {"reference": IQA_SERIES_REFERENCE, "consecutive": IQA_SERIES_CONSECUTIVE}
@@ -75,6 +75,10 @@ def _load() -> ctypes.CDLL:
     lib.iqa_fused_tiles_2d.restype = i
     lib.iqa_fused_tiles_2d.argtypes = [vp, vp, i, i, ctypes.c_longlong, ctypes.c_longlong, i, f, f, f, f,
                                        vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_aggregate_partial.restype = i
+    lib.iqa_aggregate_partial.argtypes = [vp, vp, vp, vp, i, f, f, vp, vp]
+    lib.iqa_aggregate_finish.restype = i
+    lib.iqa_aggregate_finish.argtypes = [vp, ctypes.c_longlong, f, f, vp, vp]
     lib.iqa_tiles_below.restype = i
     lib.iqa_tiles_below.argtypes = [vp, i, i, f, vp, i, vp, vp]
     lib.iqa_tiles_bottom_k.restype = i
@@ -220,6 +224,15 @@ def iqa_tiles_bottom_k(values, n_tiles, n_maps, k, indices, vals=None, stream=No
 def iqa_aggregate(lisi, auglisi, sum_x, sum_y, n_tiles, C2, C, out2, stream=None) -> int:
     return lib.iqa_aggregate(_ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), int(n_tiles),
                              C2, C, _ptr(out2), _stream(stream))
+
+
+def iqa_aggregate_partial(lisi, auglisi, sum_x, sum_y, n_tiles, C2, C, sums4, stream=None) -> int:
+    return lib.iqa_aggregate_partial(_ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), int(n_tiles),
+                                     C2, C, _ptr(sums4), _stream(stream))
+
+
+def iqa_aggregate_finish(sums4, n_tiles_total, C2, C, out2, stream=None) -> int:
+    return lib.iqa_aggregate_finish(_ptr(sums4), int(n_tiles_total), C2, C, _ptr(out2), _stream(stream))
 
 
 def iqa_merge_tiles(lisi, auglisi, sum_x, sum_y, nt, g, C2, C,
@@ -445,6 +458,26 @@ def aggregate(lisi, auglisi, X, Y, C2, C, out2=None):
     rc = iqa_aggregate(lisi, auglisi, X, Y, n, C2, C, out2, _current_stream(lisi.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_aggregate")
+    return out2
+
+
+def aggregate_partial(lisi, auglisi, X, Y, C2, C):
+    """The four double sums of Eqs. 3-4 over the given tiles (one band of a sharded image) -> float64 CUDA tensor [4]."""
+    import torch
+    sums4 = torch.empty(4, dtype=torch.float64, device=lisi.device)
+    rc = iqa_aggregate_partial(lisi, auglisi, X, Y, lisi.numel(), C2, C, sums4, _current_stream(lisi.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_aggregate_partial")
+    return sums4
+
+
+def aggregate_finish(sums4, n_tiles_total, C2, C):
+    """Eqs. 3-4 from the all-reduced sums of every band -> float32 CUDA tensor [LISI, augLISI]."""
+    import torch
+    out2 = torch.empty(2, dtype=torch.float32, device=sums4.device)
+    rc = iqa_aggregate_finish(sums4, n_tiles_total, C2, C, out2, _current_stream(sums4.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_aggregate_finish")
     return out2
 
 

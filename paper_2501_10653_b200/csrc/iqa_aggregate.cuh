@@ -64,7 +64,7 @@ constexpr int kAggUnroll = 4;
 __global__ void __launch_bounds__(kAggThreads)
 aggregate_kernel(const float* __restrict__ lisi, const float* __restrict__ aug,
                  const float* __restrict__ X, const float* __restrict__ Y, int n,
-                 float C2f, float Cf, float* __restrict__ out2) {
+                 float C2f, float Cf, float* __restrict__ out2, double* __restrict__ sums4) {
     namespace cg = cooperative_groups;
     __shared__ Agg4 part[kAggThreads / 32];
     __shared__ Agg4 cta_part;
@@ -74,7 +74,7 @@ aggregate_kernel(const float* __restrict__ lisi, const float* __restrict__ aug,
     const int csize = (int)cluster.num_blocks();              // launch attribute: agg_cluster_size(n)
     const size_t pair = blockIdx.x / csize;
     const size_t base = pair * (size_t)n;
-    lisi += base; aug += base; X += base; Y += base; out2 += 2 * pair;
+    lisi += base; aug += base; X += base; Y += base;
     const double C2 = (double)C2f, C = (double)Cf;
     Agg4 a = {0.0, 0.0, 0.0, 0.0};
     // this CTA's element range; a multiple of 4 long so the 128-bit groups never straddle ranks
@@ -122,9 +122,24 @@ aggregate_kernel(const float* __restrict__ lisi, const float* __restrict__ aug,
             const Agg4* q = cluster.map_shared_rank(&cta_part, r);
             s.n3 += q->n3; s.n4 += q->n4; s.sx += q->sx; s.sy += q->sy;
         }
-        agg_finish(s, (double)n, C2, C, out2, out2 + 1);
+        if (out2) agg_finish(s, (double)n, C2, C, out2 + 2 * pair, out2 + 2 * pair + 1);
+        if (sums4) {                                          // raw sums of Eqs. 3-4 (a band of a sharded image)
+            double* q4 = sums4 + 4 * pair;
+            q4[0] = s.n3; q4[1] = s.n4; q4[2] = s.sx; q4[3] = s.sy;
+        }
     }
     cluster.sync();                                           // nobody exits while CTA 0 reads its shared memory
+}
+
+// Eqs. 3-4 from the (all-reduced) sums of all bands: sums4 = {sum lisi_t (max(X_t,Y_t)+C2),
+// sum auglisi_t (X_t+Y_t+C), sum X_t, sum Y_t} over the n tiles of the whole image.
+__global__ void aggregate_finish_kernel(const double* __restrict__ sums4, double n, float C2f, float Cf,
+                                        float* __restrict__ out2) {
+    pdl_prologue();
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        const Agg4 s = {sums4[0], sums4[1], sums4[2], sums4[3]};
+        agg_finish(s, n, (double)C2f, (double)Cf, out2, out2 + 1);
+    }
 }
 
 // P:66 merge: one warp per output tile; lanes stride over the g*g input tiles (row-major

@@ -437,7 +437,7 @@ int finish_comparisons(const Outputs& out, float* out2, int n_cmp, long long n, 
         const unsigned cs = (unsigned)agg_cluster_size(n);
         if (launch_cluster(aggregate_kernel, (unsigned)n_cmp * cs, kAggThreads, 0, st, cs,
                    (const float*)out.lisi, (const float*)out.auglisi, (const float*)out.sum_x,
-                   (const float*)out.sum_y, (int)n, k.C2, k.C, out2) != cudaSuccess)
+                   (const float*)out.sum_y, (int)n, k.C2, k.C, out2, (double*)nullptr) != cudaSuccess)
             return IQA_ERR_CUDA;
     }
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
@@ -663,7 +663,32 @@ int iqa_aggregate(const float* lisi, const float* auglisi,
     if (!pos_finite(C2) || !pos_finite(C)) return IQA_ERR_PARAM;
     const unsigned cs = (unsigned)agg_cluster_size(n_tiles);
     if (launch_cluster(aggregate_kernel, cs, kAggThreads, 0, (cudaStream_t)stream, cs, lisi, auglisi, sum_x, sum_y,
-               n_tiles, C2, C, out2) != cudaSuccess)
+               n_tiles, C2, C, out2, (double*)nullptr) != cudaSuccess)
+        return IQA_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+}
+
+int iqa_aggregate_partial(const float* lisi, const float* auglisi,
+                          const float* sum_x, const float* sum_y, int n_tiles,
+                          float C2, float C, double* sums4, void* stream) {
+    if (!lisi || !auglisi || !sum_x || !sum_y || !sums4) return IQA_ERR_NULL;
+    if (n_tiles <= 0) return IQA_ERR_SHAPE;
+    if (!pos_finite(C2) || !pos_finite(C)) return IQA_ERR_PARAM;
+    if ((uintptr_t)sums4 & 7u) return IQA_ERR_ALIGN;
+    const unsigned cs = (unsigned)agg_cluster_size(n_tiles);
+    if (launch_cluster(aggregate_kernel, cs, kAggThreads, 0, (cudaStream_t)stream, cs, lisi, auglisi, sum_x, sum_y,
+               n_tiles, C2, C, (float*)nullptr, sums4) != cudaSuccess)
+        return IQA_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+}
+
+int iqa_aggregate_finish(const double* sums4, long long n_tiles_total, float C2, float C, float* out2, void* stream) {
+    if (!sums4 || !out2) return IQA_ERR_NULL;
+    if (n_tiles_total <= 0) return IQA_ERR_SHAPE;
+    if (!pos_finite(C2) || !pos_finite(C)) return IQA_ERR_PARAM;
+    if ((uintptr_t)sums4 & 7u) return IQA_ERR_ALIGN;
+    if (launch(aggregate_finish_kernel, 1u, 32u, 0, (cudaStream_t)stream, sums4, (double)n_tiles_total, C2, C, out2) !=
+        cudaSuccess)
         return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }

@@ -57,3 +57,43 @@ def gather_whole(whole_local, dist=None):
     parts = [torch.empty_like(whole_local) for _ in range(dist.get_world_size())]
     dist.all_gather(parts, whole_local.contiguous())
     return torch.cat(parts, dim=0)
+
+
+# ----------------------------------------------------------------------------- one pair over several GPUs
+def band_rows(H: int, N_T: int, rank: int, world: int) -> tuple:
+    """Rows [r0, r1) of an H-row image that ``rank`` owns when ONE pair is sharded over ``world`` GPUs
+    (SURVEY.md 8(e)): contiguous bands of whole tile rows (a band is one contiguous byte range of a
+    row-major image, no halo), balanced to within one tile row; the last band takes the ragged rest."""
+    if world <= 0 or not 0 <= rank < world or H <= 0 or N_T <= 0:
+        raise ValueError("bad (H, N_T, rank, world)")
+    nty = -(-H // N_T)
+    tr = pair_range(nty, rank, world)                    # tile rows of this rank
+    return min(H, tr.start * N_T), min(H, tr.stop * N_T)
+
+
+def banded_pair(binding, x_band, y_band, n_tiles_total: int, N_T: int, C1, C2, C, D, dist=None) -> dict:
+    """One rank's share of ONE image pair sharded by bands of tile rows: Eqs. 1-2 for the tiles of the band
+    (``iqa_fused_tiles_2d``; no exchange), then the whole-image pair of Eqs. 3-4 through ONE all-reduce of
+    four doubles (``iqa_aggregate_partial`` -> ``dist.all_reduce`` -> ``iqa_aggregate_finish``).
+    x_band, y_band: this rank's rows (CUDA tensors, possibly empty when there are more ranks than tile
+    rows).  Returns the band's matrices plus ``whole`` = [LISI, augLISI] of the ENTIRE image on every rank."""
+    import torch
+    dev = x_band.device
+    if x_band.shape[0] > 0:
+        out = binding.fused_tiles_2d(x_band, y_band, N_T, C1, C2, C, D)
+        sums4 = binding.aggregate_partial(out["lisi"], out["auglisi"], out["X"], out["Y"], C2, C)
+    else:
+        out = {k: torch.empty((0, -(-x_band.shape[1] // N_T)), dtype=torch.float32, device=dev)
+               for k in ("lisi", "auglisi", "X", "Y")}
+        sums4 = torch.zeros(4, dtype=torch.float64, device=dev)
+    sums4 = allreduce_sums(sums4, dist)
+    out["whole"] = binding.aggregate_finish(sums4, n_tiles_total, C2, C)
+    return out
+
+
+def allreduce_sums(sums4, dist=None):
+    """Sum of the per-band partial sums of Eqs. 3-4 over all ranks (32 bytes; the path's only exchange)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return sums4
+    dist.all_reduce(sums4, op=dist.ReduceOp.SUM)
+    return sums4

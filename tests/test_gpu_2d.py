@@ -117,3 +117,37 @@ def test_2d_error_codes(B):
     assert B.iqa_fused_tiles_2d(x, x, 64, 64, 64, 64, 128, *a, *o) == B.IQA_ERR_WORKSPACE
     assert B.iqa_workspace_bytes_2d(65, 130, 128) == 2 * 2 * 16 and B.iqa_workspace_bytes_2d(65, 130, 64) == 0
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("world", [1, 2, 3, 5])
+def test_one_pair_sharded_by_bands_of_tile_rows(B, U, world):
+    """`world` ranks each take a band of tile rows of ONE pair (run one after the other on
+    this GPU -- no kernel waits on another), reduce it with iqa_aggregate_partial, the partial sums are
+    added (the all-reduce), iqa_aggregate_finish gives the whole-image pair; bands stacked == the full matrices."""
+    import torch
+    import oracle
+    from paper_2501_10653_b200 import shard
+    H, W, N_T = 1000, 1536, 64
+    x, y = _pair(H, W, 77)
+    xd, yd = U.to_dev(x), U.to_dev(y)
+    ref = oracle.tiles_2d(x, y, N_T, **K)
+    n_total = ref["lisi"].size
+    total = torch.zeros(4, dtype=torch.float64, device="cuda")
+    stacked = {n: [] for n in ("lisi", "auglisi", "X", "Y")}
+    for rank in range(world):
+        r0, r1 = shard.band_rows(H, N_T, rank, world)
+        out = shard.banded_pair(B, xd[r0:r1], yd[r0:r1], n_total, N_T, K["C1"], K["C2"], K["C"], K["D"], dist=None)
+        part = B.aggregate_partial(out["lisi"], out["auglisi"], out["X"], out["Y"], K["C2"], K["C"])
+        total += part
+        for n in stacked:
+            stacked[n].append(out[n])
+    whole = B.aggregate_finish(total, n_total, K["C2"], K["C"]).cpu().numpy().astype(np.float64)
+    got = {n: torch.cat(v, dim=0).cpu().numpy().astype(np.float64) for n, v in stacked.items()}
+    U.assert_parity(got, ref, K["C"], f"bands world={world}")
+    exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], K["C2"], K["C"])
+    assert abs(whole[0] - exp[0]) <= 1e-5 * abs(exp[0]) and abs(whole[1] - exp[1]) <= 1e-5 * abs(exp[1]) + 1e-6
+    # the partial sums themselves: against the oracle's per-tile values (double)
+    c2, c = float(np.float32(K["C2"])), float(np.float32(K["C"]))
+    e4 = np.array([np.sum(ref["lisi"] * (np.maximum(ref["X"], ref["Y"]) + c2)),
+                   np.sum(ref["auglisi"] * (ref["X"] + ref["Y"] + c)), np.sum(ref["X"]), np.sum(ref["Y"])])
+    assert np.all(np.abs(total.cpu().numpy() - e4) <= 1e-5 * np.abs(e4))

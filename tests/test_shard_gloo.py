@@ -80,3 +80,75 @@ def test_two_ranks_gloo():
     assert abs(j0["us_per_unit"] - 62.5) < 1e-9
     assert m0 == [0, 1, 2] and m1 == [3, 4]                    # disjoint, ordered, complete
     assert w0 == w1 == [[0.0, 0.0], [1.0, 10.0], [2.0, 20.0], [3.0, 30.0]]
+
+
+# ----------------------------------------------------------------------------- one pair over several ranks
+def test_band_rows_partition_the_image():
+    for H, N_T in ((2048, 64), (100, 16), (65, 64), (7, 8), (1000, 128)):
+        for world in (1, 2, 3, 8):
+            bands = [shard.band_rows(H, N_T, r, world) for r in range(world)]
+            assert bands[0][0] == 0 and bands[-1][1] == H
+            for (a0, a1), (b0, b1) in zip(bands, bands[1:]):
+                assert a1 == b0 and a0 <= a1
+            for r0, r1 in bands:
+                if r1 > r0:                                    # more ranks than tile rows: trailing bands are empty
+                    assert r0 % N_T == 0 and (r1 % N_T == 0 or r1 == H)
+            rows = [(r1 - r0 + N_T - 1) // N_T for r0, r1 in bands]
+            assert max(rows) - min(rows) <= 1
+    with pytest.raises(ValueError):
+        shard.band_rows(64, 8, 2, 2)
+
+
+def _band_worker(rank, world, port, q):
+    """Each rank reduces ITS band of tile rows (per-tile values from the oracle: this test is about the
+    host logic, not the kernels) to the four sums of Eqs. 3-4; one all-reduce; every rank finishes."""
+    import numpy as np
+    import torch.distributed as dist
+    import oracle
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        rng = np.random.default_rng(0)                         # the same image on every rank
+        x = rng.random((100, 72)).astype(np.float32)
+        y = rng.random((100, 72)).astype(np.float32)
+        N_T, C2, C = 16, 1e-6, 1e-6
+        r0, r1 = shard.band_rows(100, N_T, rank, world)
+        t = oracle.tiles_2d(x[r0:r1], y[r0:r1], N_T, 1e-6, C2, C, 5e-7)
+        c2, c = float(np.float32(C2)), float(np.float32(C))
+        sums4 = torch.tensor([np.sum(t["lisi"] * (np.maximum(t["X"], t["Y"]) + c2)),
+                              np.sum(t["auglisi"] * (t["X"] + t["Y"] + c)), np.sum(t["X"]), np.sum(t["Y"])],
+                             dtype=torch.float64)
+        total = shard.allreduce_sums(sums4, dist)
+        q.put((rank, (r0, r1), t["lisi"].shape, total.tolist()))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_ranks_share_one_pair_by_bands():
+    import numpy as np
+    import torch.multiprocessing as mp
+    import oracle
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_band_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    (_, b0, s0, t0), (_, b1, s1, t1) = res
+    assert b0 == (0, 64) and b1 == (64, 100)                  # 7 tile rows: 4 + 3 (the last one ragged)
+    assert s0 == (4, 5) and s1 == (3, 5)
+    assert t0 == t1                                            # every rank holds the same all-reduced sums
+    rng = np.random.default_rng(0)
+    x = rng.random((100, 72)).astype(np.float32)
+    y = rng.random((100, 72)).astype(np.float32)
+    full = oracle.tiles_2d(x, y, 16, 1e-6, 1e-6, 1e-6, 5e-7)
+    exp = oracle.aggregate(full["lisi"], full["auglisi"], full["X"], full["Y"], 1e-6, 1e-6)
+    c2 = c = float(np.float32(1e-6))
+    n = full["lisi"].size
+    lisi = t0[0] / (max(t0[2], t0[3]) + c2)                    # Eq. 3 from the summed partials
+    aug = (t0[1] - (n - 1) * c) / (t0[2] + t0[3] + c)          # Eq. 4
+    assert abs(lisi - exp[0]) <= 1e-12 * abs(exp[0]) and abs(aug - exp[1]) <= 1e-12 * abs(exp[1])
