@@ -246,6 +246,17 @@ int iqa_fused_host(const float* x_host, const float* y_host, int N, int N_T,
                    float* sum_x_host, float* sum_y_host, float* out2_host,
                    void* dev_scratch, size_t dev_scratch_bytes, void* stream);
 
+/* The same, WITHOUT the final synchronisation: everything (both uploads, the kernels, the downloads) is
+ * enqueued on `stream` and the call returns; the host outputs are valid, and x_host / y_host / dev_scratch
+ * may be reused, once the caller has synchronised the stream.  With pinned host memory and two streams
+ * (two scratch blocks) the upload of the next pair overlaps the kernels, downloads and launch gaps of
+ * this one, which keeps the PCIe link busy (binding.HostPipeline; what bench.py times as `e2e`). */
+int iqa_fused_host_async(const float* x_host, const float* y_host, int N, int N_T,
+                         float C1, float C2, float C, float D,
+                         float* lisi_host, float* auglisi_host,
+                         float* sum_x_host, float* sum_y_host, float* out2_host,
+                         void* dev_scratch, size_t dev_scratch_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -25,7 +25,7 @@ IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKS
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
            "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
-           "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host")
+           "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
 SERIES_MODES = {"reference": IQA_SERIES_REFERENCE, "consecutive": IQA_SERIES_CONSECUTIVE}
@@ -89,6 +89,8 @@ def _load() -> ctypes.CDLL:
     lib.iqa_merge_tiles.argtypes = [vp, vp, vp, vp, i, i, f, f, vp, vp, vp, vp, vp]
     lib.iqa_fused_host.restype = i
     lib.iqa_fused_host.argtypes = [vp, vp, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_fused_host_async.restype = i
+    lib.iqa_fused_host_async.argtypes = [vp, vp, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, sz, vp]
     return lib
 
 
@@ -247,6 +249,13 @@ def iqa_fused_host(x_host, y_host, N, N_T, C1, C2, C, D, lisi_host, auglisi_host
     return lib.iqa_fused_host(_ptr(x_host), _ptr(y_host), int(N), int(N_T), C1, C2, C, D,
                               _ptr(lisi_host), _ptr(auglisi_host), _ptr(sum_x_host), _ptr(sum_y_host),
                               _ptr(out2_host), _ptr(dev_scratch), int(dev_scratch_bytes), _stream(stream))
+
+
+def iqa_fused_host_async(x_host, y_host, N, N_T, C1, C2, C, D, lisi_host, auglisi_host,
+                         sum_x_host, sum_y_host, out2_host, dev_scratch, dev_scratch_bytes, stream=None) -> int:
+    return lib.iqa_fused_host_async(_ptr(x_host), _ptr(y_host), int(N), int(N_T), C1, C2, C, D,
+                                    _ptr(lisi_host), _ptr(auglisi_host), _ptr(sum_x_host), _ptr(sum_y_host),
+                                    _ptr(out2_host), _ptr(dev_scratch), int(dev_scratch_bytes), _stream(stream))
 
 
 # ----------------------------------------------------------------------------- convenience
@@ -538,6 +547,38 @@ class HostRunner:
         if rc != IQA_OK:
             raise IqaError(rc, "iqa_fused_host")
         return self.out, self.out2
+
+
+class HostPipeline:
+    """``depth`` HostRunners on ``depth`` streams: ``submit`` enqueues one host pair with
+    ``iqa_fused_host_async`` on the next stream (after waiting for that stream's previous pair) and returns
+    the slot whose pinned outputs will hold the result; ``wait(slot)`` / ``drain()`` synchronise.  The upload
+    of pair i+1 overlaps the kernels, downloads and launch gaps of pair i."""
+
+    def __init__(self, N: int, N_T: int, device="cuda:0", depth: int = 2):
+        import torch
+        self.runners = [HostRunner(N, N_T, device) for _ in range(depth)]
+        self.streams = [torch.cuda.Stream(device=self.runners[0].device) for _ in range(depth)]
+        self.next = 0
+
+    def submit(self, x_host, y_host, C1, C2, C, D) -> int:
+        slot = self.next
+        self.next = (self.next + 1) % len(self.runners)
+        r, st = self.runners[slot], self.streams[slot]
+        st.synchronize()                         # the slot's previous pair is complete: its buffers are free
+        rc = iqa_fused_host_async(x_host, y_host, r.N, r.N_T, C1, C2, C, D, r.out["lisi"], r.out["auglisi"],
+                                  r.out["X"], r.out["Y"], r.out2, r.scratch, r.scratch_bytes, st)
+        if rc != IQA_OK:
+            raise IqaError(rc, "iqa_fused_host_async")
+        return slot
+
+    def wait(self, slot: int):
+        self.streams[slot].synchronize()
+        return self.runners[slot].out, self.runners[slot].out2
+
+    def drain(self):
+        for st in self.streams:
+            st.synchronize()
 
 
 def fused_host(x_host, y_host, N_T, C1, C2, C, D, device="cuda:0"):

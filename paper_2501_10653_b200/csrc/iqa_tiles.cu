@@ -341,7 +341,9 @@ int launch_tma(int mode, int series, const float* const* imgs, int n_groups, int
         p.ws = ws ? ws + cmp0 * (size_t)n * pl.pieces : nullptr;
         p.pieces_x = pl.pieces_x; p.pieces_y = pl.pieces_y;
         const long long n_items = items_per_group * ng;
-        const long long resident = (long long)geo->sms * geo->tma_ctas[pl.tma_cfg];
+        long long resident = (long long)geo->sms * geo->tma_ctas[pl.tma_cfg];
+        static const int max_ctas = env_int("IQA_TMA_MAX_CTAS", 0);     // tuning knob
+        if (max_ctas > 0 && max_ctas < resident) resident = max_ctas;
         const unsigned grid = (unsigned)(n_items < resident ? n_items : resident);
         if (launch(fn, grid, kTmaThreads, tma_smem(pl.tma_cfg), st, p) != cudaSuccess) return IQA_ERR_CUDA;
     }
@@ -740,11 +742,12 @@ size_t iqa_host_scratch_bytes(int N, int N_T) {
     return 2 * img + 4 * per_tile + 256 + align_up(workspace_bytes_for(1, N, N_T), 256);
 }
 
-int iqa_fused_host(const float* x_host, const float* y_host, int N, int N_T,
-                   float C1, float C2, float C, float D,
-                   float* lisi_host, float* auglisi_host,
-                   float* sum_x_host, float* sum_y_host, float* out2_host,
-                   void* dev_scratch, size_t dev_scratch_bytes, void* stream) {
+namespace {
+int fused_host_impl(const float* x_host, const float* y_host, int N, int N_T,
+                    float C1, float C2, float C, float D,
+                    float* lisi_host, float* auglisi_host,
+                    float* sum_x_host, float* sum_y_host, float* out2_host,
+                    void* dev_scratch, size_t dev_scratch_bytes, void* stream, bool synchronise) {
     if (!x_host || !y_host || !dev_scratch) return IQA_ERR_NULL;
     if (const int s = status_of_shape(N, N_T)) return s;
     if (!pos_finite(C1) || !pos_finite(C2) || !pos_finite(C) || !std::isfinite(D)) return IQA_ERR_PARAM;
@@ -781,8 +784,27 @@ int iqa_fused_host(const float* x_host, const float* y_host, int N, int N_T,
     if (sum_x_host && e == cudaSuccess) e = cudaMemcpyAsync(sum_x_host, d_sx, nb, cudaMemcpyDeviceToHost, st);
     if (sum_y_host && e == cudaSuccess) e = cudaMemcpyAsync(sum_y_host, d_sy, nb, cudaMemcpyDeviceToHost, st);
     if (out2_host && e == cudaSuccess) e = cudaMemcpyAsync(out2_host, d_out2, 2 * sizeof(float), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess && synchronise) e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+}
+}  // namespace
+
+int iqa_fused_host(const float* x_host, const float* y_host, int N, int N_T,
+                   float C1, float C2, float C, float D,
+                   float* lisi_host, float* auglisi_host,
+                   float* sum_x_host, float* sum_y_host, float* out2_host,
+                   void* dev_scratch, size_t dev_scratch_bytes, void* stream) {
+    return fused_host_impl(x_host, y_host, N, N_T, C1, C2, C, D, lisi_host, auglisi_host, sum_x_host, sum_y_host,
+                           out2_host, dev_scratch, dev_scratch_bytes, stream, true);
+}
+
+int iqa_fused_host_async(const float* x_host, const float* y_host, int N, int N_T,
+                         float C1, float C2, float C, float D,
+                         float* lisi_host, float* auglisi_host,
+                         float* sum_x_host, float* sum_y_host, float* out2_host,
+                         void* dev_scratch, size_t dev_scratch_bytes, void* stream) {
+    return fused_host_impl(x_host, y_host, N, N_T, C1, C2, C, D, lisi_host, auglisi_host, sum_x_host, sum_y_host,
+                           out2_host, dev_scratch, dev_scratch_bytes, stream, false);
 }
 
 }  // extern "C"

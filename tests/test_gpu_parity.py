@@ -325,6 +325,33 @@ def test_fused_host_entry_point(U, B):
     U.assert_parity({n: out_np[n].numpy().astype(np.float64) for n in out_np}, ref, k["C"], "fused_host 128")
 
 
+def test_host_pipeline_two_streams(U, B):
+    """iqa_fused_host_async on two streams (binding.HostPipeline): six distinct pairs, every result against the oracle."""
+    cfg = synth.scaled(synth.CONFIGS[1], 512)
+    k = U.consts(cfg)
+    pairs = [synth.make_pair(cfg, seed=s)[:2] for s in range(6)]
+    pinned = [(torch.from_numpy(x).pin_memory(), torch.from_numpy(y).pin_memory()) for x, y in pairs]
+    pipe = B.HostPipeline(cfg.N, cfg.N_T, "cuda:0", depth=2)
+    results, slots = [], []
+
+    def collect(slot):
+        out, out2 = pipe.wait(slot)
+        results.append(({n: v.clone() for n, v in out.items()}, out2.clone()))
+
+    for xp, yp in pinned:
+        slots.append(pipe.submit(xp, yp, k["C1"], k["C2"], k["C"], k["D"]))
+        if len(slots) > 1:
+            collect(slots[-2])
+    collect(slots[-1])
+    pipe.drain()
+    assert len(results) == 6
+    for (x, y), (out, out2) in zip(pairs, results):
+        ref = U.run_oracle(x, y, cfg.N_T, k)
+        U.assert_parity({n: out[n].numpy().astype(np.float64) for n in out}, ref, k["C"], "host pipeline")
+        exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], k["C2"], k["C"])
+        assert abs(out2[0].item() - exp[0]) <= 1e-5 * abs(exp[0]) and abs(out2[1].item() - exp[1]) <= 1e-5 * abs(exp[1])
+
+
 def test_many_small_tiles(U):
     """N=4096, N_T=8: 262144 tiles (16 tile segments per warp row)."""
     x, y = _rand_pair(4096, seed=5)
