@@ -4,8 +4,8 @@
 // PAPER.md:27; series: SURVEY.md 8(f)-2).
 //
 // Data movement is done by the Tensor Memory Accelerator: one elected thread of a producer
-// warp issues cp.async.bulk.tensor.2d (SASS UTMALDG) for BOXES of 128 columns x 32 rows
-// (16 KiB) straight into shared memory; completion is signalled on an mbarrier per box
+// warp issues cp.async.bulk.tensor.2d (SASS UTMALDG) for BOXES of 128 columns x 8 RPW rows
+// (RPW = 4: 32 rows, 16 KiB) straight into shared memory; completion is signalled on an mbarrier per box
 // ("full"), the eight consumer warps give a box back through a second mbarrier ("empty").
 // Against the per-thread cp.async ring of iqa_stream.cuh this removes every address
 // computation and 8 LDGSTS per thread and stage from the instruction stream (the cp.async
@@ -24,7 +24,7 @@
 //               kPairs        (x, y) = (I_0, I_1)
 //               kReference    (x, y) = (I_0, I_k+1)    k = 0 .. M-2
 //               kConsecutive  (x, y) = (I_k, I_k+1)
-//   item      128 columns x R rows of a group (R = 32 S; S = 1 for N_T <= 32, else 2); items
+//   item      128 columns x R rows of a group (R = S box heights; 32-row boxes: S = 1 for N_T <= 32, else 2); items
 //             are numbered group-major, then row-major over the image; CTA b takes items b,
 //             b+G, b+2G, ... (persistent grid).  For an item ALL comparisons of the group are
 //             computed before the next item, so in the series modes the x box of a comparison
@@ -35,7 +35,7 @@
 //                           comparison and, S boxes later, the x of the next
 //             kReference: I_0's S boxes live in S dedicated slots for the whole item, the
 //                           snapshots stream through a ring of kNumBoxes - S boxes
-//   consume   warp w owns rows 4w..4w+3 of a box, lane l the columns 4l..4l+3: conflict-free
+//   consume   warp w owns rows RPW w .. RPW w + RPW - 1 of a box, lane l the columns 4l..4l+3: conflict-free
 //             LDS.128, 16 fp32 accumulators per lane
 //   reduce    per item and comparison: lane -> warp (segmented reduce-scatter butterfly) ->
 //             part[buf][warp][segment] in shared memory, handed through an mbarrier to a tenth
@@ -65,7 +65,7 @@ constexpr int kPartBufs = 4;                   // per-warp partial sums in fligh
 enum : int { kPairs = 0, kReference = 1, kConsecutive = 2 };
 
 struct TmaParams {
-    CUtensorMap maps[kMaxImages];   // image i of group g is maps[g * M + i]; box 128 x 32, OOB -> 0
+    CUtensorMap maps[kMaxImages];   // image i of group g is maps[g * M + i]; box 128 x 8 RPW, OOB -> 0
     int n_groups;
     int M;               // images per group (2 for pairs)
     int W, H;            // image width and height in pixels (the square API passes N, N)
@@ -114,7 +114,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "}\n" ::"r"(bar), "r"(parity), "r"(0x989680u) /* suspend-time hint: sleep in hardware, not in a spin */
         : "memory");
 }
-// One box: 128 columns x 32 rows of the image described by `map`, top-left (col, row), -> dst.
+// One box (128 columns x 8 RPW rows, fixed by the tensor map) of the image described by `map`, top-left (col, row), -> dst.
 __device__ __forceinline__ void tma_load_box(uint32_t dst, const CUtensorMap* map, int col, int row, uint32_t bar) {
     asm volatile(
         "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
