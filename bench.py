@@ -259,6 +259,20 @@ def time_region(torch, fn, steps, dist=None):
     return ms
 
 
+def step_distribution(torch, fn, steps):
+    """Per-step device times (one CUDA event pair per step, same stream): median / min / p90 in us --
+    the statistic of the paper's own measurement (median of 10 runs) beside the mean."""
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    torch.cuda.synchronize()
+    for e0, e1 in evs:
+        e0.record()
+        fn()
+        e1.record()
+    torch.cuda.synchronize()
+    t = sorted(e0.elapsed_time(e1) * 1e3 for e0, e1 in evs)
+    return {"median": t[len(t) // 2], "min": t[0], "p90": t[min(len(t) - 1, int(0.9 * len(t)))], "steps": steps}
+
+
 def cpu_baseline(cfg, budget_s=8.0):
     """The oracle as it stands on this box's host cores, on a bounded sample of the workload."""
     import oracle
@@ -276,9 +290,13 @@ def cpu_baseline(cfg, budget_s=8.0):
         if dt >= budget_s or reps >= 200:
             break
     us = dt / reps * 1e6 * (cfg.N / N) ** 2      # scaled by pixel count when the sample is a smaller canvas
+    t1 = time.perf_counter()
+    oracle.tiles(x, y, cfg.N_T, *k, threads=1)
+    us_1 = (time.perf_counter() - t1) * 1e6 * (cfg.N / N) ** 2
     sample = (f"{reps} repetition(s) of one {N}x{N} pair of the {cfg.name} recipe (N_T={cfg.N_T}), "
               f"oracle tiles + aggregate" + ("" if N == cfg.N else f", time scaled by ({cfg.N}/{N})^2"))
-    return {"value": us, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample}
+    return {"value": us, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample,
+            "one_thread_us_per_pair": us_1}
 
 
 def run_e2e(torch, binding, cfg, pairs, steps, warmup, device, dist):
@@ -351,6 +369,7 @@ def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, us
         full()
     with ClockSampler(torch.cuda.current_device()) as clk:
         ms = time_region(torch, full, steps, dist)
+    dist_us = step_distribution(torch, full, max(10, min(steps, 100)))
     for _ in range(warmup):
         kern()
     ms_kernel = time_region(torch, kern, steps, dist)
@@ -361,7 +380,7 @@ def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, us
             fn()
         lat.append(time_region(torch, fn, reps, dist) / (reps * L))
     ms_single, ms_single_cold = lat
-    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "us_single_pair_warm": None if ms_single is None else ms_single * 1e3,
+    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "step_us": dist_us, "us_single_pair_warm": None if ms_single is None else ms_single * 1e3,
             "us_single_pair_cold": None if ms_single_cold is None else ms_single_cold * 1e3, "clocks": clk.summary()}
 
 
@@ -495,6 +514,7 @@ def run_ours(args):
     n_stream = -(-pairs // 32)                               # launches of the stream kernel per step
     us_launch = m["ms_kernel"] * 1e3 / (K * n_stream)       # per launch of the stream kernel (max over ranks)
     us_single, us_single_cold, clocks = m["us_single_pair_warm"], m["us_single_pair_cold"], m["clocks"]
+    step_us = m["step_us"]
     alg = algorithmic_bytes(cfg.N, cfg.N_T) * pairs / n_stream    # algorithmic bytes one launch moves
     peak, peak_src = measured_peak()
     achieved = alg / (us_launch * 1e-6) / 1e9
@@ -552,6 +572,7 @@ def run_ours(args):
                          "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
                          "us_per_launch": us_launch, "pairs_per_launch": pairs / n_stream,
                          "frac_of_nominal_8000": achieved / 8000.0},
+            "step_us": dict(step_us, per_pair_median=step_us["median"] / pairs),
             "us_single_pair_warm": us_single,
             "us_single_pair_cold": us_single_cold,
             "e2e": e2e,

@@ -426,6 +426,18 @@ def tiles_bottom_k(values, k):
     return idx, val
 
 
+def find_transients(images, mode, N_T, C1, C2, C, D, k: int = 16, index: str = "auglisi") -> dict:
+    """The finder end to end on the device: the K comparisons of a time series
+    (``series_tiles``), then for every comparison the ``k`` tiles of lowest ``index`` ("auglisi" or "lisi";
+    low = dissimilar) by ``tiles_bottom_k``.  Returns the series outputs plus ``candidates``
+    (int32 (K, k) tile indices t = ty * nt + tx, ascending by (value, index)) and ``candidate_values`` (K, k)."""
+    if index not in ("auglisi", "lisi"):
+        raise ValueError("index must be 'auglisi' or 'lisi'")
+    out = series_tiles(images, mode, N_T, C1, C2, C, D)
+    out["candidates"], out["candidate_values"] = tiles_bottom_k(out[index], k)
+    return out
+
+
 def lisi_tiles(x, y, N_T, C1, C2, D, workspace=None):
     import torch
     N = _check_images(x, y)

@@ -96,6 +96,30 @@ def test_candidates_on_oracle_matrices_of_config1(B):
             _check_below(B, maps, thr)
 
 
+def test_find_transients_end_to_end(B):
+    """Series -> bottom-k on the device: the switched-off transients of a config-[0] series are among the
+    flagged tiles of each comparison, and the flagged tiles are exactly the bottom-k of the device matrix."""
+    import torch
+    import oracle
+    from paper_2501_10653_b200 import synth
+    cfg = synth.CONFIGS[0]
+    imgs, meta = synth.make_series(cfg, 4)
+    dev = [torch.from_numpy(a).cuda() for a in imgs]
+    out = B.find_transients(dev, "reference", cfg.N_T, cfg.C1, cfg.C2, cfg.C, cfg.D, k=12)
+    torch.cuda.synchronize()
+    cand = out["candidates"].cpu().numpy()
+    mats = out["auglisi"].cpu().numpy()
+    nt = cfg.N // cfg.N_T
+    src, ch = meta["sources"], meta["changed"]
+    for c in range(3):
+        ei, ev = oracle.bottom_k(mats[c], 12)            # selection is exact on the same fp32 matrix
+        assert np.array_equal(cand[c], ei)
+        assert np.array_equal(out["candidate_values"][c].cpu().numpy(), ev)
+        off = [i for i, s in zip(ch, meta["state_y"][c + 1]) if s and src["amp_x"][i] > 10 * cfg.noise_sigma]
+        tiles = {int(src["cy"][i]) // cfg.N_T * nt + int(src["cx"][i]) // cfg.N_T for i in off}
+        assert tiles <= set(cand[c].tolist()), (c, tiles, cand[c])
+
+
 def test_candidate_error_codes(B):
     import torch
     v = torch.zeros((4, 4), dtype=torch.float32, device="cuda")
