@@ -141,6 +141,42 @@ generic_kernel(const GenericParams g) {
     }
 }
 
+// Small tiles (N_T * N_T <= kWarpTilePixels): one WARP per tile, eight tiles per CTA -- a CTA per
+// 64-pixel tile would be all launch overhead.  Lanes stride over the tile's pixels, warp butterfly,
+// lane 0 applies Eqs. 1-2.  Same sums, same edge-tile rule as generic_kernel.
+constexpr int kWarpTilePixels = 2048;
+
+template <int MODE>
+__global__ void __launch_bounds__(kCtaThreads)
+generic_warp_kernel(const GenericParams g, long long n_tiles) {
+    pdl_prologue();
+    const TileParams& p = g.tp;
+    const int N_T = g.N_T;
+    const long long tile = (long long)blockIdx.x * kWarpsPerCta + (threadIdx.x >> 5);
+    if (tile >= n_tiles) return;
+    const int lane = threadIdx.x & 31;
+    const int ty = (int)(tile / p.nt), tx = (int)(tile % p.nt);
+    const int rows_t = min(N_T, p.H - ty * N_T);
+    const int cols_t = min(N_T, p.N - tx * N_T);
+    const int npix = rows_t * cols_t;
+    const size_t row0 = (size_t)ty * N_T, col0 = (size_t)tx * N_T;
+    float aL = 0.f, aA = 0.f, aX = 0.f, aY = 0.f;
+    for (int k = lane; k < npix; k += 32) {
+        const int r = k / cols_t, c = k % cols_t;
+        const size_t ox = (row0 + r) * (size_t)p.pitch_x + col0 + c;
+        const size_t oy = (row0 + r) * (size_t)p.pitch_y + col0 + c;
+        pixel_terms<MODE>(__ldg(p.x + ox), __ldg(p.y + oy), p.C1, aL, aA, aX, aY);
+    }
+    float4 v = make_float4(aL, aA, aX, aY);
+    for (int o = 16; o > 0; o >>= 1) {
+        v.x += __shfl_xor_sync(0xffffffffu, v.x, o);
+        v.y += __shfl_xor_sync(0xffffffffu, v.y, o);
+        v.z += __shfl_xor_sync(0xffffffffu, v.z, o);
+        v.w += __shfl_xor_sync(0xffffffffu, v.w, o);
+    }
+    if (lane == 0) finalise_tile(p, (size_t)tile, v);
+}
+
 // -----------------------------------------------------------------------------
 // Finalise kernel (split tiles): one CTA per tile sums the tile's pieces in a fixed order
 // (thread-strided, then warp butterfly, then warp order) and applies Eqs. 1-2.

@@ -406,10 +406,19 @@ int launch_pairs(int mode, const float* const* xs, const float* const* ys, int n
             p.ws = ws ? ws + (size_t)i * (size_t)n * pl.pieces : nullptr;
             g.N_T = N_T; g.pieces = pl.pieces;
             cudaError_t e;
-            switch (mode) {
-                case kModeLisi: e = launch(generic_kernel<kModeLisi>, (unsigned)grid, kCtaThreads, 0, st, g); break;
-                case kModeAug: e = launch(generic_kernel<kModeAug>, (unsigned)grid, kCtaThreads, 0, st, g); break;
-                default: e = launch(generic_kernel<kModeFused>, (unsigned)grid, kCtaThreads, 0, st, g); break;
+            if ((long long)N_T * N_T <= kWarpTilePixels) {        // small tiles: one warp per tile (pieces == 1 here)
+                const unsigned wgrid = (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta);
+                switch (mode) {
+                    case kModeLisi: e = launch(generic_warp_kernel<kModeLisi>, wgrid, kCtaThreads, 0, st, g, n); break;
+                    case kModeAug: e = launch(generic_warp_kernel<kModeAug>, wgrid, kCtaThreads, 0, st, g, n); break;
+                    default: e = launch(generic_warp_kernel<kModeFused>, wgrid, kCtaThreads, 0, st, g, n); break;
+                }
+            } else {
+                switch (mode) {
+                    case kModeLisi: e = launch(generic_kernel<kModeLisi>, (unsigned)grid, kCtaThreads, 0, st, g); break;
+                    case kModeAug: e = launch(generic_kernel<kModeAug>, (unsigned)grid, kCtaThreads, 0, st, g); break;
+                    default: e = launch(generic_kernel<kModeFused>, (unsigned)grid, kCtaThreads, 0, st, g); break;
+                }
             }
             if (e != cudaSuccess) return IQA_ERR_CUDA;
         }
