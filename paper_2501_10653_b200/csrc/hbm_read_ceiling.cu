@@ -7,6 +7,7 @@
 // CTAs per SM, i.e. the bytes in flight per SM, and prints one line per point plus "best".
 // Result on B200 (profiles/r01f_read_ceiling.md): 7.30-7.34 TB/s for EVERY shape once 96-128 KiB
 // are in flight per SM; 64 KiB gives 6.9, 192 KiB 7.16.  Not part of libiqa_tiles.so.
+// Usage: hbm_read_ceiling [image width, default 8192]
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -o hbm_read_ceiling hbm_read_ceiling.cu
 // =============================================================================
 #include <cuda.h>
@@ -53,7 +54,9 @@ __global__ void __launch_bounds__(64) k(const __grid_constant__ P p){
 }
 typedef CUresult (*Enc)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 int main(int argc, char** argv){
-  int N = 8192; int rows_total = 8192*8; // 8 images stacked: 2 GiB
+  // image width N (default 8192; argv[1]) and as many rows as make 2 GiB
+  int N = argc > 1 ? atoi(argv[1]) : 8192; if (N < 256 || N % 256) { printf("N must be a multiple of 256\n"); return 1; }
+  int rows_total = (int)((2ll << 30) / 4 / N);
   float* d; cudaMalloc(&d, (size_t)N*rows_total*4); cudaMemset(d, 0, (size_t)N*rows_total*4);
   void* f; cudaDriverEntryPointQueryResult q; cudaGetDriverEntryPoint("cuTensorMapEncodeTiled",&f,cudaEnableDefault,&q); Enc enc=(Enc)f;
   int modes[][3] = {{0,128,32},{1,256,16},{2,128,32},{3,256,32},{4,128,16},{5,64,64},{6,256,8}};

@@ -105,3 +105,36 @@ def test_series_soak_bitwise(B, U):
             torch.cuda.synchronize()
             for n in first:
                 assert torch.equal(first[n], again[n]), (mode, n)
+
+
+def test_n32768_sampled_tiles(B, U):
+    """Maximum size of the suite: N = 32768 (4 GiB per image, element offsets beyond 2^30), N_T = 128.
+    The oracle checks 48 sampled tiles (incl. the four corners) on crops copied to the host -- crop
+    consistency is pinned for the oracle (tests/test_oracle_pins.py P9) -- plus the column sums of X and Y
+    of every tile row against torch reductions of the clamped images (a property that holds at any size)."""
+    import torch
+    import oracle
+    N, N_T = 32768, 128
+    nt = N // N_T
+    k = dict(C1=1e-6, C2=1e-6, C=1e-6, D=5e-7)
+    g = torch.Generator(device="cuda").manual_seed(7)
+    x = torch.empty((N, N), dtype=torch.float32, device="cuda").normal_(0.0, 1e-3, generator=g)
+    y = torch.empty((N, N), dtype=torch.float32, device="cuda").normal_(0.0, 1e-3, generator=g)
+    x[N - 100:N - 90, N - 300:N - 200] += 0.5                  # a source in the last tile row
+    out = B.fused_tiles(x, y, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(0)
+    picks = {(0, 0), (0, nt - 1), (nt - 1, 0), (nt - 1, nt - 1), (nt - 1, nt - 3)}
+    while len(picks) < 48:
+        picks.add((int(rng.integers(nt)), int(rng.integers(nt))))
+    for ty, tx in sorted(picks):
+        xc = x[ty * N_T:(ty + 1) * N_T, tx * N_T:(tx + 1) * N_T].contiguous().cpu().numpy()
+        yc = y[ty * N_T:(ty + 1) * N_T, tx * N_T:(tx + 1) * N_T].contiguous().cpu().numpy()
+        ref = oracle.tiles(xc, yc, N_T, **k)
+        got = {n: out[n][ty:ty + 1, tx:tx + 1].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+        U.assert_parity(got, ref, k["C"], f"N=32768 tile ({ty},{tx})")
+    # every tile contributes: sums over tile columns == sums of the clamped image over the same row bands (fp64)
+    for name, img in (("X", x), ("Y", y)):
+        rows = img.clamp_min(0).view(nt, N_T * N).sum(dim=1, dtype=torch.float64)
+        got = out[name].sum(dim=1, dtype=torch.float64)
+        assert torch.all((got - rows).abs() <= 1e-6 * rows.abs()), name
