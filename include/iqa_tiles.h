@@ -118,6 +118,20 @@ int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long p
                        float* lisi_num, float* auglisi_num,
                        void* workspace, size_t workspace_bytes, void* stream);
 
+/* The batch and time-series entry points (below) for general images: all images of the call share
+ * H, W and ONE row pitch.  Workspace: n_pairs (resp. n_images - 1) * iqa_workspace_bytes_2d(H, W, N_T).
+ * Outputs as for the square entry points with n = ceil(H / N_T) * ceil(W / N_T) tiles per comparison. */
+int iqa_fused_batch_2d(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,
+                       int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
+                       float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                       float* lisi_num, float* auglisi_num, float* out2,
+                       void* workspace, size_t workspace_bytes, void* stream);
+int iqa_series_tiles_2d(const float* const* img_ptrs_host, int n_images, int mode,
+                        int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
+                        float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                        float* lisi_num, float* auglisi_num, float* out2,
+                        void* workspace, size_t workspace_bytes, void* stream);
+
 /* Bytes of device workspace iqa_fused_batch needs: n_pairs * iqa_workspace_bytes(N, N_T). */
 size_t iqa_batch_workspace_bytes(int n_pairs, int N, int N_T);
 

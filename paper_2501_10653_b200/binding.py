@@ -24,7 +24,7 @@ IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKS
 
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
-           "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
+           "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_batch_2d", "iqa_series_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
            "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
@@ -79,6 +79,12 @@ def _load() -> ctypes.CDLL:
     lib.iqa_aggregate_partial.argtypes = [vp, vp, vp, vp, i, f, f, vp, vp]
     lib.iqa_aggregate_finish.restype = i
     lib.iqa_aggregate_finish.argtypes = [vp, ctypes.c_longlong, f, f, vp, vp]
+    lib.iqa_fused_batch_2d.restype = i
+    lib.iqa_fused_batch_2d.argtypes = [vp, vp, i, i, i, ctypes.c_longlong, i, f, f, f, f,
+                                       vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_series_tiles_2d.restype = i
+    lib.iqa_series_tiles_2d.argtypes = [vp, i, i, i, i, ctypes.c_longlong, i, f, f, f, f,
+                                        vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.iqa_tiles_below.restype = i
     lib.iqa_tiles_below.argtypes = [vp, i, i, f, vp, i, vp, vp]
     lib.iqa_tiles_bottom_k.restype = i
@@ -196,6 +202,25 @@ def iqa_fused_tiles_2d(x, y, H, W, pitch_x, pitch_y, N_T, C1, C2, C, D, lisi, au
                                   C1, C2, C, D, _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
                                   _ptr(lisi_num), _ptr(auglisi_num), _ptr(workspace), int(workspace_bytes),
                                   _stream(stream))
+
+
+def iqa_fused_batch_2d(x_ptrs_host, y_ptrs_host, n_pairs, H, W, pitch, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
+                       lisi_num=None, auglisi_num=None, out2=None, workspace=None, workspace_bytes=0,
+                       stream=None) -> int:
+    xt, _ = _ptr_table(x_ptrs_host)
+    yt, _ = _ptr_table(y_ptrs_host)
+    return lib.iqa_fused_batch_2d(xt, yt, int(n_pairs), int(H), int(W), int(pitch), int(N_T), C1, C2, C, D,
+                                  _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), _ptr(lisi_num),
+                                  _ptr(auglisi_num), _ptr(out2), _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
+def iqa_series_tiles_2d(img_ptrs_host, n_images, mode, H, W, pitch, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
+                        lisi_num=None, auglisi_num=None, out2=None, workspace=None, workspace_bytes=0,
+                        stream=None) -> int:
+    it, _ = _ptr_table(img_ptrs_host)
+    return lib.iqa_series_tiles_2d(it, int(n_images), int(mode), int(H), int(W), int(pitch), int(N_T), C1, C2, C, D,
+                                   _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), _ptr(lisi_num),
+                                   _ptr(auglisi_num), _ptr(out2), _ptr(workspace), int(workspace_bytes), _stream(stream))
 
 
 def iqa_series_workspace_bytes(n_images: int, N: int, N_T: int) -> int:
@@ -354,6 +379,61 @@ def fused_tiles_2d(x, y, N_T, C1, C2, C, D, numerators: bool = False) -> dict:
                             out["X"], out["Y"], out.get("L"), out.get("A"), ws, nbytes, _current_stream(x.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_fused_tiles_2d")
+    return out
+
+
+def _check_2d_list(images):
+    import torch
+    H, W = int(images[0].shape[0]), int(images[0].shape[1])
+    pitch = int(images[0].stride(0))
+    for t in images:
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.dim() == 2):
+            raise TypeError("images must be 2-D float32 CUDA tensors (no CPU fallback)")
+        if tuple(t.shape) != (H, W) or t.stride(1) != 1 or int(t.stride(0)) != pitch or t.device != images[0].device:
+            raise ValueError("all images of a call must share shape, row pitch and device")
+    return H, W, pitch
+
+
+def series_tiles_2d(images, mode, N_T, C1, C2, C, D, numerators: bool = False, aggregate: bool = True) -> dict:
+    """``series_tiles`` for H x W images with a common row pitch and edge tiles (SURVEY.md 8(f)-2 + 8(f)-4)."""
+    import torch
+    if mode not in SERIES_MODES:
+        raise ValueError(f"mode must be one of {tuple(SERIES_MODES)}")
+    if len(images) < 2 or N_T <= 0:
+        raise IqaError(IQA_ERR_SHAPE, "series_tiles_2d")
+    H, W, pitch = _check_2d_list(images)
+    K, nty, ntx, dev = len(images) - 1, -(-H // N_T), -(-W // N_T), images[0].device
+    names = ["lisi", "auglisi", "X", "Y"] + (["L", "A"] if numerators else [])
+    out = {k: torch.empty((K, nty, ntx), dtype=torch.float32, device=dev) for k in names}
+    if aggregate:
+        out["whole"] = torch.empty((K, 2), dtype=torch.float32, device=dev)
+    nbytes = K * iqa_workspace_bytes_2d(H, W, N_T)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev) if nbytes else None
+    rc = iqa_series_tiles_2d(images, len(images), SERIES_MODES[mode], H, W, pitch, N_T, C1, C2, C, D,
+                             out["lisi"], out["auglisi"], out["X"], out["Y"], out.get("L"), out.get("A"),
+                             out.get("whole"), ws, nbytes, _current_stream(dev))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_series_tiles_2d")
+    return out
+
+
+def fused_batch_2d(xs, ys, N_T, C1, C2, C, D, numerators: bool = False, aggregate: bool = True) -> dict:
+    """``fused_batch`` for H x W images with a common row pitch and edge tiles."""
+    import torch
+    if len(xs) != len(ys) or not xs or N_T <= 0:
+        raise IqaError(IQA_ERR_SHAPE, "fused_batch_2d")
+    H, W, pitch = _check_2d_list(list(xs) + list(ys))
+    P, nty, ntx, dev = len(xs), -(-H // N_T), -(-W // N_T), xs[0].device
+    names = ["lisi", "auglisi", "X", "Y"] + (["L", "A"] if numerators else [])
+    out = {k: torch.empty((P, nty, ntx), dtype=torch.float32, device=dev) for k in names}
+    if aggregate:
+        out["whole"] = torch.empty((P, 2), dtype=torch.float32, device=dev)
+    nbytes = P * iqa_workspace_bytes_2d(H, W, N_T)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev) if nbytes else None
+    rc = iqa_fused_batch_2d(xs, ys, P, H, W, pitch, N_T, C1, C2, C, D, out["lisi"], out["auglisi"], out["X"], out["Y"],
+                            out.get("L"), out.get("A"), out.get("whole"), ws, nbytes, _current_stream(dev))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_fused_batch_2d")
     return out
 
 

@@ -455,15 +455,29 @@ int finish_comparisons(const Outputs& out, float* out2, int n_cmp, long long n, 
 }
 
 // Validation shared by the batch and the series entry points (everything but the image lists).
+// Shape of a general image (g2) or of the paper's square N x N image: status and tile count.
+int status_of_geometry(int N, int N_T, const Geom2D* g2, long long* n_tiles) {
+    if (!g2) {
+        if (const int s = status_of_shape(N, N_T)) return s;
+        *n_tiles = (long long)(N / N_T) * (N / N_T);
+        return IQA_OK;
+    }
+    if (g2->H <= 0 || g2->W <= 0 || N_T <= 0 || g2->H > kMaxN || g2->W > kMaxN || g2->pitch_x < g2->W ||
+        g2->pitch_y < g2->W)
+        return IQA_ERR_SHAPE;
+    *n_tiles = (long long)((g2->W + N_T - 1) / N_T) * ((g2->H + N_T - 1) / N_T);
+    return *n_tiles > 0x7fffffffLL ? IQA_ERR_SHAPE : IQA_OK;
+}
+
 int validate_common(int mode, int n_cmp, int N, int N_T, float C1, float C2, float C, float D, const Outputs& out,
-                    const float* out2) {
+                    const float* out2, const Geom2D* g2 = nullptr) {
     if (n_cmp <= 0) return IQA_ERR_SHAPE;
     if ((mode & kModeLisi) && !out.lisi) return IQA_ERR_NULL;
     if ((mode & kModeAug) && !out.auglisi) return IQA_ERR_NULL;
     if (mode == kModeFused && (!out.sum_x || !out.sum_y)) return IQA_ERR_NULL;
-    if (const int s = status_of_shape(N, N_T)) return s;
-    const long long nt = N / N_T;
-    if (nt * nt * n_cmp > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    long long n = 0;
+    if (const int s = status_of_geometry(N, N_T, g2, &n)) return s;
+    if (n * n_cmp > 0x7fffffffLL) return IQA_ERR_SHAPE;
     if ((mode & kModeLisi) && (!pos_finite(C1) || !pos_finite(C2) || !std::isfinite(D))) return IQA_ERR_PARAM;
     if ((mode & kModeAug) && !pos_finite(C)) return IQA_ERR_PARAM;
     if (out2 && (!pos_finite(C2) || !pos_finite(C))) return IQA_ERR_PARAM;
@@ -474,27 +488,28 @@ int validate_common(int mode, int n_cmp, int N, int N_T, float C1, float C2, flo
 // xs, ys: HOST arrays of n_pairs device pointers.  out2 (nullable): Eqs. 3-4 per pair.
 int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pairs, int N, int N_T,
               float C1, float C2, float C, float D, Outputs out, float* out2,
-              void* workspace, size_t workspace_bytes, void* stream) {
+              void* workspace, size_t workspace_bytes, void* stream, const Geom2D* g2 = nullptr) {
     if (!xs || !ys) return IQA_ERR_NULL;
     if (n_pairs <= 0) return IQA_ERR_SHAPE;
     for (int i = 0; i < n_pairs; ++i)
         if (!xs[i] || !ys[i]) return IQA_ERR_NULL;
-    if (const int s = validate_common(mode, n_pairs, N, N_T, C1, C2, C, D, out, out2)) return s;
+    if (const int s = validate_common(mode, n_pairs, N, N_T, C1, C2, C, D, out, out2, g2)) return s;
+    long long n = 0;
+    status_of_geometry(N, N_T, g2, &n);
     uintptr_t bits = 0;
     for (int i = 0; i < n_pairs; ++i) bits |= (uintptr_t)xs[i] | (uintptr_t)ys[i];
     if (bits & 3u) return IQA_ERR_ALIGN;
-    const size_t need = workspace_bytes_for(n_pairs, N, N_T);
+    const size_t need = (size_t)n_pairs * (size_t)n * (max_pieces(N_T) > 1 ? max_pieces(N_T) : 0) * sizeof(float4);
     if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
     if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
 
-    const bool aligned16 = ((bits & 15u) == 0) && (N % 4 == 0);
-    const Plan pl = make_plan(N, N_T, aligned16, xs[0], false);
+    const bool aligned16 = ((bits & 15u) == 0) && (g2 ? (g2->pitch_x % 4 == 0 && g2->pitch_y % 4 == 0) : (N % 4 == 0));
+    const Plan pl = make_plan(g2 ? g2->W : N, N_T, aligned16, xs[0], false, g2);
     cudaStream_t st = (cudaStream_t)stream;
     float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
     out = out.for_mode(mode);
     const Consts k{C1, C2, C, D};
-    if (const int rc = launch_pairs(mode, xs, ys, n_pairs, N, N_T, k, out, ws, pl, st)) return rc;
-    const long long n = (long long)(N / N_T) * (N / N_T);
+    if (const int rc = launch_pairs(mode, xs, ys, n_pairs, g2 ? g2->W : N, N_T, k, out, ws, pl, st, g2)) return rc;
     return finish_comparisons(out, out2, n_pairs, n, k, ws, pl, st);
 }
 
@@ -504,26 +519,28 @@ int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pa
 // everything else is computed pair by pair with the kernels of the pair entry points.
 int run_series(const float* const* imgs, int n_images, int series, int N, int N_T,
                float C1, float C2, float C, float D, Outputs out, float* out2,
-               void* workspace, size_t workspace_bytes, void* stream) {
+               void* workspace, size_t workspace_bytes, void* stream, const Geom2D* g2 = nullptr) {
     if (!imgs) return IQA_ERR_NULL;
     if (n_images < 2 || (series != kReference && series != kConsecutive)) return IQA_ERR_SHAPE;
     for (int i = 0; i < n_images; ++i)
         if (!imgs[i]) return IQA_ERR_NULL;
     const int K = n_images - 1;
-    if (const int s = validate_common(kModeFused, K, N, N_T, C1, C2, C, D, out, out2)) return s;
+    if (const int s = validate_common(kModeFused, K, N, N_T, C1, C2, C, D, out, out2, g2)) return s;
+    long long n = 0;
+    status_of_geometry(N, N_T, g2, &n);
     uintptr_t bits = 0;
     for (int i = 0; i < n_images; ++i) bits |= (uintptr_t)imgs[i];
     if (bits & 3u) return IQA_ERR_ALIGN;
-    const size_t need = workspace_bytes_for(K, N, N_T);
+    const size_t need = (size_t)K * (size_t)n * (max_pieces(N_T) > 1 ? max_pieces(N_T) : 0) * sizeof(float4);
     if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
     if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
 
-    const bool aligned16 = ((bits & 15u) == 0) && (N % 4 == 0);
-    const Plan pl = make_plan(N, N_T, aligned16, imgs[0], true);
+    const bool aligned16 = ((bits & 15u) == 0) && (g2 ? g2->pitch_x % 4 == 0 : N % 4 == 0);
+    if (g2) N = g2->W;
+    const Plan pl = make_plan(N, N_T, aligned16, imgs[0], true, g2);
     cudaStream_t st = (cudaStream_t)stream;
     float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
     const Consts k{C1, C2, C, D};
-    const long long n = (long long)(N / N_T) * (N / N_T);
     if (pl.kind == kPlanTma) {
         // chunks of at most kMaxImages images; consecutive chunks share one image
         const float* chunk[kMaxImages];
@@ -532,7 +549,7 @@ int run_series(const float* const* imgs, int n_images, int series, int N, int N_
             chunk[0] = series == kReference ? imgs[0] : imgs[first];
             for (int i = 0; i < kc; ++i) chunk[1 + i] = imgs[first + 1 + i];
             const int rc = launch_tma(kModeFused, series, chunk, 1, kc + 1, N, N_T, k, out.offset((size_t)first * (size_t)n),
-                                      ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st);
+                                      ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st, g2);
             if (rc != IQA_OK) return rc;
         }
     } else {
@@ -545,7 +562,7 @@ int run_series(const float* const* imgs, int n_images, int series, int N, int N_
                 ys[i] = imgs[first + i + 1];
             }
             const int rc = launch_pairs(kModeFused, xs, ys, kc, N, N_T, k, out.offset((size_t)first * (size_t)n),
-                                        ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st);
+                                        ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st, g2);
             if (rc != IQA_OK) return rc;
         }
     }
@@ -638,6 +655,29 @@ int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long p
     const Consts k{C1, C2, C, D};
     if (const int rc = launch_pairs(kModeFused, &x, &y, 1, W, N_T, k, out, ws, pl, st, &g2)) return rc;
     return finish_comparisons(out, nullptr, 1, ntx * nty, k, ws, pl, st);
+}
+
+int iqa_fused_batch_2d(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,
+                       int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
+                       float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                       float* lisi_num, float* auglisi_num, float* out2,
+                       void* workspace, size_t workspace_bytes, void* stream) {
+    const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
+    const Geom2D g2{H, W, pitch, pitch};
+    return run_batch(kModeFused, x_ptrs_host, y_ptrs_host, n_pairs, W, N_T, C1, C2, C, D, o, out2,
+                     workspace, workspace_bytes, stream, &g2);
+}
+
+int iqa_series_tiles_2d(const float* const* img_ptrs_host, int n_images, int mode,
+                        int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
+                        float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                        float* lisi_num, float* auglisi_num, float* out2,
+                        void* workspace, size_t workspace_bytes, void* stream) {
+    const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
+    const int series = mode == IQA_SERIES_REFERENCE ? kReference : mode == IQA_SERIES_CONSECUTIVE ? kConsecutive : -1;
+    const Geom2D g2{H, W, pitch, pitch};
+    return run_series(img_ptrs_host, n_images, series, W, N_T, C1, C2, C, D, o, out2,
+                      workspace, workspace_bytes, stream, &g2);
 }
 
 int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,

@@ -151,3 +151,32 @@ def test_one_pair_sharded_by_bands_of_tile_rows(B, U, world):
     e4 = np.array([np.sum(ref["lisi"] * (np.maximum(ref["X"], ref["Y"]) + c2)),
                    np.sum(ref["auglisi"] * (ref["X"] + ref["Y"] + c)), np.sum(ref["X"]), np.sum(ref["Y"])])
     assert np.all(np.abs(total.cpu().numpy() - e4) <= 1e-5 * np.abs(e4))
+
+
+@pytest.mark.parametrize("H,W,N_T,pitch,off", [(300, 500, 64, 512, 0), (513, 260, 128, 260, 0), (100, 130, 16, 131, 1),
+                                               (90, 70, 20, 72, 0)])
+def test_batch_and_series_2d(B, U, H, W, N_T, pitch, off):
+    """iqa_fused_batch_2d / iqa_series_tiles_2d (common pitch; TMA and generic paths) against oracle.tiles_2d."""
+    import torch
+    import oracle
+    rng = np.random.default_rng(H + W)
+    imgs = [rng.normal(0.05, 0.2, (H, W)).astype(np.float32) for _ in range(4)]
+    imgs[2][: H // 2] = imgs[1][: H // 2]
+    dev = [_window(a, pitch, off) for a in imgs]
+    xs, ys = [dev[0], dev[2]], [dev[1], dev[3]]
+    out = B.fused_batch_2d(xs, ys, N_T, K["C1"], K["C2"], K["C"], K["D"], numerators=True)
+    torch.cuda.synchronize()
+    for p, (ix, iy) in enumerate(((0, 1), (2, 3))):
+        ref = oracle.tiles_2d(imgs[ix], imgs[iy], N_T, **K)
+        got = {n: out[n][p].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+        U.assert_parity(got, ref, K["C"], f"batch_2d pair {p}")
+        exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], K["C2"], K["C"])
+        w = out["whole"][p].cpu().numpy()
+        assert abs(w[0] - exp[0]) <= 1e-5 * abs(exp[0]) and abs(w[1] - exp[1]) <= 1e-5 * abs(exp[1]) + 1e-6
+    for mode in ("reference", "consecutive"):
+        so = B.series_tiles_2d(dev, mode, N_T, K["C1"], K["C2"], K["C"], K["D"], numerators=True)
+        torch.cuda.synchronize()
+        for c, (ix, iy) in enumerate(oracle.comparison_indices(4, mode)):
+            ref = oracle.tiles_2d(imgs[ix], imgs[iy], N_T, **K)
+            got = {n: so[n][c].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+            U.assert_parity(got, ref, K["C"], f"series_2d {mode} {c}")
