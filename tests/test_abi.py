@@ -187,6 +187,16 @@ def test_2d_validation():
     assert B.iqa_fused_tiles_2d(FAKE, FAKE, 100, 300, 300, 300, 128, *a, *o) == B.IQA_ERR_WORKSPACE
     assert B.iqa_workspace_bytes_2d(100, 300, 128) == 1 * 3 * 2 * 16
     assert B.iqa_workspace_bytes_2d(100, 300, 64) == 0 and B.iqa_workspace_bytes_2d(0, 300, 128) == 0
+    tbl = (ctypes.c_void_p * 3)(FAKE, FAKE, FAKE)
+    bad = (ctypes.c_void_p * 3)(FAKE, 0, FAKE)
+    assert B.iqa_fused_batch_2d(tbl, bad, 3, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_NULL
+    assert B.iqa_fused_batch_2d(tbl, tbl, 3, 64, 80, 79, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_fused_batch_2d(tbl, tbl, 3, 100, 300, 300, 128, *a, *o) == B.IQA_ERR_WORKSPACE
+    assert B.iqa_series_tiles_2d(tbl, 3, 0, 64, 80, 80, 8, *a, FAKE, FAKE, FAKE, None) == B.IQA_ERR_NULL
+    assert B.iqa_series_tiles_2d(tbl, 3, 5, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_series_tiles_2d(tbl, 1, 0, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_series_tiles_2d(bad, 3, 0, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_NULL
+    assert B.iqa_series_tiles_2d(tbl, 3, 0, 64, 80, 80, 8, 1e-6, 1e-6, 0.0, 5e-7, *o) == B.IQA_ERR_PARAM
     # the square entry points keep the paper's divisibility requirement
     assert B.iqa_fused_tiles(FAKE, FAKE, 100, 64, *a, *o) == B.IQA_ERR_SHAPE
 
