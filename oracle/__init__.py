@@ -49,6 +49,10 @@ def _load():
         lib.iqa_oracle_tiles_2d.argtypes = [fp, fp, ctypes.c_long, ctypes.c_long, ctypes.c_long, ctypes.c_long,
                                             ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_double,
                                             ctypes.c_double, dp, dp, dp, dp, dp, dp, ctypes.c_int]
+        lib.iqa_oracle_tiles_2d_f64.restype = ctypes.c_int
+        lib.iqa_oracle_tiles_2d_f64.argtypes = [dp, dp, ctypes.c_long, ctypes.c_long, ctypes.c_long, ctypes.c_long,
+                                                ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                                ctypes.c_double, dp, dp, dp, dp, dp, dp, ctypes.c_int]
         lib.iqa_oracle_aggregate.restype = ctypes.c_int
         lib.iqa_oracle_aggregate.argtypes = [dp, dp, dp, dp, ctypes.c_long,
                                              ctypes.c_double, ctypes.c_double, dp]
@@ -152,6 +156,34 @@ def tiles_2d(x, y, N_T: int, C1, C2, C, D, threads: int = 0) -> dict:
         _dptr(out["L"]), _dptr(out["A"]), int(threads) if threads > 0 else max_threads())
     if rc != 0:
         raise RuntimeError(f"iqa_oracle_tiles_2d failed with code {rc}")
+    return out
+
+
+PIXEL_DTYPES = (np.float32, np.float64, np.float16, np.int16, np.int32, np.uint8)   # FITS BITPIX -32, -64, (fp16), 16, 32, 8
+
+
+def tiles_2d_any(x, y, N_T: int, C1, C2, C, D, threads: int = 0) -> dict:
+    """``tiles_2d`` for images of any supported pixel type: the pixels are converted to
+    double -- exact for every type in ``PIXEL_DTYPES`` -- and Eqs. 1-2 are evaluated in double on those values."""
+    x, y = np.asarray(x), np.asarray(y)
+    if x.dtype != y.dtype or x.dtype.type not in PIXEL_DTYPES:
+        raise ValueError(f"x and y must share one of the pixel types {[t.__name__ for t in PIXEL_DTYPES]}")
+    if x.ndim != 2 or x.shape != y.shape:
+        raise ValueError("need two equally shaped 2-D images")
+    xd = np.ascontiguousarray(x, dtype=np.float64)
+    yd = np.ascontiguousarray(y, dtype=np.float64)
+    H, W = xd.shape
+    if N_T <= 0:
+        raise ValueError("N_T must be positive")
+    nty, ntx = -(-H // N_T), -(-W // N_T)
+    out = {k: np.empty((nty, ntx), dtype=np.float64) for k in ("lisi", "auglisi", "X", "Y", "L", "A")}
+    rc = _load().iqa_oracle_tiles_2d_f64(
+        _dptr(xd), _dptr(yd), H, W, W, W, N_T,
+        float(np.float32(C1)), float(np.float32(C2)), float(np.float32(C)), float(np.float32(D)),
+        _dptr(out["lisi"]), _dptr(out["auglisi"]), _dptr(out["X"]), _dptr(out["Y"]),
+        _dptr(out["L"]), _dptr(out["A"]), int(threads) if threads > 0 else max_threads())
+    if rc != 0:
+        raise RuntimeError(f"iqa_oracle_tiles_2d_f64 failed with code {rc}")
     return out
 
 

@@ -146,6 +146,49 @@ int iqa_oracle_tiles_2d(const float* x, const float* y, long H, long W, long pit
     return 0;
 }
 
+// The same for pixels given as DOUBLES (FITS planes come as BITPIX -64, 16, 32, 8 ...;
+// every such pixel value converts to double exactly, so the caller converts and this routine is the
+// definition for all of them).  Identical loop nest; only the element type of x and y differs.
+int iqa_oracle_tiles_2d_f64(const double* x, const double* y, long H, long W, long pitch_x, long pitch_y, long N_T,
+                            double C1, double C2, double C, double D,
+                            double* lisi, double* auglisi, double* X, double* Y, double* L, double* A,
+                            int threads) {
+    if (!x || !y || !lisi || !auglisi || !X || !Y || !L || !A) return 1;
+    if (H <= 0 || W <= 0 || N_T <= 0 || pitch_x < W || pitch_y < W) return 1;
+    const long nty = (H + N_T - 1) / N_T, ntx = (W + N_T - 1) / N_T;
+    const long n = nty * ntx;
+#ifdef _OPENMP
+    const int nthreads = threads > 0 ? threads : omp_get_max_threads();
+#pragma omp parallel for schedule(static) num_threads(nthreads)
+#else
+    (void)threads;
+#endif
+    for (long t = 0; t < n; ++t) {
+        const long ty = t / ntx, tx = t % ntx;
+        const long r_end = (ty + 1) * N_T < H ? (ty + 1) * N_T : H;
+        const long c_end = (tx + 1) * N_T < W ? (tx + 1) * N_T : W;
+        double sumL = 0.0, sumA = 0.0, sumX = 0.0, sumY = 0.0;
+        for (long r = ty * N_T; r < r_end; ++r) {
+            for (long c = tx * N_T; c < c_end; ++c) {
+                const double xv = x[r * pitch_x + c], yv = y[r * pitch_y + c];
+                const double xd = (xv > 0.0) ? xv : 0.0;                 // P:27 (NaN -> 0 as well)
+                const double yd = (yv > 0.0) ? yv : 0.0;
+                const double s = std::fabs(xd + yd);
+                const double d = std::fabs(xd - yd);
+                sumL += s / (d + C1);
+                sumA += s * d;
+                sumX += xd;
+                sumY += yd;
+            }
+        }
+        const double mx = sumX > sumY ? sumX : sumY;
+        lisi[t] = D * sumL / (mx + C2);                  // Eq. 1
+        auglisi[t] = 1.0 - sumA / (sumX + sumY + C);     // Eq. 2
+        X[t] = sumX; Y[t] = sumY; L[t] = sumL; A[t] = sumA;
+    }
+    return 0;
+}
+
 // Tile -> whole-image aggregation, Eqs. 3-4, over n tiles (n >= 1).
 //   out2[0] = LISI of the whole image, out2[1] = augLISI of the whole image.
 // "Whole image" may be any set of tiles merged into a larger tile: the caller

@@ -105,3 +105,48 @@ def test_hand_checked_3x5():
     assert np.allclose(t["auglisi"], expA, rtol=1e-15)
     with pytest.raises(ValueError):
         oracle.tiles_2d(x, y[:2], 2, **k)
+
+
+# ----------------------------------------------------------------------------- other pixel types
+def test_any_dtype_reduces_to_the_fp32_oracle_on_fp32_values():
+    """T1: fp32 images through the double-input oracle == tiles_2d bit for bit (the fp32 routine is pinned above);
+    fp16 / int16 / uint8 / int32 images == the same values stored as fp32 (all exactly representable)."""
+    x, y = _pair(37, 53, 11)
+    a, b = oracle.tiles_2d_any(x, y, 16, **K), oracle.tiles_2d(x, y, 16, **K)
+    for n in NAMES:
+        assert np.array_equal(a[n], b[n]), n
+    rng = np.random.default_rng(3)
+    for dt, lo, hi in ((np.int16, -300, 3000), (np.uint8, 0, 255), (np.int32, -1000, 1 << 20), (np.float16, -2, 8)):
+        xi = rng.uniform(lo, hi, (20, 28)).astype(dt)
+        yi = rng.uniform(lo, hi, (20, 28)).astype(dt)
+        yi[:10] = xi[:10]
+        a = oracle.tiles_2d_any(xi, yi, 8, **K)
+        b = oracle.tiles_2d(xi.astype(np.float32), yi.astype(np.float32), 8, **K)
+        for n in NAMES:
+            assert np.array_equal(a[n], b[n]), (dt, n)
+    with pytest.raises(ValueError):
+        oracle.tiles_2d_any(x, y.astype(np.float64), 16, **K)
+
+
+def test_fp64_pixels_vs_exact_rational_incl_ill_conditioned_differences():
+    """T2: doubles whose differences (|x - y| ~ 3e-7) are of the order of C1 and only a few fp32 ulps of the
+    values: the Eq. 1 term 2x/(|x-y|+C1) depends on that difference, so rounding the INPUTS to fp32 first
+    (|x - y| off by up to an ulp, 6e-8) would be wrong by percents; exact rationals decide."""
+    rng = np.random.default_rng(4)
+    x = rng.normal(0.5, 0.5, (6, 8))
+    y = x + rng.normal(0.0, 3e-7, (6, 8))
+    y[0, :4] = rng.normal(0.5, 0.5, 4)
+    x[5, 5] = -0.25
+    k = dict(C1=1e-6, C2=1e-6, C=1e-6, D=5e-7)
+    got = oracle.tiles_2d_any(x, y, 4, **k)
+    kk = {n: np.float32(v) for n, v in k.items()}
+    for ty in range(2):
+        for tx in range(2):
+            ref = er.lisi_auglisi(x[ty * 4:ty * 4 + 4, tx * 4:tx * 4 + 4].tolist(),
+                                  y[ty * 4:ty * 4 + 4, tx * 4:tx * 4 + 4].tolist(), **kk)
+            for n, v in zip(NAMES, ref):
+                f = float(v)
+                assert abs(got[n][ty, tx] - f) <= 1e-11 * max(abs(f), 1e-30) + 1e-15, (ty, tx, n)
+    # and the fp32-rounded inputs give a visibly different LISI (the reason the kernel subtracts in fp64)
+    lo = oracle.tiles_2d(x.astype(np.float32), y.astype(np.float32), 4, **k)
+    assert np.max(np.abs(lo["L"] - got["L"]) / got["L"]) > 1e-3
