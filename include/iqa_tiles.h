@@ -118,6 +118,22 @@ int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long p
                        float* lisi_num, float* auglisi_num,
                        void* workspace, size_t workspace_bytes, void* stream);
 
+/* Other pixel types (FITS BITPIX -64, 16, 32, 8; fp16 from a GPU imager): the same computation on an
+ * H x W image of `pixel_type` pixels (pitches in ELEMENTS of that type; pointers aligned to the element
+ * size).  Every such value is exact in double; types that are exact in fp32 (F16, I16, U8) are converted
+ * and follow the fp32 arithmetic, F64 and I32 are clamped, added and subtracted in fp64 before rounding
+ * (the Eq. 1 term is ill-conditioned in x - y).  IQA_PIXEL_F32 forwards to iqa_fused_tiles_2d (TMA
+ * kernel); the other types take the generic kernels.  Unknown pixel_type: IQA_ERR_SHAPE. */
+typedef enum {
+    IQA_PIXEL_F32 = 0, IQA_PIXEL_F64 = 1, IQA_PIXEL_F16 = 2, IQA_PIXEL_I16 = 3, IQA_PIXEL_I32 = 4, IQA_PIXEL_U8 = 5
+} iqa_pixel_type;
+int iqa_fused_tiles_2d_typed(const void* x, const void* y, int pixel_type,
+                             int H, int W, long long pitch_x, long long pitch_y, int N_T,
+                             float C1, float C2, float C, float D,
+                             float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                             float* lisi_num, float* auglisi_num,
+                             void* workspace, size_t workspace_bytes, void* stream);
+
 /* The batch and time-series entry points (below) for general images: all images of the call share
  * H, W and ONE row pitch.  Workspace: n_pairs (resp. n_images - 1) * iqa_workspace_bytes_2d(H, W, N_T).
  * Outputs as for the square entry points with n = ceil(H / N_T) * ceil(W / N_T) tiles per comparison. */

@@ -24,10 +24,11 @@ IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKS
 
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
-           "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_batch_2d", "iqa_series_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
+           "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_tiles_2d_typed", "iqa_fused_batch_2d", "iqa_series_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
            "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
+IQA_PIXEL_F32, IQA_PIXEL_F64, IQA_PIXEL_F16, IQA_PIXEL_I16, IQA_PIXEL_I32, IQA_PIXEL_U8 = range(6)
 SERIES_MODES = {"reference": IQA_SERIES_REFERENCE, "consecutive": IQA_SERIES_CONSECUTIVE}
 
 
@@ -79,6 +80,9 @@ def _load() -> ctypes.CDLL:
     lib.iqa_aggregate_partial.argtypes = [vp, vp, vp, vp, i, f, f, vp, vp]
     lib.iqa_aggregate_finish.restype = i
     lib.iqa_aggregate_finish.argtypes = [vp, ctypes.c_longlong, f, f, vp, vp]
+    lib.iqa_fused_tiles_2d_typed.restype = i
+    lib.iqa_fused_tiles_2d_typed.argtypes = [vp, vp, i, i, i, ctypes.c_longlong, ctypes.c_longlong, i, f, f, f, f,
+                                             vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.iqa_fused_batch_2d.restype = i
     lib.iqa_fused_batch_2d.argtypes = [vp, vp, i, i, i, ctypes.c_longlong, i, f, f, f, f,
                                        vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -202,6 +206,14 @@ def iqa_fused_tiles_2d(x, y, H, W, pitch_x, pitch_y, N_T, C1, C2, C, D, lisi, au
                                   C1, C2, C, D, _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
                                   _ptr(lisi_num), _ptr(auglisi_num), _ptr(workspace), int(workspace_bytes),
                                   _stream(stream))
+
+
+def iqa_fused_tiles_2d_typed(x, y, pixel_type, H, W, pitch_x, pitch_y, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
+                             lisi_num=None, auglisi_num=None, workspace=None, workspace_bytes=0, stream=None) -> int:
+    return lib.iqa_fused_tiles_2d_typed(_ptr(x), _ptr(y), int(pixel_type), int(H), int(W), int(pitch_x), int(pitch_y),
+                                        int(N_T), C1, C2, C, D, _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
+                                        _ptr(lisi_num), _ptr(auglisi_num), _ptr(workspace), int(workspace_bytes),
+                                        _stream(stream))
 
 
 def iqa_fused_batch_2d(x_ptrs_host, y_ptrs_host, n_pairs, H, W, pitch, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
@@ -356,13 +368,18 @@ def fused_batch(xs, ys, N_T, C1, C2, C, D, numerators: bool = False, aggregate: 
 
 
 def fused_tiles_2d(x, y, N_T, C1, C2, C, D, numerators: bool = False) -> dict:
-    """Eqs. 1-2 per tile of two H x W float32 CUDA tensors with EDGE TILES.  x and y
+    """Eqs. 1-2 per tile of two H x W CUDA tensors with EDGE TILES; pixel types float32
+    (TMA kernel), float64, float16, int16, int32, uint8 (generic kernels).  x and y
     may be row-pitched views (``stride(1) == 1``, e.g. a window ``big[r0:r1, c0:c1]``); nothing is copied.
     Returns dict of (ceil(H/N_T), ceil(W/N_T)) float32 CUDA tensors: lisi, auglisi, X, Y (+ L, A)."""
     import torch
+    ptypes = {torch.float32: IQA_PIXEL_F32, torch.float64: IQA_PIXEL_F64, torch.float16: IQA_PIXEL_F16,
+              torch.int16: IQA_PIXEL_I16, torch.int32: IQA_PIXEL_I32, torch.uint8: IQA_PIXEL_U8}
     for t in (x, y):
-        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.dim() == 2):
-            raise TypeError("x and y must be 2-D float32 CUDA tensors (no CPU fallback)")
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype in ptypes and t.dim() == 2):
+            raise TypeError("x and y must be 2-D CUDA tensors of a supported pixel type (no CPU fallback)")
+        if t.dtype != x.dtype:
+            raise TypeError("x and y must share their pixel type")
         if t.stride(1) != 1 or t.stride(0) < t.shape[1]:
             raise ValueError("rows must be contiguous (stride(1) == 1) and must not overlap")
     if x.shape != y.shape or x.device != y.device:
@@ -375,10 +392,11 @@ def fused_tiles_2d(x, y, N_T, C1, C2, C, D, numerators: bool = False) -> dict:
     out = {k: torch.empty((nty, ntx), dtype=torch.float32, device=x.device) for k in names}
     nbytes = iqa_workspace_bytes_2d(H, W, N_T)
     ws = torch.empty(nbytes, dtype=torch.uint8, device=x.device) if nbytes else None
-    rc = iqa_fused_tiles_2d(x, y, H, W, x.stride(0), y.stride(0), N_T, C1, C2, C, D, out["lisi"], out["auglisi"],
-                            out["X"], out["Y"], out.get("L"), out.get("A"), ws, nbytes, _current_stream(x.device))
+    rc = iqa_fused_tiles_2d_typed(x, y, ptypes[x.dtype], H, W, x.stride(0), y.stride(0), N_T, C1, C2, C, D,
+                                  out["lisi"], out["auglisi"], out["X"], out["Y"], out.get("L"), out.get("A"),
+                                  ws, nbytes, _current_stream(x.device))
     if rc != IQA_OK:
-        raise IqaError(rc, "iqa_fused_tiles_2d")
+        raise IqaError(rc, "iqa_fused_tiles_2d_typed")
     return out
 
 

@@ -13,6 +13,7 @@
 // No floating-point atomics anywhere, so results are bit-reproducible.
 // =============================================================================
 #pragma once
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -25,7 +26,7 @@ constexpr int kUnitCols = 128;          // 32 lanes x 4 columns
 enum : int { kModeLisi = 1, kModeAug = 2, kModeFused = 3 };
 
 struct TileParams {
-    const float* __restrict__ x;
+    const float* __restrict__ x;   // typed entry point: pixels of another type behind the same pointer
     const float* __restrict__ y;
     int N;               // image width W (= side N of the square API)
     int H;               // image height
@@ -71,6 +72,33 @@ __device__ __forceinline__ void pixel_terms(float xv, float yv, float C1,
     aY += yc;
 }
 
+// S1 + S2 for one pixel pair of ANY supported pixel type T (the generic kernels).
+// Types whose values are exact in fp32 (float, half, int16, uint8) are converted and go through
+// pixel_terms.  double and int32 are clamped, added and SUBTRACTED in fp64 and only then rounded: the
+// Eq. 1 term (x+y)/(|x-y|+C1) is ill-conditioned in the inputs once |x-y| is of the order of C1, so
+// rounding x and y to fp32 first would be wrong by percents (tests/test_oracle_2d_pins.py T2).
+template <typename T> struct PixelExactInFloat { static constexpr bool value = true; };
+template <> struct PixelExactInFloat<double> { static constexpr bool value = false; };
+template <> struct PixelExactInFloat<int> { static constexpr bool value = false; };
+
+template <int MODE, typename T>
+__device__ __forceinline__ void pixel_terms_any(const T* __restrict__ x, const T* __restrict__ y, size_t ox, size_t oy,
+                                                float C1, float& aL, float& aA, float& aX, float& aY) {
+    if constexpr (PixelExactInFloat<T>::value) {
+        pixel_terms<MODE>((float)x[ox], (float)y[oy], C1, aL, aA, aX, aY);
+    } else {
+        const double xv = (double)x[ox], yv = (double)y[oy];
+        const double xc = xv > 0.0 ? xv : 0.0;      // P:27; NaN -> 0
+        const double yc = yv > 0.0 ? yv : 0.0;
+        const float s = (float)(xc + yc);
+        const float d = (float)fabs(xc - yc);
+        if (MODE & kModeLisi) aL = fmaf(s, rcp_approx(d + C1), aL);
+        if (MODE & kModeAug) aA = fmaf(s, d, aA);
+        aX += (float)xc;
+        aY += (float)yc;
+    }
+}
+
 // S4: Eq. 1 / Eq. 2 from the four sums of one tile, true fp32 division.
 template <class Params>
 __device__ __forceinline__ void finalise_tile(const Params& p, size_t t, float4 v /*L,A,X,Y*/) {
@@ -97,7 +125,7 @@ struct GenericParams {
     int pieces;               // ceil(N_T / kGenericRows)
 };
 
-template <int MODE>
+template <int MODE, typename T = float>
 __global__ void __launch_bounds__(kCtaThreads)
 generic_kernel(const GenericParams g) {
     __shared__ float4 part[kWarpsPerCta];
@@ -120,7 +148,8 @@ generic_kernel(const GenericParams g) {
         const int r = (int)(k / cols_t), c = (int)(k % cols_t);
         const size_t ox = (row0 + r) * (size_t)p.pitch_x + col0 + c;
         const size_t oy = (row0 + r) * (size_t)p.pitch_y + col0 + c;
-        pixel_terms<MODE>(__ldg(p.x + ox), __ldg(p.y + oy), p.C1, aL, aA, aX, aY);
+        pixel_terms_any<MODE, T>(reinterpret_cast<const T*>(p.x), reinterpret_cast<const T*>(p.y), ox, oy, p.C1,
+                                 aL, aA, aX, aY);
     }
     float4 v = make_float4(aL, aA, aX, aY);
     for (int o = 16; o > 0; o >>= 1) {
@@ -146,7 +175,7 @@ generic_kernel(const GenericParams g) {
 // lane 0 applies Eqs. 1-2.  Same sums, same edge-tile rule as generic_kernel.
 constexpr int kWarpTilePixels = 2048;
 
-template <int MODE>
+template <int MODE, typename T = float>
 __global__ void __launch_bounds__(kCtaThreads)
 generic_warp_kernel(const GenericParams g, long long n_tiles) {
     pdl_prologue();
@@ -165,7 +194,8 @@ generic_warp_kernel(const GenericParams g, long long n_tiles) {
         const int r = k / cols_t, c = k % cols_t;
         const size_t ox = (row0 + r) * (size_t)p.pitch_x + col0 + c;
         const size_t oy = (row0 + r) * (size_t)p.pitch_y + col0 + c;
-        pixel_terms<MODE>(__ldg(p.x + ox), __ldg(p.y + oy), p.C1, aL, aA, aX, aY);
+        pixel_terms_any<MODE, T>(reinterpret_cast<const T*>(p.x), reinterpret_cast<const T*>(p.y), ox, oy, p.C1,
+                                 aL, aA, aX, aY);
     }
     float4 v = make_float4(aL, aA, aX, aY);
     for (int o = 16; o > 0; o >>= 1) {

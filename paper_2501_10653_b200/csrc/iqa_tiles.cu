@@ -569,6 +569,29 @@ int run_series(const float* const* imgs, int n_images, int series, int N, int N_
     return finish_comparisons(out, out2, K, n, k, ws, pl, st);
 }
 
+// Generic kernels on pixels of type T (iqa_fused_tiles_2d_typed).
+template <typename T>
+int launch_typed(const void* x, const void* y, const Geom2D& g2, int N_T, const Consts& k, const Outputs& out, float4* ws,
+                 const Plan& pl, cudaStream_t st) {
+    const int nt = (g2.W + N_T - 1) / N_T;
+    const long long n = (long long)nt * ((g2.H + N_T - 1) / N_T);
+    GenericParams g{};
+    TileParams& p = g.tp;
+    p.x = (const float*)x; p.y = (const float*)y; p.N = g2.W; p.H = g2.H; p.nt = nt;
+    p.pitch_x = g2.pitch_x; p.pitch_y = g2.pitch_y;
+    p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
+    p.lisi = out.lisi; p.auglisi = out.auglisi; p.sum_x = out.sum_x; p.sum_y = out.sum_y;
+    p.lisi_num = out.lisi_num; p.aug_num = out.aug_num;
+    p.ws = ws;
+    g.N_T = N_T; g.pieces = pl.pieces;
+    cudaError_t e;
+    if ((long long)N_T * N_T <= kWarpTilePixels)
+        e = launch(generic_warp_kernel<kModeFused, T>, (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta), kCtaThreads, 0, st, g, n);
+    else
+        e = launch(generic_kernel<kModeFused, T>, (unsigned)(n * pl.pieces), kCtaThreads, 0, st, g);
+    return e == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+}
+
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace
@@ -655,6 +678,55 @@ int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long p
     const Consts k{C1, C2, C, D};
     if (const int rc = launch_pairs(kModeFused, &x, &y, 1, W, N_T, k, out, ws, pl, st, &g2)) return rc;
     return finish_comparisons(out, nullptr, 1, ntx * nty, k, ws, pl, st);
+}
+
+int iqa_fused_tiles_2d_typed(const void* x, const void* y, int pixel_type,
+                             int H, int W, long long pitch_x, long long pitch_y, int N_T,
+                             float C1, float C2, float C, float D,
+                             float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                             float* lisi_num, float* auglisi_num,
+                             void* workspace, size_t workspace_bytes, void* stream) {
+    if (pixel_type == IQA_PIXEL_F32)
+        return iqa_fused_tiles_2d((const float*)x, (const float*)y, H, W, pitch_x, pitch_y, N_T, C1, C2, C, D, lisi, auglisi,
+                                  sum_x, sum_y, lisi_num, auglisi_num, workspace, workspace_bytes, stream);
+    if (!x || !y || !lisi || !auglisi || !sum_x || !sum_y) return IQA_ERR_NULL;
+    size_t esize = 0;
+    switch (pixel_type) {
+        case IQA_PIXEL_F64: esize = 8; break;
+        case IQA_PIXEL_F16: case IQA_PIXEL_I16: esize = 2; break;
+        case IQA_PIXEL_I32: esize = 4; break;
+        case IQA_PIXEL_U8: esize = 1; break;
+        default: return IQA_ERR_SHAPE;
+    }
+    if (H <= 0 || W <= 0 || N_T <= 0 || H > kMaxN || W > kMaxN || pitch_x < W || pitch_y < W) return IQA_ERR_SHAPE;
+    const long long n = (long long)((W + N_T - 1) / N_T) * ((H + N_T - 1) / N_T);
+    if (n * (long long)((N_T + kGenericRows - 1) / kGenericRows) > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    if (!pos_finite(C1) || !pos_finite(C2) || !pos_finite(C) || !std::isfinite(D)) return IQA_ERR_PARAM;
+    if ((((uintptr_t)x | (uintptr_t)y) & (esize - 1)) != 0) return IQA_ERR_ALIGN;
+    const size_t need = iqa_workspace_bytes_2d(H, W, N_T);
+    if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
+    if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
+
+    const Geom2D g2{H, W, pitch_x, pitch_y};
+    Plan pl{};
+    pl.kind = kPlanGeneric;
+    pl.pieces_x = 1;
+    pl.pieces_y = (N_T + kGenericRows - 1) / kGenericRows;
+    pl.pieces = pl.pieces_y;
+    cudaStream_t st = (cudaStream_t)stream;
+    float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
+    const Outputs out{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
+    const Consts k{C1, C2, C, D};
+    int rc;
+    switch (pixel_type) {
+        case IQA_PIXEL_F64: rc = launch_typed<double>(x, y, g2, N_T, k, out, ws, pl, st); break;
+        case IQA_PIXEL_F16: rc = launch_typed<__half>(x, y, g2, N_T, k, out, ws, pl, st); break;
+        case IQA_PIXEL_I16: rc = launch_typed<short>(x, y, g2, N_T, k, out, ws, pl, st); break;
+        case IQA_PIXEL_I32: rc = launch_typed<int>(x, y, g2, N_T, k, out, ws, pl, st); break;
+        default: rc = launch_typed<unsigned char>(x, y, g2, N_T, k, out, ws, pl, st); break;
+    }
+    if (rc != IQA_OK) return rc;
+    return finish_comparisons(out, nullptr, 1, n, k, ws, pl, st);
 }
 
 int iqa_fused_batch_2d(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,

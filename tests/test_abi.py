@@ -197,6 +197,11 @@ def test_2d_validation():
     assert B.iqa_series_tiles_2d(tbl, 1, 0, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_SHAPE
     assert B.iqa_series_tiles_2d(bad, 3, 0, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_NULL
     assert B.iqa_series_tiles_2d(tbl, 3, 0, 64, 80, 80, 8, 1e-6, 1e-6, 0.0, 5e-7, *o) == B.IQA_ERR_PARAM
+    assert B.iqa_fused_tiles_2d_typed(FAKE, FAKE, 9, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_SHAPE          # unknown type
+    assert B.iqa_fused_tiles_2d_typed(FAKE, None, B.IQA_PIXEL_I16, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_NULL
+    assert B.iqa_fused_tiles_2d_typed(FAKE + 4, FAKE, B.IQA_PIXEL_F64, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_ALIGN
+    assert B.iqa_fused_tiles_2d_typed(FAKE, FAKE, B.IQA_PIXEL_F16, 64, 64, 60, 64, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_fused_tiles_2d_typed(FAKE, FAKE, B.IQA_PIXEL_F32, 64, 0, 64, 64, 8, *a, *o) == B.IQA_ERR_SHAPE
     # the square entry points keep the paper's divisibility requirement
     assert B.iqa_fused_tiles(FAKE, FAKE, 100, 64, *a, *o) == B.IQA_ERR_SHAPE
 

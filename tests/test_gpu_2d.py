@@ -180,3 +180,56 @@ def test_batch_and_series_2d(B, U, H, W, N_T, pitch, off):
             ref = oracle.tiles_2d(imgs[ix], imgs[iy], N_T, **K)
             got = {n: so[n][c].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
             U.assert_parity(got, ref, K["C"], f"series_2d {mode} {c}")
+
+
+@pytest.mark.parametrize("dtype,lo,hi", [("float64", -0.2, 1.0), ("float16", -2.0, 8.0), ("int16", -300, 3000),
+                                         ("int32", -1000, 1 << 20), ("uint8", 0, 255)])
+@pytest.mark.parametrize("H,W,N_T", [(100, 130, 16), (257, 300, 64), (300, 200, 150), (64, 64, 8)])
+def test_other_pixel_types(B, U, dtype, lo, hi, H, W, N_T):
+    """iqa_fused_tiles_2d_typed against oracle.tiles_2d_any (pixels -> double exactly, Eqs. 1-2 in double)."""
+    import torch
+    import oracle
+    rng = np.random.default_rng(H + W + N_T)
+    dt = np.dtype(dtype)
+    x = rng.uniform(lo, hi, (H, W)).astype(dt)
+    y = rng.uniform(lo, hi, (H, W)).astype(dt)
+    m = rng.random((H, W)) < 0.3
+    y[m] = x[m]
+    k = dict(C1=1e-3, C2=1e-3, C=1e-3, D=5e-4) if dt.kind in "iu" else K      # integer counts: C's of that scale
+    xd, yd = torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda()
+    got = B.fused_tiles_2d(xd, yd, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    torch.cuda.synchronize()
+    g = {n: v.cpu().numpy().astype(np.float64) for n, v in got.items()}
+    ref = oracle.tiles_2d_any(x, y, N_T, **k)
+    U.assert_parity(g, ref, k["C"], f"{dtype} {H}x{W} N_T={N_T}")
+
+
+def test_fp64_pixels_keep_their_small_differences(B, U):
+    """Doubles that differ by ~3e-7 (a few fp32 ulps, the order of C1): the kernel subtracts in fp64 and stays
+    within 1e-5 of the oracle, where rounding the inputs to fp32 first is off by percents."""
+    import torch
+    import oracle
+    rng = np.random.default_rng(4)
+    x = rng.normal(0.5, 0.5, (128, 192))
+    y = x + rng.normal(0.0, 3e-7, (128, 192))
+    got = B.fused_tiles_2d(torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda(), 32, K["C1"], K["C2"], K["C"], K["D"],
+                           numerators=True)
+    torch.cuda.synchronize()
+    g = {n: v.cpu().numpy().astype(np.float64) for n, v in got.items()}
+    ref = oracle.tiles_2d_any(x, y, 32, **K)
+    U.assert_parity(g, ref, K["C"], "fp64 small differences")
+    rounded = oracle.tiles_2d(x.astype(np.float32), y.astype(np.float32), 32, **K)
+    assert np.max(np.abs(rounded["L"] - ref["L"]) / ref["L"]) > 1e-3
+
+
+def test_typed_error_codes(B):
+    import torch
+    x = torch.zeros((64, 64), dtype=torch.float64, device="cuda")
+    o = [torch.zeros(64, dtype=torch.float32, device="cuda") for _ in range(4)]
+    a = (K["C1"], K["C2"], K["C"], K["D"])
+    assert B.iqa_fused_tiles_2d_typed(x, x, B.IQA_PIXEL_F64, 64, 64, 64, 64, 8, *a, *o) == B.IQA_OK
+    assert B.iqa_fused_tiles_2d_typed(x, x, 9, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_fused_tiles_2d_typed(x, None, B.IQA_PIXEL_F64, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_NULL
+    assert B.iqa_fused_tiles_2d_typed(x.data_ptr() + 4, x, B.IQA_PIXEL_F64, 32, 32, 64, 64, 8, *a, *o) == B.IQA_ERR_ALIGN
+    assert B.iqa_fused_tiles_2d_typed(x, x, B.IQA_PIXEL_F64, 64, 64, 64, 64, 128, *a, *o) == B.IQA_ERR_WORKSPACE
+    torch.cuda.synchronize()
