@@ -474,8 +474,11 @@ def measure_read_ceiling():
     over box shapes / ring depths / CTAs per SM, and prints the best rate."""
     import subprocess
     from paper_2501_10653_b200 import build
-    exe = build.build_read_ceiling()
-    out = subprocess.run([exe], capture_output=True, text=True, timeout=300).stdout
+    try:
+        exe = build.build_read_ceiling()
+        out = subprocess.run([exe], capture_output=True, text=True, timeout=300).stdout
+    except Exception as exc:           # the probe is a diagnostic: never let it take the bench line down
+        return {"GBps": None, "error": repr(exc)[:300]}
     best = [ln for ln in out.splitlines() if ln.startswith("best")]
     if not best:
         return {"GBps": None, "error": out[-300:]}
