@@ -547,8 +547,12 @@ def run_ours(args):
         # read-only ceiling of the kernel's own access pattern, and the time-series modes at N = 8192
         also["read_ceiling"] = measure_read_ceiling()
         cs = synth.CONFIGS[3] if args.workload in ("cfg1", "cfg3") else cfg
-        also[f"series_{cs.name}_M{args.series_images}"] = measure_series(
-            torch, binding, cs, args.series_images, max(3, min(K, 10)), 3, device, use_graph)
+        try:                                   # an extra: its failure must not cost the headline line
+            also[f"series_{cs.name}_M{args.series_images}"] = measure_series(
+                torch, binding, cs, args.series_images, max(3, min(K, 10)), 3, device, use_graph)
+        except Exception as exc:
+            also[f"series_{cs.name}_M{args.series_images}"] = {"error": repr(exc)[:300]}
+            torch.cuda.empty_cache()
     if args.entry_points and world == 1:
         also["entry_points_cold"] = measure_entry_points(torch, cfg, pairs, max(3, min(K, 20)), max(3, W), device, use_graph)
     if args.sweep and world == 1:
