@@ -209,7 +209,8 @@ def test_symmetry_bitwise(U):
 
 
 def test_determinism_and_mapping_independence(U, monkeypatch):
-    """P12: two runs bit-identical; every mapping (stream variants 0-2, generic kernel) agrees to 2e-6."""
+    """P12: two runs bit-identical; every mapping (TMA ring / box configurations, cp.async variants 0-2, generic
+    kernel) agrees with the oracle and with the default mapping to 2e-6."""
     cfg = synth.CONFIGS[0]
     x, y, _ = synth.make_pair(synth.scaled(synth.CONFIGS[3], 1024))
     xd, yd = U.to_dev(x), U.to_dev(y)
@@ -221,7 +222,8 @@ def test_determinism_and_mapping_independence(U, monkeypatch):
             assert np.array_equal(base[nm], again[nm]), (N_T, nm)
         ref = U.run_oracle(x, y, N_T, k)
         for env, val in (("IQA_FORCE_VARIANT", "0"), ("IQA_FORCE_VARIANT", "1"), ("IQA_FORCE_VARIANT", "2"),
-                         ("IQA_FORCE_GENERIC", "1")):
+                         ("IQA_FORCE_GENERIC", "1"), ("IQA_TMA_CONFIG", "0"), ("IQA_TMA_CONFIG", "2"),
+                         ("IQA_TMA_CONFIG", "3"), ("IQA_TMA_CONFIG", "4")):
             monkeypatch.setenv(env, val)
             other = U.run_gpu(xd, yd, N_T, k)
             monkeypatch.delenv(env)
