@@ -76,7 +76,7 @@ size_t stream_smem(int variant) {
 using TmaFn = void (*)(const TmaParams);
 
 // TMA kernel configurations: {box slots per CTA, rows per warp and box}.  Measured on B200
-// (profiles/r01f_tma_configs.md): pairs are HBM-bound and want FEW bytes in flight (config 1: two
+// (profiles/r01g_tma_configs.md): pairs are HBM-bound and want FEW bytes in flight (config 1: two
 // 16 KiB boxes in flight per CTA while two are consumed; six boxes lose 3-6 % to DRAM locality, as
 // the cp.async variants did); the series modes keep S + 1 boxes alive and want the deeper ring of
 // config 0.  IQA_TMA_CONFIG=c forces one (tuning knob).
