@@ -144,12 +144,14 @@ generic_kernel(const GenericParams g) {
     const size_t row0 = (size_t)ty * N_T + r_begin, col0 = (size_t)tx * N_T;
 
     float aL = 0.f, aA = 0.f, aX = 0.f, aY = 0.f;
-    for (long long k = threadIdx.x; k < npix; k += kCtaThreads) {
-        const int r = (int)(k / cols_t), c = (int)(k % cols_t);
-        const size_t ox = (row0 + r) * (size_t)p.pitch_x + col0 + c;
-        const size_t oy = (row0 + r) * (size_t)p.pitch_y + col0 + c;
-        pixel_terms_any<MODE, T>(reinterpret_cast<const T*>(p.x), reinterpret_cast<const T*>(p.y), ox, oy, p.C1,
-                                 aL, aA, aX, aY);
+    // warp w takes rows w, w + 8, ...; lanes stride over the columns (coalesced, no division per pixel)
+    (void)npix;
+    for (int r = (int)(threadIdx.x >> 5); r < r_end - r_begin; r += kWarpsPerCta) {
+        const size_t bx = (row0 + r) * (size_t)p.pitch_x + col0;
+        const size_t by = (row0 + r) * (size_t)p.pitch_y + col0;
+        for (int c = (int)(threadIdx.x & 31); c < cols_t; c += 32)
+            pixel_terms_any<MODE, T>(reinterpret_cast<const T*>(p.x), reinterpret_cast<const T*>(p.y), bx + c, by + c,
+                                     p.C1, aL, aA, aX, aY);
     }
     float4 v = make_float4(aL, aA, aX, aY);
     for (int o = 16; o > 0; o >>= 1) {
@@ -190,6 +192,9 @@ generic_warp_kernel(const GenericParams g, long long n_tiles) {
     const int npix = rows_t * cols_t;
     const size_t row0 = (size_t)ty * N_T, col0 = (size_t)tx * N_T;
     float aL = 0.f, aA = 0.f, aX = 0.f, aY = 0.f;
+    // independent addresses per iteration (the divisions are cheap next to the load latency of a lone warp,
+    // and the unrolled loop keeps several loads in flight)
+#pragma unroll 4
     for (int k = lane; k < npix; k += 32) {
         const int r = k / cols_t, c = k % cols_t;
         const size_t ox = (row0 + r) * (size_t)p.pitch_x + col0 + c;
