@@ -25,6 +25,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+PAIRS_PER_LAUNCH = 64      # kMaxImages / 2 of csrc/iqa_tma.cuh: tensor maps that fit one launch's parameters
 METRIC = "us_per_image_pair"
 UNIT = "us/pair"
 
@@ -223,7 +224,7 @@ class Batch:
 
     def launches_per_step(self, aggregate=True):
         split = self.wsb > 0
-        return -(-self.P // 32) + (1 if split else 0) + (1 if aggregate else 0)
+        return -(-self.P // PAIRS_PER_LAUNCH) + (1 if split else 0) + (1 if aggregate else 0)
 
     def graph(self, fn):
         torch = self.torch
@@ -514,7 +515,7 @@ def run_ours(args):
     m = measure_workload(torch, binding, cfg, pairs, K, W, device, dist, use_graph, rank, latency=not args.no_latency)
     total_pairs = K * pairs * world
     us_per_pair = m["ms"] * 1e3 / total_pairs
-    n_stream = -(-pairs // 32)                               # launches of the stream kernel per step
+    n_stream = -(-pairs // PAIRS_PER_LAUNCH)                 # launches of the tile kernel per step
     us_launch = m["ms_kernel"] * 1e3 / (K * n_stream)       # per launch of the stream kernel (max over ranks)
     us_single, us_single_cold, clocks = m["us_single_pair_warm"], m["us_single_pair_cold"], m["clocks"]
     step_us = m["step_us"]

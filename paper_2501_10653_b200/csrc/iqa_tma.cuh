@@ -54,7 +54,7 @@
 
 namespace iqa {
 
-constexpr int kMaxImages = 64;                 // tensor maps per launch (kernel parameter space: 8 KiB)
+constexpr int kMaxImages = 128;                // tensor maps per launch (kernel parameter space: 16 KiB of the 32 KiB limit)
 // Box geometry and ring size are template parameters of the kernel:
 //   RPW  rows per consumer warp and box (box = 8 RPW rows x 128 columns: 16 KiB for RPW = 4)
 //   NB   box slots per CTA (NB boxes of shared memory; 2 CTAs per SM)

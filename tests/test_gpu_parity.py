@@ -245,7 +245,7 @@ def test_standalone_entry_points_match_fused(U, B):
 
 
 @pytest.mark.parametrize("N,N_T,P", [(256, 16, 5), (2048, 64, 3), (1024, 8, 2), (1024, 256, 3), (392, 8, 4),
-                                     (200, 100, 2), (512, 128, 40)])
+                                     (200, 100, 2), (512, 128, 40), (256, 16, 70)])
 def test_fused_batch_matches_per_pair_calls_and_oracle(U, B, N, N_T, P):
     """iqa_fused_batch == P calls of iqa_fused_tiles + iqa_aggregate, bit for bit, and == the oracle."""
     cfg = synth.scaled(synth.CONFIGS[3], N, N_T)

@@ -89,8 +89,8 @@ def test_series_config1_sky(B, U, mode):
 
 @pytest.mark.parametrize("mode", MODES)
 def test_long_series_spans_several_launches(B, U, mode):
-    """More images than tensor maps fit in one launch (64): chunks that share one image."""
-    _run_and_check(B, U, _rand_series(128, 70, seed=5), mode, 16, _consts(), "M=70")
+    """More images than tensor maps fit in one launch (128): chunks that share one image."""
+    _run_and_check(B, U, _rand_series(128, 140, seed=5), mode, 16, _consts(), "M=140")
 
 
 @pytest.mark.parametrize("mode", MODES)
