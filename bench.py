@@ -524,6 +524,7 @@ def run_ours(args):
     achieved = alg / (us_launch * 1e-6) / 1e9
     split = binding.iqa_workspace_bytes(cfg.N, cfg.N_T) > 0
     launches = m["batch"].launches_per_step(True)
+    plan = binding.plan_name(m["batch"].x[0], cfg.N_T)           # the kernel the library really picked
     del m
     torch.cuda.empty_cache()
 
@@ -573,6 +574,7 @@ def run_ours(args):
             "launch": ("cuda graph of the step" if use_graph else "direct launches through ctypes")
                       + ": one iqa_fused_batch call per step",
             "gpu_launches": K * world * launches,
+            "plan": plan,
             "kernels": ["iqa::tma_kernel<3,0,NB,RPW> (fused S1-S4, all pairs of the step)"]
                        + (["iqa::finalise_*_kernel"] if split else []) + ["iqa::aggregate_kernel (S5, one CTA per pair)"],
             "roofline": {"bound": "hbm", "kernel": "iqa::tma_kernel<fused, pairs>", "achieved": achieved, "peak": peak,

@@ -98,6 +98,17 @@ int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
                     float* lisi_num, float* auglisi_num,
                     void* workspace, size_t workspace_bytes, void* stream);
 
+/* Diagnostic: which kernel a call on this image would take (host-side decision only, nothing is enqueued).
+ *   x, H, W, pitch, N_T as for iqa_fused_tiles_2d (H == W == pitch, W % N_T == 0: as for the square entry points);
+ *   series != 0: as for the time-series entry points.
+ * Returns IQA_PLAN_GENERIC, IQA_PLAN_CP_ASYNC, or IQA_PLAN_TMA + c (c = ring / box configuration of the TMA
+ * kernel, 0..4); -1 for bad arguments.  bench.py reports it, and the GPU tests assert that every
+ * BASELINE.json configuration takes the TMA kernel -- a silent fall-back would cost bandwidth, not parity. */
+#define IQA_PLAN_GENERIC 0
+#define IQA_PLAN_CP_ASYNC 1
+#define IQA_PLAN_TMA 16
+int iqa_query_plan(const float* x, int H, int W, long long pitch, int N_T, int series);
+
 /* ---- general images -------------------------------------------------------
  * The paper's images are square and N is a multiple of N_T.  This entry point drops
  * both: an H x W image with a row pitch (elements between rows; a sub-window of a larger array, a

@@ -24,7 +24,7 @@ IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKS
 
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
-           "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_tiles_2d_typed", "iqa_fused_batch_2d", "iqa_series_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
+           "iqa_query_plan", "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_tiles_2d_typed", "iqa_fused_batch_2d", "iqa_series_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
            "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
@@ -71,6 +71,8 @@ def _load() -> ctypes.CDLL:
     lib.iqa_series_workspace_bytes.argtypes = [i, i, i]
     lib.iqa_series_tiles.restype = i
     lib.iqa_series_tiles.argtypes = [vp, i, i, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_query_plan.restype = i
+    lib.iqa_query_plan.argtypes = [vp, i, i, ctypes.c_longlong, i, i]
     lib.iqa_workspace_bytes_2d.restype = sz
     lib.iqa_workspace_bytes_2d.argtypes = [i, i, i]
     lib.iqa_fused_tiles_2d.restype = i
@@ -194,6 +196,19 @@ def iqa_fused_batch(x_ptrs_host, y_ptrs_host, n_pairs, N, N_T, C1, C2, C, D, lis
                                _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
                                _ptr(lisi_num), _ptr(auglisi_num), _ptr(out2),
                                _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
+IQA_PLAN_GENERIC, IQA_PLAN_CP_ASYNC, IQA_PLAN_TMA = 0, 1, 16
+
+
+def iqa_query_plan(x, H, W, pitch, N_T, series=0) -> int:
+    return int(lib.iqa_query_plan(_ptr(x), int(H), int(W), int(pitch), int(N_T), int(series)))
+
+
+def plan_name(x, N_T, series=False) -> str:
+    """Which kernel a call on the CUDA tensor ``x`` would take: 'tma:c<k>', 'cp.async' or 'generic'."""
+    p = iqa_query_plan(x, x.shape[0], x.shape[1], x.stride(0), N_T, 1 if series else 0)
+    return f"tma:c{p - IQA_PLAN_TMA}" if p >= IQA_PLAN_TMA else {0: "generic", 1: "cp.async"}.get(p, "invalid")
 
 
 def iqa_workspace_bytes_2d(H: int, W: int, N_T: int) -> int:

@@ -645,6 +645,15 @@ int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
     return run_batch(kModeFused, &x, &y, 1, N, N_T, C1, C2, C, D, o, nullptr, workspace, workspace_bytes, stream);
 }
 
+int iqa_query_plan(const float* x, int H, int W, long long pitch, int N_T, int series) {
+    if (!x || H <= 0 || W <= 0 || N_T <= 0 || pitch < W) return -1;
+    const Geom2D g2{H, W, pitch, pitch};
+    const bool aligned16 = (((uintptr_t)x & 15u) == 0) && (pitch % 4 == 0);
+    const bool square = H == W && pitch == W && W % N_T == 0;      // what the paper-named entry points see
+    const Plan pl = make_plan(W, N_T, aligned16, x, series != 0, square ? nullptr : &g2);
+    return pl.kind == kPlanTma ? IQA_PLAN_TMA + pl.tma_cfg : pl.kind == kPlanStream ? IQA_PLAN_CP_ASYNC : IQA_PLAN_GENERIC;
+}
+
 size_t iqa_workspace_bytes_2d(int H, int W, int N_T) {
     if (H <= 0 || W <= 0 || N_T <= 0 || H > kMaxN || W > kMaxN) return 0;
     const size_t pieces = max_pieces(N_T);

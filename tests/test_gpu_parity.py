@@ -354,6 +354,21 @@ def test_host_pipeline_two_streams(U, B):
         assert abs(out2[0].item() - exp[0]) <= 1e-5 * abs(exp[0]) and abs(out2[1].item() - exp[1]) <= 1e-5 * abs(exp[1])
 
 
+def test_every_baseline_configuration_takes_the_tma_kernel(B):
+    """A silent fall-back to the cp.async or generic kernel would keep parity and lose bandwidth: assert the plan."""
+    for idx in range(5):
+        cfg = synth.CONFIGS[idx]
+        x = torch.empty((cfg.N, cfg.N), dtype=torch.float32, device="cuda")
+        for N_T in (cfg.sweep_N_T or (cfg.N_T,)):
+            assert B.plan_name(x, N_T) == "tma:c1", (cfg.name, N_T)
+            assert B.plan_name(x, N_T, series=True) == "tma:c0", (cfg.name, N_T)
+        del x
+    x = torch.empty((300, 516), dtype=torch.float32, device="cuda")
+    assert B.plan_name(x[:, :513], 64).startswith("tma")            # pitched window, W % 4 != 0
+    assert B.plan_name(x[:, 1:514], 64) == "generic"                # base not 16-byte aligned
+    assert B.plan_name(x, 100) == "generic"                         # tile side not a power of two
+
+
 def test_many_small_tiles(U):
     """N=4096, N_T=8: 262144 tiles (16 tile segments per warp row)."""
     x, y = _rand_pair(4096, seed=5)
