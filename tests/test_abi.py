@@ -202,6 +202,10 @@ def test_2d_validation():
     assert B.iqa_fused_tiles_2d_typed(FAKE + 4, FAKE, B.IQA_PIXEL_F64, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_ALIGN
     assert B.iqa_fused_tiles_2d_typed(FAKE, FAKE, B.IQA_PIXEL_F16, 64, 64, 60, 64, 8, *a, *o) == B.IQA_ERR_SHAPE
     assert B.iqa_fused_tiles_2d_typed(FAKE, FAKE, B.IQA_PIXEL_F32, 64, 0, 64, 64, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_query_plan(None, 64, 64, 64, 8) == -1 and B.iqa_query_plan(FAKE, 64, 64, 60, 8) == -1
+    assert B.iqa_query_plan(FAKE, 64, 64, 64, 7) == B.IQA_PLAN_GENERIC           # tile side not a power of two
+    assert B.iqa_query_plan(FAKE + 4, 64, 64, 64, 8) == B.IQA_PLAN_GENERIC       # base not 16-byte aligned
+    assert B.iqa_query_plan(FAKE, 64, 64, 64, 8) in (B.IQA_PLAN_CP_ASYNC, B.IQA_PLAN_TMA + 1)   # no driver here: cp.async
     # the square entry points keep the paper's divisibility requirement
     assert B.iqa_fused_tiles(FAKE, FAKE, 100, 64, *a, *o) == B.IQA_ERR_SHAPE
 
