@@ -58,7 +58,6 @@ constexpr int kMaxImages = 128;                // tensor maps per launch (kernel
 // Box geometry and ring size are template parameters of the kernel:
 //   RPW  rows per consumer warp and box (box = 8 RPW rows x 128 columns: 16 KiB for RPW = 4)
 //   NB   box slots per CTA (NB boxes of shared memory; 2 CTAs per SM)
-constexpr int kMaxBoxSlots = 12;
 constexpr int kTmaThreads = kCtaThreads + 64;  // + the producer warp + the finaliser warp
 constexpr int kPartBufs = 4;                   // per-warp partial sums in flight between consumers and finaliser
 
