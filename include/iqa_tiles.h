@@ -271,6 +271,14 @@ int iqa_merge_tiles(const float* lisi, const float* auglisi,
                     float* lisi_out, float* auglisi_out,
                     float* sum_x_out, float* sum_y_out, void* stream);
 
+/* The same for n_maps matrices at once ([n_maps][nt*nt] in, [n_maps][(nt/g)^2] out): the comparisons of a
+ * time series or the pairs of a batch -- multi-scale localisation of every comparison in one launch. */
+int iqa_merge_tiles_batch(const float* lisi, const float* auglisi,
+                          const float* sum_x, const float* sum_y, int nt, int g, int n_maps,
+                          float C2, float C,
+                          float* lisi_out, float* auglisi_out,
+                          float* sum_x_out, float* sum_y_out, void* stream);
+
 /* Bytes of DEVICE scratch iqa_fused_host needs for (N, N_T): both images, the four per-tile
  * arrays, out2 and the kernel workspace.  0 for invalid shapes. */
 size_t iqa_host_scratch_bytes(int N, int N_T);

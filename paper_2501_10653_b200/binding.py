@@ -25,7 +25,7 @@ IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKS
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
            "iqa_query_plan", "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_tiles_2d_typed", "iqa_fused_batch_2d", "iqa_series_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
-           "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
+           "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_merge_tiles_batch", "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
 IQA_PIXEL_F32, IQA_PIXEL_F64, IQA_PIXEL_F16, IQA_PIXEL_I16, IQA_PIXEL_I32, IQA_PIXEL_U8 = range(6)
@@ -97,6 +97,8 @@ def _load() -> ctypes.CDLL:
     lib.iqa_tiles_bottom_k.argtypes = [vp, i, i, i, vp, vp, vp]
     lib.iqa_aggregate.restype = i
     lib.iqa_aggregate.argtypes = [vp, vp, vp, vp, i, f, f, vp, vp]
+    lib.iqa_merge_tiles_batch.restype = i
+    lib.iqa_merge_tiles_batch.argtypes = [vp, vp, vp, vp, i, i, i, f, f, vp, vp, vp, vp, vp]
     lib.iqa_merge_tiles.restype = i
     lib.iqa_merge_tiles.argtypes = [vp, vp, vp, vp, i, i, f, f, vp, vp, vp, vp, vp]
     lib.iqa_fused_host.restype = i
@@ -615,19 +617,30 @@ def aggregate_finish(sums4, n_tiles_total, C2, C):
     return out2
 
 
+def iqa_merge_tiles_batch(lisi, auglisi, sum_x, sum_y, nt, g, n_maps, C2, C,
+                          lisi_out, auglisi_out, sum_x_out, sum_y_out, stream=None) -> int:
+    return lib.iqa_merge_tiles_batch(_ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), int(nt), int(g), int(n_maps),
+                                     C2, C, _ptr(lisi_out), _ptr(auglisi_out), _ptr(sum_x_out),
+                                     _ptr(sum_y_out), _stream(stream))
+
+
 def merge_tiles(lisi, auglisi, X, Y, g, C2, C) -> dict:
-    """Eqs. 3-4 on every g x g block of the (nt, nt) matrices -> (nt/g, nt/g) matrices."""
+    """Eqs. 3-4 on every g x g block of the (nt, nt) matrices -> (nt/g, nt/g) matrices; (n_maps, nt, nt)
+    stacks (the comparisons of a series, the pairs of a batch) are merged map by map in one launch."""
     import torch
-    nt = int(lisi.shape[0])
-    if g <= 0 or nt % g:
+    batched = lisi.dim() == 3
+    nt = int(lisi.shape[-1])
+    n_maps = int(lisi.shape[0]) if batched else 1
+    if g <= 0 or nt % g or lisi.shape[-2] != nt or not lisi.is_contiguous():
         raise IqaError(IQA_ERR_SHAPE, "merge_tiles")
     no = nt // g
-    out = {k: torch.empty((no, no), dtype=torch.float32, device=lisi.device)
+    shape = (n_maps, no, no) if batched else (no, no)
+    out = {k: torch.empty(shape, dtype=torch.float32, device=lisi.device)
            for k in ("lisi", "auglisi", "X", "Y")}
-    rc = iqa_merge_tiles(lisi, auglisi, X, Y, nt, g, C2, C, out["lisi"], out["auglisi"], out["X"],
-                         out["Y"], _current_stream(lisi.device))
+    rc = iqa_merge_tiles_batch(lisi, auglisi, X, Y, nt, g, n_maps, C2, C, out["lisi"], out["auglisi"], out["X"],
+                               out["Y"], _current_stream(lisi.device))
     if rc != IQA_OK:
-        raise IqaError(rc, "iqa_merge_tiles")
+        raise IqaError(rc, "iqa_merge_tiles_batch")
     return out
 
 
@@ -635,7 +648,7 @@ def pyramid(tiles: dict, C2, C) -> list:
     """All levels N_T, 2 N_T, 4 N_T, ... up to the coarsest the tile count allows (factor-2 merges)."""
     levels = [tiles]
     cur = tiles
-    while cur["lisi"].shape[0] % 2 == 0 and cur["lisi"].shape[0] > 1:
+    while cur["lisi"].shape[-1] % 2 == 0 and cur["lisi"].shape[-1] > 1:
         cur = merge_tiles(cur["lisi"], cur["auglisi"], cur["X"], cur["Y"], 2, C2, C)
         levels.append(cur)
     return levels

@@ -147,28 +147,31 @@ __global__ void aggregate_finish_kernel(const double* __restrict__ sums4, double
 // (oy*g .. oy*g+g-1, ox*g .. ox*g+g-1) of the nt x nt matrix.
 __global__ void __launch_bounds__(256)
 merge_kernel(const float* __restrict__ lisi, const float* __restrict__ aug,
-             const float* __restrict__ X, const float* __restrict__ Y, int nt, int g,
+             const float* __restrict__ X, const float* __restrict__ Y, int nt, int g, int n_maps,
              float C2f, float Cf,
              float* __restrict__ lisi_o, float* __restrict__ aug_o,
              float* __restrict__ X_o, float* __restrict__ Y_o) {
     pdl_prologue();
     const int nto = nt / g;
-    const long long o = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
-    if (o >= (long long)nto * nto) return;
+    const long long per_map = (long long)nto * nto;
+    const long long og = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);      // output tile over all maps
+    if (og >= per_map * n_maps) return;
+    const long long map = og / per_map, o = og % per_map;
+    const size_t in0 = (size_t)map * nt * nt;
     const int lane = threadIdx.x & 31;
     const int oy = (int)(o / nto), ox = (int)(o % nto);
     const double C2 = (double)C2f, C = (double)Cf;
     Agg4 a = {0.0, 0.0, 0.0, 0.0};
     const int gg = g * g;
     for (int k = lane; k < gg; k += 32) {
-        const size_t t = (size_t)(oy * g + k / g) * nt + (size_t)(ox * g + k % g);
+        const size_t t = in0 + (size_t)(oy * g + k / g) * nt + (size_t)(ox * g + k % g);
         agg_add(a, lisi[t], aug[t], X[t], Y[t], C2, C);
     }
     a = agg_warp_sum(a);
     if (lane == 0) {
-        agg_finish(a, (double)gg, C2, C, lisi_o + o, aug_o + o);
-        X_o[o] = (float)a.sx;
-        Y_o[o] = (float)a.sy;
+        agg_finish(a, (double)gg, C2, C, lisi_o + og, aug_o + og);
+        X_o[og] = (float)a.sx;
+        Y_o[og] = (float)a.sy;
     }
 }
 

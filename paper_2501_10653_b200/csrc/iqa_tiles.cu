@@ -846,22 +846,31 @@ int iqa_tiles_bottom_k(const float* values, int n_tiles, int n_maps, int k,
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }
 
+int iqa_merge_tiles_batch(const float* lisi, const float* auglisi,
+                          const float* sum_x, const float* sum_y, int nt, int g, int n_maps,
+                          float C2, float C,
+                          float* lisi_out, float* auglisi_out,
+                          float* sum_x_out, float* sum_y_out, void* stream) {
+    if (!lisi || !auglisi || !sum_x || !sum_y || !lisi_out || !auglisi_out || !sum_x_out || !sum_y_out)
+        return IQA_ERR_NULL;
+    if (nt <= 0 || g <= 0 || g > nt || nt % g != 0 || n_maps <= 0 || (long long)nt * nt * n_maps > 0x7fffffffLL)
+        return IQA_ERR_SHAPE;
+    if (!pos_finite(C2) || !pos_finite(C)) return IQA_ERR_PARAM;
+    const long long n_out = (long long)(nt / g) * (nt / g) * n_maps;
+    const unsigned grid = (unsigned)((n_out + 7) / 8);
+    if (launch(merge_kernel, grid, 256u, 0, (cudaStream_t)stream, lisi, auglisi, sum_x, sum_y, nt, g, n_maps, C2, C,
+               lisi_out, auglisi_out, sum_x_out, sum_y_out) != cudaSuccess)
+        return IQA_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+}
+
 int iqa_merge_tiles(const float* lisi, const float* auglisi,
                     const float* sum_x, const float* sum_y, int nt, int g,
                     float C2, float C,
                     float* lisi_out, float* auglisi_out,
                     float* sum_x_out, float* sum_y_out, void* stream) {
-    if (!lisi || !auglisi || !sum_x || !sum_y || !lisi_out || !auglisi_out || !sum_x_out || !sum_y_out)
-        return IQA_ERR_NULL;
-    if (nt <= 0 || g <= 0 || g > nt || nt % g != 0 || (long long)nt * nt > 0x7fffffffLL)
-        return IQA_ERR_SHAPE;
-    if (!pos_finite(C2) || !pos_finite(C)) return IQA_ERR_PARAM;
-    const long long n_out = (long long)(nt / g) * (nt / g);
-    const unsigned grid = (unsigned)((n_out + 7) / 8);
-    if (launch(merge_kernel, grid, 256u, 0, (cudaStream_t)stream, lisi, auglisi, sum_x, sum_y, nt, g, C2, C,
-               lisi_out, auglisi_out, sum_x_out, sum_y_out) != cudaSuccess)
-        return IQA_ERR_CUDA;
-    return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+    return iqa_merge_tiles_batch(lisi, auglisi, sum_x, sum_y, nt, g, 1, C2, C, lisi_out, auglisi_out, sum_x_out,
+                                 sum_y_out, stream);
 }
 
 size_t iqa_host_scratch_bytes(int N, int N_T) {

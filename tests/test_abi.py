@@ -108,6 +108,8 @@ def test_standalone_and_aggregate_validation():
     assert B.iqa_merge_tiles(FAKE, FAKE, FAKE, FAKE, 8, 3, 1e-6, 1e-6, FAKE, FAKE, FAKE, FAKE) == B.IQA_ERR_SHAPE
     assert B.iqa_merge_tiles(FAKE, FAKE, FAKE, FAKE, 8, 0, 1e-6, 1e-6, FAKE, FAKE, FAKE, FAKE) == B.IQA_ERR_SHAPE
     assert B.iqa_merge_tiles(FAKE, FAKE, FAKE, FAKE, 8, 2, 1e-6, math.nan, FAKE, FAKE, FAKE, FAKE) == B.IQA_ERR_PARAM
+    assert B.iqa_merge_tiles_batch(FAKE, FAKE, FAKE, FAKE, 8, 2, 0, 1e-6, 1e-6, FAKE, FAKE, FAKE, FAKE) == B.IQA_ERR_SHAPE
+    assert B.iqa_merge_tiles_batch(FAKE, FAKE, FAKE, FAKE, 8, 2, 3, 1e-6, 1e-6, FAKE, None, FAKE, FAKE) == B.IQA_ERR_NULL
     assert B.iqa_fused_host(None, FAKE, 256, 16, 1e-6, 1e-6, 1e-6, 5e-7, None, None, None, None, None,
                             FAKE, 1 << 30) == B.IQA_ERR_NULL
     assert B.iqa_fused_host(FAKE, FAKE, 256, 16, 1e-6, 1e-6, 1e-6, 5e-7, None, None, None, None, None,

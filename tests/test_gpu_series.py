@@ -142,6 +142,33 @@ def test_series_ring_configurations(B, U, monkeypatch, cfg_id, N_T):
         _run_and_check(B, U, imgs, mode, N_T, _consts(), f"tma config {cfg_id} N_T={N_T}")
 
 
+@pytest.mark.parametrize("mode", MODES)
+def test_pyramid_of_a_series(B, U, mode):
+    """P:66 on every comparison of a series in one launch per level (iqa_merge_tiles_batch): the g x g merge of the
+    N_T = 16 matrices equals the oracle's series at tile size 16 g."""
+    import torch
+    import oracle
+    imgs = _rand_series(256, 4, seed=21)
+    dev = [U.to_dev(a) for a in imgs]
+    k = _consts()
+    base = B.series_tiles(dev, mode, 16, k["C1"], k["C2"], k["C"], k["D"])
+    for g in (2, 4, 16):
+        m = B.merge_tiles(base["lisi"], base["auglisi"], base["X"], base["Y"], g, k["C2"], k["C"])
+        torch.cuda.synchronize()
+        ref = oracle.series(imgs, mode, 16 * g, **k)
+        assert m["lisi"].shape == (3, 16 // g, 16 // g)
+        for c in range(3):
+            got = {n: m[n][c].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y")}
+            U.assert_parity(got, {n: ref[n][c] for n in list(got) + ["A"]}, k["C"], f"series merge g={g} cmp {c}")
+    levels = B.pyramid(base, k["C2"], k["C"])
+    assert [tuple(l["lisi"].shape) for l in levels] == [(3, 16, 16), (3, 8, 8), (3, 4, 4), (3, 2, 2), (3, 1, 1)]
+    top = levels[-1]
+    for c in range(3):                      # the top of the pyramid is the whole-image pair of Eqs. 3-4
+        w = base["whole"][c].cpu().numpy()
+        assert abs(top["lisi"][c, 0, 0].item() - w[0]) <= 1e-5 * abs(w[0])
+        assert abs(top["auglisi"][c, 0, 0].item() - w[1]) <= 1e-5 * abs(w[1]) + 1e-6
+
+
 def test_series_determinism(B, U):
     import torch
     imgs = [U.to_dev(a) for a in _rand_series(1024, 5, seed=2)]
