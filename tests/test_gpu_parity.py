@@ -94,6 +94,18 @@ def test_config2_tile_sweep(U, N_T):
     U.check_pair(x, y, N_T, U.consts(cfg), f"cfg2 N_T={N_T}", *_cfg2_dev(U))
 
 
+def test_config2_other_reading_of_the_generator(U):
+    """BASELINE.json config [2] says "same generator as config 1, seed 1"; R13 reads that as BJ index [1].
+    The other reading -- the FIRST listed config's generator (30 sources, sigma 1.5 px, log-uniform flux) on the
+    2048 canvas -- is run here too, over the ends and the middle of the sweep."""
+    from dataclasses import replace
+    cfg = replace(synth.CONFIGS[0], name="cfg2_alt_N2048", N=2048, N_T=64, seed=1)
+    x, y, _ = synth.make_pair(cfg)
+    xd, yd = U.to_dev(x), U.to_dev(y)
+    for N_T in (8, 64, 512):
+        U.check_pair(x, y, N_T, U.consts(cfg), f"cfg2 alt N_T={N_T}", xd, yd)
+
+
 _CFG2 = {}
 
 
