@@ -33,9 +33,9 @@ UNIT = "us/pair"
 WORKLOADS = {"cfg1": (1, 32, 8), "cfg3": (3, 8, 2), "cfg4": (4, 16, 1), "cfg0": (0, 64, 8)}
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused TMA kernel at the default pairs
-# per step, from the `ncu --set full` captures summarised under profiles/r01f_ncu_full_*_tma.md
+# per step, from the `ncu --set full` captures summarised under profiles/r01g_ncu_full_*_tma.md
 # (null when not captured for that workload; algorithmic bytes: cfg1 1.07427e9, cfg3 4.29706e9).
-NCU_TRAFFIC_BYTES = {"cfg1": 1.073819e9 + 4.387e6, "cfg3": 4.295092e9 + 6.723e6}
+NCU_TRAFFIC_BYTES = {"cfg1": 1.073771e9 + 4.429e6, "cfg3": 4.295015e9 + 4.734e6}
 
 
 def algorithmic_bytes(N: int, N_T: int) -> int:
