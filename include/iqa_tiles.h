@@ -13,6 +13,11 @@
  *   Eq. 3/4   tile -> whole-image aggregation of the two matrices
  *   merge     the "entire image" of Eqs. 3-4 may be a larger tile formed by
  *             merging g x g smaller ones
+ * and, built on the same kernels (each section below cites its passage):
+ *   series    K comparisons of a time series, every snapshot read from HBM once
+ *   finder    tiles below a threshold / the k lowest tiles of a matrix
+ *   general   H x W images with a row pitch, edge tiles, other pixel types
+ *   sharding  one pair over several GPUs by bands of tile rows
  *
  * Conventions (the paper states none; DESIGN.md "Boundary" and "Readings"):
  *   * Every pointer is a DEVICE pointer owned by the caller unless the argument name ends
