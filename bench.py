@@ -462,6 +462,20 @@ def measure_series(torch, binding, cfg, M, steps, warmup, device, use_graph):
                      "hbm_GBps": series_bytes(cfg.N, cfg.N_T, M) / (us * 1e-6) / 1e9,
                      "pairwise_equivalent_GBps": K * algorithmic_bytes(cfg.N, cfg.N_T) / (us * 1e-6) / 1e9,
                      "bytes_per_pixel_and_comparison": 4.0 * M / K}
+    # candidate extraction on the K augLISI matrices of the last call: bottom-16 and a threshold
+    aug3 = outs[1].view(K, cfg.N // cfg.N_T, cfg.N // cfg.N_T)
+    thr = float(torch.quantile(outs[1][0], 0.01))
+    idx = torch.empty((K, 16), dtype=torch.int32, device=device)
+    cnt = torch.empty(K, dtype=torch.int32, device=device)
+    cap = torch.empty((K, 1024), dtype=torch.int32, device=device)
+    st = lambda: torch.cuda.current_stream().cuda_stream
+    cand = {}
+    for name, fn in (("bottom_16", lambda: binding.iqa_tiles_bottom_k(aug3, n, K, 16, idx, None, st())),
+                     ("below_1pct_quantile", lambda: binding.iqa_tiles_below(aug3, n, K, thr, cap, 1024, cnt, st()))):
+        for _ in range(3):
+            assert fn() == 0
+        cand[name + "_us_per_call"] = time_region(torch, lambda: [fn() for _ in range(10)], 5) * 1e3 / 50
+    res["candidates"] = dict(cand, maps=K, tiles_per_map=n)
     res.update({"images": M, "comparisons": K, "N": cfg.N, "N_T": cfg.N_T,
                 "l2": f"{M * 4 * cfg.N * cfg.N / 2**20:.0f} MiB of snapshots per call"})
     del imgs, outs

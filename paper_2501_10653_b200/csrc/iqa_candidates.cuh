@@ -9,8 +9,8 @@
 // deterministic (the only atomics are integer histogram counts, which commute).
 //   order key   u = bits(v + 0.0f) (so -0 == +0), flipped so that unsigned order == float order;
 //               NaN (never produced: C2, C > 0) sorts last
-//   bottom-k    radix select (4 passes of 8 bits) finds the k-th smallest key and how many of its
-//               equals belong to the answer; an ordered compaction gathers the k selected
+//   bottom-k    radix select (8-bit digits, starting below the bits ALL keys share) finds the k-th smallest
+//               key and how many of its equals belong to the answer; an ordered compaction gathers the k selected
 //               (key, index) pairs in index order into shared memory; a bitonic sort orders them
 // =============================================================================
 #pragma once
@@ -21,9 +21,16 @@
 
 namespace iqa {
 
-constexpr int kCandThreads = 256;
-constexpr int kCandPerThread = 4;
-constexpr int kCandChunk = kCandThreads * kCandPerThread;
+constexpr int kCandThreads = 1024;     // at most: one CTA per matrix, as many threads as the matrix has 16-tile runs
+constexpr int kCandPerThread = 16;
+
+// Threads of the CTA for a matrix of n tiles: a power of two in [64, 1024] covering n / 16 (a small matrix must
+// not pay for 32 warps walking through the whole kernel).
+inline int cand_threads(int n) {
+    int t = 64;
+    while (t < kCandThreads && t * kCandPerThread < n) t <<= 1;
+    return t;
+}
 constexpr int kMaxBottomK = 1024;
 
 __device__ __forceinline__ uint32_t order_key(float v) {
@@ -32,7 +39,7 @@ __device__ __forceinline__ uint32_t order_key(float v) {
     return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 
-// Exclusive scan of one int per thread over the CTA (256 threads); returns the offset of this
+// Exclusive scan of one int per thread over the CTA (blockDim.x threads); returns the offset of this
 // thread and the CTA total.  `warp_tot` is shared scratch of kCandThreads / 32 ints.
 __device__ __forceinline__ int block_exclusive_scan(int c, int* warp_tot, int& total) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -46,8 +53,7 @@ __device__ __forceinline__ int block_exclusive_scan(int c, int* warp_tot, int& t
     if (lane == 31) warp_tot[w] = inc;
     __syncthreads();
     int base = 0, tot = 0;
-#pragma unroll
-    for (int i = 0; i < kCandThreads / 32; ++i) {
+    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) {
         const int t = warp_tot[i];
         if (i < w) base += t;
         tot += t;
@@ -55,6 +61,10 @@ __device__ __forceinline__ int block_exclusive_scan(int c, int* warp_tot, int& t
     total = tot;
     return base + inc - c;
 }
+
+// Work layout of both kernels: a SUPER-CHUNK is 16 blockDim.x consecutive tiles (16384 for 1024 threads); thread t
+// owns the kCandPerThread = 16 consecutive tiles [16 t, 16 t + 16) of it, so index order == (thread, j) order and one
+// block scan per super-chunk orders everything.  Matrices of up to one super-chunk are read from memory once.
 
 // values [n_maps][n]; indices [n_maps][capacity] (ascending tile index, first `capacity` only);
 // counts [n_maps] = number of tiles below the threshold (may exceed capacity).
@@ -65,24 +75,20 @@ below_kernel(const float* __restrict__ values, int n, float threshold, int* __re
     pdl_prologue();
     const float* v = values + (size_t)blockIdx.x * n;
     int* out = indices + (size_t)blockIdx.x * capacity;
+    const int kCandChunk = (int)blockDim.x * kCandPerThread;
     int base = 0;
     for (int c0 = 0; c0 < n; c0 += kCandChunk) {
         const int i0 = c0 + threadIdx.x * kCandPerThread;
-        bool f[kCandPerThread];
-        int c = 0;
-#pragma unroll
-        for (int j = 0; j < kCandPerThread; ++j) {
-            f[j] = (i0 + j < n) && (v[i0 + j] < threshold);
-            c += f[j];
-        }
-        int total;
-        int pos = base + block_exclusive_scan(c, warp_tot, total);
+        uint32_t flags = 0;
 #pragma unroll
         for (int j = 0; j < kCandPerThread; ++j)
-            if (f[j]) {
-                if (pos < capacity) out[pos] = i0 + j;
-                ++pos;
-            }
+            if (i0 + j < n && v[i0 + j] < threshold) flags |= 1u << j;
+        int total;
+        int pos = base + block_exclusive_scan(__popc(flags), warp_tot, total);
+        for (uint32_t f = flags; f; f &= f - 1) {
+            if (pos < capacity) out[pos] = i0 + (__ffs(f) - 1);
+            ++pos;
+        }
         base += total;
     }
     if (threadIdx.x == 0) counts[blockIdx.x] = base;
@@ -94,39 +100,82 @@ __global__ void __launch_bounds__(kCandThreads)
 bottom_k_kernel(const float* __restrict__ values, int n, int k, int* __restrict__ indices, float* __restrict__ vals) {
     __shared__ int hist[256];
     __shared__ int warp_tot[kCandThreads / 32];
-    __shared__ uint32_t s_prefix;
+    __shared__ uint32_t s_prefix, s_and[kCandThreads / 32], s_or[kCandThreads / 32];
     __shared__ int s_rank;
     __shared__ unsigned long long keys[kMaxBottomK];
     pdl_prologue();
     const float* v = values + (size_t)blockIdx.x * n;
     const int kk = k < n ? k : n;                           // entries that exist
     const int tid = threadIdx.x;
+    const int kCandChunk = (int)blockDim.x * kCandPerThread;
+    const bool resident = n <= kCandChunk;                  // the whole matrix sits in registers: read once
+    uint32_t u[kCandPerThread];                             // order keys of this thread's tiles of a super-chunk
+    auto load_keys = [&](int c0) {
+        const int i0 = c0 + tid * kCandPerThread;
+#pragma unroll
+        for (int j = 0; j < kCandPerThread; ++j) u[j] = i0 + j < n ? order_key(v[i0 + j]) : 0xffffffffu;
+    };
+    if (resident) load_keys(0);
 
-    // ---- radix select: the kk-th smallest order key (rank counts from 1) ----
-    uint32_t prefix = 0, mask = 0;
+    // ---- the bits all keys share: similarity values cluster (augLISI ~ 0.99x), so their leading bits are equal;
+    //      a digit on which every key agrees would send all the atomics of a pass to ONE histogram bucket ----
+    uint32_t k_and = 0xffffffffu, k_or = 0u;
+    for (int c0 = 0; c0 < n; c0 += kCandChunk) {
+        if (!resident) load_keys(c0);
+        const int i0 = c0 + tid * kCandPerThread;
+#pragma unroll
+        for (int j = 0; j < kCandPerThread; ++j)
+            if (i0 + j < n) { k_and &= u[j]; k_or |= u[j]; }
+    }
+    k_and = __reduce_and_sync(0xffffffffu, k_and);
+    k_or = __reduce_or_sync(0xffffffffu, k_or);
+    if ((tid & 31) == 0) { s_and[tid >> 5] = k_and; s_or[tid >> 5] = k_or; }
+    __syncthreads();
+    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) { k_and &= s_and[i]; k_or |= s_or[i]; }
+    const uint32_t diff = k_and ^ k_or;                     // bits on which the keys differ
+    const int hi = 31 - __clz(diff | 1u);                   // highest such bit (0 when all keys are equal)
+
+    // ---- radix select below the common prefix: the kk-th smallest order key (rank counts from 1) ----
+    uint32_t mask = hi >= 31 ? 0u : ~((2u << hi) - 1u);     // bits above `hi` are settled
+    uint32_t prefix = k_and & mask;
     int rank = kk;
-    for (int shift = 24; shift >= 0 && kk > 0; shift -= 8) {
-        hist[tid] = 0;
+    for (int shift = hi > 7 ? hi - 7 : 0; kk > 0; shift = shift > 8 ? shift - 8 : 0) {
+        for (int i = tid; i < 256; i += (int)blockDim.x) hist[i] = 0;
         __syncthreads();
-        for (int i = tid; i < n; i += kCandThreads) {
-            const uint32_t u = order_key(v[i]);
-            if ((u & mask) == prefix) atomicAdd(&hist[(u >> shift) & 255u], 1);
+        for (int c0 = 0; c0 < n; c0 += kCandChunk) {
+            if (!resident) load_keys(c0);
+            const int i0 = c0 + tid * kCandPerThread;
+#pragma unroll
+            for (int j = 0; j < kCandPerThread; ++j)
+                if (i0 + j < n && (u[j] & mask) == prefix) atomicAdd(&hist[(u[j] >> shift) & 255u], 1);
         }
         __syncthreads();
-        if (tid == 0) {
-            int cum = 0, b = 0;
-            for (; b < 255; ++b) {
-                if (cum + hist[b] >= rank) break;
-                cum += hist[b];
+        if (tid < 32) {                                     // warp 0 finds the bucket that holds the rank-th key
+            int c[8], sum = 0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { c[j] = hist[tid * 8 + j]; sum += c[j]; }
+            int inc = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (tid >= o) inc += t;
             }
-            s_prefix = prefix | ((uint32_t)b << shift);
-            s_rank = rank - cum;
+            int cum = inc - sum;                            // keys in the buckets before this lane's eight
+            if (cum < rank && rank <= inc) {                // exactly one lane (the histogram holds >= rank keys)
+                int b = 0;
+                for (; b < 7; ++b) {
+                    if (cum + c[b] >= rank) break;
+                    cum += c[b];
+                }
+                s_prefix = prefix | ((uint32_t)(tid * 8 + b) << shift);   // digits may overlap settled bits: same bits
+                s_rank = rank - cum;
+            }
         }
         __syncthreads();
         prefix = s_prefix;
         rank = s_rank;
         mask |= 255u << shift;
-        __syncthreads();
+        if (shift == 0) break;
     }
     const uint32_t pivot = prefix;                          // key of the kk-th smallest value
     const int take_eq = rank;                               // how many tiles equal to it belong to the answer
@@ -134,42 +183,35 @@ bottom_k_kernel(const float* __restrict__ values, int n, int k, int* __restrict_
     // ---- ordered compaction of the selected (key, index) pairs into shared memory ----
     int base = 0, eq_seen = 0;
     for (int c0 = 0; c0 < n && kk > 0; c0 += kCandChunk) {
+        if (!resident) load_keys(c0);
         const int i0 = c0 + tid * kCandPerThread;
-        uint32_t u[kCandPerThread];
-        bool eq[kCandPerThread];
-        int ce = 0;
-#pragma unroll
-        for (int j = 0; j < kCandPerThread; ++j) {
-            u[j] = i0 + j < n ? order_key(v[i0 + j]) : 0xffffffffu;
-            eq[j] = (i0 + j < n) && u[j] == pivot;
-            ce += eq[j];
-        }
-        int tot_e;
-        int erank = eq_seen + block_exclusive_scan(ce, warp_tot, tot_e);
-        bool sel[kCandPerThread];
-        int cs = 0;
-#pragma unroll
-        for (int j = 0; j < kCandPerThread; ++j) {
-            sel[j] = (i0 + j < n) && (u[j] < pivot || (eq[j] && erank < take_eq));
-            erank += eq[j];
-            cs += sel[j];
-        }
-        int tot_s;
-        int pos = base + block_exclusive_scan(cs, warp_tot, tot_s);
+        uint32_t eq = 0, less = 0;
 #pragma unroll
         for (int j = 0; j < kCandPerThread; ++j)
-            if (sel[j]) keys[pos++] = ((unsigned long long)u[j] << 32) | (uint32_t)(i0 + j);
+            if (i0 + j < n) {
+                if (u[j] == pivot) eq |= 1u << j;
+                if (u[j] < pivot) less |= 1u << j;
+            }
+        int tot_e;
+        int erank = eq_seen + block_exclusive_scan(__popc(eq), warp_tot, tot_e);
+        uint32_t sel = less;                                // plus the first take_eq equals, in index order
+        for (uint32_t f = eq; f && erank < take_eq; f &= f - 1, ++erank) sel |= f & (0u - f);
+        int tot_s;
+        int pos = base + block_exclusive_scan(__popc(sel), warp_tot, tot_s);
+#pragma unroll
+        for (int j = 0; j < kCandPerThread; ++j)
+            if (sel & (1u << j)) keys[pos++] = ((unsigned long long)u[j] << 32) | (uint32_t)(i0 + j);
         base += tot_s;
         eq_seen += tot_e;
     }
     // base == kk here.  Pad to a power of two and sort ascending by (key, index).
     int P = 1;
     while (P < kk) P <<= 1;
-    for (int i = kk + tid; i < P; i += kCandThreads) keys[i] = ~0ull;
+    for (int i = kk + tid; i < P; i += (int)blockDim.x) keys[i] = ~0ull;
     __syncthreads();
     for (int size = 2; size <= P; size <<= 1)
         for (int stride = size >> 1; stride > 0; stride >>= 1) {
-            for (int i = tid; i < P / 2; i += kCandThreads) {
+            for (int i = tid; i < P / 2; i += (int)blockDim.x) {
                 const int lo = 2 * i - (i & (stride - 1));  // index with the `stride` bit clear
                 const int hi = lo + stride;
                 const bool up = (lo & size) == 0;
@@ -180,7 +222,7 @@ bottom_k_kernel(const float* __restrict__ values, int n, int k, int* __restrict_
         }
     int* out_i = indices + (size_t)blockIdx.x * k;
     float* out_v = vals ? vals + (size_t)blockIdx.x * k : nullptr;
-    for (int i = tid; i < k; i += kCandThreads) {
+    for (int i = tid; i < k; i += (int)blockDim.x) {
         if (i < kk) {
             const int idx = (int)(uint32_t)keys[i];
             out_i[i] = idx;

@@ -830,7 +830,7 @@ int iqa_tiles_below(const float* values, int n_tiles, int n_maps, float threshol
     if (!values || !counts || (capacity > 0 && !indices)) return IQA_ERR_NULL;
     if (n_tiles <= 0 || n_maps <= 0 || capacity < 0) return IQA_ERR_SHAPE;
     if (threshold != threshold) return IQA_ERR_PARAM;
-    if (launch(below_kernel, (unsigned)n_maps, kCandThreads, 0, (cudaStream_t)stream, values, n_tiles, threshold,
+    if (launch(below_kernel, (unsigned)n_maps, (unsigned)cand_threads(n_tiles), 0, (cudaStream_t)stream, values, n_tiles, threshold,
                indices, capacity, counts) != cudaSuccess)
         return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
@@ -840,7 +840,7 @@ int iqa_tiles_bottom_k(const float* values, int n_tiles, int n_maps, int k,
                        int* indices, float* vals, void* stream) {
     if (!values || !indices) return IQA_ERR_NULL;
     if (n_tiles <= 0 || n_maps <= 0 || k <= 0 || k > kMaxBottomK) return IQA_ERR_SHAPE;
-    if (launch(bottom_k_kernel, (unsigned)n_maps, kCandThreads, 0, (cudaStream_t)stream, values, n_tiles, k,
+    if (launch(bottom_k_kernel, (unsigned)n_maps, (unsigned)cand_threads(n_tiles), 0, (cudaStream_t)stream, values, n_tiles, k,
                indices, vals) != cudaSuccess)
         return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
