@@ -14,6 +14,7 @@
 //               (key, index) pairs in index order into shared memory; a bitonic sort orders them
 // =============================================================================
 #pragma once
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -232,6 +233,208 @@ bottom_k_kernel(const float* __restrict__ values, int n, int k, int* __restrict_
             if (out_v) out_v[i] = __int_as_float(0x7f800000);
         }
     }
+}
+
+// -----------------------------------------------------------------------------
+// bottom-k of a LARGE matrix (16384 < n <= 8 x 16384 tiles: N = 16384 at N_T = 64, N = 2048 at N_T = 8): one
+// thread-block CLUSTER of C = ceil(n / 16384) CTAs per matrix instead of one CTA looping over super-chunks and
+// re-reading them in every radix pass.  CTA r keeps tiles [16384 r, 16384 (r+1)) in registers; the per-CTA
+// AND / OR words, histograms and selection counts are read across the cluster through distributed shared memory
+// (every CTA sums the C histograms itself and reaches the same bucket, so nothing is broadcast); the selected
+// (key, index) pairs are written straight into CTA 0's shared memory at their global position, and CTA 0 sorts
+// and stores them.  Same selection, same order, same output as bottom_k_kernel.
+// -----------------------------------------------------------------------------
+constexpr int kCandMaxCluster = 8;
+
+inline int cand_cluster_size(int n) {                       // 0: use the single-CTA kernel
+    const int chunk = kCandThreads * kCandPerThread;
+    if (n <= chunk || n > kCandMaxCluster * chunk) return 0;
+    return (n + chunk - 1) / chunk;
+}
+
+__global__ void __launch_bounds__(kCandThreads)
+bottom_k_cluster_kernel(const float* __restrict__ values, int n, int k, int* __restrict__ indices,
+                        float* __restrict__ vals) {
+    namespace cg = cooperative_groups;
+    __shared__ int hist[256];
+    __shared__ int warp_tot[kCandThreads / 32];
+    __shared__ uint32_t s_prefix, s_and[kCandThreads / 32], s_or[kCandThreads / 32];
+    __shared__ int s_rank;
+    __shared__ uint32_t cta_and, cta_or;                    // this CTA's words, read by the others
+    __shared__ int cta_tot_e, cta_tot_s;
+    __shared__ unsigned long long keys[kMaxBottomK];        // used in CTA 0 only
+    cg::cluster_group cluster = cg::this_cluster();
+    pdl_prologue();
+    const int C = (int)cluster.num_blocks(), r = (int)cluster.block_rank();
+    const size_t map = blockIdx.x / C;
+    const float* v = values + map * (size_t)n;
+    const int kk = k < n ? k : n;
+    const int tid = threadIdx.x;
+    const int i0 = (r * kCandThreads + tid) * kCandPerThread;               // first tile of this thread
+    uint32_t u[kCandPerThread];
+#pragma unroll
+    for (int j = 0; j < kCandPerThread; ++j) u[j] = i0 + j < n ? order_key(v[i0 + j]) : 0xffffffffu;
+
+    // ---- bits all keys of the matrix share ----
+    uint32_t k_and = 0xffffffffu, k_or = 0u;
+#pragma unroll
+    for (int j = 0; j < kCandPerThread; ++j)
+        if (i0 + j < n) { k_and &= u[j]; k_or |= u[j]; }
+    k_and = __reduce_and_sync(0xffffffffu, k_and);
+    k_or = __reduce_or_sync(0xffffffffu, k_or);
+    if ((tid & 31) == 0) { s_and[tid >> 5] = k_and; s_or[tid >> 5] = k_or; }
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t a = 0xffffffffu, o = 0u;
+        for (int i = 0; i < kCandThreads / 32; ++i) { a &= s_and[i]; o |= s_or[i]; }
+        cta_and = a; cta_or = o;
+    }
+    cluster.sync();
+    k_and = 0xffffffffu; k_or = 0u;
+    for (int q = 0; q < C; ++q) { k_and &= *cluster.map_shared_rank(&cta_and, q); k_or |= *cluster.map_shared_rank(&cta_or, q); }
+    const uint32_t diff = k_and ^ k_or;
+    const int hi = 31 - __clz(diff | 1u);
+
+    // ---- radix select below the common prefix; every CTA sums the C histograms and finds the same bucket ----
+    uint32_t mask = hi >= 31 ? 0u : ~((2u << hi) - 1u);
+    uint32_t prefix = k_and & mask;
+    int rank = kk;
+    for (int shift = hi > 7 ? hi - 7 : 0; kk > 0; shift = shift > 8 ? shift - 8 : 0) {
+        if (tid < 256) hist[tid] = 0;
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < kCandPerThread; ++j)
+            if (i0 + j < n && (u[j] & mask) == prefix) atomicAdd(&hist[(u[j] >> shift) & 255u], 1);
+        cluster.sync();                                     // every CTA's histogram is complete
+        if (tid < 32) {
+            int c[8], sum = 0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) c[j] = 0;
+            for (int q = 0; q < C; ++q) {
+                const int* h = cluster.map_shared_rank(hist, q);
+#pragma unroll
+                for (int j = 0; j < 8; ++j) c[j] += h[tid * 8 + j];
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) sum += c[j];
+            int inc = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (tid >= o) inc += t;
+            }
+            int cum = inc - sum;
+            if (cum < rank && rank <= inc) {
+                int b = 0;
+                for (; b < 7; ++b) {
+                    if (cum + c[b] >= rank) break;
+                    cum += c[b];
+                }
+                s_prefix = prefix | ((uint32_t)(tid * 8 + b) << shift);
+                s_rank = rank - cum;
+            }
+        }
+        cluster.sync();                                     // all histograms have been read: they may be cleared
+        prefix = s_prefix;
+        rank = s_rank;
+        mask |= 255u << shift;
+        if (shift == 0) break;
+    }
+    const uint32_t pivot = prefix;
+    const int take_eq = rank;
+
+    // ---- ordered compaction across the cluster into CTA 0's shared memory ----
+    uint32_t eq = 0, less = 0;
+#pragma unroll
+    for (int j = 0; j < kCandPerThread; ++j)
+        if (i0 + j < n) {
+            if (u[j] == pivot) eq |= 1u << j;
+            if (u[j] < pivot) less |= 1u << j;
+        }
+    int tot_e;
+    int erank = block_exclusive_scan(__popc(eq), warp_tot, tot_e);
+    if (tid == 0) cta_tot_e = tot_e;
+    cluster.sync();
+    for (int q = 0; q < r; ++q) erank += *cluster.map_shared_rank(&cta_tot_e, q);       // equals in the CTAs before this one
+    uint32_t sel = less;
+    for (uint32_t f = eq; f && erank < take_eq; f &= f - 1, ++erank) sel |= f & (0u - f);
+    int tot_s;
+    int pos = block_exclusive_scan(__popc(sel), warp_tot, tot_s);
+    if (tid == 0) cta_tot_s = tot_s;
+    cluster.sync();
+    for (int q = 0; q < r; ++q) pos += *cluster.map_shared_rank(&cta_tot_s, q);
+    unsigned long long* keys0 = cluster.map_shared_rank(keys, 0);
+#pragma unroll
+    for (int j = 0; j < kCandPerThread; ++j)
+        if (kk > 0 && (sel & (1u << j))) keys0[pos++] = ((unsigned long long)u[j] << 32) | (uint32_t)(i0 + j);
+    cluster.sync();                                         // CTA 0 holds all kk pairs; the other CTAs are done
+    if (r != 0) return;
+
+    int P = 1;
+    while (P < kk) P <<= 1;
+    for (int i = kk + tid; i < P; i += kCandThreads) keys[i] = ~0ull;
+    __syncthreads();
+    for (int size = 2; size <= P; size <<= 1)
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            for (int i = tid; i < P / 2; i += kCandThreads) {
+                const int lo = 2 * i - (i & (stride - 1));
+                const int hi2 = lo + stride;
+                const bool up = (lo & size) == 0;
+                const unsigned long long a = keys[lo], b = keys[hi2];
+                if ((a > b) == up) { keys[lo] = b; keys[hi2] = a; }
+            }
+            __syncthreads();
+        }
+    int* out_i = indices + map * (size_t)k;
+    float* out_v = vals ? vals + map * (size_t)k : nullptr;
+    for (int i = tid; i < k; i += kCandThreads) {
+        if (i < kk) {
+            const int idx = (int)(uint32_t)keys[i];
+            out_i[i] = idx;
+            if (out_v) out_v[i] = v[idx];
+        } else {
+            out_i[i] = -1;
+            if (out_v) out_v[i] = __int_as_float(0x7f800000);
+        }
+    }
+}
+
+// Threshold list of a large matrix with the same cluster layout: CTA r flags its 16384 tiles, the counts of the
+// CTAs before it (distributed shared memory) give its offset in the ascending list.
+__global__ void __launch_bounds__(kCandThreads)
+below_cluster_kernel(const float* __restrict__ values, int n, float threshold, int* __restrict__ indices, int capacity,
+                     int* __restrict__ counts) {
+    namespace cg = cooperative_groups;
+    __shared__ int warp_tot[kCandThreads / 32];
+    __shared__ int cta_total;
+    cg::cluster_group cluster = cg::this_cluster();
+    pdl_prologue();
+    const int C = (int)cluster.num_blocks(), r = (int)cluster.block_rank();
+    const size_t map = blockIdx.x / C;
+    const float* v = values + map * (size_t)n;
+    int* out = indices + map * (size_t)capacity;
+    const int i0 = (r * kCandThreads + (int)threadIdx.x) * kCandPerThread;
+    uint32_t flags = 0;
+#pragma unroll
+    for (int j = 0; j < kCandPerThread; ++j)
+        if (i0 + j < n && v[i0 + j] < threshold) flags |= 1u << j;
+    int total;
+    int pos = block_exclusive_scan(__popc(flags), warp_tot, total);
+    if (threadIdx.x == 0) cta_total = total;
+    cluster.sync();
+    int before = 0, all = 0;
+    for (int q = 0; q < C; ++q) {
+        const int t = *cluster.map_shared_rank(&cta_total, q);
+        if (q < r) before += t;
+        all += t;
+    }
+    pos += before;
+    for (uint32_t f = flags; f; f &= f - 1) {
+        if (pos < capacity) out[pos] = i0 + (__ffs(f) - 1);
+        ++pos;
+    }
+    if (r == 0 && threadIdx.x == 0) counts[map] = all;
+    cluster.sync();                                         // nobody exits while its total may still be read
 }
 
 }  // namespace iqa

@@ -830,9 +830,13 @@ int iqa_tiles_below(const float* values, int n_tiles, int n_maps, float threshol
     if (!values || !counts || (capacity > 0 && !indices)) return IQA_ERR_NULL;
     if (n_tiles <= 0 || n_maps <= 0 || capacity < 0) return IQA_ERR_SHAPE;
     if (threshold != threshold) return IQA_ERR_PARAM;
-    if (launch(below_kernel, (unsigned)n_maps, (unsigned)cand_threads(n_tiles), 0, (cudaStream_t)stream, values, n_tiles, threshold,
-               indices, capacity, counts) != cudaSuccess)
-        return IQA_ERR_CUDA;
+    const int cs = env_int("IQA_CAND_NO_CLUSTER", 0) ? 0 : cand_cluster_size(n_tiles);
+    const cudaError_t e = cs > 0
+        ? launch_cluster(below_cluster_kernel, (unsigned)n_maps * (unsigned)cs, (unsigned)kCandThreads, 0,
+                         (cudaStream_t)stream, (unsigned)cs, values, n_tiles, threshold, indices, capacity, counts)
+        : launch(below_kernel, (unsigned)n_maps, (unsigned)cand_threads(n_tiles), 0, (cudaStream_t)stream, values,
+                 n_tiles, threshold, indices, capacity, counts);
+    if (e != cudaSuccess) return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }
 
@@ -840,9 +844,13 @@ int iqa_tiles_bottom_k(const float* values, int n_tiles, int n_maps, int k,
                        int* indices, float* vals, void* stream) {
     if (!values || !indices) return IQA_ERR_NULL;
     if (n_tiles <= 0 || n_maps <= 0 || k <= 0 || k > kMaxBottomK) return IQA_ERR_SHAPE;
-    if (launch(bottom_k_kernel, (unsigned)n_maps, (unsigned)cand_threads(n_tiles), 0, (cudaStream_t)stream, values, n_tiles, k,
-               indices, vals) != cudaSuccess)
-        return IQA_ERR_CUDA;
+    const int cs = env_int("IQA_CAND_NO_CLUSTER", 0) ? 0 : cand_cluster_size(n_tiles);
+    const cudaError_t e = cs > 0
+        ? launch_cluster(bottom_k_cluster_kernel, (unsigned)n_maps * (unsigned)cs, (unsigned)kCandThreads, 0,
+                         (cudaStream_t)stream, (unsigned)cs, values, n_tiles, k, indices, vals)
+        : launch(bottom_k_kernel, (unsigned)n_maps, (unsigned)cand_threads(n_tiles), 0, (cudaStream_t)stream, values,
+                 n_tiles, k, indices, vals);
+    if (e != cudaSuccess) return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }
 
