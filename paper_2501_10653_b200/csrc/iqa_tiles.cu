@@ -611,7 +611,7 @@ const char* iqa_status_string(int status) {
     }
 }
 
-const char* iqa_version(void) { return "0.3.0"; }
+const char* iqa_version(void) { return "0.4.0"; }
 
 size_t iqa_workspace_bytes(int N, int N_T) {
     if (status_of_shape(N, N_T) != IQA_OK) return 0;
