@@ -32,10 +32,29 @@ UNIT = "us/pair"
 # workload name -> (BASELINE.json config index, pairs per step, pairs per e2e step)
 WORKLOADS = {"cfg1": (1, 32, 8), "cfg3": (3, 8, 2), "cfg4": (4, 16, 1), "cfg0": (0, 64, 8)}
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused TMA kernel at the default pairs
-# per step, from the `ncu --set full` captures summarised under profiles/r01g_ncu_full_*_tma.md
-# (null when not captured for that workload; algorithmic bytes: cfg1 1.07427e9, cfg3 4.29706e9).
-NCU_TRAFFIC_BYTES = {"cfg1": 1.073771e9 + 4.429e6, "cfg3": 4.295015e9 + 4.734e6}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel come from the table in this file
+# (written by hand from `ncu --set full` captures; each row names the library version it was captured on).
+NCU_TRAFFIC_FILE = os.path.join("profiles", "ncu_traffic.md")
+
+
+def ncu_traffic(workload: str, pairs: int, version: str):
+    """(bytes per launch, source) from the row `| workload | pairs per launch | library version | read | write | capture |`
+    of profiles/ncu_traffic.md -- (None, why) when there is no row for this workload / batch size or the row was
+    captured on another library version: a number that does not describe the timed binary is not printed."""
+    try:
+        with open(os.path.join(ROOT, NCU_TRAFFIC_FILE)) as f:
+            rows = [[c.strip() for c in ln.strip().strip("|").split("|")] for ln in f if ln.lstrip().startswith("|")]
+    except OSError as exc:
+        return None, f"{NCU_TRAFFIC_FILE}: {exc.strerror}"
+    stale = None
+    for r in rows:
+        if len(r) >= 6 and r[0] == workload and r[1] == str(pairs):
+            if r[2] == version:
+                return float(r[3]) + float(r[4]), f"{NCU_TRAFFIC_FILE} row {workload}/{pairs} pairs, libiqa_tiles {r[2]}, capture {r[5]}"
+            stale = r[2]
+    if stale:
+        return None, f"{NCU_TRAFFIC_FILE}: row captured on libiqa_tiles {stale}, this run is {version}"
+    return None, f"{NCU_TRAFFIC_FILE}: no row for {workload} with {pairs} pairs per launch"
 
 
 def algorithmic_bytes(N: int, N_T: int) -> int:
@@ -374,6 +393,11 @@ def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, us
     for _ in range(warmup):
         kern()
     ms_kernel = time_region(torch, kern, steps, dist)
+    # the same step WITHOUT the graph: the ctypes call, the host-side tensor-map encodes and the launches are inside
+    direct = lambda: batch.step(True)
+    for _ in range(warmup):
+        direct()
+    ms_direct = time_region(torch, direct, max(3, min(steps, 20)), dist) / max(3, min(steps, 20)) * steps
     reps = max(3, min(steps, 20))
     lat = [] if latency else [None, None]
     for fn in ((single_warm, single_cold) if latency else ()):
@@ -381,7 +405,7 @@ def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, us
             fn()
         lat.append(time_region(torch, fn, reps, dist) / (reps * L))
     ms_single, ms_single_cold = lat
-    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "step_us": dist_us, "us_single_pair_warm": None if ms_single is None else ms_single * 1e3,
+    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "ms_direct": ms_direct, "step_us": dist_us, "us_single_pair_warm": None if ms_single is None else ms_single * 1e3,
             "us_single_pair_cold": None if ms_single_cold is None else ms_single_cold * 1e3, "clocks": clk.summary()}
 
 
@@ -421,6 +445,83 @@ def measure_sweep(torch, binding, base_cfg, pairs, steps, warmup, device, use_gr
         del m
         torch.cuda.empty_cache()
     return rows
+
+
+def graph_of(torch, fn):
+    g = torch.cuda.CUDAGraph()
+    fn()
+    torch.cuda.synchronize()
+    with torch.cuda.graph(g):
+        fn()
+    return g.replay
+
+
+# (row name, pixel dtype, H, W, row pitch in elements, base offset in elements, N_T): the paths SURVEY.md 8(f)-4 added
+PATH_ROWS = [
+    ("f32_NT48", "float32", 8192, 8192, 8192, 0, 48), ("f32_NT100", "float32", 8192, 8192, 8192, 0, 100),
+    ("f32_NT50", "float32", 8192, 8192, 8192, 0, 50), ("f32_NT64_base4B", "float32", 8192, 8188, 8192, 1, 64),
+    ("f32_NT100_base4B", "float32", 8192, 8188, 8192, 3, 100), ("f32_NT300_split", "float32", 8192, 8192, 8192, 0, 300),
+    ("f16_NT64", "float16", 8192, 8192, 8192, 0, 64), ("i16_NT64", "int16", 8192, 8192, 8192, 0, 64),
+    ("u8_NT64", "uint8", 8192, 8192, 8192, 0, 64), ("f64_NT64", "float64", 8192, 8192, 8192, 0, 64),
+    ("i32_NT64", "int32", 8192, 8192, 8192, 0, 64), ("f16_NT100", "float16", 8192, 8192, 8192, 0, 100),
+    ("u8_NT100", "uint8", 8192, 8192, 8192, 0, 100),
+    # no tensor map can describe these (row pitch not a multiple of 16 bytes): the generic kernels
+    ("generic_f32_NT64_pitch8190", "float32", 8192, 8190, 8190, 0, 64),
+    ("generic_f32_NT32_pitch8190", "float32", 8192, 8190, 8190, 0, 32),
+    ("generic_i16_NT64_pitch8190", "int16", 8192, 8190, 8190, 0, 64),
+]
+
+
+def measure_paths(torch, binding, steps, warmup, device, use_graph, rows=PATH_ROWS, pairs=4):
+    """One row per kernel path beyond the power-of-two fp32 one: `pairs` distinct pairs per step through
+    iqa_fused_batch_2d_typed (one launch of any_kernel, or `pairs` launches of a generic kernel), Eqs. 3-4 included.
+    GB/s on each path's OWN algorithmic bytes: 2 sizeof(pixel) per pixel pair + 16 B per tile."""
+    out = {}
+    k = (1e-6, 1e-6, 1e-6, 5e-7)
+    for name, dtype, H, W, pitch, off, N_T in rows:
+        dt = getattr(torch, dtype)
+        es = torch.empty((), dtype=dt).element_size()
+        g = torch.Generator(device=device).manual_seed(len(name) + N_T)
+        imgs = []
+        for _ in range(2 * pairs):
+            buf = torch.empty(H * pitch + 64, dtype=dt, device=device)
+            if dt.is_floating_point:
+                buf.copy_(torch.randn(buf.shape, generator=g, device=device, dtype=torch.float32) * 1e-3 + 2e-4)
+            else:
+                buf.copy_(torch.randint(-20 if dt != torch.uint8 else 0, 200, buf.shape, generator=g, device=device,
+                                        dtype=torch.int32))
+            imgs.append(torch.as_strided(buf, (H, W), (pitch, 1), off))
+        xs, ys = imgs[0::2], imgs[1::2]
+        nty, ntx = -(-H // N_T), -(-W // N_T)
+        n = nty * ntx
+        o = [torch.empty((pairs, n), dtype=torch.float32, device=device) for _ in range(4)]
+        out2 = torch.empty((pairs, 2), dtype=torch.float32, device=device)
+        wsb = pairs * binding.iqa_workspace_bytes_2d(H, W, N_T)
+        ws = torch.empty(wsb, dtype=torch.uint8, device=device) if wsb else None
+        xt, _ = binding._ptr_table(xs)
+        yt, _ = binding._ptr_table(ys)
+        ptype = binding._pixel_types()[dt]
+
+        def step():
+            rc = binding.iqa_fused_batch_2d_typed(xt, yt, pairs, ptype, H, W, pitch, N_T, *k, *o, None, None, out2, ws, wsb,
+                                                  torch.cuda.current_stream().cuda_stream)
+            if rc:
+                raise binding.IqaError(rc, "iqa_fused_batch_2d_typed")
+
+        fn = graph_of(torch, step) if use_graph else step
+        for _ in range(warmup):
+            fn()
+        with ClockSampler(torch.cuda.current_device()) as clk:
+            us = time_region(torch, fn, steps) * 1e3 / (steps * pairs)
+        alg = 2 * es * H * W + 16 * n
+        gbs = alg / (us * 1e-6) / 1e9
+        out[name] = {"plan": binding.plan_name(xs[0], N_T), "pixel": dtype, "H": H, "W": W, "pitch": pitch,
+                     "base_offset_bytes": off * es, "N_T": N_T, "pairs_per_step": pairs, "us_per_pair": us,
+                     "algorithmic_bytes_per_pair": alg, "GBps": gbs, "frac_of_nominal_8000": gbs / 8000.0,
+                     "clocks": clk.summary()}
+        del imgs, xs, ys, o, ws
+        torch.cuda.empty_cache()
+    return out
 
 
 def series_bytes(N: int, N_T: int, M: int) -> int:
@@ -539,39 +640,58 @@ def run_ours(args):
     split = binding.iqa_workspace_bytes(cfg.N, cfg.N_T) > 0
     launches = m["batch"].launches_per_step(True)
     plan = binding.plan_name(m["batch"].x[0], cfg.N_T)           # the kernel the library really picked
+    us_per_pair_direct = m["ms_direct"] * 1e3 / total_pairs
+    traffic, traffic_src = ncu_traffic(args.workload, pairs // n_stream, binding.iqa_version())
     del m
     torch.cuda.empty_cache()
 
     e2e = run_e2e(torch, binding, cfg, pairs_e2e, max(2, min(K, 10)), min(W, 2), device, dist)
 
     also = {}
-    if args.workload == "cfg1" and not args.no_also and world == 1:
-        # the north-star bar (>= 75 % of HBM peak) is quoted at N >= 8192: measure config [3] beside the headline
-        c3, p3, k3 = synth.CONFIGS[3], 4, max(3, min(K, 10))
-        m3 = measure_workload(torch, binding, c3, p3, k3, max(3, W), device, None, use_graph, rank)
-        us3 = m3["ms_kernel"] * 1e3 / (k3 * p3)
-        gbs3 = algorithmic_bytes(c3.N, c3.N_T) / (us3 * 1e-6) / 1e9
-        also[c3.name] = {"us_per_pair_step": m3["ms"] * 1e3 / (k3 * p3), "us_per_pair_tiles_kernel": us3,
-                         "us_single_pair_warm": m3["us_single_pair_warm"],
-                         "us_single_pair_cold": m3["us_single_pair_cold"],
-                         "achieved_GBps": gbs3, "frac_of_measured_peak": gbs3 / peak,
-                         "frac_of_nominal_8000": gbs3 / 8000.0, "pairs_per_step": p3, "clocks": m3["clocks"]}
-        del m3
+
+    def guarded(name, fn):
+        """An extra row: its failure must not cost the headline line."""
+        try:
+            also[name] = fn()
+        except Exception as exc:
+            also[name] = {"error": repr(exc)[:300]}
         torch.cuda.empty_cache()
 
-    if world == 1 and not args.no_also:
+    def workload_row(c, p, k, w):
+        m2 = measure_workload(torch, binding, c, p, k, w, device, None, use_graph, rank)
+        n_l = -(-p // PAIRS_PER_LAUNCH)
+        usk = m2["ms_kernel"] * 1e3 / (k * p)
+        gbs = algorithmic_bytes(c.N, c.N_T) / (usk * 1e-6) / 1e9
+        row = {"us_per_pair_step": m2["ms"] * 1e3 / (k * p), "us_per_pair_step_no_graph": m2["ms_direct"] * 1e3 / (k * p),
+               "us_per_pair_tiles_kernel": usk, "step_us": m2["step_us"],
+               "us_single_pair_warm": m2["us_single_pair_warm"], "us_single_pair_cold": m2["us_single_pair_cold"],
+               "achieved_GBps": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_nominal_8000": gbs / 8000.0,
+               "pairs_per_step": p, "launches_per_step": m2["batch"].launches_per_step(True),
+               "tile_kernel_launches_per_step": n_l, "plan": binding.plan_name(m2["batch"].x[0], c.N_T),
+               "clocks": m2["clocks"]}
+        del m2
+        return row
+
+    extras = world == 1 and not args.no_also
+    if extras and args.workload == "cfg1":
+        # the north-star bar (>= 75 % of HBM peak) is quoted at N >= 8192: config [3] and config [4]'s 16-pair loop
+        # (SURVEY.md 8(d): <= 89.5 us and <= 358 us per pair), config [0], and the config [2] sweep beside the headline
+        c3, c4, c0 = synth.CONFIGS[3], synth.CONFIGS[4], synth.CONFIGS[0]
+        guarded(c3.name, lambda: workload_row(c3, 4, max(3, min(K, 10)), max(3, W)))
+        guarded(c4.name + "_loop16", lambda: dict(workload_row(c4, 16, 3, 3), bar_us_per_pair=358.0))
+        guarded(c0.name, lambda: workload_row(c0, 64, max(3, min(K, 20)), max(3, W)))
+        guarded("cfg2_sweep", lambda: measure_sweep(torch, binding, synth.CONFIGS[2], 32, max(3, min(K, 10)), 3,
+                                                    device, use_graph))
+    if extras:
         # read-only ceiling of the kernel's own access pattern, and the time-series modes at N = 8192
         also["read_ceiling"] = measure_read_ceiling()
         cs = synth.CONFIGS[3] if args.workload in ("cfg1", "cfg3") else cfg
-        try:                                   # an extra: its failure must not cost the headline line
-            also[f"series_{cs.name}_M{args.series_images}"] = measure_series(
-                torch, binding, cs, args.series_images, max(3, min(K, 10)), 3, device, use_graph)
-        except Exception as exc:
-            also[f"series_{cs.name}_M{args.series_images}"] = {"error": repr(exc)[:300]}
-            torch.cuda.empty_cache()
-    if args.entry_points and world == 1:
-        also["entry_points_cold"] = measure_entry_points(torch, cfg, pairs, max(3, min(K, 20)), max(3, W), device, use_graph)
-    if args.sweep and world == 1:
+        guarded(f"series_{cs.name}_M{args.series_images}",
+                lambda: measure_series(torch, binding, cs, args.series_images, max(3, min(K, 10)), 3, device, use_graph))
+        guarded("entry_points_cold", lambda: measure_entry_points(torch, cfg, pairs, max(3, min(K, 20)), max(3, W),
+                                                                  device, use_graph))
+        guarded("paths", lambda: measure_paths(torch, binding, max(3, min(K, 10)), 3, device, use_graph))
+    if args.sweep and world == 1 and "cfg2_sweep" not in also:
         also["cfg2_sweep"] = measure_sweep(torch, binding, synth.CONFIGS[2], 32, max(3, min(K, 20)), max(3, W),
                                            device, use_graph)
 
@@ -585,6 +705,10 @@ def run_ours(args):
             "config": workload_config(cfg, pairs, f"inputs {pairs * 8 * cfg.N * cfg.N / 2**20:.0f} MiB per step > 126 MB L2: "
                                       "every pair is read cold from HBM; no explicit flush"),
             "pairs_per_s": 1e6 / us_per_pair,
+            "no_graph": {"value": us_per_pair_direct, "unit": UNIT,
+                         "what": "the same step launched directly through ctypes every time: the iqa_fused_batch call, its "
+                                 "host-side tensor-map encodes and the launches are inside the timed region"},
+            "library_version": binding.iqa_version(),
             "launch": ("cuda graph of the step" if use_graph else "direct launches through ctypes")
                       + ": one iqa_fused_batch call per step",
             "gpu_launches": K * world * launches,
@@ -592,7 +716,7 @@ def run_ours(args):
             "kernels": ["iqa::tma_kernel<3,0,NB,RPW> (fused S1-S4, all pairs of the step)"]
                        + (["iqa::finalise_*_kernel"] if split else []) + ["iqa::aggregate_kernel (S5, one CTA per pair)"],
             "roofline": {"bound": "hbm", "kernel": "iqa::tma_kernel<fused, pairs>", "achieved": achieved, "peak": peak,
-                         "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if not args.pairs else None,
+                         "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
                          "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
                          "us_per_launch": us_launch, "pairs_per_launch": pairs / n_stream,
                          "frac_of_nominal_8000": achieved / 8000.0},
@@ -625,13 +749,12 @@ def main():
     ap.add_argument("--workload", default="cfg1", choices=sorted(WORKLOADS))
     ap.add_argument("--pairs", type=int, default=0, help="pairs per step (default per workload)")
     ap.add_argument("--no-graph", action="store_true", help="launch through ctypes each step instead of replaying a CUDA graph")
-    ap.add_argument("--no-also", action="store_true", help="skip the extra N=8192 measurement")
+    ap.add_argument("--no-also", action="store_true",
+                    help="skip the extra rows (configs [0], [2], [3], [4], series, entry points, other kernel paths)")
     ap.add_argument("--no-latency", action="store_true",
                     help="skip the single-pair latency loops (keeps the launch list short under ncu)")
     ap.add_argument("--series-images", type=int, default=9, help="snapshots of the time-series measurement in `also`")
     ap.add_argument("--sweep", action="store_true", help="also time BASELINE.json config [2] (N=2048, N_T = 8..512)")
-    ap.add_argument("--entry-points", action="store_true",
-                    help="also time iqa_fused_tiles / iqa_lisi_tiles / iqa_auglisi_tiles per pair, cold")
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)
     if args.impl == "reference":

@@ -37,14 +37,22 @@
  *     enqueued when the status is not IQA_OK (validation precedes the first launch).
  *       NULL required pointer ....................................... IQA_ERR_NULL
  *       N <= 0, N_T <= 0, N % N_T != 0, n_tiles <= 0,
- *       n_pairs <= 0, g bad ......................................... IQA_ERR_SHAPE
- *       C1, C2 or C not finite or <= 0, D not finite ................ IQA_ERR_PARAM
- *       x or y not 4-byte aligned ................................... IQA_ERR_ALIGN
+ *       n_pairs <= 0, g bad, unknown pixel type ..................... IQA_ERR_SHAPE
+ *       C2 or C not finite or <= 0, D not finite, C1 not a NORMAL
+ *       positive float (C1 >= FLT_MIN: |x - y| + C1 feeds a
+ *       flush-to-zero reciprocal) ................................... IQA_ERR_PARAM
+ *       x or y not aligned to their element size (4 bytes for fp32) . IQA_ERR_ALIGN
  *       workspace NULL / too small when iqa_workspace_bytes() > 0 ... IQA_ERR_WORKSPACE
  *       CUDA launch / copy failure .................................. IQA_ERR_CUDA
- *   * Any N_T that divides N is accepted.  Power-of-two N_T >= 8 with 16-byte aligned
- *     x and y (and N % 4 == 0) take the persistent TMA-fed kernel; everything else takes a
- *     generic (slower, still CUDA) kernel.  Results are deterministic: fixed reduction order,
+ *     Every tensor map of a call is encoded on the host BEFORE its first launch (a map that cannot be
+ *     encoded downgrades the whole call to the generic kernels), so validation, planning and encoding
+ *     never leave work behind.  IQA_ERR_CUDA from a failing launch or copy is the one exception: earlier
+ *     launches of the same call may already be enqueued and the outputs are then undefined.
+ *   * Any N_T that divides N is accepted.  Images whose row pitch is a multiple of 16 bytes (N % 4 == 0
+ *     for the square fp32 entry points) take a persistent TMA-fed kernel whatever the alignment of
+ *     their base: tma_kernel for power-of-two N_T >= 8, any_kernel for every other N_T >= 4 and for
+ *     the other pixel types.  Other pitches and N_T < 4 take a generic (slower, still CUDA) kernel.
+ *     Results are deterministic: fixed reduction order,
  *     no floating-point atomics; two calls on the same inputs are bit-identical.
  * ============================================================================= */
 #ifndef IQA_TILES_H
@@ -104,15 +112,24 @@ int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
                     void* workspace, size_t workspace_bytes, void* stream);
 
 /* Diagnostic: which kernel a call on this image would take (host-side decision only, nothing is enqueued).
- *   x, H, W, pitch, N_T as for iqa_fused_tiles_2d (H == W == pitch, W % N_T == 0: as for the square entry points);
- *   series != 0: as for the time-series entry points.
- * Returns IQA_PLAN_GENERIC, IQA_PLAN_CP_ASYNC, or IQA_PLAN_TMA + c (c = ring / box configuration of the TMA
- * kernel, 0..4); -1 for bad arguments.  bench.py reports it, and the GPU tests assert that every
- * BASELINE.json configuration takes the TMA kernel -- a silent fall-back would cost bandwidth, not parity. */
+ *   x, pixel_type, H, W, pitch, N_T as for iqa_fused_tiles_2d_typed; series != 0: as for the time-series entry points.
+ * Returns IQA_PLAN_GENERIC, IQA_PLAN_TMA_ANY (any_kernel: any N_T >= 4, any pixel type; the time-series entry points
+ * run it pair by pair), or IQA_PLAN_TMA + c (tma_kernel, c = its ring / box configuration, 0..4); -1 for bad
+ * arguments.  bench.py reports it, and the GPU tests assert that every BASELINE.json configuration takes tma_kernel
+ * -- a silent fall-back would cost bandwidth, not parity. */
 #define IQA_PLAN_GENERIC 0
-#define IQA_PLAN_CP_ASYNC 1
+#define IQA_PLAN_TMA_ANY 2
 #define IQA_PLAN_TMA 16
-int iqa_query_plan(const float* x, int H, int W, long long pitch, int N_T, int series);
+int iqa_query_plan(const void* x, int pixel_type, int H, int W, long long pitch, int N_T, int series);
+
+/* Test and tuning hook: sets one of the library's process-wide knobs and returns its previous value (-1: unknown
+ * name).  The knobs take their initial value from the environment variable of the same name, read once:
+ *   IQA_FORCE_GENERIC 1: generic kernels only        IQA_FORCE_ANY 1: any_kernel instead of tma_kernel
+ *   IQA_TMA_CONFIG 0..4: tma_kernel ring / box configuration (-1: default)
+ *   IQA_TMA_MAX_CTAS n: cap of the persistent grid (0: none)     IQA_NO_PDL 1: no programmatic dependent launch
+ *   IQA_CAND_NO_CLUSTER 1: candidate kernels without thread-block clusters
+ * They select among kernels that all satisfy the same parity bar (tests/test_gpu_parity.py runs every one). */
+int iqa_debug_knob(const char* name, int value);
 
 /* ---- general images -------------------------------------------------------
  * The paper's images are square and N is a multiple of N_T.  This entry point drops
@@ -124,9 +141,9 @@ int iqa_query_plan(const float* x, int H, int W, long long pitch, int N_T, int s
  *   x, y            pixel (r, c) is x[r * pitch_x + c] / y[r * pitch_y + c]; pitch >= W
  *   outputs         [nty * ntx], nty = ceil(H / N_T), ntx = ceil(W / N_T), t = ty * ntx + tx
  *   workspace       >= iqa_workspace_bytes_2d(H, W, N_T) bytes (may be NULL when 0)
- * Eqs. 3-4 over the result: iqa_aggregate with n_tiles = nty * ntx.  16-byte aligned bases, pitches
- * that are multiples of 4 and a power-of-two N_T >= 8 take the TMA kernel (the TMA unit zero-fills
- * what lies outside the image); everything else takes the generic kernel. */
+ * Eqs. 3-4 over the result: iqa_aggregate with n_tiles = nty * ntx.  Pitches that are multiples of 4 take a
+ * TMA-fed kernel (the TMA unit zero-fills what lies outside the image; the base needs 4-byte alignment only);
+ * other pitches and N_T < 4 take the generic kernel. */
 size_t iqa_workspace_bytes_2d(int H, int W, int N_T);
 int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long pitch_x, long long pitch_y, int N_T,
                        float C1, float C2, float C, float D,
@@ -138,8 +155,9 @@ int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long p
  * H x W image of `pixel_type` pixels (pitches in ELEMENTS of that type; pointers aligned to the element
  * size).  Every such value is exact in double; types that are exact in fp32 (F16, I16, U8) are converted
  * and follow the fp32 arithmetic, F64 and I32 are clamped, added and subtracted in fp64 before rounding
- * (the Eq. 1 term is ill-conditioned in x - y).  IQA_PIXEL_F32 forwards to iqa_fused_tiles_2d (TMA
- * kernel); the other types take the generic kernels.  Unknown pixel_type: IQA_ERR_SHAPE. */
+ * (the Eq. 1 term is ill-conditioned in x - y).  Row pitches that are multiples of 16 BYTES and N_T >= 4 take the
+ * TMA-fed any_kernel (tensor maps of the element type; algorithmic bytes 2 sizeof(pixel) per pixel pair); other
+ * pitches take the generic kernels.  Unknown pixel_type: IQA_ERR_SHAPE. */
 typedef enum {
     IQA_PIXEL_F32 = 0, IQA_PIXEL_F64 = 1, IQA_PIXEL_F16 = 2, IQA_PIXEL_I16 = 3, IQA_PIXEL_I32 = 4, IQA_PIXEL_U8 = 5
 } iqa_pixel_type;
@@ -163,6 +181,20 @@ int iqa_series_tiles_2d(const float* const* img_ptrs_host, int n_images, int mod
                         float* lisi, float* auglisi, float* sum_x, float* sum_y,
                         float* lisi_num, float* auglisi_num, float* out2,
                         void* workspace, size_t workspace_bytes, void* stream);
+
+/* The same two entry points for images of `pixel_type` pixels (pitch in ELEMENTS of that type).  Batches run in
+ * one any_kernel launch per 32 pairs; a typed time series is computed pair by pair (2 sizeof(pixel) bytes per pixel
+ * and comparison -- only fp32 images with a power-of-two N_T have the read-once series kernel). */
+int iqa_fused_batch_2d_typed(const void* const* x_ptrs_host, const void* const* y_ptrs_host, int n_pairs, int pixel_type,
+                             int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
+                             float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                             float* lisi_num, float* auglisi_num, float* out2,
+                             void* workspace, size_t workspace_bytes, void* stream);
+int iqa_series_tiles_2d_typed(const void* const* img_ptrs_host, int n_images, int mode, int pixel_type,
+                              int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
+                              float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                              float* lisi_num, float* auglisi_num, float* out2,
+                              void* workspace, size_t workspace_bytes, void* stream);
 
 /* Bytes of device workspace iqa_fused_batch needs: n_pairs * iqa_workspace_bytes(N, N_T). */
 size_t iqa_batch_workspace_bytes(int n_pairs, int N, int N_T);

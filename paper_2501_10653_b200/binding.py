@@ -22,10 +22,13 @@ from . import build as _build
 
 IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKSPACE, IQA_ERR_CUDA = range(7)
 
-EXPORTS = ("iqa_status_string", "iqa_version", "iqa_workspace_bytes", "iqa_lisi_tiles",
+EXPORTS = ("iqa_status_string", "iqa_version", "iqa_debug_knob", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
-           "iqa_query_plan", "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_tiles_2d_typed", "iqa_fused_batch_2d", "iqa_series_tiles_2d", "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
-           "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_merge_tiles_batch", "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
+           "iqa_query_plan", "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_tiles_2d_typed",
+           "iqa_fused_batch_2d", "iqa_fused_batch_2d_typed", "iqa_series_tiles_2d", "iqa_series_tiles_2d_typed",
+           "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
+           "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_merge_tiles_batch",
+           "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
 IQA_PIXEL_F32, IQA_PIXEL_F64, IQA_PIXEL_F16, IQA_PIXEL_I16, IQA_PIXEL_I32, IQA_PIXEL_U8 = range(6)
@@ -38,15 +41,23 @@ class IqaError(RuntimeError):
         super().__init__(f"{where}: iqa_status {status} ({iqa_status_string(status)})")
 
 
+STALE = False      # True when an out-of-date libiqa_tiles.so had to be loaded because no nvcc is available
+
+
 def _load() -> ctypes.CDLL:
+    global STALE
     try:
         path = _build.build()
-    except Exception as exc:  # no nvcc and no prebuilt library
+    except _build.NoCompiler as exc:   # no nvcc on this machine: a prebuilt library may stand in, and says so
         if not os.path.exists(_build.LIB):
             raise ImportError(
                 "libiqa_tiles.so is not built and nvcc could not build it "
                 f"({exc}); run `python -m paper_2501_10653_b200.build`. There is no CPU fallback.") from exc
-        path = _build.LIB      # stale but present (e.g. read-only tree): use it
+        import warnings
+        warnings.warn("libiqa_tiles.so is older than its sources and nvcc is not available: loading the stale library")
+        STALE = True
+        path = _build.LIB
+    # a compile error is never swallowed: results must describe the sources in the tree
     lib = ctypes.CDLL(path)
     vp, f, i, sz = ctypes.c_void_p, ctypes.c_float, ctypes.c_int, ctypes.c_size_t
     lib.iqa_status_string.restype = ctypes.c_char_p
@@ -72,7 +83,15 @@ def _load() -> ctypes.CDLL:
     lib.iqa_series_tiles.restype = i
     lib.iqa_series_tiles.argtypes = [vp, i, i, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.iqa_query_plan.restype = i
-    lib.iqa_query_plan.argtypes = [vp, i, i, ctypes.c_longlong, i, i]
+    lib.iqa_query_plan.argtypes = [vp, i, i, i, ctypes.c_longlong, i, i]
+    lib.iqa_debug_knob.restype = i
+    lib.iqa_debug_knob.argtypes = [ctypes.c_char_p, i]
+    lib.iqa_fused_batch_2d_typed.restype = i
+    lib.iqa_fused_batch_2d_typed.argtypes = [vp, vp, i, i, i, i, ctypes.c_longlong, i, f, f, f, f,
+                                             vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_series_tiles_2d_typed.restype = i
+    lib.iqa_series_tiles_2d_typed.argtypes = [vp, i, i, i, i, i, ctypes.c_longlong, i, f, f, f, f,
+                                              vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.iqa_workspace_bytes_2d.restype = sz
     lib.iqa_workspace_bytes_2d.argtypes = [i, i, i]
     lib.iqa_fused_tiles_2d.restype = i
@@ -139,6 +158,13 @@ def _current_stream(device=None):
     return torch.cuda.current_stream(device).cuda_stream
 
 
+def _device_of(t):
+    """Context manager making the device of tensor ``t`` (or a torch.device) current: the library launches on, and
+    caches launch geometry for, the CURRENT device, so a call on tensors of another device must switch first."""
+    import torch
+    return torch.cuda.device(t.device if hasattr(t, "device") else t)
+
+
 # ----------------------------------------------------------------------------- C names
 def iqa_status_string(status: int) -> str:
     return lib.iqa_status_string(int(status)).decode()
@@ -200,17 +226,43 @@ def iqa_fused_batch(x_ptrs_host, y_ptrs_host, n_pairs, N, N_T, C1, C2, C, D, lis
                                _ptr(workspace), int(workspace_bytes), _stream(stream))
 
 
-IQA_PLAN_GENERIC, IQA_PLAN_CP_ASYNC, IQA_PLAN_TMA = 0, 1, 16
+IQA_PLAN_GENERIC, IQA_PLAN_TMA_ANY, IQA_PLAN_TMA = 0, 2, 16
 
 
-def iqa_query_plan(x, H, W, pitch, N_T, series=0) -> int:
-    return int(lib.iqa_query_plan(_ptr(x), int(H), int(W), int(pitch), int(N_T), int(series)))
+def iqa_query_plan(x, pixel_type, H, W, pitch, N_T, series=0) -> int:
+    return int(lib.iqa_query_plan(_ptr(x), int(pixel_type), int(H), int(W), int(pitch), int(N_T), int(series)))
+
+
+def iqa_debug_knob(name: str, value: int) -> int:
+    """Test / tuning hook (include/iqa_tiles.h): sets a knob, returns its previous value (-1: unknown name)."""
+    return int(lib.iqa_debug_knob(name.encode(), int(value)))
+
+
+class knob:
+    """``with binding.knob("IQA_FORCE_ANY", 1): ...`` -- sets a library knob for the block and restores it."""
+
+    def __init__(self, name: str, value: int):
+        self.name, self.value = name, int(value)
+
+    def __enter__(self):
+        self.prev = iqa_debug_knob(self.name, self.value)
+        return self
+
+    def __exit__(self, *a):
+        iqa_debug_knob(self.name, self.prev)
+
+
+def _pixel_types():
+    import torch
+    return {torch.float32: IQA_PIXEL_F32, torch.float64: IQA_PIXEL_F64, torch.float16: IQA_PIXEL_F16,
+            torch.int16: IQA_PIXEL_I16, torch.int32: IQA_PIXEL_I32, torch.uint8: IQA_PIXEL_U8}
 
 
 def plan_name(x, N_T, series=False) -> str:
-    """Which kernel a call on the CUDA tensor ``x`` would take: 'tma:c<k>', 'cp.async' or 'generic'."""
-    p = iqa_query_plan(x, x.shape[0], x.shape[1], x.stride(0), N_T, 1 if series else 0)
-    return f"tma:c{p - IQA_PLAN_TMA}" if p >= IQA_PLAN_TMA else {0: "generic", 1: "cp.async"}.get(p, "invalid")
+    """Which kernel a call on the CUDA tensor ``x`` would take: 'tma:c<k>' (tma_kernel), 'tma_any' (any_kernel)
+    or 'generic'."""
+    p = iqa_query_plan(x, _pixel_types()[x.dtype], x.shape[0], x.shape[1], x.stride(0), N_T, 1 if series else 0)
+    return f"tma:c{p - IQA_PLAN_TMA}" if p >= IQA_PLAN_TMA else {0: "generic", 2: "tma_any"}.get(p, "invalid")
 
 
 def iqa_workspace_bytes_2d(H: int, W: int, N_T: int) -> int:
@@ -250,6 +302,27 @@ def iqa_series_tiles_2d(img_ptrs_host, n_images, mode, H, W, pitch, N_T, C1, C2,
     return lib.iqa_series_tiles_2d(it, int(n_images), int(mode), int(H), int(W), int(pitch), int(N_T), C1, C2, C, D,
                                    _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), _ptr(lisi_num),
                                    _ptr(auglisi_num), _ptr(out2), _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
+def iqa_fused_batch_2d_typed(x_ptrs_host, y_ptrs_host, n_pairs, pixel_type, H, W, pitch, N_T, C1, C2, C, D,
+                             lisi, auglisi, sum_x, sum_y, lisi_num=None, auglisi_num=None, out2=None,
+                             workspace=None, workspace_bytes=0, stream=None) -> int:
+    xt, _ = _ptr_table(x_ptrs_host)
+    yt, _ = _ptr_table(y_ptrs_host)
+    return lib.iqa_fused_batch_2d_typed(xt, yt, int(n_pairs), int(pixel_type), int(H), int(W), int(pitch), int(N_T),
+                                        C1, C2, C, D, _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
+                                        _ptr(lisi_num), _ptr(auglisi_num), _ptr(out2), _ptr(workspace),
+                                        int(workspace_bytes), _stream(stream))
+
+
+def iqa_series_tiles_2d_typed(img_ptrs_host, n_images, mode, pixel_type, H, W, pitch, N_T, C1, C2, C, D,
+                              lisi, auglisi, sum_x, sum_y, lisi_num=None, auglisi_num=None, out2=None,
+                              workspace=None, workspace_bytes=0, stream=None) -> int:
+    it, _ = _ptr_table(img_ptrs_host)
+    return lib.iqa_series_tiles_2d_typed(it, int(n_images), int(mode), int(pixel_type), int(H), int(W), int(pitch),
+                                         int(N_T), C1, C2, C, D, _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
+                                         _ptr(lisi_num), _ptr(auglisi_num), _ptr(out2), _ptr(workspace),
+                                         int(workspace_bytes), _stream(stream))
 
 
 def iqa_series_workspace_bytes(n_images: int, N: int, N_T: int) -> int:
@@ -350,8 +423,9 @@ def fused_tiles(x, y, N_T, C1, C2, C, D, numerators: bool = False, workspace=Non
     if workspace is None:
         workspace, _ = make_workspace(N, N_T, x.device)
     wsb = 0 if workspace is None else workspace.numel() * workspace.element_size()
-    rc = iqa_fused_tiles(x, y, N, N_T, C1, C2, C, D, out["lisi"], out["auglisi"], out["X"], out["Y"],
-                         out.get("L"), out.get("A"), workspace, wsb, _current_stream(x.device))
+    with _device_of(x.device):
+        rc = iqa_fused_tiles(x, y, N, N_T, C1, C2, C, D, out["lisi"], out["auglisi"], out["X"], out["Y"],
+                             out.get("L"), out.get("A"), workspace, wsb, _current_stream(x.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_fused_tiles")
     return out
@@ -377,8 +451,9 @@ def fused_batch(xs, ys, N_T, C1, C2, C, D, numerators: bool = False, aggregate: 
         out["whole"] = torch.empty((P, 2), dtype=torch.float32, device=dev)
     nbytes = iqa_batch_workspace_bytes(P, N, N_T)
     ws = torch.empty(nbytes, dtype=torch.uint8, device=dev) if nbytes else None
-    rc = iqa_fused_batch(xs, ys, P, N, N_T, C1, C2, C, D, out["lisi"], out["auglisi"], out["X"], out["Y"],
-                         out.get("L"), out.get("A"), out.get("whole"), ws, nbytes, _current_stream(dev))
+    with _device_of(dev):
+        rc = iqa_fused_batch(xs, ys, P, N, N_T, C1, C2, C, D, out["lisi"], out["auglisi"], out["X"], out["Y"],
+                             out.get("L"), out.get("A"), out.get("whole"), ws, nbytes, _current_stream(dev))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_fused_batch")
     return out
@@ -390,8 +465,7 @@ def fused_tiles_2d(x, y, N_T, C1, C2, C, D, numerators: bool = False) -> dict:
     may be row-pitched views (``stride(1) == 1``, e.g. a window ``big[r0:r1, c0:c1]``); nothing is copied.
     Returns dict of (ceil(H/N_T), ceil(W/N_T)) float32 CUDA tensors: lisi, auglisi, X, Y (+ L, A)."""
     import torch
-    ptypes = {torch.float32: IQA_PIXEL_F32, torch.float64: IQA_PIXEL_F64, torch.float16: IQA_PIXEL_F16,
-              torch.int16: IQA_PIXEL_I16, torch.int32: IQA_PIXEL_I32, torch.uint8: IQA_PIXEL_U8}
+    ptypes = _pixel_types()
     for t in (x, y):
         if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype in ptypes and t.dim() == 2):
             raise TypeError("x and y must be 2-D CUDA tensors of a supported pixel type (no CPU fallback)")
@@ -409,24 +483,28 @@ def fused_tiles_2d(x, y, N_T, C1, C2, C, D, numerators: bool = False) -> dict:
     out = {k: torch.empty((nty, ntx), dtype=torch.float32, device=x.device) for k in names}
     nbytes = iqa_workspace_bytes_2d(H, W, N_T)
     ws = torch.empty(nbytes, dtype=torch.uint8, device=x.device) if nbytes else None
-    rc = iqa_fused_tiles_2d_typed(x, y, ptypes[x.dtype], H, W, x.stride(0), y.stride(0), N_T, C1, C2, C, D,
-                                  out["lisi"], out["auglisi"], out["X"], out["Y"], out.get("L"), out.get("A"),
-                                  ws, nbytes, _current_stream(x.device))
+    with _device_of(x.device):
+        rc = iqa_fused_tiles_2d_typed(x, y, ptypes[x.dtype], H, W, x.stride(0), y.stride(0), N_T, C1, C2, C, D,
+                                      out["lisi"], out["auglisi"], out["X"], out["Y"], out.get("L"), out.get("A"),
+                                      ws, nbytes, _current_stream(x.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_fused_tiles_2d_typed")
     return out
 
 
 def _check_2d_list(images):
+    """Shape, common row pitch and pixel type (IQA_PIXEL_*) of the images of a batch / series call."""
     import torch
+    ptypes = _pixel_types()
     H, W = int(images[0].shape[0]), int(images[0].shape[1])
     pitch = int(images[0].stride(0))
     for t in images:
-        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.dim() == 2):
-            raise TypeError("images must be 2-D float32 CUDA tensors (no CPU fallback)")
-        if tuple(t.shape) != (H, W) or t.stride(1) != 1 or int(t.stride(0)) != pitch or t.device != images[0].device:
-            raise ValueError("all images of a call must share shape, row pitch and device")
-    return H, W, pitch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype in ptypes and t.dim() == 2):
+            raise TypeError("images must be 2-D CUDA tensors of a supported pixel type (no CPU fallback)")
+        if (tuple(t.shape) != (H, W) or t.stride(1) != 1 or int(t.stride(0)) != pitch or t.device != images[0].device
+                or t.dtype != images[0].dtype):
+            raise ValueError("all images of a call must share shape, row pitch, pixel type and device")
+    return H, W, pitch, ptypes[images[0].dtype]
 
 
 def series_tiles_2d(images, mode, N_T, C1, C2, C, D, numerators: bool = False, aggregate: bool = True) -> dict:
@@ -436,7 +514,7 @@ def series_tiles_2d(images, mode, N_T, C1, C2, C, D, numerators: bool = False, a
         raise ValueError(f"mode must be one of {tuple(SERIES_MODES)}")
     if len(images) < 2 or N_T <= 0:
         raise IqaError(IQA_ERR_SHAPE, "series_tiles_2d")
-    H, W, pitch = _check_2d_list(images)
+    H, W, pitch, ptype = _check_2d_list(images)
     K, nty, ntx, dev = len(images) - 1, -(-H // N_T), -(-W // N_T), images[0].device
     names = ["lisi", "auglisi", "X", "Y"] + (["L", "A"] if numerators else [])
     out = {k: torch.empty((K, nty, ntx), dtype=torch.float32, device=dev) for k in names}
@@ -444,11 +522,12 @@ def series_tiles_2d(images, mode, N_T, C1, C2, C, D, numerators: bool = False, a
         out["whole"] = torch.empty((K, 2), dtype=torch.float32, device=dev)
     nbytes = K * iqa_workspace_bytes_2d(H, W, N_T)
     ws = torch.empty(nbytes, dtype=torch.uint8, device=dev) if nbytes else None
-    rc = iqa_series_tiles_2d(images, len(images), SERIES_MODES[mode], H, W, pitch, N_T, C1, C2, C, D,
-                             out["lisi"], out["auglisi"], out["X"], out["Y"], out.get("L"), out.get("A"),
-                             out.get("whole"), ws, nbytes, _current_stream(dev))
+    with _device_of(images[0]):
+        rc = iqa_series_tiles_2d_typed(images, len(images), SERIES_MODES[mode], ptype, H, W, pitch, N_T, C1, C2, C, D,
+                                       out["lisi"], out["auglisi"], out["X"], out["Y"], out.get("L"), out.get("A"),
+                                       out.get("whole"), ws, nbytes, _current_stream(dev))
     if rc != IQA_OK:
-        raise IqaError(rc, "iqa_series_tiles_2d")
+        raise IqaError(rc, "iqa_series_tiles_2d_typed")
     return out
 
 
@@ -457,7 +536,7 @@ def fused_batch_2d(xs, ys, N_T, C1, C2, C, D, numerators: bool = False, aggregat
     import torch
     if len(xs) != len(ys) or not xs or N_T <= 0:
         raise IqaError(IQA_ERR_SHAPE, "fused_batch_2d")
-    H, W, pitch = _check_2d_list(list(xs) + list(ys))
+    H, W, pitch, ptype = _check_2d_list(list(xs) + list(ys))
     P, nty, ntx, dev = len(xs), -(-H // N_T), -(-W // N_T), xs[0].device
     names = ["lisi", "auglisi", "X", "Y"] + (["L", "A"] if numerators else [])
     out = {k: torch.empty((P, nty, ntx), dtype=torch.float32, device=dev) for k in names}
@@ -465,10 +544,12 @@ def fused_batch_2d(xs, ys, N_T, C1, C2, C, D, numerators: bool = False, aggregat
         out["whole"] = torch.empty((P, 2), dtype=torch.float32, device=dev)
     nbytes = P * iqa_workspace_bytes_2d(H, W, N_T)
     ws = torch.empty(nbytes, dtype=torch.uint8, device=dev) if nbytes else None
-    rc = iqa_fused_batch_2d(xs, ys, P, H, W, pitch, N_T, C1, C2, C, D, out["lisi"], out["auglisi"], out["X"], out["Y"],
-                            out.get("L"), out.get("A"), out.get("whole"), ws, nbytes, _current_stream(dev))
+    with _device_of(xs[0]):
+        rc = iqa_fused_batch_2d_typed(xs, ys, P, ptype, H, W, pitch, N_T, C1, C2, C, D, out["lisi"], out["auglisi"],
+                                      out["X"], out["Y"], out.get("L"), out.get("A"), out.get("whole"), ws, nbytes,
+                                      _current_stream(dev))
     if rc != IQA_OK:
-        raise IqaError(rc, "iqa_fused_batch_2d")
+        raise IqaError(rc, "iqa_fused_batch_2d_typed")
     return out
 
 
@@ -494,9 +575,10 @@ def series_tiles(images, mode, N_T, C1, C2, C, D, numerators: bool = False, aggr
         out["whole"] = torch.empty((K, 2), dtype=torch.float32, device=dev)
     nbytes = iqa_series_workspace_bytes(len(images), N, N_T)
     ws = torch.empty(nbytes, dtype=torch.uint8, device=dev) if nbytes else None
-    rc = iqa_series_tiles(images, len(images), SERIES_MODES[mode], N, N_T, C1, C2, C, D,
-                          out["lisi"], out["auglisi"], out["X"], out["Y"], out.get("L"), out.get("A"),
-                          out.get("whole"), ws, nbytes, _current_stream(dev))
+    with _device_of(dev):
+        rc = iqa_series_tiles(images, len(images), SERIES_MODES[mode], N, N_T, C1, C2, C, D,
+                              out["lisi"], out["auglisi"], out["X"], out["Y"], out.get("L"), out.get("A"),
+                              out.get("whole"), ws, nbytes, _current_stream(dev))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_series_tiles")
     return out
@@ -522,7 +604,8 @@ def tiles_below(values, threshold, capacity=None):
     capacity = n if capacity is None else int(capacity)
     idx = torch.full((n_maps, capacity), -1, dtype=torch.int32, device=values.device)
     cnt = torch.empty(n_maps, dtype=torch.int32, device=values.device)
-    rc = iqa_tiles_below(values, n, n_maps, float(threshold), idx, capacity, cnt, _current_stream(values.device))
+    with _device_of(values.device):
+        rc = iqa_tiles_below(values, n, n_maps, float(threshold), idx, capacity, cnt, _current_stream(values.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_tiles_below")
     return idx, cnt
@@ -535,7 +618,8 @@ def tiles_bottom_k(values, k):
     n_maps, n = _check_maps(values)
     idx = torch.empty((n_maps, k), dtype=torch.int32, device=values.device)
     val = torch.empty((n_maps, k), dtype=torch.float32, device=values.device)
-    rc = iqa_tiles_bottom_k(values, n, n_maps, k, idx, val, _current_stream(values.device))
+    with _device_of(values.device):
+        rc = iqa_tiles_bottom_k(values, n, n_maps, k, idx, val, _current_stream(values.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_tiles_bottom_k")
     return idx, val
@@ -563,7 +647,8 @@ def lisi_tiles(x, y, N_T, C1, C2, D, workspace=None):
     if workspace is None:
         workspace, _ = make_workspace(N, N_T, x.device)
     wsb = 0 if workspace is None else workspace.numel() * workspace.element_size()
-    rc = iqa_lisi_tiles(x, y, N, N_T, C1, C2, D, out, workspace, wsb, _current_stream(x.device))
+    with _device_of(x.device):
+        rc = iqa_lisi_tiles(x, y, N, N_T, C1, C2, D, out, workspace, wsb, _current_stream(x.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_lisi_tiles")
     return out
@@ -579,7 +664,8 @@ def auglisi_tiles(x, y, N_T, C, workspace=None):
     if workspace is None:
         workspace, _ = make_workspace(N, N_T, x.device)
     wsb = 0 if workspace is None else workspace.numel() * workspace.element_size()
-    rc = iqa_auglisi_tiles(x, y, N, N_T, C, out, workspace, wsb, _current_stream(x.device))
+    with _device_of(x.device):
+        rc = iqa_auglisi_tiles(x, y, N, N_T, C, out, workspace, wsb, _current_stream(x.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_auglisi_tiles")
     return out
@@ -591,7 +677,8 @@ def aggregate(lisi, auglisi, X, Y, C2, C, out2=None):
     n = lisi.numel()
     if out2 is None:
         out2 = torch.empty(2, dtype=torch.float32, device=lisi.device)
-    rc = iqa_aggregate(lisi, auglisi, X, Y, n, C2, C, out2, _current_stream(lisi.device))
+    with _device_of(lisi.device):
+        rc = iqa_aggregate(lisi, auglisi, X, Y, n, C2, C, out2, _current_stream(lisi.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_aggregate")
     return out2
@@ -601,7 +688,8 @@ def aggregate_partial(lisi, auglisi, X, Y, C2, C):
     """The four double sums of Eqs. 3-4 over the given tiles (one band of a sharded image) -> float64 CUDA tensor [4]."""
     import torch
     sums4 = torch.empty(4, dtype=torch.float64, device=lisi.device)
-    rc = iqa_aggregate_partial(lisi, auglisi, X, Y, lisi.numel(), C2, C, sums4, _current_stream(lisi.device))
+    with _device_of(lisi.device):
+        rc = iqa_aggregate_partial(lisi, auglisi, X, Y, lisi.numel(), C2, C, sums4, _current_stream(lisi.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_aggregate_partial")
     return sums4
@@ -611,7 +699,8 @@ def aggregate_finish(sums4, n_tiles_total, C2, C):
     """Eqs. 3-4 from the all-reduced sums of every band -> float32 CUDA tensor [LISI, augLISI]."""
     import torch
     out2 = torch.empty(2, dtype=torch.float32, device=sums4.device)
-    rc = iqa_aggregate_finish(sums4, n_tiles_total, C2, C, out2, _current_stream(sums4.device))
+    with _device_of(sums4.device):
+        rc = iqa_aggregate_finish(sums4, n_tiles_total, C2, C, out2, _current_stream(sums4.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_aggregate_finish")
     return out2
@@ -637,8 +726,9 @@ def merge_tiles(lisi, auglisi, X, Y, g, C2, C) -> dict:
     shape = (n_maps, no, no) if batched else (no, no)
     out = {k: torch.empty(shape, dtype=torch.float32, device=lisi.device)
            for k in ("lisi", "auglisi", "X", "Y")}
-    rc = iqa_merge_tiles_batch(lisi, auglisi, X, Y, nt, g, n_maps, C2, C, out["lisi"], out["auglisi"], out["X"],
-                               out["Y"], _current_stream(lisi.device))
+    with _device_of(lisi.device):
+        rc = iqa_merge_tiles_batch(lisi, auglisi, X, Y, nt, g, n_maps, C2, C, out["lisi"], out["auglisi"], out["X"],
+                                   out["Y"], _current_stream(lisi.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_merge_tiles_batch")
     return out
@@ -679,9 +769,10 @@ class HostRunner:
         return 4 * 4 * self.nt * self.nt + 8
 
     def __call__(self, x_host, y_host, C1, C2, C, D):
-        rc = iqa_fused_host(x_host, y_host, self.N, self.N_T, C1, C2, C, D,
-                            self.out["lisi"], self.out["auglisi"], self.out["X"], self.out["Y"],
-                            self.out2, self.scratch, self.scratch_bytes, _current_stream(self.device))
+        with _device_of(self.device):
+            rc = iqa_fused_host(x_host, y_host, self.N, self.N_T, C1, C2, C, D,
+                                self.out["lisi"], self.out["auglisi"], self.out["X"], self.out["Y"],
+                                self.out2, self.scratch, self.scratch_bytes, _current_stream(self.device))
         if rc != IQA_OK:
             raise IqaError(rc, "iqa_fused_host")
         return self.out, self.out2
@@ -704,8 +795,9 @@ class HostPipeline:
         self.next = (self.next + 1) % len(self.runners)
         r, st = self.runners[slot], self.streams[slot]
         st.synchronize()                         # the slot's previous pair is complete: its buffers are free
-        rc = iqa_fused_host_async(x_host, y_host, r.N, r.N_T, C1, C2, C, D, r.out["lisi"], r.out["auglisi"],
-                                  r.out["X"], r.out["Y"], r.out2, r.scratch, r.scratch_bytes, st)
+        with _device_of(r.device):
+            rc = iqa_fused_host_async(x_host, y_host, r.N, r.N_T, C1, C2, C, D, r.out["lisi"], r.out["auglisi"],
+                                      r.out["X"], r.out["Y"], r.out2, r.scratch, r.scratch_bytes, st)
         if rc != IQA_OK:
             raise IqaError(rc, "iqa_fused_host_async")
         return slot

@@ -17,7 +17,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "iqa_tiles.cu")]
 HEADERS = [os.path.join(CSRC, "iqa_kernels.cuh"), os.path.join(CSRC, "iqa_aggregate.cuh"),
-           os.path.join(CSRC, "iqa_stream.cuh"), os.path.join(CSRC, "iqa_tma.cuh"), os.path.join(CSRC, "iqa_candidates.cuh"),
+           os.path.join(CSRC, "iqa_any.cuh"), os.path.join(CSRC, "iqa_tma.cuh"), os.path.join(CSRC, "iqa_candidates.cuh"),
            os.path.join(_ROOT, "include", "iqa_tiles.h")]
 LIB = os.path.join(_HERE, "libiqa_tiles.so")
 
@@ -25,11 +25,15 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-shared", "-Xcompiler", "-fPIC", "--cudart", "shared"]
 
 
+class NoCompiler(RuntimeError):
+    """nvcc is not installed (as opposed to: nvcc ran and the sources did not compile)."""
+
+
 def _nvcc() -> str:
     for cand in (os.environ.get("NVCC"), shutil.which("nvcc"), "/usr/local/cuda/bin/nvcc"):
         if cand and os.path.exists(cand):
             return cand
-    raise RuntimeError("nvcc not found: libiqa_tiles.so cannot be built (there is no CPU fallback)")
+    raise NoCompiler("nvcc not found: libiqa_tiles.so cannot be built (there is no CPU fallback)")
 
 
 def is_stale() -> bool:

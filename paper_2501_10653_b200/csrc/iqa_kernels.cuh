@@ -5,7 +5,7 @@
 //   finalise_tile    S4: Eq. 1 / Eq. 2 from the four sums of one tile
 //   generic_kernel   any N_T dividing N, any 4-byte aligned pointers (slow path, still CUDA)
 //   finalise_*       second pass for tiles that were split over several CTAs (workspace)
-// The fast path (power-of-two N_T >= 8, 16-byte aligned images) is iqa_stream.cuh.
+// The fast paths are iqa_tma.cuh (fp32, power-of-two N_T >= 8) and iqa_any.cuh (any N_T >= 4, any pixel type).
 // Every kernel starts with pdl_prologue(): when launched with the programmatic-stream-
 // serialisation attribute its CTAs may become resident while the previous kernel of the
 // stream drains; griddepcontrol.wait then blocks until that kernel has completed and its
@@ -53,6 +53,29 @@ __device__ __forceinline__ float rcp_approx(float v) {
     float r;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
     return r;
+}
+
+// Position of one persistent CTA in its item sequence b, b+G, b+2G, ... kept as (pair, uy, ux) and advanced
+// by the decoded stride (no integer division in the loop).  Items are numbered pair-major, then row-major.
+struct ItemCursor {
+    int pair, uy, ux;
+    __device__ __forceinline__ void advance(const ItemCursor& d, int units_x, int units_y) {
+        ux += d.ux;
+        const int cx = ux >= units_x;
+        ux -= cx ? units_x : 0;
+        uy += d.uy + cx;
+        const int cy = uy >= units_y;
+        uy -= cy ? units_y : 0;
+        pair += d.pair + cy;
+    }
+};
+__device__ __forceinline__ ItemCursor decode_item(int q, int units_x, int units_y) {
+    ItemCursor c;
+    const int t = q / units_x;
+    c.ux = q - t * units_x;
+    c.pair = t / units_y;
+    c.uy = t - c.pair * units_y;
+    return c;
 }
 
 // S1 + S2 for one pixel pair: clamp, then the Eq. 1 and Eq. 2 terms.
@@ -124,8 +147,8 @@ __device__ __forceinline__ void finalise_tile(const Params& p, size_t t, float4 
 }
 
 // -----------------------------------------------------------------------------
-// Generic kernel: any N_T, any H x W with row pitches (edge tiles), any 4-byte aligned pointers (the stream kernel needs a
-// power-of-two N_T >= 8 and 16-byte alignment).  One CTA per (tile, piece), a piece being up
+// Generic kernel: any N_T, any H x W with ANY row pitch (edge tiles), any element-aligned pointers -- what is
+// left when no tensor map can describe the image (row pitch not a multiple of 16 bytes) or N_T < 4.  One CTA per (tile, piece), a piece being up
 // to kGenericRows rows of the tile; scalar coalesced loads, thread-strided partial sums,
 // warp butterfly, warp order.  pieces == 1: the CTA finalises its tile; otherwise the
 // partial goes to the workspace and finalise_kernel finishes.

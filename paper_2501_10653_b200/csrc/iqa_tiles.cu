@@ -1,21 +1,27 @@
 // =============================================================================
-// iqa_tiles.cu -- the C ABI of include/iqa_tiles.h: argument validation, the N_T-dependent
-// choice of mapping, and the launches.  No torch types, no allocation; the only thing kept
-// between calls is a per-device cache of launch geometry (SM count, CTAs per SM).
+// iqa_tiles.cu -- the C ABI of include/iqa_tiles.h: argument validation, the choice of kernel and
+// mapping, tensor-map encoding, and the launches.  No torch types, no allocation of device memory; the
+// only things kept between calls are a per-device cache of launch geometry (SM count, CTAs per SM) and
+// the test / tuning knobs of iqa_debug_knob.
+// Order of every entry point: validate -> plan -> encode EVERY tensor map of the call on the host ->
+// launch.  Nothing is enqueued unless all of the first three succeeded.
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -shared -Xcompiler -fPIC
 // =============================================================================
 #include "../../include/iqa_tiles.h"
 
 #include <atomic>
+#include <cfloat>
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
+#include <cstring>
 #include <utility>
+#include <vector>
 
 #include "iqa_aggregate.cuh"
+#include "iqa_any.cuh"
 #include "iqa_candidates.cuh"
 #include "iqa_kernels.cuh"
-#include "iqa_stream.cuh"
 #include "iqa_tma.cuh"
 
 namespace {
@@ -24,66 +30,69 @@ using namespace iqa;
 
 constexpr int kMaxN = 1 << 20;   // 2^40 pixels; keeps every grid and tile index inside int
 constexpr int kMaxDevices = 64;
+constexpr int kGenericBatch = 32;   // pairs per chunk of the pair-by-pair paths
 
 bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+int ceil_div(int a, int b) { return (a + b - 1) / b; }
+int round_up(int a, int b) { return ceil_div(a, b) * b; }
 bool pos_finite(float v) { return std::isfinite(v) && v > 0.0f; }
+// C1 feeds rcp.approx.ftz (|x - y| + C1 with x == y): a subnormal C1 would be flushed to zero there
+bool pos_normal(float v) { return std::isfinite(v) && v >= FLT_MIN; }
 
-int env_int(const char* name, int dflt) {
-    const char* s = std::getenv(name);
-    return (s && *s) ? std::atoi(s) : dflt;
-}
+// ---- test / tuning knobs (iqa_debug_knob): read from the environment ONCE, then plain atomics -------------------
+//   IQA_FORCE_GENERIC    1: every call takes the generic kernels
+//   IQA_FORCE_ANY        1: fp32 power-of-two shapes take the general TMA kernel (iqa_any.cuh) instead of tma_kernel
+//   IQA_TMA_CONFIG       0..4: ring / box configuration of tma_kernel (-1: default)
+//   IQA_TMA_MAX_CTAS     cap of the persistent grid (0: none)
+//   IQA_NO_PDL           1: launch without programmatic dependent launch
+//   IQA_CAND_NO_CLUSTER  1: candidate kernels never use the cluster twins
+enum Knob { kKnobForceGeneric, kKnobForceAny, kKnobTmaConfig, kKnobTmaMaxCtas, kKnobNoPdl, kKnobCandNoCluster, kNumKnobs };
+const char* const kKnobNames[kNumKnobs] = {"IQA_FORCE_GENERIC", "IQA_FORCE_ANY", "IQA_TMA_CONFIG", "IQA_TMA_MAX_CTAS",
+                                           "IQA_NO_PDL", "IQA_CAND_NO_CLUSTER"};
+const int kKnobDefaults[kNumKnobs] = {0, 0, -1, 0, 0, 0};
+struct Knobs {
+    std::atomic<int> v[kNumKnobs];
+    Knobs() {
+        for (int i = 0; i < kNumKnobs; ++i) {
+            const char* s = std::getenv(kKnobNames[i]);
+            v[i].store((s && *s) ? std::atoi(s) : kKnobDefaults[i], std::memory_order_relaxed);
+        }
+    }
+};
+Knobs& knobs() { static Knobs k; return k; }
+int knob(Knob k) { return knobs().v[k].load(std::memory_order_relaxed); }
 
-// ---- stream-kernel variants (rows per warp and stage K, ring depth, CTAs per SM) -----------
-// Measured on B200 (profiles/r01*_variants.md): 48-64 KiB of copies in
-// flight per SM is the sweet spot; deeper rings or more CTAs lose DRAM locality (down to
-// 6.1-6.4 TB/s), fewer warps lose latency hiding.  Variants 0 and 1 are within 1 % of each other.
-//   variant 0  K=4, depth 2, 2 CTAs/SM  (stage = 32 rows, 68 KiB smem/CTA, 64 KiB in flight per SM)  default
-//   variant 1  K=2, depth 2, 3 CTAs/SM  (stage = 16 rows, 36 KiB smem/CTA, 48 KiB in flight per SM)
-//   variant 2  K=8, depth 2, 1 CTA/SM   (stage = 64 rows, 132 KiB smem/CTA)  mapping-independence tests only
-// The default path is the TMA-fed kernel of iqa_tma.cuh (kTmaConfigs below); the cp.async variants stay as the
-// fallback when a tensor map cannot be encoded and for the mapping-independence tests.
-// IQA_FORCE_VARIANT=v selects one of them (debug / tuning knob); all kernels agree to ~1e-7 relative.
-constexpr int kNumVariants = 3;
-struct VariantInfo { int K, depth, min_ctas; };
-constexpr VariantInfo kVariants[kNumVariants] = {{4, 2, 2}, {2, 2, 3}, {8, 2, 1}};
-
-using StreamFn = void (*)(const BatchParams);
-
-template <int MODE>
-StreamFn stream_fn(int variant) {
-    switch (variant) {
-        case 1: return stream_kernel<MODE, 2, 2, 3>;
-        case 2: return stream_kernel<MODE, 8, 2, 1>;
-        default: return stream_kernel<MODE, 4, 2, 2>;
+// ---- pixel types -----------------------------------------------------------------------------------------
+int esize_of(int ptype) {
+    switch (ptype) {
+        case IQA_PIXEL_F32: case IQA_PIXEL_I32: return 4;
+        case IQA_PIXEL_F64: return 8;
+        case IQA_PIXEL_F16: case IQA_PIXEL_I16: return 2;
+        case IQA_PIXEL_U8: return 1;
+        default: return 0;
     }
 }
-StreamFn stream_fn(int mode, int variant) {
-    switch (mode) {
-        case kModeLisi: return stream_fn<kModeLisi>(variant);
-        case kModeAug: return stream_fn<kModeAug>(variant);
-        default: return stream_fn<kModeFused>(variant);
-    }
-}
-size_t stream_smem(int variant) {
-    switch (variant) {
-        case 1: return stream_smem_bytes<2, 2>();
-        case 2: return stream_smem_bytes<8, 2>();
-        default: return stream_smem_bytes<4, 2>();
+CUtensorMapDataType tma_type_of(int ptype) {
+    switch (ptype) {
+        case IQA_PIXEL_F64: return CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
+        case IQA_PIXEL_F16: return CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
+        case IQA_PIXEL_I16: return CU_TENSOR_MAP_DATA_TYPE_UINT16;     // bits only; the kernel reinterprets
+        case IQA_PIXEL_I32: return CU_TENSOR_MAP_DATA_TYPE_INT32;
+        case IQA_PIXEL_U8: return CU_TENSOR_MAP_DATA_TYPE_UINT8;
+        default: return CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
     }
 }
 
-using TmaFn = void (*)(const TmaParams);
-
-// TMA kernel configurations: {box slots per CTA, rows per warp and box}.  Measured on B200
-// (profiles/r01g_tma_configs.md): pairs are HBM-bound and want FEW bytes in flight (config 1: two
-// 16 KiB boxes in flight per CTA while two are consumed; six boxes lose 3-6 % to DRAM locality, as
-// the cp.async variants did); the series modes keep S + 1 boxes alive and want the deeper ring of
-// config 0.  IQA_TMA_CONFIG=c forces one (tuning knob).
+// ---- tma_kernel configurations: {box slots per CTA, rows per warp and box} ------------------------------------
+// Measured on B200 (profiles/r01g_tma_configs.md): pairs are HBM-bound and want FEW bytes in flight (config 1: two
+// 16 KiB boxes in flight per CTA while two are consumed; six boxes lose 3-6 % to DRAM locality); the series modes
+// keep S + 1 boxes alive and want the deeper ring of config 0.
 struct TmaConfig { int boxes, rpw; };
 constexpr int kNumTmaConfigs = 5;
 constexpr TmaConfig kTmaConfigs[kNumTmaConfigs] = {{6, 4}, {4, 4}, {8, 2}, {6, 2}, {4, 2}};
 
+using TmaFn = void (*)(const TmaParams);
 template <int MODE, int SERIES>
 TmaFn tma_fn_cfg(int cfg) {
     switch (cfg) {
@@ -108,6 +117,35 @@ TmaFn tma_fn(int mode, int series, int cfg) {
 }
 size_t tma_smem(int cfg) { return tma_smem_bytes(kTmaConfigs[cfg].boxes, kTmaConfigs[cfg].rpw); }
 
+// any_kernel instantiations: the three modes for fp32 (paper-named entry points with odd N_T), fused for the rest.
+using AnyFn = void (*)(const AnyParams);
+constexpr int kNumAnyFns = 8;
+AnyFn any_fn_at(int i) {
+    switch (i) {
+        case 0: return any_kernel<kModeLisi, float>;
+        case 1: return any_kernel<kModeAug, float>;
+        case 2: return any_kernel<kModeFused, float>;
+        case 3: return any_kernel<kModeFused, double>;
+        case 4: return any_kernel<kModeFused, __half>;
+        case 5: return any_kernel<kModeFused, short>;
+        case 6: return any_kernel<kModeFused, int>;
+        default: return any_kernel<kModeFused, unsigned char>;
+    }
+}
+int any_fn_index(int mode, int ptype) {
+    switch (ptype) {
+        case IQA_PIXEL_F32: return mode == kModeLisi ? 0 : mode == kModeAug ? 1 : 2;
+        case IQA_PIXEL_F64: return 3;
+        case IQA_PIXEL_F16: return 4;
+        case IQA_PIXEL_I16: return 5;
+        case IQA_PIXEL_I32: return 6;
+        default: return 7;
+    }
+}
+constexpr int kAnyBoxBudget = 20480;    // bytes of one box
+constexpr int kAnyRingBudget = 81920;   // bytes of the ring of boxes of one CTA (2 CTAs per SM)
+constexpr size_t kAnyMaxSmem = 1024 + kAnyRingBudget + 128 * kAnyMaxSlots + kAnyPartBufs * kWarpsPerCta * 32 * 16 + 256;
+
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda).
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -124,23 +162,30 @@ EncodeTiledFn encode_tiled_fn() {
     return fn;
 }
 
-// Tensor map of one H x W fp32 row-major image with a row pitch (in elements): boxes of 128 columns x box_rows rows, no swizzle (a box
-// lands as [box_rows][128] floats), out-of-bounds elements read as zero.  Needs a 16-byte aligned base
-// and pitch % 4 == 0 (row pitch a multiple of 16 bytes); W itself is free.
-bool encode_image_map(CUtensorMap* map, const float* img, int H, int W, long long pitch, int box_rows) {
+// Tensor map of one H x W row-major image of `ptype` pixels with a row pitch (in elements): boxes of box_w columns x
+// box_rows rows, no swizzle (a box lands as [box_rows][box_w] elements), out-of-bounds elements read as zero.
+// The image base only needs the alignment of its element type: the tensor starts at the 16-byte boundary below it and
+// is (base & 15) / sizeof(pixel) elements wider on the left; any_kernel works in tensor columns and masks those
+// elements (they lie in the same 16-byte line as pixel (0, 0), hence inside the allocation).  The row pitch must be
+// a multiple of 16 bytes.
+bool encode_image_map(CUtensorMap* map, const void* img, int ptype, int H, int W, long long pitch,
+                      int box_w, int box_rows) {
     const EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return false;
-    const cuuint64_t dims[2] = {(cuuint64_t)W, (cuuint64_t)H};
-    const cuuint64_t strides[1] = {(cuuint64_t)pitch * sizeof(float)};
-    const cuuint32_t box[2] = {(cuuint32_t)kUnitCols, (cuuint32_t)box_rows};
+    const int es = esize_of(ptype);
+    const uintptr_t addr = (uintptr_t)img;
+    const unsigned sh = (unsigned)((addr & 15u) / (unsigned)es);
+    const cuuint64_t dims[2] = {(cuuint64_t)W + sh, (cuuint64_t)H};
+    const cuuint64_t strides[1] = {(cuuint64_t)pitch * (cuuint64_t)es};
+    const cuuint32_t box[2] = {(cuuint32_t)box_w, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1u, 1u};
-    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2u, const_cast<float*>(img), dims, strides, box, estr,
+    return enc(map, tma_type_of(ptype), 2u, (void*)(addr & ~(uintptr_t)15u), dims, strides, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // Per-device launch geometry, filled on first use (benign race: every thread computes the same values).
-struct Geometry { std::atomic<int> ready{0}; int sms; int ctas[3][kNumVariants]; int tma_ctas[kNumTmaConfigs]; };
+struct Geometry { std::atomic<int> ready{0}; int sms; int tma_ctas[kNumTmaConfigs]; };
 Geometry g_geo[kMaxDevices];
 
 const Geometry* geometry() {
@@ -150,15 +195,6 @@ const Geometry* geometry() {
     if (g.ready.load(std::memory_order_acquire)) return &g;
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return nullptr;
-    for (int m = 0; m < 3; ++m)
-        for (int v = 0; v < kNumVariants; ++v) {
-            StreamFn fn = stream_fn(m + 1, v);
-            const size_t smem = stream_smem(v);
-            if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return nullptr;
-            int occ = 0;
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kCtaThreads, smem) != cudaSuccess || occ <= 0) return nullptr;
-            g.ctas[m][v] = occ < kVariants[v].min_ctas ? occ : kVariants[v].min_ctas;
-        }
     for (int c = 0; c < kNumTmaConfigs; ++c) {
         g.tma_ctas[c] = 0;
         for (int m = 1; m <= 3; ++m)
@@ -172,6 +208,9 @@ const Geometry* geometry() {
                 g.tma_ctas[c] = g.tma_ctas[c] == 0 || occ < g.tma_ctas[c] ? occ : g.tma_ctas[c];
             }
     }
+    for (int i = 0; i < kNumAnyFns; ++i)
+        if (cudaFuncSetAttribute(any_fn_at(i), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAnyMaxSmem) != cudaSuccess)
+            return nullptr;
     g.sms = sms;
     g.ready.store(1, std::memory_order_release);
     return &g;
@@ -190,8 +229,7 @@ cudaError_t launch_cluster(void (*kernel)(KArgs...), unsigned grid, unsigned blo
     cfg.stream = st;
     cudaLaunchAttribute attr[2];
     unsigned na = 0;
-    static const bool no_pdl = env_int("IQA_NO_PDL", 0) != 0;
-    if (!no_pdl) {
+    if (!knob(kKnobNoPdl)) {
         attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[na].val.programmaticStreamSerializationAllowed = 1;
         ++na;
@@ -220,42 +258,138 @@ int status_of_shape(int N, int N_T) {
     return IQA_OK;
 }
 
-// How (N, N_T) is mapped onto CTAs.  DESIGN.md "Mapping".
-enum PlanKind { kPlanGeneric = 0, kPlanStream = 1, kPlanTma = 2 };
+// Geometry of the images of one call: the x images share pitch_x, the y images pitch_y (elements).
+struct Geom { int H, W; long long pitch_x, pitch_y; int ptype; };
+Geom square_geom(int N) { return Geom{N, N, (long long)N, (long long)N, IQA_PIXEL_F32}; }
+
+// ---- run-time geometry of any_kernel (iqa_any.cuh) ------------------------------------------------------------
+struct AnyGeom {
+    int kx, ky, px, py, pw, ph, box_w, box_rows, row_bytes, slot_bytes, n_slots, rpw, wpt, fin_gsz, units_x, units_y;
+    int const_s;       // every item sits at the same column offset inside its box
+};
+constexpr int kAnySplitAbove = 112;   // tiles wider than this are split (128 lanes-columns minus the widest 16-byte pad)
+// Pieces per split tile (N_T > kAnySplitAbove): pw x 64 pixels each, pw a multiple of 16 columns; the same for every
+// pixel type and alignment, so that the workspace size is a function of N_T alone.
+void any_pieces(int N_T, int* pw, int* px, int* py) {
+    const int px0 = ceil_div(N_T, kAnySplitAbove);
+    *pw = round_up(ceil_div(N_T, px0), 16);
+    *px = ceil_div(N_T, *pw);
+    *py = ceil_div(N_T, 64);
+}
+// shift: elements between the 16-byte boundary below the image bases and pixel (0, 0) (the same for every image).
+AnyGeom any_geometry(int esize, int N_T, int H, int W, int shift) {
+    AnyGeom g{};
+    const int pad = 16 / esize;                       // elements per 16 bytes: a TMA box starts at a multiple of it
+    const int wpad = pad < 4 ? 4 : pad;               // box widths are whole lanes (4 columns) as well
+    const int ntx = ceil_div(W, N_T), nty = ceil_div(H, N_T);
+    if (N_T <= kAnySplitAbove) {                      // whole tiles inside one item: kx across, ky down
+        // kx_a: items that start on 16-byte boundaries (s = 0 everywhere); kx_s: items at any column, which costs
+        // pad - 1 columns of the box
+        int kx_a = 0;
+        if (shift == 0)
+            for (int k = kUnitCols / N_T; k >= 1; --k)
+                if ((k * N_T) % pad == 0) { kx_a = k; break; }
+        int kx_s = (kUnitCols - pad + 1) / N_T;
+        if (kx_a > ntx) kx_a = ntx;
+        if (kx_s > ntx) kx_s = ntx;
+        if (kx_a > 0 && kx_a * 8 >= kx_s * 7) {
+            g.kx = kx_a;
+            g.const_s = 1;
+            g.box_w = round_up(g.kx * N_T, wpad);
+        } else {
+            g.kx = kx_s;
+            g.const_s = (g.kx * N_T) % pad == 0 || g.kx >= ntx;      // one item column: c0 = 0 everywhere
+            g.box_w = round_up(g.kx * N_T + pad - 1, wpad);
+        }
+        g.pw = g.kx * N_T;
+        g.row_bytes = g.box_w * esize;
+        int rows_fit = kAnyBoxBudget / g.row_bytes;
+        if (rows_fit > 256) rows_fit = 256;
+        g.ky = 1;
+        if (N_T <= rows_fit) {                        // several tile rows per box, 8 / ky warps each
+            while (g.ky < kWarpsPerCta && 2 * g.ky * N_T <= rows_fit && g.ky < nty) g.ky *= 2;
+            g.box_rows = g.ky * N_T;
+            g.wpt = kWarpsPerCta / g.ky;
+            g.rpw = ceil_div(N_T, g.wpt);
+        } else {                                      // the tile's rows in S boxes
+            const int S = ceil_div(N_T, rows_fit);
+            g.box_rows = ceil_div(N_T, S);
+            g.wpt = kWarpsPerCta;
+            g.rpw = ceil_div(g.box_rows, kWarpsPerCta);
+        }
+        g.ph = g.ky * N_T;
+        g.px = g.py = 1;
+    } else {                                          // split tiles: pieces of pw x 64 pixels
+        any_pieces(N_T, &g.pw, &g.px, &g.py);
+        g.kx = g.ky = 1;
+        g.const_s = N_T % pad == 0;                   // pw is a multiple of 16 columns
+        g.box_w = g.const_s && shift == 0 ? g.pw : round_up(g.pw + pad - 1, wpad);
+        g.row_bytes = g.box_w * esize;
+        g.box_rows = 64;
+        while (g.box_rows * g.row_bytes > kAnyBoxBudget) g.box_rows /= 2;
+        g.ph = 64;
+        g.wpt = kWarpsPerCta;
+        g.rpw = ceil_div(g.box_rows, kWarpsPerCta);
+    }
+    g.slot_bytes = round_up(g.box_rows * g.row_bytes, 128);
+    g.n_slots = (kAnyRingBudget / g.slot_bytes) & ~1;
+    if (g.n_slots < 4) g.n_slots = 4;
+    if (g.n_slots > kAnyMaxSlots) g.n_slots = kAnyMaxSlots;
+    int p2 = 1;
+    while (p2 < g.kx * g.ky) p2 <<= 1;
+    g.fin_gsz = p2 >= 32 ? 1 : 32 / p2;
+    g.units_x = ceil_div(ntx, g.kx) * g.px;
+    g.units_y = ceil_div(nty, g.ky) * g.py;
+    return g;
+}
+
+// How a call is mapped onto kernels.  DESIGN.md "Kernels".
+enum PlanKind { kPlanGeneric = 0, kPlanTma = 2, kPlanAny = 3 };
 struct Plan {
-    PlanKind kind;     // generic kernel / cp.async stream kernel / TMA kernel
-    int variant;       // stream: index into kVariants
+    PlanKind kind;     // generic kernels / tma_kernel (fp32, power-of-two N_T) / any_kernel
     int tma_cfg;       // tma: index into kTmaConfigs
-    int item_rows;     // stream, tma: R
+    int item_rows;     // tma: R
     int pieces_x, pieces_y, pieces;   // pieces per tile; pieces == 1 -> finished inside one CTA
+    AnyGeom any;
 };
 
-constexpr int kSplitItemRows = 64;   // tiles of side >= 128: items of 128 x 64, pieces to the workspace
+constexpr int kSplitItemRows = 64;   // tma_kernel, tiles of side >= 128: items of 128 x 64, pieces to the workspace
 
-// General image geometry of the 2-D entry point (pairs only): x has pitch_x, y has pitch_y.
-struct Geom2D { int H, W; long long pitch_x, pitch_y; };
+void generic_plan(Plan& pl, int N_T) {
+    pl.kind = kPlanGeneric;
+    pl.pieces_x = 1;
+    pl.pieces_y = ceil_div(N_T, kGenericRows);
+    pl.pieces = pl.pieces_y;
+}
 
-// first_image: one image of the call (the TMA path is taken only when its tensor map encodes).
-Plan make_plan(int N, int N_T, bool aligned16, const float* first_image, bool series, const Geom2D* g2 = nullptr) {
+// Alignment of the images of a call: `lo16` = the offset of every base inside its 16-byte line when all images
+// share it (-1 when they differ: no common column grid for the TMA boxes).
+struct Align { int lo16; };
+Align align_of(const void* const* a, int na, const void* const* b, int nb) {
+    const int lo = (int)((uintptr_t)a[0] & 15u);
+    for (int i = 0; i < na; ++i)
+        if ((int)((uintptr_t)a[i] & 15u) != lo) return Align{-1};
+    for (int i = 0; i < nb; ++i)
+        if ((int)((uintptr_t)b[i] & 15u) != lo) return Align{-1};
+    return Align{lo};
+}
+
+// A tensor map can describe the images when every row pitch is a multiple of 16 bytes; the boxes of x and y share
+// their column grid when all bases have the same offset inside a 16-byte line (al.lo16 >= 0).
+Plan make_plan(const Geom& g, int N_T, Align al, bool series) {
     Plan pl{};
-    const bool fast = is_pow2(N_T) && N_T >= 8 && aligned16 && !env_int("IQA_FORCE_GENERIC", 0);
-    pl.kind = fast ? kPlanTma : kPlanGeneric;
-    if (fast) {
-        const int forced = env_int("IQA_FORCE_VARIANT", -1);     // debug knob (tests: mapping independence)
-        if (forced >= 0 && forced < kNumVariants && !g2) { pl.kind = kPlanStream; pl.variant = forced; }
-        if (pl.kind == kPlanTma) {
-            const int dflt = series ? 0 : 1;
-            const int c = env_int("IQA_TMA_CONFIG", dflt);
-            pl.tma_cfg = c >= 0 && c < kNumTmaConfigs ? c : dflt;
-            // the series modes keep S + 1 boxes alive (S = 64 / box rows for N_T >= 64): small rings fall back
-            if (series && kTmaConfigs[pl.tma_cfg].boxes < 64 / (kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw) + 2) pl.tma_cfg = 0;
-            CUtensorMap probe;
-            const bool ok = g2 ? encode_image_map(&probe, first_image, g2->H, g2->W, g2->pitch_x, kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw)
-                               : encode_image_map(&probe, first_image, N, N, N, kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw);
-            if (!ok) { pl.kind = g2 ? kPlanGeneric : kPlanStream; pl.variant = 0; }
-        }
-        const int rs = pl.kind == kPlanTma ? kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw
-                                           : kWarpsPerCta * kVariants[pl.variant].K;   // stage height
+    generic_plan(pl, N_T);
+    const int es = esize_of(g.ptype);
+    const bool tma_able = (g.pitch_x * es) % 16 == 0 && (g.pitch_y * es) % 16 == 0 && al.lo16 >= 0;
+    if (!tma_able || N_T < 4 || knob(kKnobForceGeneric)) return pl;
+    if (g.ptype == IQA_PIXEL_F32 && is_pow2(N_T) && N_T >= 8 && al.lo16 == 0 && !knob(kKnobForceAny)) {
+        pl.kind = kPlanTma;
+        const int dflt = series ? 0 : 1;
+        const int c = knob(kKnobTmaConfig);
+        pl.tma_cfg = c >= 0 && c < kNumTmaConfigs ? c : dflt;
+        // the series modes keep S + 1 boxes alive (S = 64 / box rows for N_T >= 64): small rings fall back
+        if (series && kTmaConfigs[pl.tma_cfg].boxes < 64 / (kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw) + 2) pl.tma_cfg = 0;
+        const int rs = kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw;       // box height
         if (N_T <= 64) {
             pl.item_rows = N_T > rs ? N_T : rs;                  // whole tiles inside one item
             pl.pieces_x = pl.pieces_y = 1;
@@ -264,19 +398,26 @@ Plan make_plan(int N, int N_T, bool aligned16, const float* first_image, bool se
             pl.pieces_x = N_T / kUnitCols;
             pl.pieces_y = N_T / kSplitItemRows;
         }
+        pl.pieces = pl.pieces_x * pl.pieces_y;
+        return pl;
     }
-    if (pl.kind == kPlanGeneric) {
-        pl.pieces_x = 1;
-        pl.pieces_y = (N_T + kGenericRows - 1) / kGenericRows;
-    }
+    pl.kind = kPlanAny;
+    pl.any = any_geometry(es, N_T, g.H, g.W, al.lo16 / es);
+    pl.pieces_x = pl.any.px;
+    pl.pieces_y = pl.any.py;
     pl.pieces = pl.pieces_x * pl.pieces_y;
     return pl;
 }
 
-// Pieces per tile in the worst case over the mappings a call may take (tma, stream or generic).
+// Pieces per tile in the worst case over the mappings a call may take (tma, any or generic).
 size_t max_pieces(int N_T) {
     if (N_T <= 64) return 1;                                      // every path finishes tiles inside one CTA
-    size_t pieces = (size_t)(N_T + kGenericRows - 1) / kGenericRows;
+    size_t pieces = (size_t)ceil_div(N_T, kGenericRows);
+    if (N_T > kAnySplitAbove) {
+        int pw, px, py;
+        any_pieces(N_T, &pw, &px, &py);
+        if ((size_t)px * py > pieces) pieces = (size_t)px * py;
+    }
     if (is_pow2(N_T)) {
         const size_t s = (size_t)(N_T / kUnitCols) * (size_t)(N_T / kSplitItemRows);
         if (s > pieces) pieces = s;
@@ -305,32 +446,39 @@ struct Outputs {
 
 struct Consts { float C1, C2, C, D; };
 
-// The TMA kernel over n_groups groups of M images (imgs[g * M + i], HOST array of device pointers);
-// `out` and `ws` point at the first comparison of the first group.  n_groups * M may exceed
-// kMaxImages (several launches); M itself may not.
-int launch_tma(int mode, int series, const float* const* imgs, int n_groups, int M, int N, int N_T, const Consts& k,
-               const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st, const Geom2D* g2 = nullptr) {
+// ---- tma_kernel: encode, then launch --------------------------------------------------------------------------
+struct TmaLaunch { TmaParams p; TmaFn fn; unsigned grid; size_t smem; };
+
+// n_groups groups of M images (imgs[g * M + i], HOST array of device pointers); `out` and `ws` point at the first
+// comparison of the first group.  n_groups * M may exceed kMaxImages (several launches); M itself may not.  Image i of
+// a group has pitch_y when (i & 1) else pitch_x (pairs: x, y; series: both pitches are equal).
+// Appends the prepared launches; false when a tensor map could not be encoded (nothing was launched).
+bool prepare_tma(std::vector<TmaLaunch>& q, int mode, int series, const void* const* imgs, int n_groups, int M,
+                 const Geom& g, int N_T, const Consts& k, const Outputs& out, float4* ws, const Plan& pl) {
     const Geometry* geo = geometry();
     TmaFn fn = tma_fn(mode, series, pl.tma_cfg);
     const int box_rows = kWarpsPerCta * kTmaConfigs[pl.tma_cfg].rpw;
-    if (!geo || !fn || geo->tma_ctas[pl.tma_cfg] <= 0 || M < 2 || M > kMaxImages) return IQA_ERR_CUDA;
-    const int H = g2 ? g2->H : N, W = g2 ? g2->W : N;
-    const int ntx = (W + N_T - 1) / N_T, nty = (H + N_T - 1) / N_T;
+    if (!geo || !fn || geo->tma_ctas[pl.tma_cfg] <= 0 || M < 2 || M > kMaxImages) return false;
+    const int H = g.H, W = g.W;
+    const int ntx = ceil_div(W, N_T), nty = ceil_div(H, N_T);
     const long long n = (long long)ntx * nty;
     // split tiles: the items cover the whole tile grid, so that every piece of an edge tile is written
     // (boxes entirely outside the image are zero-filled by the TMA unit without touching memory)
-    const int units_x = pl.pieces > 1 ? ntx * pl.pieces_x : (W + kUnitCols - 1) / kUnitCols;
-    const int units_y = pl.pieces > 1 ? nty * pl.pieces_y : (H + pl.item_rows - 1) / pl.item_rows;
+    const int units_x = pl.pieces > 1 ? ntx * pl.pieces_x : ceil_div(W, kUnitCols);
+    const int units_y = pl.pieces > 1 ? nty * pl.pieces_y : ceil_div(H, pl.item_rows);
     const long long items_per_group = (long long)units_x * units_y;
     const int groups_per_launch = kMaxImages / M;
-    if (items_per_group * groups_per_launch > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    if (items_per_group * groups_per_launch > 0x7fffffffLL) return false;
     for (int first = 0; first < n_groups; first += groups_per_launch) {
         const int ng = n_groups - first < groups_per_launch ? n_groups - first : groups_per_launch;
-        TmaParams p{};
+        q.emplace_back();
+        TmaLaunch& L = q.back();
+        TmaParams& p = L.p;
+        std::memset(&p, 0, sizeof(p));
         for (int i = 0; i < ng * M; ++i)
-            if (!encode_image_map(&p.maps[i], imgs[(size_t)first * M + i], H, W,
-                                  g2 ? ((i & 1) ? g2->pitch_y : g2->pitch_x) : (long long)N, box_rows))
-                return IQA_ERR_CUDA;
+            if (!encode_image_map(&p.maps[i], imgs[(size_t)first * M + i], IQA_PIXEL_F32, H, W,
+                                  (i & 1) ? g.pitch_y : g.pitch_x, kUnitCols, box_rows))
+                return false;
         p.n_groups = ng; p.M = M; p.W = W; p.H = H; p.log2_nt = ilog2(N_T); p.ntx = ntx; p.n_tiles = (int)n;
         p.units_x = units_x; p.units_y = units_y; p.S = pl.item_rows / box_rows;
         p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
@@ -338,92 +486,142 @@ int launch_tma(int mode, int series, const float* const* imgs, int n_groups, int
         const Outputs o = out.offset(cmp0 * (size_t)n);
         p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
         p.lisi_num = o.lisi_num; p.aug_num = o.aug_num;
-        p.ws = ws ? ws + cmp0 * (size_t)n * pl.pieces : nullptr;
+        p.ws = (ws && pl.pieces > 1) ? ws + cmp0 * (size_t)n * pl.pieces : nullptr;
         p.pieces_x = pl.pieces_x; p.pieces_y = pl.pieces_y;
         const long long n_items = items_per_group * ng;
         long long resident = (long long)geo->sms * geo->tma_ctas[pl.tma_cfg];
-        static const int max_ctas = env_int("IQA_TMA_MAX_CTAS", 0);     // tuning knob
+        const int max_ctas = knob(kKnobTmaMaxCtas);
         if (max_ctas > 0 && max_ctas < resident) resident = max_ctas;
-        const unsigned grid = (unsigned)(n_items < resident ? n_items : resident);
-        if (launch(fn, grid, kTmaThreads, tma_smem(pl.tma_cfg), st, p) != cudaSuccess) return IQA_ERR_CUDA;
+        L.fn = fn;
+        L.grid = (unsigned)(n_items < resident ? n_items : resident);
+        L.smem = tma_smem(pl.tma_cfg);
+    }
+    return true;
+}
+int fire(const std::vector<TmaLaunch>& q, cudaStream_t st) {
+    for (const TmaLaunch& L : q)
+        if (launch(L.fn, L.grid, kTmaThreads, L.smem, st, L.p) != cudaSuccess) return IQA_ERR_CUDA;
+    return IQA_OK;
+}
+
+// ---- any_kernel: encode, then launch ---------------------------------------------------------------------------
+struct AnyLaunch { AnyParams p; AnyFn fn; unsigned grid; size_t smem; };
+
+bool prepare_any(std::vector<AnyLaunch>& q, int mode, const void* const* xs, const void* const* ys, int n_pairs,
+                 const Geom& g, int N_T, const Consts& k, const Outputs& out, float4* ws, const Plan& pl) {
+    const Geometry* geo = geometry();
+    if (!geo) return false;
+    const AnyGeom& a = pl.any;
+    AnyFn fn = any_fn_at(any_fn_index(mode, g.ptype));
+    const size_t smem = any_smem_bytes(a.n_slots, a.slot_bytes);
+    if (smem > kAnyMaxSmem) return false;
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kTmaThreads, smem) != cudaSuccess || occ <= 0) return false;
+    if (occ > 2) occ = 2;
+    const int ntx = ceil_div(g.W, N_T), nty = ceil_div(g.H, N_T);
+    const long long n = (long long)ntx * nty;
+    const long long items_per_pair = (long long)a.units_x * a.units_y;
+    const int pairs_per_launch = kAnyMaxImages / 2;
+    if (items_per_pair * pairs_per_launch > 0x7fffffffLL) return false;
+    for (int first = 0; first < n_pairs; first += pairs_per_launch) {
+        const int np = n_pairs - first < pairs_per_launch ? n_pairs - first : pairs_per_launch;
+        q.emplace_back();
+        AnyLaunch& L = q.back();
+        AnyParams& p = L.p;
+        std::memset(&p, 0, sizeof(p));
+        for (int i = 0; i < np; ++i) {
+            if (!encode_image_map(&p.maps[2 * i], xs[first + i], g.ptype, g.H, g.W, g.pitch_x, a.box_w, a.box_rows) ||
+                !encode_image_map(&p.maps[2 * i + 1], ys[first + i], g.ptype, g.H, g.W, g.pitch_y, a.box_w, a.box_rows))
+                return false;
+        }
+        p.shift = (int)(((uintptr_t)xs[0] & 15u) / (unsigned)esize_of(g.ptype));
+        p.pad_mask = 16 / esize_of(g.ptype) - 1;
+        p.const_s = a.const_s;
+        p.n_pairs = np; p.W = g.W; p.H = g.H; p.N_T = N_T; p.ntx = ntx; p.nty = nty; p.n_tiles = (int)n;
+        p.kx = a.kx; p.ky = a.ky; p.px = a.px; p.py = a.py; p.pw = a.pw; p.ph = a.ph;
+        p.units_x = a.units_x; p.units_y = a.units_y; p.box_rows = a.box_rows; p.row_bytes = a.row_bytes;
+        p.slot_bytes = a.slot_bytes; p.n_slots = a.n_slots; p.rpw = a.rpw; p.wpt = a.wpt; p.fin_gsz = a.fin_gsz;
+        p.boxes_per_item = ceil_div(a.ph, a.box_rows);
+        p.nt_magic = (unsigned)(0x100000000ull / (unsigned)N_T) + 1u;
+        p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
+        const Outputs o = out.offset((size_t)first * (size_t)n);
+        p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
+        p.lisi_num = o.lisi_num; p.aug_num = o.aug_num;
+        p.ws = (ws && pl.pieces > 1) ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr;
+        const long long n_items = items_per_pair * np;
+        long long resident = (long long)geo->sms * occ;
+        const int max_ctas = knob(kKnobTmaMaxCtas);
+        if (max_ctas > 0 && max_ctas < resident) resident = max_ctas;
+        L.fn = fn;
+        L.grid = (unsigned)(n_items < resident ? n_items : resident);
+        L.smem = smem;
+    }
+    return true;
+}
+int fire(const std::vector<AnyLaunch>& q, cudaStream_t st) {
+    for (const AnyLaunch& L : q)
+        if (launch(L.fn, L.grid, kTmaThreads, L.smem, st, L.p) != cudaSuccess) return IQA_ERR_CUDA;
+    return IQA_OK;
+}
+
+// ---- generic kernels (pair by pair) ---------------------------------------------------------------------------
+template <int MODE, typename T>
+cudaError_t launch_generic_one(const GenericParams& g, long long n, int N_T, int pieces, cudaStream_t st) {
+    if ((long long)N_T * N_T <= kWarpTilePixels)          // small tiles: one warp per tile (pieces == 1 here)
+        return launch(generic_warp_kernel<MODE, T>, (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta), kCtaThreads, 0, st, g, n);
+    return launch(generic_kernel<MODE, T>, (unsigned)(n * pieces), kCtaThreads, 0, st, g);
+}
+int launch_generic(int mode, const void* const* xs, const void* const* ys, int n_pairs, const Geom& g2, int N_T,
+                   const Consts& k, const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st) {
+    const int nt = ceil_div(g2.W, N_T);
+    const long long n = (long long)nt * ceil_div(g2.H, N_T);
+    if (n * pl.pieces > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    for (int i = 0; i < n_pairs; ++i) {
+        GenericParams g{};
+        TileParams& p = g.tp;
+        p.x = (const float*)xs[i]; p.y = (const float*)ys[i]; p.N = g2.W; p.H = g2.H; p.nt = nt;
+        p.pitch_x = g2.pitch_x; p.pitch_y = g2.pitch_y;
+        p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
+        const Outputs o = out.offset((size_t)i * (size_t)n);
+        p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
+        p.lisi_num = o.lisi_num; p.aug_num = o.aug_num;
+        p.ws = (ws && pl.pieces > 1) ? ws + (size_t)i * (size_t)n * pl.pieces : nullptr;
+        g.N_T = N_T; g.pieces = pl.pieces;
+        cudaError_t e;
+        switch (g2.ptype) {
+            case IQA_PIXEL_F64: e = launch_generic_one<kModeFused, double>(g, n, N_T, pl.pieces, st); break;
+            case IQA_PIXEL_F16: e = launch_generic_one<kModeFused, __half>(g, n, N_T, pl.pieces, st); break;
+            case IQA_PIXEL_I16: e = launch_generic_one<kModeFused, short>(g, n, N_T, pl.pieces, st); break;
+            case IQA_PIXEL_I32: e = launch_generic_one<kModeFused, int>(g, n, N_T, pl.pieces, st); break;
+            case IQA_PIXEL_U8: e = launch_generic_one<kModeFused, unsigned char>(g, n, N_T, pl.pieces, st); break;
+            default:
+                e = mode == kModeLisi  ? launch_generic_one<kModeLisi, float>(g, n, N_T, pl.pieces, st)
+                    : mode == kModeAug ? launch_generic_one<kModeAug, float>(g, n, N_T, pl.pieces, st)
+                                       : launch_generic_one<kModeFused, float>(g, n, N_T, pl.pieces, st);
+        }
+        if (e != cudaSuccess) return IQA_ERR_CUDA;
     }
     return IQA_OK;
 }
 
-// S1-S4 for n_pairs pairs (xs[i], ys[i]) with the plan's kernel; `out` / `ws` point at pair 0.
-int launch_pairs(int mode, const float* const* xs, const float* const* ys, int n_pairs, int N, int N_T,
-                 const Consts& k, const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st,
-                 const Geom2D* g2 = nullptr) {
-    const int H = g2 ? g2->H : N, W = g2 ? g2->W : N;
-    const int nt = (W + N_T - 1) / N_T;                       // tiles per row
-    const long long n = (long long)nt * ((H + N_T - 1) / N_T);
+// S1-S4 for n_pairs pairs (xs[i], ys[i]) with the plan's kernel; `out` / `ws` point at pair 0.  The plan is
+// downgraded to the generic kernels (before anything is launched) when a tensor map cannot be encoded.
+int launch_pairs(int mode, const void* const* xs, const void* const* ys, int n_pairs, const Geom& g, int N_T,
+                 const Consts& k, const Outputs& out, float4* ws, Plan& pl, cudaStream_t st) {
     if (pl.kind == kPlanTma) {
-        const float* imgs[kMaxImages];
-        for (int first = 0; first < n_pairs; first += kMaxImages / 2) {
-            const int np = n_pairs - first < kMaxImages / 2 ? n_pairs - first : kMaxImages / 2;
-            for (int i = 0; i < np; ++i) { imgs[2 * i] = xs[first + i]; imgs[2 * i + 1] = ys[first + i]; }
-            const int rc = launch_tma(mode, kPairs, imgs, np, 2, N, N_T, k, out.offset((size_t)first * (size_t)n),
-                                      ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st, g2);
-            if (rc != IQA_OK) return rc;
-        }
-    } else if (pl.kind == kPlanStream) {
-        const Geometry* geo = geometry();
-        if (!geo) return IQA_ERR_CUDA;
-        const int units_x = (N + kUnitCols - 1) / kUnitCols;
-        const int units_y = (N + pl.item_rows - 1) / pl.item_rows;
-        const long long items_per_pair = (long long)units_x * units_y;
-        if (items_per_pair * kMaxBatch > 0x7fffffffLL) return IQA_ERR_SHAPE;
-        StreamFn fn = stream_fn(mode, pl.variant);
-        for (int first = 0; first < n_pairs; first += kMaxBatch) {
-            const int np = n_pairs - first < kMaxBatch ? n_pairs - first : kMaxBatch;
-            BatchParams p{};
-            for (int i = 0; i < np; ++i) { p.x[i] = xs[first + i]; p.y[i] = ys[first + i]; }
-            p.n_pairs = np; p.N = N; p.log2_nt = ilog2(N_T); p.nt = nt; p.n_tiles = (int)n;
-            p.units_x = units_x; p.units_y = units_y; p.item_rows = pl.item_rows;
-            p.n_items = (int)(items_per_pair * np);
-            p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
-            const Outputs o = out.offset((size_t)first * (size_t)n);
-            p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
-            p.lisi_num = o.lisi_num; p.aug_num = o.aug_num;
-            p.ws = ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr;
-            p.pieces_x = pl.pieces_x; p.pieces_y = pl.pieces_y;
-            const long long resident = (long long)geo->sms * geo->ctas[mode - 1][pl.variant];
-            const unsigned grid = (unsigned)(p.n_items < resident ? p.n_items : resident);
-            if (launch(fn, grid, kCtaThreads, stream_smem(pl.variant), st, p) != cudaSuccess) return IQA_ERR_CUDA;
-        }
-    } else {
-        const long long grid = n * pl.pieces;
-        if (grid > 0x7fffffffLL) return IQA_ERR_SHAPE;
-        for (int i = 0; i < n_pairs; ++i) {
-            GenericParams g{};
-            TileParams& p = g.tp;
-            p.x = xs[i]; p.y = ys[i]; p.N = W; p.H = H; p.nt = nt;
-            p.pitch_x = g2 ? g2->pitch_x : (long long)N; p.pitch_y = g2 ? g2->pitch_y : (long long)N;
-            p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
-            const Outputs o = out.offset((size_t)i * (size_t)n);
-            p.lisi = o.lisi; p.auglisi = o.auglisi; p.sum_x = o.sum_x; p.sum_y = o.sum_y;
-            p.lisi_num = o.lisi_num; p.aug_num = o.aug_num;
-            p.ws = ws ? ws + (size_t)i * (size_t)n * pl.pieces : nullptr;
-            g.N_T = N_T; g.pieces = pl.pieces;
-            cudaError_t e;
-            if ((long long)N_T * N_T <= kWarpTilePixels) {        // small tiles: one warp per tile (pieces == 1 here)
-                const unsigned wgrid = (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta);
-                switch (mode) {
-                    case kModeLisi: e = launch(generic_warp_kernel<kModeLisi>, wgrid, kCtaThreads, 0, st, g, n); break;
-                    case kModeAug: e = launch(generic_warp_kernel<kModeAug>, wgrid, kCtaThreads, 0, st, g, n); break;
-                    default: e = launch(generic_warp_kernel<kModeFused>, wgrid, kCtaThreads, 0, st, g, n); break;
-                }
-            } else {
-                switch (mode) {
-                    case kModeLisi: e = launch(generic_kernel<kModeLisi>, (unsigned)grid, kCtaThreads, 0, st, g); break;
-                    case kModeAug: e = launch(generic_kernel<kModeAug>, (unsigned)grid, kCtaThreads, 0, st, g); break;
-                    default: e = launch(generic_kernel<kModeFused>, (unsigned)grid, kCtaThreads, 0, st, g); break;
-                }
-            }
-            if (e != cudaSuccess) return IQA_ERR_CUDA;
-        }
+        std::vector<TmaLaunch> q;
+        q.reserve((size_t)ceil_div(n_pairs, kMaxImages / 2));
+        std::vector<const void*> imgs((size_t)2 * n_pairs);
+        for (int i = 0; i < n_pairs; ++i) { imgs[2 * (size_t)i] = xs[i]; imgs[2 * (size_t)i + 1] = ys[i]; }
+        if (prepare_tma(q, mode, kPairs, imgs.data(), n_pairs, 2, g, N_T, k, out, ws, pl)) return fire(q, st);
+        generic_plan(pl, N_T);
+    } else if (pl.kind == kPlanAny) {
+        std::vector<AnyLaunch> q;
+        q.reserve((size_t)ceil_div(n_pairs, kAnyMaxImages / 2));
+        if (prepare_any(q, mode, xs, ys, n_pairs, g, N_T, k, out, ws, pl)) return fire(q, st);
+        generic_plan(pl, N_T);
     }
-    return IQA_OK;
+    return launch_generic(mode, xs, ys, n_pairs, g, N_T, k, out, ws, pl, st);
 }
 
 // After S1-S4 of n_cmp comparisons: the second pass of split tiles, then Eqs. 3-4 per comparison.
@@ -454,142 +652,122 @@ int finish_comparisons(const Outputs& out, float* out2, int n_cmp, long long n, 
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }
 
-// Validation shared by the batch and the series entry points (everything but the image lists).
-// Shape of a general image (g2) or of the paper's square N x N image: status and tile count.
-int status_of_geometry(int N, int N_T, const Geom2D* g2, long long* n_tiles) {
-    if (!g2) {
-        if (const int s = status_of_shape(N, N_T)) return s;
-        *n_tiles = (long long)(N / N_T) * (N / N_T);
+// Shape of the images of a call: status and tile count.  `square`: the paper-named entry points keep the paper's
+// requirement N % N_T == 0.
+int status_of_geometry(const Geom& g, int N_T, bool square, long long* n_tiles) {
+    if (square) {
+        if (const int s = status_of_shape(g.W, N_T)) return s;
+        *n_tiles = (long long)(g.W / N_T) * (g.W / N_T);
         return IQA_OK;
     }
-    if (g2->H <= 0 || g2->W <= 0 || N_T <= 0 || g2->H > kMaxN || g2->W > kMaxN || g2->pitch_x < g2->W ||
-        g2->pitch_y < g2->W)
+    if (esize_of(g.ptype) == 0) return IQA_ERR_SHAPE;
+    if (g.H <= 0 || g.W <= 0 || N_T <= 0 || g.H > kMaxN || g.W > kMaxN || g.pitch_x < g.W || g.pitch_y < g.W)
         return IQA_ERR_SHAPE;
-    *n_tiles = (long long)((g2->W + N_T - 1) / N_T) * ((g2->H + N_T - 1) / N_T);
+    *n_tiles = (long long)ceil_div(g.W, N_T) * ceil_div(g.H, N_T);
     return *n_tiles > 0x7fffffffLL ? IQA_ERR_SHAPE : IQA_OK;
 }
 
-int validate_common(int mode, int n_cmp, int N, int N_T, float C1, float C2, float C, float D, const Outputs& out,
-                    const float* out2, const Geom2D* g2 = nullptr) {
+int validate_common(int mode, int n_cmp, const Geom& g, int N_T, bool square, float C1, float C2, float C, float D,
+                    const Outputs& out, const float* out2) {
     if (n_cmp <= 0) return IQA_ERR_SHAPE;
     if ((mode & kModeLisi) && !out.lisi) return IQA_ERR_NULL;
     if ((mode & kModeAug) && !out.auglisi) return IQA_ERR_NULL;
     if (mode == kModeFused && (!out.sum_x || !out.sum_y)) return IQA_ERR_NULL;
     long long n = 0;
-    if (const int s = status_of_geometry(N, N_T, g2, &n)) return s;
+    if (const int s = status_of_geometry(g, N_T, square, &n)) return s;
     if (n * n_cmp > 0x7fffffffLL) return IQA_ERR_SHAPE;
-    if ((mode & kModeLisi) && (!pos_finite(C1) || !pos_finite(C2) || !std::isfinite(D))) return IQA_ERR_PARAM;
+    if ((mode & kModeLisi) && (!pos_normal(C1) || !pos_finite(C2) || !std::isfinite(D))) return IQA_ERR_PARAM;
     if ((mode & kModeAug) && !pos_finite(C)) return IQA_ERR_PARAM;
     if (out2 && (!pos_finite(C2) || !pos_finite(C))) return IQA_ERR_PARAM;
     return IQA_OK;
 }
 
+size_t pieces_bytes(long long n_cmp, long long n, int N_T) {
+    const size_t mp = max_pieces(N_T);
+    return mp > 1 ? (size_t)n_cmp * (size_t)n * mp * sizeof(float4) : 0;
+}
+
 // Shared body of every *_tiles / *_batch entry point: validation, then the launches.
 // xs, ys: HOST arrays of n_pairs device pointers.  out2 (nullable): Eqs. 3-4 per pair.
-int run_batch(int mode, const float* const* xs, const float* const* ys, int n_pairs, int N, int N_T,
+int run_batch(int mode, const void* const* xs, const void* const* ys, int n_pairs, const Geom& g, int N_T, bool square,
               float C1, float C2, float C, float D, Outputs out, float* out2,
-              void* workspace, size_t workspace_bytes, void* stream, const Geom2D* g2 = nullptr) {
+              void* workspace, size_t workspace_bytes, void* stream) {
     if (!xs || !ys) return IQA_ERR_NULL;
     if (n_pairs <= 0) return IQA_ERR_SHAPE;
     for (int i = 0; i < n_pairs; ++i)
         if (!xs[i] || !ys[i]) return IQA_ERR_NULL;
-    if (const int s = validate_common(mode, n_pairs, N, N_T, C1, C2, C, D, out, out2, g2)) return s;
+    if (const int s = validate_common(mode, n_pairs, g, N_T, square, C1, C2, C, D, out, out2)) return s;
     long long n = 0;
-    status_of_geometry(N, N_T, g2, &n);
+    status_of_geometry(g, N_T, square, &n);
     uintptr_t bits = 0;
     for (int i = 0; i < n_pairs; ++i) bits |= (uintptr_t)xs[i] | (uintptr_t)ys[i];
-    if (bits & 3u) return IQA_ERR_ALIGN;
-    const size_t need = (size_t)n_pairs * (size_t)n * (max_pieces(N_T) > 1 ? max_pieces(N_T) : 0) * sizeof(float4);
+    if (bits & (uintptr_t)(esize_of(g.ptype) - 1)) return IQA_ERR_ALIGN;
+    const size_t need = pieces_bytes(n_pairs, n, N_T);
     if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
     if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
 
-    const bool aligned16 = ((bits & 15u) == 0) && (g2 ? (g2->pitch_x % 4 == 0 && g2->pitch_y % 4 == 0) : (N % 4 == 0));
-    const Plan pl = make_plan(g2 ? g2->W : N, N_T, aligned16, xs[0], false, g2);
+    Plan pl = make_plan(g, N_T, align_of(xs, n_pairs, ys, n_pairs), false);
     cudaStream_t st = (cudaStream_t)stream;
-    float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
+    float4* ws = need > 0 ? (float4*)workspace : nullptr;
     out = out.for_mode(mode);
     const Consts k{C1, C2, C, D};
-    if (const int rc = launch_pairs(mode, xs, ys, n_pairs, g2 ? g2->W : N, N_T, k, out, ws, pl, st, g2)) return rc;
+    if (const int rc = launch_pairs(mode, xs, ys, n_pairs, g, N_T, k, out, ws, pl, st)) return rc;
     return finish_comparisons(out, out2, n_pairs, n, k, ws, pl, st);
 }
 
 // Time series: imgs = HOST array of n_images device pointers; K = n_images - 1
-// comparisons, (I_0, I_k+1) or (I_k, I_k+1).  Aligned power-of-two shapes take the TMA kernel, which
+// comparisons, (I_0, I_k+1) or (I_k, I_k+1).  fp32 images with a power-of-two N_T take tma_kernel, which
 // keeps the x box of every comparison in shared memory (each image is read from HBM once);
 // everything else is computed pair by pair with the kernels of the pair entry points.
-int run_series(const float* const* imgs, int n_images, int series, int N, int N_T,
+int run_series(const void* const* imgs, int n_images, int series, const Geom& g, int N_T, bool square,
                float C1, float C2, float C, float D, Outputs out, float* out2,
-               void* workspace, size_t workspace_bytes, void* stream, const Geom2D* g2 = nullptr) {
+               void* workspace, size_t workspace_bytes, void* stream) {
     if (!imgs) return IQA_ERR_NULL;
     if (n_images < 2 || (series != kReference && series != kConsecutive)) return IQA_ERR_SHAPE;
     for (int i = 0; i < n_images; ++i)
         if (!imgs[i]) return IQA_ERR_NULL;
     const int K = n_images - 1;
-    if (const int s = validate_common(kModeFused, K, N, N_T, C1, C2, C, D, out, out2, g2)) return s;
+    if (const int s = validate_common(kModeFused, K, g, N_T, square, C1, C2, C, D, out, out2)) return s;
     long long n = 0;
-    status_of_geometry(N, N_T, g2, &n);
+    status_of_geometry(g, N_T, square, &n);
     uintptr_t bits = 0;
     for (int i = 0; i < n_images; ++i) bits |= (uintptr_t)imgs[i];
-    if (bits & 3u) return IQA_ERR_ALIGN;
-    const size_t need = (size_t)K * (size_t)n * (max_pieces(N_T) > 1 ? max_pieces(N_T) : 0) * sizeof(float4);
+    if (bits & (uintptr_t)(esize_of(g.ptype) - 1)) return IQA_ERR_ALIGN;
+    const size_t need = pieces_bytes(K, n, N_T);
     if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
     if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
 
-    const bool aligned16 = ((bits & 15u) == 0) && (g2 ? g2->pitch_x % 4 == 0 : N % 4 == 0);
-    if (g2) N = g2->W;
-    const Plan pl = make_plan(N, N_T, aligned16, imgs[0], true, g2);
+    Plan pl = make_plan(g, N_T, align_of(imgs, n_images, imgs, 0), true);
     cudaStream_t st = (cudaStream_t)stream;
-    float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
+    float4* ws = need > 0 ? (float4*)workspace : nullptr;
     const Consts k{C1, C2, C, D};
     if (pl.kind == kPlanTma) {
         // chunks of at most kMaxImages images; consecutive chunks share one image
-        const float* chunk[kMaxImages];
-        for (int first = 0; first < K; first += kMaxImages - 1) {       // first = first comparison of the chunk
+        std::vector<TmaLaunch> q;
+        q.reserve((size_t)ceil_div(K, kMaxImages - 1));
+        const void* chunk[kMaxImages];
+        bool ok = true;
+        for (int first = 0; first < K && ok; first += kMaxImages - 1) {       // first = first comparison of the chunk
             const int kc = K - first < kMaxImages - 1 ? K - first : kMaxImages - 1;
             chunk[0] = series == kReference ? imgs[0] : imgs[first];
             for (int i = 0; i < kc; ++i) chunk[1 + i] = imgs[first + 1 + i];
-            const int rc = launch_tma(kModeFused, series, chunk, 1, kc + 1, N, N_T, k, out.offset((size_t)first * (size_t)n),
-                                      ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st, g2);
-            if (rc != IQA_OK) return rc;
+            ok = prepare_tma(q, kModeFused, series, chunk, 1, kc + 1, g, N_T, k, out.offset((size_t)first * (size_t)n),
+                             ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl);
         }
-    } else {
-        const float* xs[kMaxBatch];
-        const float* ys[kMaxBatch];
-        for (int first = 0; first < K; first += kMaxBatch) {
-            const int kc = K - first < kMaxBatch ? K - first : kMaxBatch;
-            for (int i = 0; i < kc; ++i) {
-                xs[i] = series == kReference ? imgs[0] : imgs[first + i];
-                ys[i] = imgs[first + i + 1];
-            }
-            const int rc = launch_pairs(kModeFused, xs, ys, kc, N, N_T, k, out.offset((size_t)first * (size_t)n),
-                                        ws ? ws + (size_t)first * (size_t)n * pl.pieces : nullptr, pl, st, g2);
-            if (rc != IQA_OK) return rc;
+        if (ok) {
+            if (const int rc = fire(q, st)) return rc;
+            return finish_comparisons(out, out2, K, n, k, ws, pl, st);
         }
+        generic_plan(pl, N_T);
     }
+    // pair by pair; a plan downgraded by one chunk stays downgraded for the rest (one finalise pass fits all)
+    std::vector<const void*> xs((size_t)K), ys((size_t)K);
+    for (int i = 0; i < K; ++i) {
+        xs[i] = series == kReference ? imgs[0] : imgs[i];
+        ys[i] = imgs[i + 1];
+    }
+    if (const int rc = launch_pairs(kModeFused, xs.data(), ys.data(), K, g, N_T, k, out, ws, pl, st)) return rc;
     return finish_comparisons(out, out2, K, n, k, ws, pl, st);
-}
-
-// Generic kernels on pixels of type T (iqa_fused_tiles_2d_typed).
-template <typename T>
-int launch_typed(const void* x, const void* y, const Geom2D& g2, int N_T, const Consts& k, const Outputs& out, float4* ws,
-                 const Plan& pl, cudaStream_t st) {
-    const int nt = (g2.W + N_T - 1) / N_T;
-    const long long n = (long long)nt * ((g2.H + N_T - 1) / N_T);
-    GenericParams g{};
-    TileParams& p = g.tp;
-    p.x = (const float*)x; p.y = (const float*)y; p.N = g2.W; p.H = g2.H; p.nt = nt;
-    p.pitch_x = g2.pitch_x; p.pitch_y = g2.pitch_y;
-    p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;
-    p.lisi = out.lisi; p.auglisi = out.auglisi; p.sum_x = out.sum_x; p.sum_y = out.sum_y;
-    p.lisi_num = out.lisi_num; p.aug_num = out.aug_num;
-    p.ws = ws;
-    g.N_T = N_T; g.pieces = pl.pieces;
-    cudaError_t e;
-    if ((long long)N_T * N_T <= kWarpTilePixels)
-        e = launch(generic_warp_kernel<kModeFused, T>, (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta), kCtaThreads, 0, st, g, n);
-    else
-        e = launch(generic_kernel<kModeFused, T>, (unsigned)(n * pl.pieces), kCtaThreads, 0, st, g);
-    return e == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -602,16 +780,23 @@ const char* iqa_status_string(int status) {
     switch (status) {
         case IQA_OK: return "ok";
         case IQA_ERR_NULL: return "required pointer is NULL";
-        case IQA_ERR_SHAPE: return "bad shape: need 0 < N_T <= N <= 2^20, N % N_T == 0, n_pairs >= 1, tile count < 2^31";
-        case IQA_ERR_PARAM: return "bad constant: C1, C2, C must be finite and > 0, D finite";
-        case IQA_ERR_ALIGN: return "pointer alignment: images 4-byte, workspace 16-byte";
+        case IQA_ERR_SHAPE: return "bad shape: need 0 < N_T <= N <= 2^20, N % N_T == 0, n_pairs >= 1, tile count < 2^31, a known pixel type";
+        case IQA_ERR_PARAM: return "bad constant: C1 must be a normal float > 0, C2 and C finite and > 0, D finite";
+        case IQA_ERR_ALIGN: return "pointer alignment: images to their element size, workspace 16-byte";
         case IQA_ERR_WORKSPACE: return "workspace missing or smaller than iqa_workspace_bytes / iqa_batch_workspace_bytes";
         case IQA_ERR_CUDA: return "CUDA launch or copy failed";
         default: return "unknown status";
     }
 }
 
-const char* iqa_version(void) { return "0.4.0"; }
+const char* iqa_version(void) { return "0.5.0"; }
+
+int iqa_debug_knob(const char* name, int value) {
+    if (!name) return -1;
+    for (int i = 0; i < kNumKnobs; ++i)
+        if (std::strcmp(name, kKnobNames[i]) == 0) return knobs().v[i].exchange(value, std::memory_order_relaxed);
+    return -1;
+}
 
 size_t iqa_workspace_bytes(int N, int N_T) {
     if (status_of_shape(N, N_T) != IQA_OK) return 0;
@@ -627,13 +812,19 @@ int iqa_lisi_tiles(const float* x, const float* y, int N, int N_T,
                    float C1, float C2, float D, float* lisi,
                    void* workspace, size_t workspace_bytes, void* stream) {
     const Outputs o{lisi, nullptr, nullptr, nullptr, nullptr, nullptr};
-    return run_batch(kModeLisi, &x, &y, 1, N, N_T, C1, C2, 1.0f, D, o, nullptr, workspace, workspace_bytes, stream);
+    const void* xs[1] = {x};
+    const void* ys[1] = {y};
+    return run_batch(kModeLisi, xs, ys, 1, square_geom(N), N_T, true, C1, C2, 1.0f, D, o, nullptr, workspace,
+                     workspace_bytes, stream);
 }
 
 int iqa_auglisi_tiles(const float* x, const float* y, int N, int N_T, float C,
                       float* auglisi, void* workspace, size_t workspace_bytes, void* stream) {
     const Outputs o{nullptr, auglisi, nullptr, nullptr, nullptr, nullptr};
-    return run_batch(kModeAug, &x, &y, 1, N, N_T, 1.0f, 1.0f, C, 0.0f, o, nullptr, workspace, workspace_bytes, stream);
+    const void* xs[1] = {x};
+    const void* ys[1] = {y};
+    return run_batch(kModeAug, xs, ys, 1, square_geom(N), N_T, true, 1.0f, 1.0f, C, 0.0f, o, nullptr, workspace,
+                     workspace_bytes, stream);
 }
 
 int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
@@ -642,51 +833,28 @@ int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
                     float* lisi_num, float* auglisi_num,
                     void* workspace, size_t workspace_bytes, void* stream) {
     const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
-    return run_batch(kModeFused, &x, &y, 1, N, N_T, C1, C2, C, D, o, nullptr, workspace, workspace_bytes, stream);
+    const void* xs[1] = {x};
+    const void* ys[1] = {y};
+    return run_batch(kModeFused, xs, ys, 1, square_geom(N), N_T, true, C1, C2, C, D, o, nullptr, workspace,
+                     workspace_bytes, stream);
 }
 
-int iqa_query_plan(const float* x, int H, int W, long long pitch, int N_T, int series) {
-    if (!x || H <= 0 || W <= 0 || N_T <= 0 || pitch < W) return -1;
-    const Geom2D g2{H, W, pitch, pitch};
-    const bool aligned16 = (((uintptr_t)x & 15u) == 0) && (pitch % 4 == 0);
-    const bool square = H == W && pitch == W && W % N_T == 0;      // what the paper-named entry points see
-    const Plan pl = make_plan(W, N_T, aligned16, x, series != 0, square ? nullptr : &g2);
-    return pl.kind == kPlanTma ? IQA_PLAN_TMA + pl.tma_cfg : pl.kind == kPlanStream ? IQA_PLAN_CP_ASYNC : IQA_PLAN_GENERIC;
+int iqa_query_plan(const void* x, int pixel_type, int H, int W, long long pitch, int N_T, int series) {
+    const int es = esize_of(pixel_type);
+    if (!x || es == 0 || H <= 0 || W <= 0 || N_T <= 0 || pitch < W || ((uintptr_t)x & (uintptr_t)(es - 1))) return -1;
+    const Geom g{H, W, pitch, pitch, pixel_type};
+    const Plan pl = make_plan(g, N_T, align_of(&x, 1, &x, 0), series != 0);
+    if (pl.kind == kPlanTma) return IQA_PLAN_TMA + pl.tma_cfg;
+    // the time-series entry points run any_kernel pair by pair (8 bytes per pixel and comparison)
+    return pl.kind == kPlanAny ? IQA_PLAN_TMA_ANY : IQA_PLAN_GENERIC;
 }
 
 size_t iqa_workspace_bytes_2d(int H, int W, int N_T) {
     if (H <= 0 || W <= 0 || N_T <= 0 || H > kMaxN || W > kMaxN) return 0;
     const size_t pieces = max_pieces(N_T);
     if (pieces <= 1) return 0;
-    const size_t n = (size_t)((H + N_T - 1) / N_T) * (size_t)((W + N_T - 1) / N_T);
+    const size_t n = (size_t)ceil_div(H, N_T) * (size_t)ceil_div(W, N_T);
     return n * pieces * sizeof(float4);
-}
-
-int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long pitch_x, long long pitch_y, int N_T,
-                       float C1, float C2, float C, float D,
-                       float* lisi, float* auglisi, float* sum_x, float* sum_y,
-                       float* lisi_num, float* auglisi_num,
-                       void* workspace, size_t workspace_bytes, void* stream) {
-    if (!x || !y || !lisi || !auglisi || !sum_x || !sum_y) return IQA_ERR_NULL;
-    if (H <= 0 || W <= 0 || N_T <= 0 || H > kMaxN || W > kMaxN || pitch_x < W || pitch_y < W) return IQA_ERR_SHAPE;
-    const long long ntx = (W + N_T - 1) / N_T, nty = (H + N_T - 1) / N_T;
-    if (ntx * nty > 0x7fffffffLL) return IQA_ERR_SHAPE;
-    if (!pos_finite(C1) || !pos_finite(C2) || !pos_finite(C) || !std::isfinite(D)) return IQA_ERR_PARAM;
-    const uintptr_t bits = (uintptr_t)x | (uintptr_t)y;
-    if (bits & 3u) return IQA_ERR_ALIGN;
-    const size_t need = iqa_workspace_bytes_2d(H, W, N_T);
-    if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
-    if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
-
-    const Geom2D g2{H, W, pitch_x, pitch_y};
-    const bool aligned16 = ((bits & 15u) == 0) && (pitch_x % 4 == 0) && (pitch_y % 4 == 0);
-    const Plan pl = make_plan(W, N_T, aligned16, x, false, &g2);
-    cudaStream_t st = (cudaStream_t)stream;
-    float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
-    const Outputs out{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
-    const Consts k{C1, C2, C, D};
-    if (const int rc = launch_pairs(kModeFused, &x, &y, 1, W, N_T, k, out, ws, pl, st, &g2)) return rc;
-    return finish_comparisons(out, nullptr, 1, ntx * nty, k, ws, pl, st);
 }
 
 int iqa_fused_tiles_2d_typed(const void* x, const void* y, int pixel_type,
@@ -695,47 +863,31 @@ int iqa_fused_tiles_2d_typed(const void* x, const void* y, int pixel_type,
                              float* lisi, float* auglisi, float* sum_x, float* sum_y,
                              float* lisi_num, float* auglisi_num,
                              void* workspace, size_t workspace_bytes, void* stream) {
-    if (pixel_type == IQA_PIXEL_F32)
-        return iqa_fused_tiles_2d((const float*)x, (const float*)y, H, W, pitch_x, pitch_y, N_T, C1, C2, C, D, lisi, auglisi,
-                                  sum_x, sum_y, lisi_num, auglisi_num, workspace, workspace_bytes, stream);
-    if (!x || !y || !lisi || !auglisi || !sum_x || !sum_y) return IQA_ERR_NULL;
-    size_t esize = 0;
-    switch (pixel_type) {
-        case IQA_PIXEL_F64: esize = 8; break;
-        case IQA_PIXEL_F16: case IQA_PIXEL_I16: esize = 2; break;
-        case IQA_PIXEL_I32: esize = 4; break;
-        case IQA_PIXEL_U8: esize = 1; break;
-        default: return IQA_ERR_SHAPE;
-    }
-    if (H <= 0 || W <= 0 || N_T <= 0 || H > kMaxN || W > kMaxN || pitch_x < W || pitch_y < W) return IQA_ERR_SHAPE;
-    const long long n = (long long)((W + N_T - 1) / N_T) * ((H + N_T - 1) / N_T);
-    if (n * (long long)((N_T + kGenericRows - 1) / kGenericRows) > 0x7fffffffLL) return IQA_ERR_SHAPE;
-    if (!pos_finite(C1) || !pos_finite(C2) || !pos_finite(C) || !std::isfinite(D)) return IQA_ERR_PARAM;
-    if ((((uintptr_t)x | (uintptr_t)y) & (esize - 1)) != 0) return IQA_ERR_ALIGN;
-    const size_t need = iqa_workspace_bytes_2d(H, W, N_T);
-    if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
-    if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
+    const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
+    const Geom g{H, W, pitch_x, pitch_y, pixel_type};
+    const void* xs[1] = {x};
+    const void* ys[1] = {y};
+    return run_batch(kModeFused, xs, ys, 1, g, N_T, false, C1, C2, C, D, o, nullptr, workspace, workspace_bytes, stream);
+}
 
-    const Geom2D g2{H, W, pitch_x, pitch_y};
-    Plan pl{};
-    pl.kind = kPlanGeneric;
-    pl.pieces_x = 1;
-    pl.pieces_y = (N_T + kGenericRows - 1) / kGenericRows;
-    pl.pieces = pl.pieces_y;
-    cudaStream_t st = (cudaStream_t)stream;
-    float4* ws = pl.pieces > 1 ? (float4*)workspace : nullptr;
-    const Outputs out{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
-    const Consts k{C1, C2, C, D};
-    int rc;
-    switch (pixel_type) {
-        case IQA_PIXEL_F64: rc = launch_typed<double>(x, y, g2, N_T, k, out, ws, pl, st); break;
-        case IQA_PIXEL_F16: rc = launch_typed<__half>(x, y, g2, N_T, k, out, ws, pl, st); break;
-        case IQA_PIXEL_I16: rc = launch_typed<short>(x, y, g2, N_T, k, out, ws, pl, st); break;
-        case IQA_PIXEL_I32: rc = launch_typed<int>(x, y, g2, N_T, k, out, ws, pl, st); break;
-        default: rc = launch_typed<unsigned char>(x, y, g2, N_T, k, out, ws, pl, st); break;
-    }
-    if (rc != IQA_OK) return rc;
-    return finish_comparisons(out, nullptr, 1, n, k, ws, pl, st);
+int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long pitch_x, long long pitch_y, int N_T,
+                       float C1, float C2, float C, float D,
+                       float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                       float* lisi_num, float* auglisi_num,
+                       void* workspace, size_t workspace_bytes, void* stream) {
+    return iqa_fused_tiles_2d_typed(x, y, IQA_PIXEL_F32, H, W, pitch_x, pitch_y, N_T, C1, C2, C, D, lisi, auglisi, sum_x,
+                                    sum_y, lisi_num, auglisi_num, workspace, workspace_bytes, stream);
+}
+
+int iqa_fused_batch_2d_typed(const void* const* x_ptrs_host, const void* const* y_ptrs_host, int n_pairs, int pixel_type,
+                             int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
+                             float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                             float* lisi_num, float* auglisi_num, float* out2,
+                             void* workspace, size_t workspace_bytes, void* stream) {
+    const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
+    const Geom g{H, W, pitch, pitch, pixel_type};
+    return run_batch(kModeFused, x_ptrs_host, y_ptrs_host, n_pairs, g, N_T, false, C1, C2, C, D, o, out2,
+                     workspace, workspace_bytes, stream);
 }
 
 int iqa_fused_batch_2d(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,
@@ -743,10 +895,21 @@ int iqa_fused_batch_2d(const float* const* x_ptrs_host, const float* const* y_pt
                        float* lisi, float* auglisi, float* sum_x, float* sum_y,
                        float* lisi_num, float* auglisi_num, float* out2,
                        void* workspace, size_t workspace_bytes, void* stream) {
+    return iqa_fused_batch_2d_typed((const void* const*)x_ptrs_host, (const void* const*)y_ptrs_host, n_pairs, IQA_PIXEL_F32,
+                                    H, W, pitch, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num,
+                                    out2, workspace, workspace_bytes, stream);
+}
+
+int iqa_series_tiles_2d_typed(const void* const* img_ptrs_host, int n_images, int mode, int pixel_type,
+                              int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
+                              float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                              float* lisi_num, float* auglisi_num, float* out2,
+                              void* workspace, size_t workspace_bytes, void* stream) {
     const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
-    const Geom2D g2{H, W, pitch, pitch};
-    return run_batch(kModeFused, x_ptrs_host, y_ptrs_host, n_pairs, W, N_T, C1, C2, C, D, o, out2,
-                     workspace, workspace_bytes, stream, &g2);
+    const int series = mode == IQA_SERIES_REFERENCE ? kReference : mode == IQA_SERIES_CONSECUTIVE ? kConsecutive : -1;
+    const Geom g{H, W, pitch, pitch, pixel_type};
+    return run_series(img_ptrs_host, n_images, series, g, N_T, false, C1, C2, C, D, o, out2,
+                      workspace, workspace_bytes, stream);
 }
 
 int iqa_series_tiles_2d(const float* const* img_ptrs_host, int n_images, int mode,
@@ -754,11 +917,9 @@ int iqa_series_tiles_2d(const float* const* img_ptrs_host, int n_images, int mod
                         float* lisi, float* auglisi, float* sum_x, float* sum_y,
                         float* lisi_num, float* auglisi_num, float* out2,
                         void* workspace, size_t workspace_bytes, void* stream) {
-    const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
-    const int series = mode == IQA_SERIES_REFERENCE ? kReference : mode == IQA_SERIES_CONSECUTIVE ? kConsecutive : -1;
-    const Geom2D g2{H, W, pitch, pitch};
-    return run_series(img_ptrs_host, n_images, series, W, N_T, C1, C2, C, D, o, out2,
-                      workspace, workspace_bytes, stream, &g2);
+    return iqa_series_tiles_2d_typed((const void* const*)img_ptrs_host, n_images, mode, IQA_PIXEL_F32, H, W, pitch, N_T,
+                                     C1, C2, C, D, lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num, out2,
+                                     workspace, workspace_bytes, stream);
 }
 
 int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,
@@ -767,8 +928,8 @@ int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_
                     float* lisi_num, float* auglisi_num, float* out2,
                     void* workspace, size_t workspace_bytes, void* stream) {
     const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
-    return run_batch(kModeFused, x_ptrs_host, y_ptrs_host, n_pairs, N, N_T, C1, C2, C, D, o, out2,
-                     workspace, workspace_bytes, stream);
+    return run_batch(kModeFused, (const void* const*)x_ptrs_host, (const void* const*)y_ptrs_host, n_pairs, square_geom(N),
+                     N_T, true, C1, C2, C, D, o, out2, workspace, workspace_bytes, stream);
 }
 
 size_t iqa_series_workspace_bytes(int n_images, int N, int N_T) {
@@ -783,7 +944,7 @@ int iqa_series_tiles(const float* const* img_ptrs_host, int n_images, int mode,
                      void* workspace, size_t workspace_bytes, void* stream) {
     const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
     const int series = mode == IQA_SERIES_REFERENCE ? kReference : mode == IQA_SERIES_CONSECUTIVE ? kConsecutive : -1;
-    return run_series(img_ptrs_host, n_images, series, N, N_T, C1, C2, C, D, o, out2,
+    return run_series((const void* const*)img_ptrs_host, n_images, series, square_geom(N), N_T, true, C1, C2, C, D, o, out2,
                       workspace, workspace_bytes, stream);
 }
 
@@ -830,7 +991,7 @@ int iqa_tiles_below(const float* values, int n_tiles, int n_maps, float threshol
     if (!values || !counts || (capacity > 0 && !indices)) return IQA_ERR_NULL;
     if (n_tiles <= 0 || n_maps <= 0 || capacity < 0) return IQA_ERR_SHAPE;
     if (threshold != threshold) return IQA_ERR_PARAM;
-    const int cs = env_int("IQA_CAND_NO_CLUSTER", 0) ? 0 : cand_cluster_size(n_tiles);
+    const int cs = knob(kKnobCandNoCluster) ? 0 : cand_cluster_size(n_tiles);
     const cudaError_t e = cs > 0
         ? launch_cluster(below_cluster_kernel, (unsigned)n_maps * (unsigned)cs, (unsigned)kCandThreads, 0,
                          (cudaStream_t)stream, (unsigned)cs, values, n_tiles, threshold, indices, capacity, counts)
@@ -844,7 +1005,7 @@ int iqa_tiles_bottom_k(const float* values, int n_tiles, int n_maps, int k,
                        int* indices, float* vals, void* stream) {
     if (!values || !indices) return IQA_ERR_NULL;
     if (n_tiles <= 0 || n_maps <= 0 || k <= 0 || k > kMaxBottomK) return IQA_ERR_SHAPE;
-    const int cs = env_int("IQA_CAND_NO_CLUSTER", 0) ? 0 : cand_cluster_size(n_tiles);
+    const int cs = knob(kKnobCandNoCluster) ? 0 : cand_cluster_size(n_tiles);
     const cudaError_t e = cs > 0
         ? launch_cluster(bottom_k_cluster_kernel, (unsigned)n_maps * (unsigned)cs, (unsigned)kCandThreads, 0,
                          (cudaStream_t)stream, (unsigned)cs, values, n_tiles, k, indices, vals)
@@ -897,7 +1058,7 @@ int fused_host_impl(const float* x_host, const float* y_host, int N, int N_T,
                     void* dev_scratch, size_t dev_scratch_bytes, void* stream, bool synchronise) {
     if (!x_host || !y_host || !dev_scratch) return IQA_ERR_NULL;
     if (const int s = status_of_shape(N, N_T)) return s;
-    if (!pos_finite(C1) || !pos_finite(C2) || !pos_finite(C) || !std::isfinite(D)) return IQA_ERR_PARAM;
+    if (!pos_normal(C1) || !pos_finite(C2) || !pos_finite(C) || !std::isfinite(D)) return IQA_ERR_PARAM;
     if (dev_scratch_bytes < iqa_host_scratch_bytes(N, N_T)) return IQA_ERR_WORKSPACE;
     if ((uintptr_t)dev_scratch & 255u) return IQA_ERR_ALIGN;
 

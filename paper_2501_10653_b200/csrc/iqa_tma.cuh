@@ -7,9 +7,9 @@
 // warp issues cp.async.bulk.tensor.2d (SASS UTMALDG) for BOXES of 128 columns x 8 RPW rows
 // (RPW = 4: 32 rows, 16 KiB) straight into shared memory; completion is signalled on an mbarrier per box
 // ("full"), the eight consumer warps give a box back through a second mbarrier ("empty").
-// Against the per-thread cp.async ring of iqa_stream.cuh this removes every address
-// computation and 8 LDGSTS per thread and stage from the instruction stream (the cp.async
-// kernel spends ~19.5 instructions per pixel pair, ~10.5 of them arithmetic), which is what
+// Against a per-thread cp.async ring (the first version of this kernel, profiles/r01d_variants.md)
+// this removes every address computation and 8 LDGSTS per thread and stage from the instruction
+// stream (that kernel spent ~19.5 instructions per pixel pair, ~10.5 of them arithmetic), which is what
 // the time-series modes need: they halve the HBM bytes per comparison, so the instruction
 // issue rate, not HBM, would otherwise bound them.  Rows / columns outside the image are
 // zero-filled by the TMA unit, and zeros add exact zeros to all four sums.
@@ -50,7 +50,6 @@
 #include <stdint.h>
 
 #include "iqa_kernels.cuh"
-#include "iqa_stream.cuh"     // ItemCursor, decode_item
 
 namespace iqa {
 

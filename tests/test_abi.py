@@ -40,12 +40,14 @@ def test_workspace_bytes():
     # tiles of side <= 64 are always finished inside one CTA: no second pass, no workspace
     for N, N_T in [(256, 16), (2048, 8), (2048, 64), (8192, 64), (10, 5), (192, 48)]:
         assert B.iqa_workspace_bytes(N, N_T) == 0
-    # split tiles: 16 B per piece of 128 x 64 pixels -> (N_T/128) x (N_T/64) pieces per tile
-    assert B.iqa_workspace_bytes(2048, 128) == 256 * 1 * 2 * 16
-    assert B.iqa_workspace_bytes(2048, 512) == 16 * 4 * 8 * 16
-    assert B.iqa_workspace_bytes(16384, 128) == 16384 * 2 * 16
-    assert B.iqa_workspace_bytes(16384, 16384) == 128 * 256 * 16
-    assert B.iqa_batch_workspace_bytes(16, 16384, 128) == 16 * 16384 * 2 * 16
+    # split tiles: 16 B per piece; the worst case over the kernels a call may take: tma_kernel cuts pieces of 128 x 64
+    # pixels, any_kernel (unaligned bases, other pixel types) pieces of at most 112 x 64
+    assert B.iqa_workspace_bytes(2048, 128) == 256 * 2 * 2 * 16
+    assert B.iqa_workspace_bytes(2048, 512) == 16 * 5 * 8 * 16
+    assert B.iqa_workspace_bytes(16384, 128) == 16384 * 4 * 16
+    assert B.iqa_workspace_bytes(16384, 16384) == 147 * 256 * 16
+    assert B.iqa_batch_workspace_bytes(16, 16384, 128) == 16 * 16384 * 4 * 16
+    assert B.iqa_workspace_bytes(900, 300) == 9 * 3 * 5 * 16      # any_kernel: 3 x 5 pieces of 112 x 64
     assert B.iqa_batch_workspace_bytes(5, 2048, 64) == 0
     assert B.iqa_batch_workspace_bytes(0, 2048, 128) == 0
     assert B.iqa_workspace_bytes(200, 100) == 4 * 2 * 16          # generic: ceil(100/64) pieces
@@ -78,6 +80,8 @@ def test_fused_argument_validation():
     assert _fused(N=16, N_T=32) == B.IQA_ERR_SHAPE
     assert _fused(N=(1 << 20) + 16, N_T=16) == B.IQA_ERR_SHAPE
     assert _fused(N=1 << 20, N_T=1) == B.IQA_ERR_SHAPE       # 2^40 tiles do not fit an int index
+    assert _fused(C1=1e-40) == B.IQA_ERR_PARAM               # subnormal C1: |x - y| + C1 would be flushed to zero
+    assert _fused(C2=1e-40, C=1e-40, N=256, N_T=128) == B.IQA_ERR_WORKSPACE   # subnormal C2 / C are fine
     for bad in (0.0, -1e-6, math.inf, math.nan):
         assert _fused(C1=bad) == B.IQA_ERR_PARAM
         assert _fused(C2=bad) == B.IQA_ERR_PARAM
@@ -187,7 +191,7 @@ def test_2d_validation():
     assert B.iqa_fused_tiles_2d(FAKE, FAKE, 64, 64, 64, 64, 8, 1e-6, -1.0, 1e-6, 5e-7, *o) == B.IQA_ERR_PARAM
     assert B.iqa_fused_tiles_2d(FAKE + 2, FAKE, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_ALIGN
     assert B.iqa_fused_tiles_2d(FAKE, FAKE, 100, 300, 300, 300, 128, *a, *o) == B.IQA_ERR_WORKSPACE
-    assert B.iqa_workspace_bytes_2d(100, 300, 128) == 1 * 3 * 2 * 16
+    assert B.iqa_workspace_bytes_2d(100, 300, 128) == 1 * 3 * 4 * 16
     assert B.iqa_workspace_bytes_2d(100, 300, 64) == 0 and B.iqa_workspace_bytes_2d(0, 300, 128) == 0
     tbl = (ctypes.c_void_p * 3)(FAKE, FAKE, FAKE)
     bad = (ctypes.c_void_p * 3)(FAKE, 0, FAKE)
@@ -204,12 +208,45 @@ def test_2d_validation():
     assert B.iqa_fused_tiles_2d_typed(FAKE + 4, FAKE, B.IQA_PIXEL_F64, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_ALIGN
     assert B.iqa_fused_tiles_2d_typed(FAKE, FAKE, B.IQA_PIXEL_F16, 64, 64, 60, 64, 8, *a, *o) == B.IQA_ERR_SHAPE
     assert B.iqa_fused_tiles_2d_typed(FAKE, FAKE, B.IQA_PIXEL_F32, 64, 0, 64, 64, 8, *a, *o) == B.IQA_ERR_SHAPE
-    assert B.iqa_query_plan(None, 64, 64, 64, 8) == -1 and B.iqa_query_plan(FAKE, 64, 64, 60, 8) == -1
-    assert B.iqa_query_plan(FAKE, 64, 64, 64, 7) == B.IQA_PLAN_GENERIC           # tile side not a power of two
-    assert B.iqa_query_plan(FAKE + 4, 64, 64, 64, 8) == B.IQA_PLAN_GENERIC       # base not 16-byte aligned
-    assert B.iqa_query_plan(FAKE, 64, 64, 64, 8) in (B.IQA_PLAN_CP_ASYNC, B.IQA_PLAN_TMA + 1)   # no driver here: cp.async
+    F32, F64, U8 = B.IQA_PIXEL_F32, B.IQA_PIXEL_F64, B.IQA_PIXEL_U8
+    assert B.iqa_query_plan(None, F32, 64, 64, 64, 8) == -1 and B.iqa_query_plan(FAKE, F32, 64, 64, 60, 8) == -1
+    assert B.iqa_query_plan(FAKE, 17, 64, 64, 64, 8) == -1 and B.iqa_query_plan(FAKE + 4, F64, 64, 64, 64, 8) == -1
+    assert B.iqa_query_plan(FAKE, F32, 64, 64, 64, 7) == B.IQA_PLAN_TMA_ANY       # tile side not a power of two
+    assert B.iqa_query_plan(FAKE, F32, 64, 64, 64, 3) == B.IQA_PLAN_GENERIC       # N_T < 4
+    assert B.iqa_query_plan(FAKE + 4, F32, 64, 64, 64, 8) == B.IQA_PLAN_TMA_ANY   # 4-byte aligned base: any_kernel
+    assert B.iqa_query_plan(FAKE, F32, 64, 64, 64, 8) == B.IQA_PLAN_TMA + 1 and B.iqa_query_plan(FAKE, F32, 64, 64, 64, 8, 1) == B.IQA_PLAN_TMA
+    assert B.iqa_query_plan(FAKE, F32, 64, 63, 63, 8) == B.IQA_PLAN_GENERIC       # pitch not a multiple of 16 bytes
+    assert B.iqa_query_plan(FAKE, U8, 64, 60, 64, 8) == B.IQA_PLAN_TMA_ANY and B.iqa_query_plan(FAKE, U8, 64, 60, 60, 8) == B.IQA_PLAN_GENERIC
+    assert B.iqa_query_plan(FAKE, F64, 64, 64, 66, 100) == B.IQA_PLAN_TMA_ANY
     # the square entry points keep the paper's divisibility requirement
     assert B.iqa_fused_tiles(FAKE, FAKE, 100, 64, *a, *o) == B.IQA_ERR_SHAPE
+
+
+def test_typed_batch_series_validation_and_knobs():
+    a = (1e-6, 1e-6, 1e-6, 5e-7)
+    o = (FAKE, FAKE, FAKE, FAKE)
+    tbl = (ctypes.c_void_p * 3)(FAKE, FAKE, FAKE)
+    odd = (ctypes.c_void_p * 3)(FAKE, FAKE + 4, FAKE)
+    I16, F64 = B.IQA_PIXEL_I16, B.IQA_PIXEL_F64
+    assert B.iqa_fused_batch_2d_typed(tbl, None, 3, I16, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_NULL
+    assert B.iqa_fused_batch_2d_typed(tbl, tbl, 3, 11, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_fused_batch_2d_typed(tbl, tbl, 0, I16, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_fused_batch_2d_typed(tbl, odd, 3, F64, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_ALIGN
+    assert B.iqa_fused_batch_2d_typed(tbl, odd, 3, I16, 100, 300, 300, 128, *a, *o) == B.IQA_ERR_WORKSPACE
+    assert B.iqa_series_tiles_2d_typed(tbl, 3, 7, I16, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_series_tiles_2d_typed(odd, 3, 0, F64, 64, 80, 80, 8, *a, *o) == B.IQA_ERR_ALIGN
+    assert B.iqa_series_tiles_2d_typed(tbl, 3, 0, F64, 64, 80, 80, 8, 0.0, 1e-6, 1e-6, 5e-7, *o) == B.IQA_ERR_PARAM
+    # knobs: unknown names are refused, known ones return the previous value and change the plan
+    assert B.iqa_debug_knob("IQA_NO_SUCH_KNOB", 1) == -1
+    assert B.iqa_query_plan(FAKE, B.IQA_PIXEL_F32, 64, 64, 64, 8) == B.IQA_PLAN_TMA + 1
+    with B.knob("IQA_FORCE_ANY", 1):
+        assert B.iqa_query_plan(FAKE, B.IQA_PIXEL_F32, 64, 64, 64, 8) == B.IQA_PLAN_TMA_ANY
+        with B.knob("IQA_FORCE_GENERIC", 1):
+            assert B.iqa_query_plan(FAKE, B.IQA_PIXEL_F32, 64, 64, 64, 8) == B.IQA_PLAN_GENERIC
+    with B.knob("IQA_TMA_CONFIG", 3):
+        assert B.iqa_query_plan(FAKE, B.IQA_PIXEL_F32, 64, 64, 64, 8) == B.IQA_PLAN_TMA + 3
+    assert B.iqa_query_plan(FAKE, B.IQA_PIXEL_F32, 64, 64, 64, 8) == B.IQA_PLAN_TMA + 1
+    assert not B.STALE                                       # the library under test was built from the sources in the tree
 
 
 def test_convenience_wrappers_refuse_cpu_tensors():

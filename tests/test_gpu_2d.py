@@ -115,7 +115,7 @@ def test_2d_error_codes(B):
     assert B.iqa_fused_tiles_2d(x, None, 64, 64, 64, 64, 8, *a, *o) == B.IQA_ERR_NULL
     assert B.iqa_fused_tiles_2d(x, x, 64, 64, 64, 64, 8, 0.0, K["C2"], K["C"], K["D"], *o) == B.IQA_ERR_PARAM
     assert B.iqa_fused_tiles_2d(x, x, 64, 64, 64, 64, 128, *a, *o) == B.IQA_ERR_WORKSPACE
-    assert B.iqa_workspace_bytes_2d(65, 130, 128) == 2 * 2 * 16 and B.iqa_workspace_bytes_2d(65, 130, 64) == 0
+    assert B.iqa_workspace_bytes_2d(65, 130, 128) == 2 * 4 * 16 and B.iqa_workspace_bytes_2d(65, 130, 64) == 0
     torch.cuda.synchronize()
 
 
@@ -233,3 +233,177 @@ def test_typed_error_codes(B):
     assert B.iqa_fused_tiles_2d_typed(x.data_ptr() + 4, x, B.IQA_PIXEL_F64, 32, 32, 64, 64, 8, *a, *o) == B.IQA_ERR_ALIGN
     assert B.iqa_fused_tiles_2d_typed(x, x, B.IQA_PIXEL_F64, 64, 64, 64, 64, 128, *a, *o) == B.IQA_ERR_WORKSPACE
     torch.cuda.synchronize()
+
+
+# ---------------------------------------------------------------------------------------------- any_kernel (iqa_any.cuh)
+def _typed_pair(rng, H, W, dtype):
+    dt = np.dtype(dtype)
+    if dt.kind in "iu":
+        lo, hi = (0, 255) if dt == np.uint8 else (-300, 3000) if dt == np.int16 else (-1000, 1 << 20)
+        x = rng.integers(lo, hi, (H, W)).astype(dt)
+        y = rng.integers(lo, hi, (H, W)).astype(dt)
+        k = dict(C1=1e-3, C2=1e-3, C=1e-3, D=5e-4)
+    else:
+        x = rng.normal(0.05, 0.2, (H, W)).astype(dt)
+        y = rng.normal(0.05, 0.2, (H, W)).astype(dt)
+        k = K
+    m = rng.random((H, W)) < 0.3
+    y[m] = x[m]
+    return x, y, k
+
+
+def _typed_window(a, pitch, off):
+    """Device copy of `a` (any pixel type) as a window of a wider buffer; the halo holds NaN (floats) or a large
+    value (integers), so a stray read shows up in the sums."""
+    import torch
+    H, W = a.shape
+    t = torch.from_numpy(a)
+    fill = float("nan") if a.dtype.kind == "f" else (200 if a.dtype == np.uint8 else 30000)
+    buf = torch.full((H * pitch + off + 64,), fill, dtype=t.dtype, device="cuda")
+    view = torch.as_strided(buf, (H, W), (pitch, 1), off)
+    view.copy_(t)
+    return view
+
+
+def _check_typed(B, U, x, y, xd, yd, N_T, k, what, plan="tma_any"):
+    import torch
+    import oracle
+    if plan is not None:
+        assert B.plan_name(xd, N_T) == plan, (what, B.plan_name(xd, N_T))
+    got = B.fused_tiles_2d(xd, yd, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    torch.cuda.synchronize()
+    g = {n: v.cpu().numpy().astype(np.float64) for n, v in got.items()}
+    ref = oracle.tiles_2d_any(x, y, N_T, **k)
+    U.assert_parity(g, ref, k["C"], what)
+    return got, ref
+
+
+ANY_SHAPES = [
+    # H, W, N_T, pitch (elements), off (elements)       -- geometry of any_geometry() in the comment
+    (480, 960, 48, 960, 0),        # kx = 2, one box per item
+    (500, 700, 100, 704, 0),       # kx = 1, two boxes of 50 rows
+    (500, 700, 100, 704, 3),       # base aligned to 4 bytes only: shifted tensor map
+    (333, 777, 50, 780, 1),        # N_T % 4 != 0: lanes straddle two tiles
+    (200, 300, 7, 304, 0),         # kx = 18, ky = 4: several tile rows per box, straddling lanes
+    (64, 64, 4, 64, 0),            # smallest tile side: kx = 32, ky = 8
+    (130, 130, 5, 132, 2),
+    (257, 513, 12, 516, 0),        # kx = 10, ky = 2
+    (300, 300, 20, 300, 0), (300, 300, 36, 300, 0), (200, 650, 65, 652, 0), (400, 400, 97, 400, 0),
+    (260, 390, 127, 392, 0),       # three boxes, a ragged last one that overlaps its predecessor
+    (300, 400, 129, 400, 0),       # split tiles: px = 2, py = 3 with ragged last pieces
+    (450, 310, 150, 312, 0), (700, 900, 300, 900, 1), (1100, 1300, 1000, 1300, 0),
+    (33, 1500, 24, 1500, 0), (1000, 40, 33, 40, 0), (1, 4, 6, 4, 0), (3, 1000, 100, 1000, 0),
+]
+
+
+@pytest.mark.parametrize("H,W,N_T,pitch,off", ANY_SHAPES)
+def test_any_kernel_fp32_shapes(B, U, H, W, N_T, pitch, off):
+    """fp32, tile sides that are not powers of two, bases aligned to 4 bytes only: any_kernel against oracle.tiles_2d."""
+    rng = np.random.default_rng(H * 7 + W + N_T)
+    x, y, k = _typed_pair(rng, H, W, "float32")
+    xd, yd = _typed_window(x, pitch, off), _typed_window(y, pitch + 4, off)        # same offset inside the 16-byte line
+    got, ref = _check_typed(B, U, x, y, xd, yd, N_T, k, f"any fp32 {H}x{W} N_T={N_T} off={off}")
+    agg = B.aggregate(got["lisi"], got["auglisi"], got["X"], got["Y"], k["C2"], k["C"]).cpu().numpy()
+    import oracle
+    exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], k["C2"], k["C"])
+    assert abs(agg[0] - exp[0]) <= 1e-5 * abs(exp[0]) and abs(agg[1] - exp[1]) <= 1e-5 * abs(exp[1]) + 1e-6
+
+
+@pytest.mark.parametrize("dtype", ["float64", "float16", "int16", "int32", "uint8"])
+@pytest.mark.parametrize("H,W,N_T", [(300, 500, 64), (257, 300, 48), (300, 333, 100), (200, 210, 50), (150, 200, 7),
+                                     (400, 600, 256), (500, 300, 150), (64, 64, 8), (90, 1000, 16)])
+def test_any_kernel_pixel_types(B, U, dtype, H, W, N_T):
+    """Every pixel type through the TMA-fed any_kernel (row pitch a multiple of 16 bytes, base aligned to the element
+    only) against oracle.tiles_2d_any."""
+    rng = np.random.default_rng(H + 3 * W + N_T)
+    x, y, k = _typed_pair(rng, H, W, dtype)
+    per16 = 16 // x.dtype.itemsize
+    pitch = -(-(W + 5) // per16) * per16
+    for off in (0, 1, per16 - 1) if per16 > 2 else (0, 1):
+        xd, yd = _typed_window(x, pitch, off), _typed_window(y, pitch + per16, off)
+        _check_typed(B, U, x, y, xd, yd, N_T, k, f"any {dtype} {H}x{W} N_T={N_T} off={off}")
+
+
+def test_any_kernel_matches_tma_kernel_on_power_of_two_tiles(B, U):
+    """IQA_FORCE_ANY sends a power-of-two shape through any_kernel: the same per-pixel arithmetic in another
+    summation order, so the two kernels agree to a few ulps (and both with the oracle)."""
+    import torch
+    rng = np.random.default_rng(11)
+    x, y, k = _typed_pair(rng, 1024, 1536, "float32")
+    xd, yd = U.to_dev(x), U.to_dev(y)
+    for N_T in (8, 16, 64, 128, 512):
+        a = B.fused_tiles_2d(xd, yd, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+        with B.knob("IQA_FORCE_ANY", 1):
+            assert B.plan_name(xd, N_T) == "tma_any"
+            b, _ = _check_typed(B, U, x, y, xd, yd, N_T, k, f"forced any N_T={N_T}")
+        for n in a:
+            assert torch.all((a[n] - b[n]).abs() <= 2e-6 * a[n].abs() + 1e-30), (N_T, n)
+
+
+@pytest.mark.parametrize("dtype,N_T", [("float32", 100), ("int16", 64), ("float64", 48), ("uint8", 150)])
+def test_typed_batch_and_series(B, U, dtype, N_T):
+    """iqa_fused_batch_2d_typed (40 pairs: two launches of any_kernel) and iqa_series_tiles_2d_typed (pair by pair)."""
+    import torch
+    import oracle
+    rng = np.random.default_rng(N_T)
+    H, W = 210, 330
+    per16 = 16 // np.dtype(dtype).itemsize
+    pitch = -(-W // per16) * per16
+    imgs, k = [], None
+    for _ in range(6):
+        a, _, k = _typed_pair(rng, H, W, dtype)
+        imgs.append(a)
+    dev = [_typed_window(a, pitch, 0) for a in imgs]
+    order = [(i % 6, (i * 5 + 1) % 6) for i in range(40)]
+    out = B.fused_batch_2d([dev[i] for i, _ in order], [dev[j] for _, j in order], N_T, k["C1"], k["C2"], k["C"], k["D"],
+                           numerators=True)
+    torch.cuda.synchronize()
+    refs = {}
+    for p, (i, j) in enumerate(order):
+        if (i, j) not in refs:
+            refs[(i, j)] = oracle.tiles_2d_any(imgs[i], imgs[j], N_T, **k)
+        ref = refs[(i, j)]
+        got = {n: out[n][p].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+        U.assert_parity(got, ref, k["C"], f"typed batch {dtype} pair {p}")
+        exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], k["C2"], k["C"])
+        w = out["whole"][p].cpu().numpy()
+        assert abs(w[0] - exp[0]) <= 1e-5 * abs(exp[0]) and abs(w[1] - exp[1]) <= 1e-5 * abs(exp[1]) + 1e-6
+    for mode in ("reference", "consecutive"):
+        so = B.series_tiles_2d(dev[:4], mode, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+        torch.cuda.synchronize()
+        for c, (ix, iy) in enumerate(oracle.comparison_indices(4, mode)):
+            ref = oracle.tiles_2d_any(imgs[ix], imgs[iy], N_T, **k)
+            got = {n: so[n][c].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+            U.assert_parity(got, ref, k["C"], f"typed series {dtype} {mode} {c}")
+
+
+def test_paper_named_entry_points_with_odd_tile_sides(B, U):
+    """iqa_lisi_tiles / iqa_auglisi_tiles / iqa_fused_tiles with N_T = 48 and 100 (N % N_T == 0): the three modes of
+    any_kernel; the standalone results equal the fused ones bit for bit."""
+    import torch
+    rng = np.random.default_rng(5)
+    for N, N_T in ((960, 48), (1200, 100), (1000, 250)):
+        x, y, k = _typed_pair(rng, N, N, "float32")
+        xd, yd = U.to_dev(x), U.to_dev(y)
+        assert B.plan_name(xd, N_T) == "tma_any"
+        f, _, _ = U.check_pair(x, y, N_T, k, f"square any N_T={N_T}", xd=xd, yd=yd)
+        fo = B.fused_tiles(xd, yd, N_T, **k)
+        li = B.lisi_tiles(xd, yd, N_T, k["C1"], k["C2"], k["D"])
+        au = B.auglisi_tiles(xd, yd, N_T, k["C"])
+        assert torch.equal(li, fo["lisi"]) and torch.equal(au, fo["auglisi"])
+
+
+def test_unaligned_bases(B, U):
+    """Windows that start 1..3 elements into a 16-byte line.  Same offset for x and y (two windows cut at the same
+    column): any_kernel loads from the 16-byte boundary below and shifts the column -> tile assignment.  Different
+    offsets: no common column grid for the boxes, the generic kernel.  Both against the oracle, for a power-of-two
+    and an odd tile side."""
+    rng = np.random.default_rng(8)
+    x, y, k = _typed_pair(rng, 512, 768, "float32")
+    for N_T in (64, 100, 256):
+        for off in (1, 2, 3):
+            xd, yd = _typed_window(x, 768, off), _typed_window(y, 772, off)
+            assert xd.data_ptr() % 16 == 4 * off
+            _check_typed(B, U, x, y, xd, yd, N_T, k, f"shift {off} N_T={N_T}", plan="tma_any")
+            yd2 = _typed_window(y, 772, (off + 1) % 4)
+            _check_typed(B, U, x, y, xd, yd2, N_T, k, f"offsets {off}/{(off + 1) % 4} N_T={N_T}", plan=None)

@@ -1,5 +1,5 @@
 """-m gpu parity at BASELINE.json's FULL sizes in the launch configurations bench.py times:
-iqa_fused_batch over 32 cfg1 pairs / 8 cfg3 pairs / a cfg4 batch, and iqa_series_tiles over 9 snapshots
+iqa_fused_batch over 32 cfg1 pairs / 8 cfg3 pairs / the 16 cfg4 pairs, and iqa_series_tiles over 9 snapshots
 of the N = 8192 sky.  Every pair (cfg1) or a sample of pairs / comparisons (larger configs) is checked
 element by element against the oracle on the same device-drawn buffers copied to the host."""
 import numpy as np
@@ -20,7 +20,9 @@ def U():
     return gpu_util
 
 
-def _check_batch(B, U, cfg, pairs, sample):
+def _check_batch(B, U, cfg, pairs, sample, whole_of=None):
+    """`sample`: pairs checked element by element (all six per-tile arrays + the whole-image pair);
+    `whole_of`: pairs whose whole-image pair (Eqs. 3-4) is checked against the oracle's."""
     import torch
     import oracle
     from paper_2501_10653_b200 import synth
@@ -30,17 +32,20 @@ def _check_batch(B, U, cfg, pairs, sample):
         xd, yd, _ = synth.make_pair(cfg, seed=s, device="cuda")
         xs.append(xd)
         ys.append(yd)
+    assert B.plan_name(xs[0], cfg.N_T) == "tma:c1"
     out = B.fused_batch(xs, ys, cfg.N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True, aggregate=True)
     torch.cuda.synchronize()
     whole = out["whole"].cpu().numpy().astype(np.float64)
-    for i in sample:
+    for i in sorted(set(sample) | set(whole_of or ())):
         x, y = xs[i].cpu().numpy(), ys[i].cpu().numpy()
         ref = oracle.tiles(x, y, cfg.N_T, **k)
-        got = {n: out[n][i].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
-        U.assert_parity(got, ref, k["C"], f"{cfg.name} pair {i} of {pairs}")
+        if i in sample:
+            got = {n: out[n][i].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+            U.assert_parity(got, ref, k["C"], f"{cfg.name} pair {i} of {pairs}")
         exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], k["C2"], k["C"])
         assert abs(whole[i, 0] - exp[0]) <= 1e-5 * abs(exp[0]), (i, whole[i], exp)
         assert abs(whole[i, 1] - exp[1]) <= 1e-5 * abs(exp[1]), (i, whole[i], exp)
+        del x, y, ref
     del xs, ys, out
     torch.cuda.empty_cache()
 
@@ -55,11 +60,13 @@ def test_cfg3_batch_of_8_sampled_pairs(B, U):
     _check_batch(B, U, synth.CONFIGS[3], 8, (0, 3, 7))
 
 
-def test_cfg4_batch_sampled_pairs(B, U):
-    """Config [4]'s throughput loop runs 16 pairs per launch; the test keeps 3 (6 GiB) -- the grid is
-    persistent, so the launch shape is the same -- and checks the first and the last."""
+def test_cfg4_throughput_loop_of_16_pairs(B, U):
+    """Config [4] as BASELINE.json states it and bench.py times it: ONE iqa_fused_batch call over 16 pairs of
+    N = 16384, N_T = 128 (32 GiB of images resident, a [16 pairs][16384 tiles][2 pieces] workspace, 32 tensor maps in
+    one launch).  Pairs 0 and 15 are checked element by element, the whole-image pair of EVERY pair against the oracle
+    (SURVEY.md 8(d))."""
     from paper_2501_10653_b200 import synth
-    _check_batch(B, U, synth.CONFIGS[4], 3, (0, 2))
+    _check_batch(B, U, synth.CONFIGS[4], 16, (0, 15), whole_of=range(16))
 
 
 @pytest.mark.parametrize("mode", ["reference", "consecutive"])

@@ -62,7 +62,7 @@ def test_bottom_k_random_with_ties(B, nt, n_maps, k):
 
 
 @pytest.mark.parametrize("nt,n_maps,k", [(150, 2, 40), (181, 1, 1024), (300, 2, 7), (362, 1, 500), (363, 1, 100), (256, 3, 64)])
-def test_bottom_k_large_matrices(B, nt, n_maps, k, monkeypatch):
+def test_bottom_k_large_matrices(B, nt, n_maps, k):
     """More than 16384 tiles: a thread-block cluster of 2..8 CTAs per matrix (n <= 131072), the single-CTA loop above
     that (nt = 363) and when IQA_CAND_NO_CLUSTER is set -- all three must give the oracle's list, ties included."""
     rng = np.random.default_rng(nt + k)
@@ -72,9 +72,9 @@ def test_bottom_k_large_matrices(B, nt, n_maps, k, monkeypatch):
     _check_bottom_k(B, maps, k)
     for thr, cap in ((0.9925, None), (0.6, 10), (2.0, 1000)):
         _check_below(B, maps, thr, cap)
-    monkeypatch.setenv("IQA_CAND_NO_CLUSTER", "1")
-    _check_bottom_k(B, maps, k)
-    _check_below(B, maps, 0.9925)
+    with B.knob("IQA_CAND_NO_CLUSTER", 1):
+        _check_bottom_k(B, maps, k)
+        _check_below(B, maps, 0.9925)
 
 
 def test_bottom_k_all_equal_and_sorted_inputs(B):

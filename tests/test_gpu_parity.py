@@ -220,9 +220,9 @@ def test_symmetry_bitwise(U):
     assert np.array_equal(a["X"], b["Y"]) and np.array_equal(a["Y"], b["X"])
 
 
-def test_determinism_and_mapping_independence(U, monkeypatch):
-    """P12: two runs bit-identical; every mapping (TMA ring / box configurations, cp.async variants 0-2, generic
-    kernel) agrees with the oracle and with the default mapping to 2e-6."""
+def test_determinism_and_mapping_independence(U, B):
+    """P12: two runs bit-identical; every mapping (tma_kernel ring / box configurations, any_kernel, generic
+    kernel, a capped grid, no PDL) agrees with the oracle and with the default mapping to 2e-6."""
     cfg = synth.CONFIGS[0]
     x, y, _ = synth.make_pair(synth.scaled(synth.CONFIGS[3], 1024))
     xd, yd = U.to_dev(x), U.to_dev(y)
@@ -233,12 +233,11 @@ def test_determinism_and_mapping_independence(U, monkeypatch):
         for nm in base:
             assert np.array_equal(base[nm], again[nm]), (N_T, nm)
         ref = U.run_oracle(x, y, N_T, k)
-        for env, val in (("IQA_FORCE_VARIANT", "0"), ("IQA_FORCE_VARIANT", "1"), ("IQA_FORCE_VARIANT", "2"),
-                         ("IQA_FORCE_GENERIC", "1"), ("IQA_TMA_CONFIG", "0"), ("IQA_TMA_CONFIG", "2"),
-                         ("IQA_TMA_CONFIG", "3"), ("IQA_TMA_CONFIG", "4")):
-            monkeypatch.setenv(env, val)
-            other = U.run_gpu(xd, yd, N_T, k)
-            monkeypatch.delenv(env)
+        for env, val in (("IQA_FORCE_ANY", 1), ("IQA_TMA_MAX_CTAS", 37), ("IQA_NO_PDL", 1),
+                         ("IQA_FORCE_GENERIC", 1), ("IQA_TMA_CONFIG", 0), ("IQA_TMA_CONFIG", 2),
+                         ("IQA_TMA_CONFIG", 3), ("IQA_TMA_CONFIG", 4)):
+            with B.knob(env, val):
+                other = U.run_gpu(xd, yd, N_T, k)
             U.assert_parity(other, ref, k["C"], f"{env}={val} N_T={N_T}")
             for nm in base:
                 assert np.max(U.rel_err(other[nm], base[nm])) <= 2e-6, (env, val, N_T, nm)
@@ -367,7 +366,7 @@ def test_host_pipeline_two_streams(U, B):
 
 
 def test_every_baseline_configuration_takes_the_tma_kernel(B):
-    """A silent fall-back to the cp.async or generic kernel would keep parity and lose bandwidth: assert the plan."""
+    """A silent fall-back to the generic kernel would keep parity and lose bandwidth: assert the plan."""
     for idx in range(5):
         cfg = synth.CONFIGS[idx]
         x = torch.empty((cfg.N, cfg.N), dtype=torch.float32, device="cuda")
@@ -377,8 +376,13 @@ def test_every_baseline_configuration_takes_the_tma_kernel(B):
         del x
     x = torch.empty((300, 516), dtype=torch.float32, device="cuda")
     assert B.plan_name(x[:, :513], 64).startswith("tma")            # pitched window, W % 4 != 0
-    assert B.plan_name(x[:, 1:514], 64) == "generic"                # base not 16-byte aligned
-    assert B.plan_name(x, 100) == "generic"                         # tile side not a power of two
+    assert B.plan_name(x[:, 1:514], 64) == "tma_any"                # base 4-byte aligned only: any_kernel shifts columns
+    assert B.plan_name(x, 100) == "tma_any"                         # tile side not a power of two
+    assert B.plan_name(x[:, :515], 2) == "generic"                  # N_T < 4
+    y = torch.empty((300, 517), dtype=torch.float32, device="cuda")
+    assert B.plan_name(y, 64) == "generic"                          # row pitch not a multiple of 16 bytes
+    assert B.plan_name(y.to(torch.float64)[:, :500], 64) == "generic" and B.plan_name(x.to(torch.uint8), 64) == "generic"
+    assert B.plan_name(torch.empty((64, 528), dtype=torch.uint8, device="cuda"), 50) == "tma_any"
 
 
 def test_many_small_tiles(U):

@@ -133,13 +133,13 @@ def test_series_unaligned_images_take_the_pairwise_path(B, U, mode):
 
 @pytest.mark.parametrize("cfg_id", ["0", "1", "2", "3"])
 @pytest.mark.parametrize("N_T", [16, 64, 256])
-def test_series_ring_configurations(B, U, monkeypatch, cfg_id, N_T):
+def test_series_ring_configurations(B, U, cfg_id, N_T):
     """Every TMA ring / box configuration (IQA_TMA_CONFIG: 6 or 4 boxes of 32 rows, 8 or 6 boxes of 16 rows)
     gives the oracle's values in both series modes."""
-    monkeypatch.setenv("IQA_TMA_CONFIG", cfg_id)
     imgs = _rand_series(512, 4, seed=int(cfg_id) + N_T)
-    for mode in MODES:
-        _run_and_check(B, U, imgs, mode, N_T, _consts(), f"tma config {cfg_id} N_T={N_T}")
+    with B.knob("IQA_TMA_CONFIG", int(cfg_id)):
+        for mode in MODES:
+            _run_and_check(B, U, imgs, mode, N_T, _consts(), f"tma config {cfg_id} N_T={N_T}")
 
 
 @pytest.mark.parametrize("mode", MODES)
