@@ -47,7 +47,7 @@
 namespace iqa {
 
 constexpr int kAnyMaxImages = 64;      // tensor maps per launch: 32 pairs
-constexpr int kAnyPartBufs = 2;
+constexpr int kAnyPartBufs = 4;
 constexpr int kAnyMaxSlots = 8;
 
 struct AnyParams {
@@ -334,28 +334,43 @@ any_kernel(const __grid_constant__ AnyParams p) {
         const int gsz = p.fin_gsz;                    // lanes per tile
         const int groups = 32 / gsz;
         const int m = lane & (gsz - 1);
+        const int nw = p.ky > 1 ? p.wpt : kWarpsPerCta;        // warps that share a tile: a power of two
+        const int log2_nw = 31 - __clz(nw);
+        const uint64_t pol = policy_evict_last();
+        const int t_lane = lane / gsz;                // this lane's tile of the first round (the only one when gsz > 1)
+        const int jy_lane = t_lane / p.kx, jx_lane = t_lane - jy_lane * p.kx;
         for (ItemCursor c = decode_item((int)blockIdx.x, units_x, units_y); c.pair < p.n_pairs;
              c.advance(stride, units_x, units_y)) {
             const AnyItem it = any_item(p, c.ux, c.uy);
             mbar_wait(pfull_u32 + 8u * buf, phase);
             for (int t0 = 0; t0 < n_it; t0 += groups) {
-                const int t = t0 + lane / gsz;
+                const int t = t0 + t_lane;
                 const bool active = t < n_it;
-                const int jy = active ? t / p.kx : 0;
-                const int jx = active ? t - jy * p.kx : 0;
+                int jy = jy_lane, jx = jx_lane;
+                if (t0 > 0) { jy = t / p.kx; jx = t - jy * p.kx; }
+                if (!active) jy = jx = 0;
                 // lanes whose FIRST valid column lies in tile column jx (the columns a lane holds of the next tile
                 // were moved one lane up by the consumers); the item's column c is box column c + s
                 const int la = (split || jx == 0) ? it.s >> 2 : (jx * p.N_T + it.s + 3) >> 2;
                 const int lb = split ? (it.cv + it.s + 3) >> 2 : ((jx + 1) * p.N_T + it.s + 3) >> 2;
                 const int w0 = p.ky > 1 ? jy * p.wpt : 0;
-                const int nw = p.ky > 1 ? p.wpt : kWarpsPerCta;
-                const int nl = lb - la;
-                const int ne = active ? nw * nl : 0;
                 float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
-                for (int e = m; e < ne; e += gsz) {
-                    const int ew = e / nl;
-                    const float4 u = part[buf][w0 + ew][la + (e - ew * nl)];
-                    s.x += u.x; s.y += u.y; s.z += u.z; s.w += u.w;
+                if (active) {
+                    // the tile's entries are part[buf][w0 .. w0 + nw)[la .. lb): the gsz lanes of the tile's group
+                    // split them without a division (nw and gsz are powers of two), each in a fixed order
+                    if (gsz >= nw) {                 // gsz / nw lanes per warp row
+                        const float4* row = part[buf][w0 + (m & (nw - 1))];
+                        for (int l = la + (m >> log2_nw); l < lb; l += gsz >> log2_nw) {
+                            const float4 u = row[l];
+                            s.x += u.x; s.y += u.y; s.z += u.z; s.w += u.w;
+                        }
+                    } else {                         // several warp rows per lane
+                        for (int ew = m; ew < nw; ew += gsz)
+                            for (int l = la; l < lb; ++l) {
+                                const float4 u = part[buf][w0 + ew][l];
+                                s.x += u.x; s.y += u.y; s.z += u.z; s.w += u.w;
+                            }
+                    }
                 }
                 for (int o = gsz >> 1; o > 0; o >>= 1) {
                     s.x += __shfl_xor_sync(0xffffffffu, s.x, o);
@@ -366,7 +381,7 @@ any_kernel(const __grid_constant__ AnyParams p) {
                 const int tx = it.tx0 + jx, ty = it.ty0 + jy;
                 if (active && m == 0 && (split || (tx < p.ntx && ty < p.nty))) {
                     const size_t tile = (size_t)c.pair * p.n_tiles + (size_t)ty * p.ntx + tx;
-                    if (!split) finalise_tile(p, tile, s);
+                    if (!split) finalise_tile(p, tile, s, pol);
                     else p.ws[(tile * p.py + it.iy) * p.px + it.ix] = s;
                 }
             }

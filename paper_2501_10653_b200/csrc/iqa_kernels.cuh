@@ -126,24 +126,31 @@ __device__ __forceinline__ void pixel_terms_any(const T* __restrict__ x, const T
 // Per-tile results are stored with an L2 evict-last policy: they are a few MiB, they are read again right away
 // (finalise / aggregate / merge / candidate kernels), and keeping them in L2 keeps their write-back out of the
 // DRAM read stream of the images.
-__device__ __forceinline__ void store_result(float* dst, float v) {
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void store_result(float* dst, float v, uint64_t pol) {
 #if defined(IQA_PLAIN_STORES)
     *dst = v;
 #else
-    uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
     asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(dst), "f"(v), "l"(pol) : "memory");
 #endif
 }
 
 template <class Params>
-__device__ __forceinline__ void finalise_tile(const Params& p, size_t t, float4 v /*L,A,X,Y*/) {
-    if (p.lisi) store_result(p.lisi + t, p.D * v.x / (fmaxf(v.z, v.w) + p.C2));        // Eq. 1
-    if (p.auglisi) store_result(p.auglisi + t, 1.0f - v.y / (v.z + v.w + p.C));          // Eq. 2
-    if (p.sum_x) store_result(p.sum_x + t, v.z);
-    if (p.sum_y) store_result(p.sum_y + t, v.w);
-    if (p.lisi_num) store_result(p.lisi_num + t, v.x);
-    if (p.aug_num) store_result(p.aug_num + t, v.y);
+__device__ __forceinline__ void finalise_tile(const Params& p, size_t t, float4 v /*L,A,X,Y*/, uint64_t pol) {
+    if (p.lisi) store_result(p.lisi + t, p.D * v.x / (fmaxf(v.z, v.w) + p.C2), pol);        // Eq. 1
+    if (p.auglisi) store_result(p.auglisi + t, 1.0f - v.y / (v.z + v.w + p.C), pol);          // Eq. 2
+    if (p.sum_x) store_result(p.sum_x + t, v.z, pol);
+    if (p.sum_y) store_result(p.sum_y + t, v.w, pol);
+    if (p.lisi_num) store_result(p.lisi_num + t, v.x, pol);
+    if (p.aug_num) store_result(p.aug_num + t, v.y, pol);
+}
+template <class Params>
+__device__ __forceinline__ void finalise_tile(const Params& p, size_t t, float4 v) {
+    finalise_tile(p, t, v, policy_evict_last());
 }
 
 // -----------------------------------------------------------------------------
