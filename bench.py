@@ -209,6 +209,20 @@ class Batch:
         if rc:
             raise B.IqaError(rc, "iqa_fused_batch")
 
+    def step_one_call(self, i=0):
+        """The whole path for ONE pair in one call: iqa_fused_batch with n_pairs = 1 (S1-S4, the second pass of split
+        tiles, Eqs. 3-4)."""
+        B, cfg = self.B, self.cfg
+        st = self.torch.cuda.current_stream().cuda_stream
+        C1, C2, C, D = self.k
+        if not hasattr(self, "tables1"):
+            self.tables1 = [(B._ptr_table([x])[0], B._ptr_table([y])[0]) for x, y in zip(self.x, self.y)]
+        xt, yt = self.tables1[i]
+        rc = B.iqa_fused_batch(xt, yt, 1, cfg.N, cfg.N_T, C1, C2, C, D, self.lisi[i], self.aug[i], self.sx[i], self.sy[i],
+                               None, None, self.out2[i], self.ws1, self.wsb1, st)
+        if rc:
+            raise B.IqaError(rc, "iqa_fused_batch")
+
     def step_single(self, i=0, aggregate=True):
         """The per-pair entry points on pair i: iqa_fused_tiles then iqa_aggregate (2-3 launches)."""
         B, cfg = self.B, self.cfg
@@ -379,12 +393,14 @@ def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, us
     # to back: the same pair (warm: L2-resident when it fits -- what the paper's 10-run median measures,
     # P:31) and rotating over the batch's distinct pairs (cold: every call reads HBM)
     L = 16
-    single_warm = lambda: [batch.step_single(0, True) for _ in range(L)]
-    single_cold = lambda: [batch.step_single(i % pairs, True) for i in range(L)]
+    single_warm = lambda: [batch.step_one_call(0) for _ in range(L)]
+    single_cold = lambda: [batch.step_one_call(i % pairs) for i in range(L)]
+    two_calls = lambda: [batch.step_single(i % pairs, True) for i in range(L)]
     if use_graph:
         full, kern = batch.graph(full).replay, batch.graph(kern).replay
         if latency:
             single_warm, single_cold = batch.graph(single_warm).replay, batch.graph(single_cold).replay
+            two_calls = batch.graph(two_calls).replay
     for _ in range(warmup):
         full()
     with ClockSampler(torch.cuda.current_device()) as clk:
@@ -399,14 +415,16 @@ def measure_workload(torch, binding, cfg, pairs, steps, warmup, device, dist, us
         direct()
     ms_direct = time_region(torch, direct, max(3, min(steps, 20)), dist) / max(3, min(steps, 20)) * steps
     reps = max(3, min(steps, 20))
-    lat = [] if latency else [None, None]
-    for fn in ((single_warm, single_cold) if latency else ()):
+    lat = [] if latency else [None, None, None]
+    for fn in ((single_warm, single_cold, two_calls) if latency else ()):
         for _ in range(max(3, warmup)):
             fn()
         lat.append(time_region(torch, fn, reps, dist) / (reps * L))
-    ms_single, ms_single_cold = lat
-    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "ms_direct": ms_direct, "step_us": dist_us, "us_single_pair_warm": None if ms_single is None else ms_single * 1e3,
-            "us_single_pair_cold": None if ms_single_cold is None else ms_single_cold * 1e3, "clocks": clk.summary()}
+    ms_single, ms_single_cold, ms_two = lat
+    us = lambda v: None if v is None else v * 1e3
+    return {"batch": batch, "ms": ms, "ms_kernel": ms_kernel, "ms_direct": ms_direct, "step_us": dist_us,
+            "us_single_pair_warm": us(ms_single), "us_single_pair_cold": us(ms_single_cold),
+            "us_single_pair_two_calls_cold": us(ms_two), "clocks": clk.summary()}
 
 
 def measure_entry_points(torch, cfg, pairs, steps, warmup, device, use_graph):
@@ -584,14 +602,29 @@ def measure_series(torch, binding, cfg, M, steps, warmup, device, use_graph):
     return res
 
 
-def measure_read_ceiling():
-    """Read-only HBM ceiling of this GPU (build step 5): the standalone probe
-    paper_2501_10653_b200/csrc/hbm_read_ceiling.cu streams 2 GiB through TMA rings with no arithmetic,
-    over box shapes / ring depths / CTAs per SM, and prints the best rate."""
+CEILING_SRC = os.path.join(ROOT, "hbm_read_ceiling.cu")
+CEILING_EXE = os.path.join(ROOT, "hbm_read_ceiling")
+
+
+def build_read_ceiling(force: bool = False) -> str:
+    """Compile the standalone read-only HBM ceiling probe (hbm_read_ceiling.cu, beside this file: a measurement aid,
+    not part of the library). Returns its path."""
     import subprocess
     from paper_2501_10653_b200 import build
+    if not force and os.path.exists(CEILING_EXE) and os.path.getmtime(CEILING_EXE) >= os.path.getmtime(CEILING_SRC):
+        return CEILING_EXE
+    subprocess.run([build._nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17",
+                    "-o", CEILING_EXE, CEILING_SRC], check=True)
+    return CEILING_EXE
+
+
+def measure_read_ceiling():
+    """Read-only HBM ceiling of this GPU (build step 5): the standalone probe hbm_read_ceiling.cu
+    streams 2 GiB through TMA rings with no arithmetic, over box shapes / ring depths / CTAs per SM, and prints the
+    best rate."""
+    import subprocess
     try:
-        exe = build.build_read_ceiling()
+        exe = build_read_ceiling()
         out = subprocess.run([exe], capture_output=True, text=True, timeout=300).stdout
     except Exception as exc:           # the probe is a diagnostic: never let it take the bench line down
         return {"GBps": None, "error": repr(exc)[:300]}
@@ -633,6 +666,7 @@ def run_ours(args):
     n_stream = -(-pairs // PAIRS_PER_LAUNCH)                 # launches of the tile kernel per step
     us_launch = m["ms_kernel"] * 1e3 / (K * n_stream)       # per launch of the stream kernel (max over ranks)
     us_single, us_single_cold, clocks = m["us_single_pair_warm"], m["us_single_pair_cold"], m["clocks"]
+    us_two_calls = m["us_single_pair_two_calls_cold"]
     step_us = m["step_us"]
     alg = algorithmic_bytes(cfg.N, cfg.N_T) * pairs / n_stream    # algorithmic bytes one launch moves
     peak, peak_src = measured_peak()
@@ -665,6 +699,7 @@ def run_ours(args):
         row = {"us_per_pair_step": m2["ms"] * 1e3 / (k * p), "us_per_pair_step_no_graph": m2["ms_direct"] * 1e3 / (k * p),
                "us_per_pair_tiles_kernel": usk, "step_us": m2["step_us"],
                "us_single_pair_warm": m2["us_single_pair_warm"], "us_single_pair_cold": m2["us_single_pair_cold"],
+               "us_single_pair_two_calls_cold": m2["us_single_pair_two_calls_cold"],
                "achieved_GBps": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_nominal_8000": gbs / 8000.0,
                "pairs_per_step": p, "launches_per_step": m2["batch"].launches_per_step(True),
                "tile_kernel_launches_per_step": n_l, "plan": binding.plan_name(m2["batch"].x[0], c.N_T),
@@ -723,6 +758,10 @@ def run_ours(args):
             "step_us": dict(step_us, per_pair_median=step_us["median"] / pairs),
             "us_single_pair_warm": us_single,
             "us_single_pair_cold": us_single_cold,
+            "us_single_pair_two_calls_cold": us_two_calls,
+            "single_pair": "one iqa_fused_batch call with n_pairs = 1 per pair (tile kernel, second pass of split tiles, "
+                           "Eqs. 3-4: 2-3 dependent launches), 16 calls back to back, the same pair (warm: L2) / rotating "
+                           "over the batch (cold: HBM); two_calls = iqa_fused_tiles then iqa_aggregate per pair",
             "e2e": e2e,
             "clocks": clocks,
             "paper_context": {"note": "H100 kernel-only medians at N=2048, N_T=64 (PAPER.md:31); context, not the target",

@@ -316,6 +316,21 @@ int iqa_merge_tiles_batch(const float* lisi, const float* auglisi,
                           float* lisi_out, float* auglisi_out,
                           float* sum_x_out, float* sum_y_out, void* stream);
 
+/* P:66, the whole pyramid in ONE launch: from the per-tile arrays of an nty x ntx tile matrix (any rectangle: the
+ * output of iqa_fused_tiles_2d; n_maps of them stacked) every coarser level j = 1 .. L, L = iqa_pyramid_levels(nty, ntx)
+ * = ceil(log2(max(nty, ntx))).  Level j merges blocks of 2^j x 2^j base tiles by Eqs. 3-4 into a
+ * ceil(nty / 2^j) x ceil(ntx / 2^j) matrix, i.e. the tile matrix for tile side 2^j N_T; a block over the right / bottom
+ * border merges only the tiles that exist, and Eq. 4's n is that count.  Every output tile is summed in double
+ * directly from the BASE arrays (not from the rounded level below); level L is 1 x 1 and equals iqa_aggregate's pair.
+ *   outputs  [n_maps][iqa_pyramid_tiles(nty, ntx)]: the levels one after the other, level j row-major at offset
+ *            sum_{i<j} ceil(nty / 2^i) ceil(ntx / 2^i); may be NULL only when L == 0 (a 1 x 1 matrix).
+ * Outputs must not alias inputs. */
+int iqa_pyramid_levels(int nty, int ntx);
+size_t iqa_pyramid_tiles(int nty, int ntx);
+int iqa_pyramid(const float* lisi, const float* auglisi, const float* sum_x, const float* sum_y,
+                int nty, int ntx, int n_maps, float C2, float C,
+                float* lisi_out, float* auglisi_out, float* sum_x_out, float* sum_y_out, void* stream);
+
 /* Bytes of DEVICE scratch iqa_fused_host needs for (N, N_T): both images, the four per-tile
  * arrays, out2 and the kernel workspace.  0 for invalid shapes. */
 size_t iqa_host_scratch_bytes(int N, int N_T);

@@ -28,6 +28,7 @@ EXPORTS = ("iqa_status_string", "iqa_version", "iqa_debug_knob", "iqa_workspace_
            "iqa_fused_batch_2d", "iqa_fused_batch_2d_typed", "iqa_series_tiles_2d", "iqa_series_tiles_2d_typed",
            "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_tiles_below", "iqa_tiles_bottom_k",
            "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_merge_tiles_batch",
+           "iqa_pyramid_levels", "iqa_pyramid_tiles", "iqa_pyramid",
            "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
@@ -120,6 +121,12 @@ def _load() -> ctypes.CDLL:
     lib.iqa_merge_tiles_batch.argtypes = [vp, vp, vp, vp, i, i, i, f, f, vp, vp, vp, vp, vp]
     lib.iqa_merge_tiles.restype = i
     lib.iqa_merge_tiles.argtypes = [vp, vp, vp, vp, i, i, f, f, vp, vp, vp, vp, vp]
+    lib.iqa_pyramid_levels.restype = i
+    lib.iqa_pyramid_levels.argtypes = [i, i]
+    lib.iqa_pyramid_tiles.restype = sz
+    lib.iqa_pyramid_tiles.argtypes = [i, i]
+    lib.iqa_pyramid.restype = i
+    lib.iqa_pyramid.argtypes = [vp, vp, vp, vp, i, i, i, f, f, vp, vp, vp, vp, vp]
     lib.iqa_fused_host.restype = i
     lib.iqa_fused_host.argtypes = [vp, vp, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.iqa_fused_host_async.restype = i
@@ -734,13 +741,48 @@ def merge_tiles(lisi, auglisi, X, Y, g, C2, C) -> dict:
     return out
 
 
+def iqa_pyramid_levels(nty: int, ntx: int) -> int:
+    return int(lib.iqa_pyramid_levels(int(nty), int(ntx)))
+
+
+def iqa_pyramid_tiles(nty: int, ntx: int) -> int:
+    return int(lib.iqa_pyramid_tiles(int(nty), int(ntx)))
+
+
+def iqa_pyramid(lisi, auglisi, sum_x, sum_y, nty, ntx, n_maps, C2, C,
+                lisi_out, auglisi_out, sum_x_out, sum_y_out, stream=None) -> int:
+    return lib.iqa_pyramid(_ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y), int(nty), int(ntx), int(n_maps),
+                           C2, C, _ptr(lisi_out), _ptr(auglisi_out), _ptr(sum_x_out), _ptr(sum_y_out), _stream(stream))
+
+
 def pyramid(tiles: dict, C2, C) -> list:
-    """All levels N_T, 2 N_T, 4 N_T, ... up to the coarsest the tile count allows (factor-2 merges)."""
+    """all levels N_T, 2 N_T, 4 N_T, ... up to the whole image (a 1 x 1 matrix) from ONE ``iqa_pyramid`` launch.
+    ``tiles``: dict of (nty, ntx) or (n_maps, nty, ntx) matrices lisi, auglisi, X, Y (any rectangle).  Returns
+    ``[tiles, level 1, level 2, ...]``; level j holds (ceil(nty / 2^j), ceil(ntx / 2^j)) matrices (views of one buffer)."""
+    import torch
+    lisi = tiles["lisi"]
+    batched = lisi.dim() == 3
+    nty, ntx = int(lisi.shape[-2]), int(lisi.shape[-1])
+    n_maps = int(lisi.shape[0]) if batched else 1
+    src = [tiles[k] for k in ("lisi", "auglisi", "X", "Y")]
+    if not all(t.is_contiguous() and t.dtype == torch.float32 and t.is_cuda for t in src):
+        raise TypeError("pyramid needs contiguous float32 CUDA matrices (no CPU fallback)")
+    L, total = iqa_pyramid_levels(nty, ntx), iqa_pyramid_tiles(nty, ntx)
     levels = [tiles]
-    cur = tiles
-    while cur["lisi"].shape[-1] % 2 == 0 and cur["lisi"].shape[-1] > 1:
-        cur = merge_tiles(cur["lisi"], cur["auglisi"], cur["X"], cur["Y"], 2, C2, C)
-        levels.append(cur)
+    if L == 0:
+        return levels
+    out = [torch.empty((n_maps, total), dtype=torch.float32, device=lisi.device) for _ in range(4)]
+    with _device_of(lisi.device):
+        rc = iqa_pyramid(*src, nty, ntx, n_maps, C2, C, *out, _current_stream(lisi.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_pyramid")
+    off = 0
+    for j in range(1, L + 1):
+        ny, nx = -(-nty // (1 << j)), -(-ntx // (1 << j))
+        shape = (n_maps, ny, nx) if batched else (ny, nx)
+        levels.append({k: (o[:, off:off + ny * nx] if batched else o[0, off:off + ny * nx]).reshape(shape)
+                       for k, o in zip(("lisi", "auglisi", "X", "Y"), out)})
+        off += ny * nx
     return levels
 
 

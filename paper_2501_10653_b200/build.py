@@ -55,18 +55,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-CEILING_SRC = os.path.join(CSRC, "hbm_read_ceiling.cu")
-CEILING_EXE = os.path.join(_HERE, "hbm_read_ceiling")
-
-
-def build_read_ceiling(force: bool = False) -> str:
-    """Compile the standalone read-only HBM ceiling probe (csrc/hbm_read_ceiling.cu). Returns its path."""
-    if not force and os.path.exists(CEILING_EXE) and os.path.getmtime(CEILING_EXE) >= os.path.getmtime(CEILING_SRC):
-        return CEILING_EXE
-    subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17",
-                    "-o", CEILING_EXE, CEILING_SRC], check=True)
-    return CEILING_EXE
-
-
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose=True))

@@ -175,4 +175,69 @@ merge_kernel(const float* __restrict__ lisi, const float* __restrict__ aug,
     }
 }
 
+// ---- P:66, every level in one launch -------------------------------------------------------------------------------
+// Level j >= 1 of the pyramid over an nty x ntx tile matrix merges blocks of 2^j x 2^j base tiles (tile size 2^j N_T):
+// ceil(nty / 2^j) x ceil(ntx / 2^j) output tiles; a block over the right / bottom border holds only the base tiles that
+// exist, and Eq. 4's n is that count.  EVERY output tile is summed directly from the BASE arrays in double
+// (never from the re-rounded level below), so level j is the tile matrix of size 2^j N_T up to one fp32 rounding.
+// One launch: a unit (map, level, block) is taken by a warp (blocks of up to kPyrWarpTiles base tiles, 8 units per CTA)
+// or by a whole CTA (larger blocks); lanes / threads stride over the block's tiles, then butterflies, fixed order.
+constexpr int kPyrMaxLevels = 21;
+constexpr int kPyrWarpTiles = 1024;
+struct PyramidLevel { int shift, nby, nbx, cta_mode; long long out_off; unsigned first_cta; };
+struct PyramidParams {
+    PyramidLevel lv[kPyrMaxLevels];
+    int n_levels, nty, ntx, n_maps;
+    long long out_per_map;                  // output tiles of all levels of one map
+};
+
+__global__ void __launch_bounds__(256)
+pyramid_kernel(const float* __restrict__ lisi, const float* __restrict__ aug,
+               const float* __restrict__ X, const float* __restrict__ Y, const __grid_constant__ PyramidParams p,
+               float C2f, float Cf, float* __restrict__ lisi_o, float* __restrict__ aug_o,
+               float* __restrict__ X_o, float* __restrict__ Y_o) {
+    __shared__ Agg4 part[8];
+    pdl_prologue();
+    int l = 0;
+    while (l + 1 < p.n_levels && blockIdx.x >= p.lv[l + 1].first_cta) ++l;
+    const PyramidLevel& L = p.lv[l];
+    const long long per_map = (long long)L.nby * L.nbx;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const long long unit = L.cta_mode ? (long long)(blockIdx.x - L.first_cta)
+                                      : (long long)(blockIdx.x - L.first_cta) * 8 + w;
+    if (unit >= per_map * p.n_maps) return;                  // (whole warps / CTAs: no barrier is skipped by part of one)
+    const long long map = unit / per_map, o = unit - map * per_map;
+    const int oy = (int)(o / L.nbx), ox = (int)(o - (long long)oy * L.nbx);
+    const int r0 = oy << L.shift, c0 = ox << L.shift;
+    const int rows = min(p.nty - r0, 1 << L.shift), cols = min(p.ntx - c0, 1 << L.shift);
+    const int nb = rows * cols;                               // base tiles actually merged: Eq. 4's n
+    const size_t in0 = (size_t)map * p.nty * p.ntx + (size_t)r0 * p.ntx + c0;
+    const double C2 = (double)C2f, C = (double)Cf;
+    Agg4 a = {0.0, 0.0, 0.0, 0.0};
+    const int t0 = L.cta_mode ? (int)threadIdx.x : lane, dt = L.cta_mode ? 256 : 32;
+    int r = t0 / cols, c = t0 - r * cols;                     // tile k = r * cols + c of the block
+    const int dr = dt / cols, dc = dt - dr * cols;
+    for (int k = t0; k < nb; k += dt) {
+        const size_t t = in0 + (size_t)r * p.ntx + c;
+        agg_add(a, lisi[t], aug[t], X[t], Y[t], C2, C);
+        r += dr; c += dc;
+        if (c >= cols) { c -= cols; ++r; }
+    }
+    a = agg_warp_sum(a);
+    if (L.cta_mode) {
+        if (lane == 0) part[w] = a;
+        __syncthreads();
+        if (threadIdx.x >= 32) return;
+        Agg4 b = {0.0, 0.0, 0.0, 0.0};
+        if (lane < 8) b = part[lane];
+        a = agg_warp_sum(b);
+    }
+    if (lane == 0) {
+        const size_t og = (size_t)map * p.out_per_map + (size_t)L.out_off + (size_t)o;
+        agg_finish(a, (double)nb, C2, C, lisi_o + og, aug_o + og);
+        X_o[og] = (float)a.sx;
+        Y_o[og] = (float)a.sy;
+    }
+}
+
 }  // namespace iqa

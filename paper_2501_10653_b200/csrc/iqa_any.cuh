@@ -150,20 +150,22 @@ template <> struct Pixel4<__half> {
     static __device__ __forceinline__ void row(const unsigned char* xs, const unsigned char* ys, float C1, Acc16& a) {
         const uint2 qx = *reinterpret_cast<const uint2*>(xs);
         const uint2 qy = *reinterpret_cast<const uint2*>(ys);
-        const float2 x01 = __half22float2(*reinterpret_cast<const __half2*>(&qx.x));
-        const float2 x23 = __half22float2(*reinterpret_cast<const __half2*>(&qx.y));
-        const float2 y01 = __half22float2(*reinterpret_cast<const __half2*>(&qy.x));
-        const float2 y23 = __half22float2(*reinterpret_cast<const __half2*>(&qy.y));
-        pixel_terms2<MODE>(x01.x, x01.y, y01.x, y01.y, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
-        pixel_terms2<MODE>(x23.x, x23.y, y23.x, y23.y, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+        // the clamp on two pixels at once in fp16 (max(NaN, 0) = 0, as in fp32), then the exact conversion
+        const __half2 zero = __float2half2_rn(0.0f);
+        const float2 x01 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&qx.x), zero));
+        const float2 x23 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&qx.y), zero));
+        const float2 y01 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&qy.x), zero));
+        const float2 y23 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&qy.y), zero));
+        pixel_terms2<MODE, false>(x01.x, x01.y, y01.x, y01.y, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
+        pixel_terms2<MODE, false>(x23.x, x23.y, y23.x, y23.y, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
     }
 };
 
-// int16 -> fp32 without the conversion unit: flipping the sign bit gives u = v + 32768 in [0, 65535];
-// the float with bits 0x4B000000 | u is exactly 2^23 + u, and subtracting 2^23 + 32768 leaves v.
+// int16 -> fp32 without the conversion unit: the clamp on both halves at once leaves u in [0, 32767];
+// the float with bits 0x4B000000 | u is exactly 2^23 + u, and subtracting 2^23 leaves u.
 __device__ __forceinline__ void s16x2_to_float(uint32_t w, float& lo, float& hi) {
-    const uint32_t u = w ^ 0x80008000u;
-    const uint64_t m = pack2(8421376.0f, 8421376.0f);
+    const uint32_t u = __vmaxs2(w, 0u);
+    const uint64_t m = pack2(8388608.0f, 8388608.0f);
     const uint64_t f = sub2(pack2(__uint_as_float(__byte_perm(u, 0x4B000000u, 0x7610)),
                                   __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7632))), m);
     unpack2(f, lo, hi);
@@ -177,8 +179,8 @@ template <> struct Pixel4<short> {
         float x0, x1, x2, x3, y0, y1, y2, y3;
         s16x2_to_float(qx.x, x0, x1); s16x2_to_float(qx.y, x2, x3);
         s16x2_to_float(qy.x, y0, y1); s16x2_to_float(qy.y, y2, y3);
-        pixel_terms2<MODE>(x0, x1, y0, y1, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
-        pixel_terms2<MODE>(x2, x3, y2, y3, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+        pixel_terms2<MODE, false>(x0, x1, y0, y1, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
+        pixel_terms2<MODE, false>(x2, x3, y2, y3, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
     }
 };
 
@@ -199,8 +201,8 @@ template <> struct Pixel4<unsigned char> {
         float x0, x1, x2, x3, y0, y1, y2, y3;
         u8x4_to_float(qx, x0, x1, x2, x3);
         u8x4_to_float(qy, y0, y1, y2, y3);
-        pixel_terms2<MODE>(x0, x1, y0, y1, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
-        pixel_terms2<MODE>(x2, x3, y2, y3, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+        pixel_terms2<MODE, false>(x0, x1, y0, y1, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);      // unsigned: nothing to clamp
+        pixel_terms2<MODE, false>(x2, x3, y2, y3, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
     }
 };
 

@@ -604,6 +604,10 @@ int launch_generic(int mode, const void* const* xs, const void* const* ys, int n
     return IQA_OK;
 }
 
+// Which second pass a split-tile call takes: a function of (pieces, tiles per comparison) only, so that a batch and
+// the same pairs one by one sum the pieces in the same order.
+bool finalise_is_small(int pieces, long long n) { return pieces <= 32 && n >= 64; }
+
 // S1-S4 for n_pairs pairs (xs[i], ys[i]) with the plan's kernel; `out` / `ws` point at pair 0.  The plan is
 // downgraded to the generic kernels (before anything is launched) when a tensor map cannot be encoded.
 int launch_pairs(int mode, const void* const* xs, const void* const* ys, int n_pairs, const Geom& g, int N_T,
@@ -635,7 +639,7 @@ int finish_comparisons(const Outputs& out, float* out2, int n_cmp, long long n, 
         p.ws = ws;
         const int total = (int)(n * n_cmp);
         cudaError_t e;
-        if (pl.pieces <= 32 && total >= 64)
+        if (finalise_is_small(pl.pieces, n))
             e = launch(finalise_small_kernel, (unsigned)((total + kCtaThreads - 1) / kCtaThreads), kCtaThreads, 0, st,
                        p, pl.pieces, total);
         else
@@ -1028,6 +1032,54 @@ int iqa_merge_tiles_batch(const float* lisi, const float* auglisi,
     const long long n_out = (long long)(nt / g) * (nt / g) * n_maps;
     const unsigned grid = (unsigned)((n_out + 7) / 8);
     if (launch(merge_kernel, grid, 256u, 0, (cudaStream_t)stream, lisi, auglisi, sum_x, sum_y, nt, g, n_maps, C2, C,
+               lisi_out, auglisi_out, sum_x_out, sum_y_out) != cudaSuccess)
+        return IQA_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+}
+
+int iqa_pyramid_levels(int nty, int ntx) {
+    if (nty <= 0 || ntx <= 0) return 0;
+    int L = 0;
+    while ((1 << L) < (nty > ntx ? nty : ntx)) ++L;
+    return L;
+}
+
+size_t iqa_pyramid_tiles(int nty, int ntx) {
+    const int L = iqa_pyramid_levels(nty, ntx);
+    size_t total = 0;
+    for (int j = 1; j <= L; ++j) total += (size_t)ceil_div(nty, 1 << j) * (size_t)ceil_div(ntx, 1 << j);
+    return total;
+}
+
+int iqa_pyramid(const float* lisi, const float* auglisi, const float* sum_x, const float* sum_y,
+                int nty, int ntx, int n_maps, float C2, float C,
+                float* lisi_out, float* auglisi_out, float* sum_x_out, float* sum_y_out, void* stream) {
+    if (!lisi || !auglisi || !sum_x || !sum_y) return IQA_ERR_NULL;
+    if (nty <= 0 || ntx <= 0 || n_maps <= 0 || (long long)nty * ntx * n_maps > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    if (!pos_finite(C2) || !pos_finite(C)) return IQA_ERR_PARAM;
+    const int L = iqa_pyramid_levels(nty, ntx);
+    if (L == 0) return IQA_OK;                                // a 1 x 1 matrix is its own top: no level to emit
+    if (!lisi_out || !auglisi_out || !sum_x_out || !sum_y_out) return IQA_ERR_NULL;
+    if (L > kPyrMaxLevels) return IQA_ERR_SHAPE;
+    PyramidParams p{};
+    p.n_levels = L; p.nty = nty; p.ntx = ntx; p.n_maps = n_maps;
+    long long off = 0, cta = 0;
+    for (int j = 1; j <= L; ++j) {
+        PyramidLevel& lv = p.lv[j - 1];
+        lv.shift = j;
+        lv.nby = ceil_div(nty, 1 << j);
+        lv.nbx = ceil_div(ntx, 1 << j);
+        const long long side = 1LL << j;
+        lv.cta_mode = side * side > kPyrWarpTiles;
+        lv.out_off = off;
+        lv.first_cta = (unsigned)cta;
+        const long long units = (long long)lv.nby * lv.nbx * n_maps;
+        off += (long long)lv.nby * lv.nbx;
+        cta += lv.cta_mode ? units : (units + 7) / 8;
+    }
+    p.out_per_map = off;
+    if (cta > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    if (launch(pyramid_kernel, (unsigned)cta, 256u, 0, (cudaStream_t)stream, lisi, auglisi, sum_x, sum_y, p, C2, C,
                lisi_out, auglisi_out, sum_x_out, sum_y_out) != cudaSuccess)
         return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;

@@ -157,11 +157,12 @@ struct Acc16 {
 
 // S1 + S2 for two horizontally adjacent pixel pairs: clamp, then the Eq. 1 / Eq. 2 terms
 // with the roundings of pixel_terms() (iqa_kernels.cuh).
-template <int MODE>
+// CLAMP = false: the caller has clamped already (or the pixel type has no negative values).
+template <int MODE, bool CLAMP = true>
 __device__ __forceinline__ void pixel_terms2(float x0, float x1, float y0, float y1, float C1,
                                              uint64_t& aL, float& aA0, float& aA1, uint64_t& aX, uint64_t& aY) {
-    const uint64_t xc = pack2(fmaxf(x0, 0.0f), fmaxf(x1, 0.0f));     // NaN -> 0, negatives -> 0
-    const uint64_t yc = pack2(fmaxf(y0, 0.0f), fmaxf(y1, 0.0f));
+    const uint64_t xc = CLAMP ? pack2(fmaxf(x0, 0.0f), fmaxf(x1, 0.0f)) : pack2(x0, x1);     // NaN -> 0, negatives -> 0
+    const uint64_t yc = CLAMP ? pack2(fmaxf(y0, 0.0f), fmaxf(y1, 0.0f)) : pack2(y0, y1);
     const uint64_t s = add2(xc, yc);            // |x + y| = x + y after the clamp
     const uint64_t d = sub2(xc, yc);
     float d0, d1;

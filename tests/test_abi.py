@@ -222,6 +222,22 @@ def test_2d_validation():
     assert B.iqa_fused_tiles(FAKE, FAKE, 100, 64, *a, *o) == B.IQA_ERR_SHAPE
 
 
+def test_pyramid_geometry_and_validation():
+    assert B.iqa_pyramid_levels(1, 1) == 0 and B.iqa_pyramid_tiles(1, 1) == 0
+    assert B.iqa_pyramid_levels(32, 32) == 5 and B.iqa_pyramid_tiles(32, 32) == 256 + 64 + 16 + 4 + 1
+    assert B.iqa_pyramid_levels(16, 24) == 5            # 8x12, 4x6, 2x3, 1x2, 1x1
+    assert B.iqa_pyramid_tiles(16, 24) == 96 + 24 + 6 + 2 + 1
+    assert B.iqa_pyramid_levels(3, 1) == 2 and B.iqa_pyramid_tiles(3, 1) == 2 + 1
+    assert B.iqa_pyramid_levels(0, 4) == 0 and B.iqa_pyramid_tiles(-1, 4) == 0
+    o = (FAKE, FAKE, FAKE, FAKE)
+    assert B.iqa_pyramid(None, FAKE, FAKE, FAKE, 4, 4, 1, 1e-6, 1e-6, *o) == B.IQA_ERR_NULL
+    assert B.iqa_pyramid(FAKE, FAKE, FAKE, FAKE, 4, 4, 1, 1e-6, 1e-6, FAKE, FAKE, None, FAKE) == B.IQA_ERR_NULL
+    assert B.iqa_pyramid(FAKE, FAKE, FAKE, FAKE, 0, 4, 1, 1e-6, 1e-6, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_pyramid(FAKE, FAKE, FAKE, FAKE, 4, 4, 0, 1e-6, 1e-6, *o) == B.IQA_ERR_SHAPE
+    assert B.iqa_pyramid(FAKE, FAKE, FAKE, FAKE, 4, 4, 1, 0.0, 1e-6, *o) == B.IQA_ERR_PARAM
+    assert B.iqa_pyramid(FAKE, FAKE, FAKE, FAKE, 1, 1, 3, 1e-6, 1e-6, None, None, None, None) == B.IQA_OK   # nothing to emit
+
+
 def test_typed_batch_series_validation_and_knobs():
     a = (1e-6, 1e-6, 1e-6, 5e-7)
     o = (FAKE, FAKE, FAKE, FAKE)

@@ -407,3 +407,25 @@ def test_unaligned_bases(B, U):
             _check_typed(B, U, x, y, xd, yd, N_T, k, f"shift {off} N_T={N_T}", plan="tma_any")
             yd2 = _typed_window(y, 772, (off + 1) % 4)
             _check_typed(B, U, x, y, xd, yd2, N_T, k, f"offsets {off}/{(off + 1) % 4} N_T={N_T}", plan=None)
+
+
+@pytest.mark.parametrize("H,W,N_T", [(1000, 1536, 64), (1000, 1536, 48), (333, 2000, 8), (700, 129, 16), (64, 64, 64)])
+def test_pyramid_of_a_rectangle_every_level(B, U, H, W, N_T):
+    """iqa_pyramid on a rectangular nty x ntx tile matrix with edge tiles: level j merges 2^j x 2^j blocks, blocks over
+    the border merge only the tiles that exist (Eq. 4's n is that count) -- so level j must equal
+    oracle.tiles_2d at tile size 2^j N_T, for EVERY level up to the 1 x 1 top."""
+    import torch
+    import oracle
+    x, y = _pair(H, W, H + N_T)
+    xd, yd = U.to_dev(x), U.to_dev(y)
+    base = B.fused_tiles_2d(xd, yd, N_T, K["C1"], K["C2"], K["C"], K["D"])
+    levels = B.pyramid(base, K["C2"], K["C"])
+    torch.cuda.synchronize()
+    nty, ntx = -(-H // N_T), -(-W // N_T)
+    assert len(levels) == 1 + B.iqa_pyramid_levels(nty, ntx)
+    assert sum(l["lisi"].numel() for l in levels[1:]) == B.iqa_pyramid_tiles(nty, ntx)
+    for j, level in enumerate(levels):
+        ref = oracle.tiles_2d(x, y, N_T << j, **K)
+        got = {n: level[n].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y")}
+        U.assert_parity(got, ref, K["C"], f"pyramid {H}x{W} N_T={N_T} level {j}")
+    assert tuple(levels[-1]["lisi"].shape) == (1, 1)

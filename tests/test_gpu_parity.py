@@ -317,8 +317,22 @@ def test_aggregate_equals_whole_image_and_merge(U, B):
         ref = oracle.tiles(x, y, 32 * g, **k)
         got = {n: m[n].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y")}
         U.assert_parity(got, ref, k["C"], f"merge g={g}")
+    # iqa_pyramid: EVERY level in one launch, each against the oracle at tile size 2^j * 32
     lv = B.pyramid(o, k["C2"], k["C"])
     assert [l["lisi"].shape[0] for l in lv] == [64, 32, 16, 8, 4, 2, 1]
+    for j, level in enumerate(lv):
+        ref = oracle.tiles(x, y, 32 << j, **k)
+        got = {n: level[n].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y")}
+        U.assert_parity(got, ref, k["C"], f"pyramid level {j}")
+    agg = B.aggregate(o["lisi"], o["auglisi"], o["X"], o["Y"], k["C2"], k["C"]).cpu().numpy()
+    assert abs(lv[-1]["lisi"].item() - agg[0]) <= 1e-6 * abs(agg[0]) and abs(lv[-1]["auglisi"].item() - agg[1]) <= 1e-6 * abs(agg[1])
+    for N_T in (8, 64):                     # 65536 base tiles (CTA-wide units at the top) and the bench tile size
+        o2 = B.fused_tiles(xd, yd, N_T, **k)
+        for j, level in enumerate(B.pyramid(o2, k["C2"], k["C"])):
+            if j in (0, 1, 5) or (N_T << j) >= 1024:
+                ref = oracle.tiles(x, y, N_T << j, **k)
+                got = {n: level[n].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y")}
+                U.assert_parity(got, ref, k["C"], f"pyramid N_T={N_T} level {j}")
 
 
 def test_fused_host_entry_point(U, B):
@@ -408,3 +422,21 @@ def test_error_codes_on_device(B):
     rc = B.iqa_fused_tiles(x.data_ptr() + 2, x, N, N_T, 1e-6, 1e-6, 1e-6, 5e-7, *o, None, None, ws, need, None)
     assert rc == B.IQA_ERR_ALIGN
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("N,N_T", [(2048, 64), (2048, 256), (2048, 512), (512, 128), (256, 128)])
+def test_one_pair_calls_and_batches_sum_in_the_same_order(U, B, N, N_T):
+    """iqa_fused_batch over 1 pair, over 5 pairs, and iqa_fused_tiles + iqa_aggregate give bit-identical results: the
+    second pass of split tiles is chosen by (pieces, tiles per pair) alone, never by the batch size (n = 16 tiles with
+    32 pieces at N = 2048, N_T = 512 used to switch kernels between a single pair and a batch of four)."""
+    dev = [tuple(U.to_dev(a) for a in _rand_pair(N, seed=N_T + i)) for i in range(5)]
+    k = K6
+    batch = B.fused_batch([d[0] for d in dev], [d[1] for d in dev], N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    for i, (xd, yd) in enumerate(dev):
+        one = B.fused_batch([xd], [yd], N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+        t = B.fused_tiles(xd, yd, N_T, numerators=True, **k)
+        agg = B.aggregate(t["lisi"], t["auglisi"], t["X"], t["Y"], k["C2"], k["C"])
+        torch.cuda.synchronize()
+        for n in ("lisi", "auglisi", "X", "Y", "L", "A"):
+            assert torch.equal(batch[n][i], one[n][0]) and torch.equal(one[n][0], t[n]), (i, n)
+        assert torch.equal(batch["whole"][i], agg) and torch.equal(one["whole"][0], agg), i

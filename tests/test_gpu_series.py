@@ -162,6 +162,11 @@ def test_pyramid_of_a_series(B, U, mode):
             U.assert_parity(got, {n: ref[n][c] for n in list(got) + ["A"]}, k["C"], f"series merge g={g} cmp {c}")
     levels = B.pyramid(base, k["C2"], k["C"])
     assert [tuple(l["lisi"].shape) for l in levels] == [(3, 16, 16), (3, 8, 8), (3, 4, 4), (3, 2, 2), (3, 1, 1)]
+    for j, level in enumerate(levels):       # every level of every comparison against the series oracle at 16 * 2^j
+        ref = oracle.series(imgs, mode, 16 << j, **k)
+        for c in range(3):
+            got = {n: level[n][c].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y")}
+            U.assert_parity(got, {n: ref[n][c] for n in list(got) + ["A"]}, k["C"], f"series pyramid level {j} cmp {c}")
     top = levels[-1]
     for c in range(3):                      # the top of the pyramid is the whole-image pair of Eqs. 3-4
         w = base["whole"][c].cpu().numpy()
