@@ -653,10 +653,22 @@ def run_ours(args):
         td.init_process_group("nccl", device_id=device)
         dist = td
 
+    if args.paths:
+        # only the rows of PATH_ROWS named on the command line (ncu captures of any_kernel / the generic kernels)
+        names = set(args.paths.split(","))
+        rows = [r for r in PATH_ROWS if r[0] in names]
+        if not rows:
+            raise SystemExit(f"--paths: unknown row(s) {sorted(names)}; known: {[r[0] for r in PATH_ROWS]}")
+        res = measure_paths(torch, binding, args.steps, args.warmup, device, not args.no_graph, rows=rows)
+        print(json.dumps({"metric": METRIC, "unit": UNIT, "library_version": binding.iqa_version(), "paths": res}))
+        return
     idx, pairs, pairs_e2e = WORKLOADS[args.workload]
     if args.pairs:
         pairs = args.pairs
     cfg = synth.CONFIGS[idx]
+    if args.nt:
+        from dataclasses import replace
+        cfg = replace(cfg, N_T=args.nt, name=f"{cfg.name}_NT{args.nt}")        # one point of the config [2] sweep
     use_graph = not args.no_graph
     K, W = args.steps, args.warmup
 
@@ -675,7 +687,8 @@ def run_ours(args):
     launches = m["batch"].launches_per_step(True)
     plan = binding.plan_name(m["batch"].x[0], cfg.N_T)           # the kernel the library really picked
     us_per_pair_direct = m["ms_direct"] * 1e3 / total_pairs
-    traffic, traffic_src = ncu_traffic(args.workload, pairs // n_stream, binding.iqa_version())
+    traffic, traffic_src = ncu_traffic(args.workload + (f"_NT{args.nt}" if args.nt else ""), pairs // n_stream,
+                                       binding.iqa_version())
     del m
     torch.cuda.empty_cache()
 
@@ -793,6 +806,8 @@ def main():
     ap.add_argument("--no-latency", action="store_true",
                     help="skip the single-pair latency loops (keeps the launch list short under ncu)")
     ap.add_argument("--series-images", type=int, default=9, help="snapshots of the time-series measurement in `also`")
+    ap.add_argument("--nt", type=int, default=0, help="override the workload's tile side N_T (a point of the config [2] sweep)")
+    ap.add_argument("--paths", default="", help="comma-separated rows of PATH_ROWS: time only those kernel paths and print them")
     ap.add_argument("--sweep", action="store_true", help="also time BASELINE.json config [2] (N=2048, N_T = 8..512)")
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)

@@ -164,7 +164,7 @@ template <> struct Pixel4<__half> {
 // int16 -> fp32 without the conversion unit: the clamp on both halves at once leaves u in [0, 32767];
 // the float with bits 0x4B000000 | u is exactly 2^23 + u, and subtracting 2^23 leaves u.
 __device__ __forceinline__ void s16x2_to_float(uint32_t w, float& lo, float& hi) {
-    const uint32_t u = __vmaxs2(w, 0u);
+    const uint32_t u = __vimax_s16x2_relu(w, w);               // max(v, 0) on both halves: VIMNMX.S16x2.RELU
     const uint64_t m = pack2(8388608.0f, 8388608.0f);
     const uint64_t f = sub2(pack2(__uint_as_float(__byte_perm(u, 0x4B000000u, 0x7610)),
                                   __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7632))), m);

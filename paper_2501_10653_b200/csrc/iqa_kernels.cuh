@@ -104,13 +104,13 @@ template <typename T> struct PixelExactInFloat { static constexpr bool value = t
 template <> struct PixelExactInFloat<double> { static constexpr bool value = false; };
 template <> struct PixelExactInFloat<int> { static constexpr bool value = false; };
 
+// One pixel of type T already in a register -> the terms.  (Loads are issued by the caller, several at a time.)
 template <int MODE, typename T>
-__device__ __forceinline__ void pixel_terms_any(const T* __restrict__ x, const T* __restrict__ y, size_t ox, size_t oy,
-                                                float C1, float& aL, float& aA, float& aX, float& aY) {
+__device__ __forceinline__ void pixel_terms_val(T xr, T yr, float C1, float& aL, float& aA, float& aX, float& aY) {
     if constexpr (PixelExactInFloat<T>::value) {
-        pixel_terms<MODE>((float)x[ox], (float)y[oy], C1, aL, aA, aX, aY);
+        pixel_terms<MODE>((float)xr, (float)yr, C1, aL, aA, aX, aY);
     } else {
-        const double xv = (double)x[ox], yv = (double)y[oy];
+        const double xv = (double)xr, yv = (double)yr;
         const double xc = xv > 0.0 ? xv : 0.0;      // P:27; NaN -> 0
         const double yc = yv > 0.0 ? yv : 0.0;
         const float s = (float)(xc + yc);
@@ -120,6 +120,11 @@ __device__ __forceinline__ void pixel_terms_any(const T* __restrict__ x, const T
         aX += (float)xc;
         aY += (float)yc;
     }
+}
+template <int MODE, typename T>
+__device__ __forceinline__ void pixel_terms_any(const T* __restrict__ x, const T* __restrict__ y, size_t ox, size_t oy,
+                                                float C1, float& aL, float& aA, float& aX, float& aY) {
+    pixel_terms_val<MODE, T>(x[ox], y[oy], C1, aL, aA, aX, aY);
 }
 
 // S4: Eq. 1 / Eq. 2 from the four sums of one tile, true fp32 division.
@@ -161,6 +166,7 @@ __device__ __forceinline__ void finalise_tile(const Params& p, size_t t, float4 
 // partial goes to the workspace and finalise_kernel finishes.
 // -----------------------------------------------------------------------------
 constexpr int kGenericRows = 64;
+constexpr int kGenericInFlight = 8;      // pixel pairs a thread loads before it computes
 
 struct GenericParams {
     TileParams tp;
@@ -187,14 +193,32 @@ generic_kernel(const GenericParams g) {
     const size_t row0 = (size_t)ty * N_T + r_begin, col0 = (size_t)tx * N_T;
 
     float aL = 0.f, aA = 0.f, aX = 0.f, aY = 0.f;
-    // warp w takes rows w, w + 8, ...; lanes stride over the columns (coalesced, no division per pixel)
+    // warp w takes rows w, w + 8, ...; lanes stride over the columns (coalesced, no division per pixel).  The loads
+    // of kGenericInFlight pixels of both images are issued before the first term is computed: a lone scalar load per
+    // thread would leave the kernel waiting on the latency of each one.
     (void)npix;
-    for (int r = (int)(threadIdx.x >> 5); r < r_end - r_begin; r += kWarpsPerCta) {
-        const size_t bx = (row0 + r) * (size_t)p.pitch_x + col0;
-        const size_t by = (row0 + r) * (size_t)p.pitch_y + col0;
-        for (int c = (int)(threadIdx.x & 31); c < cols_t; c += 32)
-            pixel_terms_any<MODE, T>(reinterpret_cast<const T*>(p.x), reinterpret_cast<const T*>(p.y), bx + c, by + c,
-                                     p.C1, aL, aA, aX, aY);
+    const T* xp = reinterpret_cast<const T*>(p.x);
+    const T* yp = reinterpret_cast<const T*>(p.y);
+    const int lane = (int)(threadIdx.x & 31);
+    const int cpl = (cols_t - lane + 31) >> 5;                 // columns of this lane per row (may be 0)
+    const int rows_w = (r_end - r_begin - (int)(threadIdx.x >> 5) + kWarpsPerCta - 1) / kWarpsPerCta;   // rows of this warp
+    const int n_mine = rows_w > 0 ? rows_w * cpl : 0;          // pixels of this thread: k -> (row k / cpl, column k % cpl)
+    int kr = 0, kc = 0;                                        // row / column counters of the next pixel to load
+    for (int k0 = 0; k0 < n_mine; k0 += kGenericInFlight) {
+        T vx[kGenericInFlight], vy[kGenericInFlight];
+#pragma unroll
+        for (int u = 0; u < kGenericInFlight; ++u) {
+            if (k0 + u < n_mine) {
+                const size_t r = row0 + (threadIdx.x >> 5) + (size_t)kr * kWarpsPerCta;
+                const size_t c = col0 + lane + (size_t)kc * 32;
+                vx[u] = xp[r * (size_t)p.pitch_x + c];
+                vy[u] = yp[r * (size_t)p.pitch_y + c];
+                if (++kc == cpl) { kc = 0; ++kr; }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kGenericInFlight; ++u)
+            if (k0 + u < n_mine) pixel_terms_val<MODE, T>(vx[u], vy[u], p.C1, aL, aA, aX, aY);
     }
     float4 v = make_float4(aL, aA, aX, aY);
     for (int o = 16; o > 0; o >>= 1) {
@@ -235,15 +259,26 @@ generic_warp_kernel(const GenericParams g, long long n_tiles) {
     const int npix = rows_t * cols_t;
     const size_t row0 = (size_t)ty * N_T, col0 = (size_t)tx * N_T;
     float aL = 0.f, aA = 0.f, aX = 0.f, aY = 0.f;
-    // independent addresses per iteration (the divisions are cheap next to the load latency of a lone warp,
-    // and the unrolled loop keeps several loads in flight)
-#pragma unroll 4
-    for (int k = lane; k < npix; k += 32) {
-        const int r = k / cols_t, c = k % cols_t;
-        const size_t ox = (row0 + r) * (size_t)p.pitch_x + col0 + c;
-        const size_t oy = (row0 + r) * (size_t)p.pitch_y + col0 + c;
-        pixel_terms_any<MODE, T>(reinterpret_cast<const T*>(p.x), reinterpret_cast<const T*>(p.y), ox, oy, p.C1,
-                                 aL, aA, aX, aY);
+    // lanes stride over the tile's pixels in row-major order; (row, column) advance by additions, and the loads of
+    // kGenericInFlight pixels of both images are issued before the first term is computed
+    const T* xp = reinterpret_cast<const T*>(p.x);
+    const T* yp = reinterpret_cast<const T*>(p.y);
+    int r = lane / cols_t, c = lane - r * cols_t;
+    const int dr = 32 / cols_t, dc = 32 - dr * cols_t;
+    for (int k0 = lane; k0 < npix; k0 += 32 * kGenericInFlight) {
+        T vx[kGenericInFlight], vy[kGenericInFlight];
+#pragma unroll
+        for (int u = 0; u < kGenericInFlight; ++u) {
+            if (k0 + 32 * u < npix) {
+                vx[u] = xp[(row0 + r) * (size_t)p.pitch_x + col0 + c];
+                vy[u] = yp[(row0 + r) * (size_t)p.pitch_y + col0 + c];
+                r += dr; c += dc;
+                if (c >= cols_t) { c -= cols_t; ++r; }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kGenericInFlight; ++u)
+            if (k0 + 32 * u < npix) pixel_terms_val<MODE, T>(vx[u], vy[u], p.C1, aL, aA, aX, aY);
     }
     float4 v = make_float4(aL, aA, aX, aY);
     for (int o = 16; o > 0; o >>= 1) {
