@@ -490,26 +490,40 @@ PATH_ROWS = [
 ]
 
 
+def make_path_inputs(torch, row, pairs, device):
+    """The synthetic image pairs of one PATH_ROWS row (seeded; also what tests/test_gpu_bench_config.py checks against
+    the oracle): zero-mean noise plus a small offset for the floating-point types (about half the pixels negative
+    before the clamp, as on the BASELINE.json skies), counts in [-20, 200) / [0, 200) for the integer types; each image
+    is a window (row pitch, base offset) of its own buffer.  Returns (xs, ys)."""
+    name, dtype, H, W, pitch, off, N_T = row
+    dt = getattr(torch, dtype)
+    g = torch.Generator(device=device).manual_seed(len(name) + N_T)
+    imgs = []
+    for _ in range(2 * pairs):
+        buf = torch.empty(H * pitch + 64, dtype=dt, device=device)
+        if dt.is_floating_point:
+            buf.copy_(torch.randn(buf.shape, generator=g, device=device, dtype=torch.float32) * 1e-3 + 2e-4)
+        else:
+            buf.copy_(torch.randint(-20 if dt != torch.uint8 else 0, 200, buf.shape, generator=g, device=device,
+                                    dtype=torch.int32))
+        imgs.append(torch.as_strided(buf, (H, W), (pitch, 1), off))
+    return imgs[0::2], imgs[1::2]
+
+
+PATH_CONSTS = (1e-6, 1e-6, 1e-6, 5e-7)       # C1, C2, C, D of the path rows
+
+
 def measure_paths(torch, binding, steps, warmup, device, use_graph, rows=PATH_ROWS, pairs=4):
     """One row per kernel path beyond the power-of-two fp32 one: `pairs` distinct pairs per step through
     iqa_fused_batch_2d_typed (one launch of any_kernel, or `pairs` launches of a generic kernel), Eqs. 3-4 included.
     GB/s on each path's OWN algorithmic bytes: 2 sizeof(pixel) per pixel pair + 16 B per tile."""
     out = {}
-    k = (1e-6, 1e-6, 1e-6, 5e-7)
-    for name, dtype, H, W, pitch, off, N_T in rows:
+    k = PATH_CONSTS
+    for row in rows:
+        name, dtype, H, W, pitch, off, N_T = row
         dt = getattr(torch, dtype)
         es = torch.empty((), dtype=dt).element_size()
-        g = torch.Generator(device=device).manual_seed(len(name) + N_T)
-        imgs = []
-        for _ in range(2 * pairs):
-            buf = torch.empty(H * pitch + 64, dtype=dt, device=device)
-            if dt.is_floating_point:
-                buf.copy_(torch.randn(buf.shape, generator=g, device=device, dtype=torch.float32) * 1e-3 + 2e-4)
-            else:
-                buf.copy_(torch.randint(-20 if dt != torch.uint8 else 0, 200, buf.shape, generator=g, device=device,
-                                        dtype=torch.int32))
-            imgs.append(torch.as_strided(buf, (H, W), (pitch, 1), off))
-        xs, ys = imgs[0::2], imgs[1::2]
+        xs, ys = make_path_inputs(torch, row, pairs, device)
         nty, ntx = -(-H // N_T), -(-W // N_T)
         n = nty * ntx
         o = [torch.empty((pairs, n), dtype=torch.float32, device=device) for _ in range(4)]
@@ -537,7 +551,7 @@ def measure_paths(torch, binding, steps, warmup, device, use_graph, rows=PATH_RO
                      "base_offset_bytes": off * es, "N_T": N_T, "pairs_per_step": pairs, "us_per_pair": us,
                      "algorithmic_bytes_per_pair": alg, "GBps": gbs, "frac_of_nominal_8000": gbs / 8000.0,
                      "clocks": clk.summary()}
-        del imgs, xs, ys, o, ws
+        del xs, ys, o, ws
         torch.cuda.empty_cache()
     return out
 

@@ -145,3 +145,38 @@ def test_n32768_sampled_tiles(B, U):
         rows = img.clamp_min(0).view(nt, N_T * N).sum(dim=1, dtype=torch.float64)
         got = out[name].sum(dim=1, dtype=torch.float64)
         assert torch.all((got - rows).abs() <= 1e-6 * rows.abs()), name
+
+
+def _path_rows():
+    import bench
+    return bench.PATH_ROWS
+
+
+@pytest.mark.parametrize("row", _path_rows(), ids=[r[0] for r in _path_rows()])
+def test_bench_path_rows_at_full_size(B, U, row):
+    """The `also.paths` rows of bench.py (any_kernel on odd tile sides / other pixel types / unaligned bases, the generic
+    kernels on odd pitches) at the size and in the launch configuration bench.py times -- one iqa_fused_batch_2d_typed
+    call over 4 pairs of 8192 x 8192 windows -- against the oracle: EVERY tile and the whole-image pair of the first and
+    the last pair, on the same seeded device buffers copied to the host."""
+    import torch
+    import bench
+    import oracle
+    name, dtype, H, W, pitch, off, N_T = row
+    pairs = 4
+    xs, ys = bench.make_path_inputs(torch, row, pairs, "cuda")
+    expect = "generic" if name.startswith("generic") else "tma_any"
+    assert B.plan_name(xs[0], N_T) == expect, (name, B.plan_name(xs[0], N_T))
+    C1, C2, C, D = bench.PATH_CONSTS
+    out = B.fused_batch_2d(xs, ys, N_T, C1, C2, C, D, numerators=True, aggregate=True)
+    torch.cuda.synchronize()
+    whole = out["whole"].cpu().numpy().astype(np.float64)
+    for i in (0, pairs - 1):
+        x, y = xs[i].cpu().numpy(), ys[i].cpu().numpy()
+        ref = oracle.tiles_2d_any(x, y, N_T, C1, C2, C, D)
+        got = {n: out[n][i].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+        U.assert_parity(got, ref, C, f"{name} pair {i}")
+        exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], C2, C)
+        assert abs(whole[i, 0] - exp[0]) <= 1e-5 * abs(exp[0]) and abs(whole[i, 1] - exp[1]) <= 1e-5 * abs(exp[1]), (name, i)
+        del x, y, ref
+    del xs, ys, out
+    torch.cuda.empty_cache()
