@@ -128,6 +128,7 @@ int iqa_query_plan(const void* x, int pixel_type, int H, int W, long long pitch,
  *   IQA_TMA_CONFIG 0..4: tma_kernel ring / box configuration (-1: default)
  *   IQA_TMA_MAX_CTAS n: cap of the persistent grid (0: none)     IQA_NO_PDL 1: no programmatic dependent launch
  *   IQA_CAND_NO_CLUSTER 1: candidate kernels without thread-block clusters
+ *   IQA_ANY_NO_WIDE 1: any_kernel lanes own four columns even when eight would fit
  * They select among kernels that all satisfy the same parity bar (tests/test_gpu_parity.py runs every one). */
 int iqa_debug_knob(const char* name, int value);
 

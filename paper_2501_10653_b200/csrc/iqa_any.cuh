@@ -25,7 +25,10 @@
 //            for 4- / 2- / 1- / 8-byte pixels): 16 accumulators, the packed-pair arithmetic of
 //            pixel_terms2, no mask and no shift in the pixel loop -- the offset s only enters when the
 //            lane's four column sums are assigned to tiles at the end of the item;
-//            fp64 and int32 form x + y and |x - y| exactly before rounding to fp32
+//            fp64 and int32 form x + y and |x - y| exactly before rounding to fp32.
+//            When N_T is a multiple of 8 and the bases are 16-byte aligned, a lane owns EIGHT columns
+//            (8l .. 8l+7, all in one tile) and folds columns j and j + 4 into the same accumulator:
+//            boxes of up to 256 columns, twice the pixels per item for the same per-item bookkeeping
 //   warp     warp w owns rows [w rpw, (w+1) rpw) of a box (ky == 1), or rows of tile row w / wpt
 //            (ky > 1: several tile rows per box, wpt = 8 / ky warps each)
 //   reduce   per item: every lane folds its 4 columns into the partial of the tile its FIRST column
@@ -60,7 +63,7 @@ struct AnyParams {
     int ntx, nty, n_tiles;
     int kx, ky;            // whole tiles per item across / down (1, 1 when tiles are split)
     int px, py;            // pieces per tile across / down (1, 1 unless split)
-    int pw, ph;            // item extent: columns (pw + s <= box_w <= 128), rows
+    int pw, ph;            // item extent: columns (pw + s <= box_w <= 32 lanes x 4 or 8 columns), rows
     int units_x, units_y;  // items across / down
     int box_rows;          // b
     int row_bytes;         // bytes between two box rows in shared memory (box_w * sizeof(T), multiple of 16)
@@ -68,6 +71,7 @@ struct AnyParams {
     int n_slots;           // even, 4 .. kAnyMaxSlots
     int rpw, wpt;          // rows per warp inside a box (or inside a tile when ky > 1); warps per tile row
     int fin_gsz;           // finaliser lanes per tile: max(1, 32 / pow2ceil(kx * ky))
+    int cpl_log2;          // log2 of the columns a lane owns: 2 (four) or 3 (eight: N_T % 8 == 0, every base 16-byte aligned)
     int boxes_per_item;    // ceil(ph / box_rows)
     unsigned nt_magic;     // floor(2^32 / N_T) + 1: n / N_T == umulhi(n, nt_magic) for the small n used here
     float C1, C2, C, D;
@@ -266,6 +270,16 @@ __device__ __forceinline__ float4 acc_cols(const Acc16& a, int lo, int hi) {
                        col_sum(x0, x1, x2, x3, lo, hi), col_sum(y0, y1, y2, y3, lo, hi));
 }
 
+// All four columns: (c0 + c1) + (c2 + c3), the order of col_sum.
+__device__ __forceinline__ float4 acc_cols(const Acc16& a) {
+    float l0, l1, l2, l3, x0, x1, x2, x3, y0, y1, y2, y3;
+    unpack2(a.L[0], l0, l1); unpack2(a.L[1], l2, l3);
+    unpack2(a.X[0], x0, x1); unpack2(a.X[1], x2, x3);
+    unpack2(a.Y[0], y0, y1); unpack2(a.Y[1], y2, y3);
+    return make_float4((l0 + l1) + (l2 + l3), (a.A[0] + a.A[1]) + (a.A[2] + a.A[3]), (x0 + x1) + (x2 + x3),
+                       (y0 + y1) + (y2 + y3));
+}
+
 template <int MODE, typename T>
 __global__ void __launch_bounds__(kTmaThreads, 2)
 any_kernel(const __grid_constant__ AnyParams p) {
@@ -353,8 +367,9 @@ any_kernel(const __grid_constant__ AnyParams p) {
                 if (!active) jy = jx = 0;
                 // lanes whose FIRST valid column lies in tile column jx (the columns a lane holds of the next tile
                 // were moved one lane up by the consumers); the item's column c is box column c + s
-                const int la = (split || jx == 0) ? it.s >> 2 : (jx * p.N_T + it.s + 3) >> 2;
-                const int lb = split ? (it.cv + it.s + 3) >> 2 : ((jx + 1) * p.N_T + it.s + 3) >> 2;
+                const int cl = p.cpl_log2, cr = (1 << cl) - 1;         // a lane owns 4 or 8 box columns
+                const int la = (split || jx == 0) ? it.s >> cl : (jx * p.N_T + it.s + cr) >> cl;
+                const int lb = split ? (it.cv + it.s + cr) >> cl : ((jx + 1) * p.N_T + it.s + cr) >> cl;
                 const int w0 = p.ky > 1 ? jy * p.wpt : 0;
                 float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (active) {
@@ -423,8 +438,13 @@ any_kernel(const __grid_constant__ AnyParams p) {
         j_cb = split ? 4 : max(0, min(4, (t + 1) * p.N_T - c));
     };
     if (fixed) lane_columns(p.shift, p.pw);
-    // lanes past the box re-read its last 16-byte chunk (their columns are masked at the end)
-    const unsigned char* my_base = base + min(lane * Pixel4<T>::kBytes, row_bytes - Pixel4<T>::kBytes);
+    // every lane holds either four columns of ONE tile or none of the item: nothing to mask (lanes outside the item
+    // are never read by the finaliser)
+    const bool wide = p.cpl_log2 == 3;                         // eight columns per lane (host: fixed, N_T % 8 == 0, s == 0)
+    const bool whole_lanes = wide || (fixed && (p.N_T & 3) == 0 && (p.shift & 3) == 0);
+    // lanes past the box re-read its last chunk (their columns are masked at the end / never read by the finaliser)
+    const int lane_bytes = Pixel4<T>::kBytes << (p.cpl_log2 - 2);
+    const unsigned char* my_base = base + min(lane * lane_bytes, row_bytes - lane_bytes);
     const int boxes_full = p.boxes_per_item;                   // boxes of an item with all ph rows
     int buf = 0;
     uint32_t part_phase = 0u;
@@ -450,26 +470,43 @@ any_kernel(const __grid_constant__ AnyParams p) {
             int nr = min(row_hi, bx.hi) - ra;
             const unsigned char* xr = my_base + (size_t)xs * slot_bytes + (size_t)ra * row_bytes;
             const unsigned char* yr = my_base + (size_t)ys * slot_bytes + (size_t)ra * row_bytes;
+            if (!wide) {
 #pragma unroll 1
-            for (; nr >= 4; nr -= 4) {
+                for (; nr >= 4; nr -= 4) {
 #pragma unroll
-                for (int k = 0; k < 4; ++k) Pixel4<T>::template row<MODE>(xr + k * row_bytes, yr + k * row_bytes, C1, acc);
-                xr += 4 * row_bytes;
-                yr += 4 * row_bytes;
+                    for (int k = 0; k < 4; ++k) Pixel4<T>::template row<MODE>(xr + k * row_bytes, yr + k * row_bytes, C1, acc);
+                    xr += 4 * row_bytes;
+                    yr += 4 * row_bytes;
+                }
+                if (nr >= 2) {
+                    Pixel4<T>::template row<MODE>(xr, yr, C1, acc);
+                    Pixel4<T>::template row<MODE>(xr + row_bytes, yr + row_bytes, C1, acc);
+                    xr += 2 * row_bytes;
+                    yr += 2 * row_bytes;
+                    nr -= 2;
+                }
+                if (nr >= 1) Pixel4<T>::template row<MODE>(xr, yr, C1, acc);
+            } else {                                               // columns j and j + 4 of the lane share accumulator j
+                constexpr int kHalf = Pixel4<T>::kBytes;
+#pragma unroll 1
+                for (; nr >= 2; nr -= 2) {
+                    Pixel4<T>::template row<MODE>(xr, yr, C1, acc);
+                    Pixel4<T>::template row<MODE>(xr + kHalf, yr + kHalf, C1, acc);
+                    Pixel4<T>::template row<MODE>(xr + row_bytes, yr + row_bytes, C1, acc);
+                    Pixel4<T>::template row<MODE>(xr + row_bytes + kHalf, yr + row_bytes + kHalf, C1, acc);
+                    xr += 2 * row_bytes;
+                    yr += 2 * row_bytes;
+                }
+                if (nr >= 1) {
+                    Pixel4<T>::template row<MODE>(xr, yr, C1, acc);
+                    Pixel4<T>::template row<MODE>(xr + kHalf, yr + kHalf, C1, acc);
+                }
             }
-            if (nr >= 2) {
-                Pixel4<T>::template row<MODE>(xr, yr, C1, acc);
-                Pixel4<T>::template row<MODE>(xr + row_bytes, yr + row_bytes, C1, acc);
-                xr += 2 * row_bytes;
-                yr += 2 * row_bytes;
-                nr -= 2;
-            }
-            if (nr >= 1) Pixel4<T>::template row<MODE>(xr, yr, C1, acc);
             __syncwarp();
             if (lane == 0) { mbar_arrive(empty_u32 + 8u * xs); mbar_arrive(empty_u32 + 8u * ys); }
         }
         // lane -> (warp, lane) partial of the tile of its first valid column
-        float4 v = acc_cols(acc, j_lo, min(j_cb, j_end));
+        float4 v = whole_lanes ? acc_cols(acc) : acc_cols(acc, j_lo, min(j_cb, j_end));
         if (straddle) {
             const float4 h = acc_cols(acc, max(j_cb, j_lo), j_end);    // columns of the NEXT tile: one lane up
             const float hx = __shfl_up_sync(0xffffffffu, h.x, 1), hy = __shfl_up_sync(0xffffffffu, h.y, 1);

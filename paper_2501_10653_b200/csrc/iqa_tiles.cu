@@ -47,10 +47,12 @@ bool pos_normal(float v) { return std::isfinite(v) && v >= FLT_MIN; }
 //   IQA_TMA_MAX_CTAS     cap of the persistent grid (0: none)
 //   IQA_NO_PDL           1: launch without programmatic dependent launch
 //   IQA_CAND_NO_CLUSTER  1: candidate kernels never use the cluster twins
-enum Knob { kKnobForceGeneric, kKnobForceAny, kKnobTmaConfig, kKnobTmaMaxCtas, kKnobNoPdl, kKnobCandNoCluster, kNumKnobs };
+//   IQA_ANY_NO_WIDE      1: any_kernel never lets a lane own eight columns
+enum Knob { kKnobForceGeneric, kKnobForceAny, kKnobTmaConfig, kKnobTmaMaxCtas, kKnobNoPdl, kKnobCandNoCluster, kKnobNoWide,
+            kNumKnobs };
 const char* const kKnobNames[kNumKnobs] = {"IQA_FORCE_GENERIC", "IQA_FORCE_ANY", "IQA_TMA_CONFIG", "IQA_TMA_MAX_CTAS",
-                                           "IQA_NO_PDL", "IQA_CAND_NO_CLUSTER"};
-const int kKnobDefaults[kNumKnobs] = {0, 0, -1, 0, 0, 0};
+                                           "IQA_NO_PDL", "IQA_CAND_NO_CLUSTER", "IQA_ANY_NO_WIDE"};
+const int kKnobDefaults[kNumKnobs] = {0, 0, -1, 0, 0, 0, 0};
 struct Knobs {
     std::atomic<int> v[kNumKnobs];
     Knobs() {
@@ -266,6 +268,7 @@ Geom square_geom(int N) { return Geom{N, N, (long long)N, (long long)N, IQA_PIXE
 struct AnyGeom {
     int kx, ky, px, py, pw, ph, box_w, box_rows, row_bytes, slot_bytes, n_slots, rpw, wpt, fin_gsz, units_x, units_y;
     int const_s;       // every item sits at the same column offset inside its box
+    int cpl_log2;      // columns per lane: 2 -> four, 3 -> eight
 };
 constexpr int kAnySplitAbove = 112;   // tiles wider than this are split (128 lanes-columns minus the widest 16-byte pad)
 // Pieces per split tile (N_T > kAnySplitAbove): pw x 64 pixels each, pw a multiple of 16 columns; the same for every
@@ -282,6 +285,7 @@ AnyGeom any_geometry(int esize, int N_T, int H, int W, int shift) {
     const int pad = 16 / esize;                       // elements per 16 bytes: a TMA box starts at a multiple of it
     const int wpad = pad < 4 ? 4 : pad;               // box widths are whole lanes (4 columns) as well
     const int ntx = ceil_div(W, N_T), nty = ceil_div(H, N_T);
+    g.cpl_log2 = 2;
     if (N_T <= kAnySplitAbove) {                      // whole tiles inside one item: kx across, ky down
         // kx_a: items that start on 16-byte boundaries (s = 0 everywhere); kx_s: items at any column, which costs
         // pad - 1 columns of the box
@@ -292,7 +296,19 @@ AnyGeom any_geometry(int esize, int N_T, int H, int W, int shift) {
         int kx_s = (kUnitCols - pad + 1) / N_T;
         if (kx_a > ntx) kx_a = ntx;
         if (kx_s > ntx) kx_s = ntx;
-        if (kx_a > 0 && kx_a * 8 >= kx_s * 7) {
+        // kx_w: eight columns per lane (boxes of up to 256 columns): every lane inside one tile, items on 16-byte
+        // boundaries.  Twice the pixels per item, and tile sides such as 48 fill 30 of 32 lanes instead of 24.
+        int kx_w = 0;
+        if (shift == 0 && N_T % 8 == 0 && esize <= 4 && !knob(kKnobNoWide))     // (fp64: 64 bytes per lane and row: slower)
+            for (int k = 2 * kUnitCols / N_T; k >= 1; --k)
+                if ((k * N_T) % pad == 0) { kx_w = k; break; }
+        if (kx_w > ntx) kx_w = ntx;
+        if (kx_w > 0 && kx_w * N_T > kUnitCols) {
+            g.kx = kx_w;
+            g.const_s = 1;
+            g.cpl_log2 = 3;
+            g.box_w = g.kx * N_T;
+        } else if (kx_a > 0 && kx_a * 8 >= kx_s * 7) {
             g.kx = kx_a;
             g.const_s = 1;
             g.box_w = round_up(g.kx * N_T, wpad);
@@ -541,6 +557,7 @@ bool prepare_any(std::vector<AnyLaunch>& q, int mode, const void* const* xs, con
         p.kx = a.kx; p.ky = a.ky; p.px = a.px; p.py = a.py; p.pw = a.pw; p.ph = a.ph;
         p.units_x = a.units_x; p.units_y = a.units_y; p.box_rows = a.box_rows; p.row_bytes = a.row_bytes;
         p.slot_bytes = a.slot_bytes; p.n_slots = a.n_slots; p.rpw = a.rpw; p.wpt = a.wpt; p.fin_gsz = a.fin_gsz;
+        p.cpl_log2 = a.cpl_log2;
         p.boxes_per_item = ceil_div(a.ph, a.box_rows);
         p.nt_magic = (unsigned)(0x100000000ull / (unsigned)N_T) + 1u;
         p.C1 = k.C1; p.C2 = k.C2; p.C = k.C; p.D = k.D;

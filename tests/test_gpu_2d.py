@@ -322,6 +322,9 @@ def test_any_kernel_pixel_types(B, U, dtype, H, W, N_T):
     for off in (0, 1, per16 - 1) if per16 > 2 else (0, 1):
         xd, yd = _typed_window(x, pitch, off), _typed_window(y, pitch + per16, off)
         _check_typed(B, U, x, y, xd, yd, N_T, k, f"any {dtype} {H}x{W} N_T={N_T} off={off}")
+    with B.knob("IQA_ANY_NO_WIDE", 1):          # four columns per lane also where eight would fit (N_T % 8 == 0, aligned)
+        xd, yd = _typed_window(x, pitch, 0), _typed_window(y, pitch + per16, 0)
+        _check_typed(B, U, x, y, xd, yd, N_T, k, f"any {dtype} {H}x{W} N_T={N_T} narrow lanes")
 
 
 def test_any_kernel_matches_tma_kernel_on_power_of_two_tiles(B, U):
@@ -335,9 +338,12 @@ def test_any_kernel_matches_tma_kernel_on_power_of_two_tiles(B, U):
         a = B.fused_tiles_2d(xd, yd, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
         with B.knob("IQA_FORCE_ANY", 1):
             assert B.plan_name(xd, N_T) == "tma_any"
-            b, _ = _check_typed(B, U, x, y, xd, yd, N_T, k, f"forced any N_T={N_T}")
+            b, _ = _check_typed(B, U, x, y, xd, yd, N_T, k, f"forced any N_T={N_T}")          # eight columns per lane
+            with B.knob("IQA_ANY_NO_WIDE", 1):
+                c, _ = _check_typed(B, U, x, y, xd, yd, N_T, k, f"forced any, narrow lanes, N_T={N_T}")
         for n in a:
             assert torch.all((a[n] - b[n]).abs() <= 2e-6 * a[n].abs() + 1e-30), (N_T, n)
+            assert torch.all((a[n] - c[n]).abs() <= 2e-6 * a[n].abs() + 1e-30), (N_T, n)
 
 
 @pytest.mark.parametrize("dtype,N_T", [("float32", 100), ("int16", 64), ("float64", 48), ("uint8", 150)])
