@@ -810,7 +810,7 @@ const char* iqa_status_string(int status) {
     }
 }
 
-const char* iqa_version(void) { return "0.5.0"; }
+const char* iqa_version(void) { return "0.6.0"; }
 
 int iqa_debug_knob(const char* name, int value) {
     if (!name) return -1;

@@ -7,7 +7,7 @@
 // warp issues cp.async.bulk.tensor.2d (SASS UTMALDG) for BOXES of 128 columns x 8 RPW rows
 // (RPW = 4: 32 rows, 16 KiB) straight into shared memory; completion is signalled on an mbarrier per box
 // ("full"), the eight consumer warps give a box back through a second mbarrier ("empty").
-// Against a per-thread cp.async ring (the first version of this kernel, profiles/r01d_variants.md)
+// Against a per-thread cp.async ring (the first version of this kernel, round 1)
 // this removes every address computation and 8 LDGSTS per thread and stage from the instruction
 // stream (that kernel spent ~19.5 instructions per pixel pair, ~10.5 of them arithmetic), which is what
 // the time-series modes need: they halve the HBM bytes per comparison, so the instruction
