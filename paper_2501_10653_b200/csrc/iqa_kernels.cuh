@@ -166,7 +166,8 @@ __device__ __forceinline__ void finalise_tile(const Params& p, size_t t, float4 
 // partial goes to the workspace and finalise_kernel finishes.
 // -----------------------------------------------------------------------------
 constexpr int kGenericRows = 64;
-constexpr int kGenericInFlight = 8;      // pixel pairs a thread loads before it computes
+constexpr int kGenericInFlight = 4;      // generic_kernel: rows whose loads a thread issues before it computes
+constexpr int kWarpInFlight = 8;         // generic_warp_kernel: pixel pairs a lane loads before it computes
 
 struct GenericParams {
     TileParams tp;
@@ -194,31 +195,25 @@ generic_kernel(const GenericParams g) {
 
     float aL = 0.f, aA = 0.f, aX = 0.f, aY = 0.f;
     // warp w takes rows w, w + 8, ...; lanes stride over the columns (coalesced, no division per pixel).  The loads
-    // of kGenericInFlight pixels of both images are issued before the first term is computed: a lone scalar load per
+    // of kGenericInFlight rows of both images are issued before the first term is computed: a lone scalar load per
     // thread would leave the kernel waiting on the latency of each one.
     (void)npix;
-    const T* xp = reinterpret_cast<const T*>(p.x);
-    const T* yp = reinterpret_cast<const T*>(p.y);
-    const int lane = (int)(threadIdx.x & 31);
-    const int cpl = (cols_t - lane + 31) >> 5;                 // columns of this lane per row (may be 0)
-    const int rows_w = (r_end - r_begin - (int)(threadIdx.x >> 5) + kWarpsPerCta - 1) / kWarpsPerCta;   // rows of this warp
-    const int n_mine = rows_w > 0 ? rows_w * cpl : 0;          // pixels of this thread: k -> (row k / cpl, column k % cpl)
-    int kr = 0, kc = 0;                                        // row / column counters of the next pixel to load
-    for (int k0 = 0; k0 < n_mine; k0 += kGenericInFlight) {
-        T vx[kGenericInFlight], vy[kGenericInFlight];
+    const int lane = (int)(threadIdx.x & 31), w = (int)(threadIdx.x >> 5);
+    const int nrows = r_end - r_begin;
+    const size_t sx = (size_t)kWarpsPerCta * (size_t)p.pitch_x, sy = (size_t)kWarpsPerCta * (size_t)p.pitch_y;
+    const T* xrow = reinterpret_cast<const T*>(p.x) + (row0 + w) * (size_t)p.pitch_x + col0;     // row w of the piece
+    const T* yrow = reinterpret_cast<const T*>(p.y) + (row0 + w) * (size_t)p.pitch_y + col0;
+    for (int r = w; r < nrows; r += kWarpsPerCta * kGenericInFlight, xrow += kGenericInFlight * sx, yrow += kGenericInFlight * sy) {
+        const int nr = min(kGenericInFlight, (nrows - r + kWarpsPerCta - 1) / kWarpsPerCta);   // rows r, r + 8, ... of this round
+        for (int c = lane; c < cols_t; c += 32) {
+            T vx[kGenericInFlight], vy[kGenericInFlight];
 #pragma unroll
-        for (int u = 0; u < kGenericInFlight; ++u) {
-            if (k0 + u < n_mine) {
-                const size_t r = row0 + (threadIdx.x >> 5) + (size_t)kr * kWarpsPerCta;
-                const size_t c = col0 + lane + (size_t)kc * 32;
-                vx[u] = xp[r * (size_t)p.pitch_x + c];
-                vy[u] = yp[r * (size_t)p.pitch_y + c];
-                if (++kc == cpl) { kc = 0; ++kr; }
-            }
+            for (int u = 0; u < kGenericInFlight; ++u)
+                if (u < nr) { vx[u] = xrow[u * sx + c]; vy[u] = yrow[u * sy + c]; }
+#pragma unroll
+            for (int u = 0; u < kGenericInFlight; ++u)
+                if (u < nr) pixel_terms_val<MODE, T>(vx[u], vy[u], p.C1, aL, aA, aX, aY);
         }
-#pragma unroll
-        for (int u = 0; u < kGenericInFlight; ++u)
-            if (k0 + u < n_mine) pixel_terms_val<MODE, T>(vx[u], vy[u], p.C1, aL, aA, aX, aY);
     }
     float4 v = make_float4(aL, aA, aX, aY);
     for (int o = 16; o > 0; o >>= 1) {
@@ -260,15 +255,15 @@ generic_warp_kernel(const GenericParams g, long long n_tiles) {
     const size_t row0 = (size_t)ty * N_T, col0 = (size_t)tx * N_T;
     float aL = 0.f, aA = 0.f, aX = 0.f, aY = 0.f;
     // lanes stride over the tile's pixels in row-major order; (row, column) advance by additions, and the loads of
-    // kGenericInFlight pixels of both images are issued before the first term is computed
+    // kWarpInFlight pixels of both images are issued before the first term is computed
     const T* xp = reinterpret_cast<const T*>(p.x);
     const T* yp = reinterpret_cast<const T*>(p.y);
     int r = lane / cols_t, c = lane - r * cols_t;
     const int dr = 32 / cols_t, dc = 32 - dr * cols_t;
-    for (int k0 = lane; k0 < npix; k0 += 32 * kGenericInFlight) {
-        T vx[kGenericInFlight], vy[kGenericInFlight];
+    for (int k0 = lane; k0 < npix; k0 += 32 * kWarpInFlight) {
+        T vx[kWarpInFlight], vy[kWarpInFlight];
 #pragma unroll
-        for (int u = 0; u < kGenericInFlight; ++u) {
+        for (int u = 0; u < kWarpInFlight; ++u) {
             if (k0 + 32 * u < npix) {
                 vx[u] = xp[(row0 + r) * (size_t)p.pitch_x + col0 + c];
                 vy[u] = yp[(row0 + r) * (size_t)p.pitch_y + col0 + c];
@@ -277,7 +272,7 @@ generic_warp_kernel(const GenericParams g, long long n_tiles) {
             }
         }
 #pragma unroll
-        for (int u = 0; u < kGenericInFlight; ++u)
+        for (int u = 0; u < kWarpInFlight; ++u)
             if (k0 + 32 * u < npix) pixel_terms_val<MODE, T>(vx[u], vy[u], p.C1, aL, aA, aX, aY);
     }
     float4 v = make_float4(aL, aA, aX, aY);
