@@ -605,10 +605,33 @@ def measure_series(torch, binding, cfg, M, steps, warmup, device, use_graph):
     cand = {}
     for name, fn in (("bottom_16", lambda: binding.iqa_tiles_bottom_k(aug3, n, K, 16, idx, None, st())),
                      ("below_1pct_quantile", lambda: binding.iqa_tiles_below(aug3, n, K, thr, cap, 1024, cnt, st()))):
+        def ten(fn=fn):
+            for _ in range(10):
+                assert fn() == 0
+        run = graph_of(torch, ten) if use_graph else ten
         for _ in range(3):
-            assert fn() == 0
-        cand[name + "_us_per_call"] = time_region(torch, lambda: [fn() for _ in range(10)], 5) * 1e3 / 50
-    res["candidates"] = dict(cand, maps=K, tiles_per_map=n)
+            run()
+        cand[name + "_us_per_call"] = time_region(torch, run, 5) * 1e3 / 50
+    # the finder in one call (iqa_series_find): what the bottom-16 list + the threshold list ADD to the series call
+    bval = torch.empty((K, 16), dtype=torch.float32, device=device)
+    mode = binding.SERIES_MODES["consecutive"]
+
+    def find_step():
+        rc = binding.iqa_series_find(table, M, mode, cfg.N, cfg.N_T, *k, *outs, None, None, out2, ws, wsb,
+                                     binding.IQA_FIND_AUGLISI, 16, idx, bval, thr, cap, 1024, cnt,
+                                     torch.cuda.current_stream().cuda_stream)
+        if rc:
+            raise binding.IqaError(rc, "iqa_series_find")
+    ffn = graph_of(torch, find_step) if use_graph else find_step
+    for _ in range(warmup):
+        ffn()
+    us_find = time_region(torch, ffn, steps) * 1e3 / steps
+    cand["series_find_us_per_call"] = us_find
+    cand["series_find_adds_us_per_call"] = us_find - res["consecutive"]["us_per_call"]
+    res["candidates"] = dict(cand, maps=K, tiles_per_map=n,
+                             what="bottom_16 / below: stand-alone calls, 10 back to back (in one CUDA graph unless --no-graph); series_find: "
+                                  "iqa_series_find (consecutive mode, bottom-16 + threshold list of the augLISI matrices) "
+                                  "timed like the series rows; adds = its time minus the consecutive row's")
     res.update({"images": M, "comparisons": K, "N": cfg.N, "N_T": cfg.N_T,
                 "l2": f"{M * 4 * cfg.N * cfg.N / 2**20:.0f} MiB of snapshots per call"})
     del imgs, outs

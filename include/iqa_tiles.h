@@ -298,6 +298,25 @@ int iqa_tiles_below(const float* values, int n_tiles, int n_maps, float threshol
 int iqa_tiles_bottom_k(const float* values, int n_tiles, int n_maps, int k,
                        int* indices, float* vals, void* stream);
 
+/* iqa_series_find: the finder in ONE call (SURVEY.md 8(f)-2 + 8(f)-3) -- iqa_series_tiles followed,
+ * on the same stream and inside the same call, by the candidate lists of every comparison taken from ONE of the two
+ * matrices (`index`: IQA_FIND_LISI or IQA_FIND_AUGLISI).  The candidate kernels are launched behind the tile kernel
+ * with programmatic dependent launch, so a caller pays no second call and no host round trip; the lists are
+ * exactly those of iqa_tiles_bottom_k / iqa_tiles_below on that matrix.
+ *   arguments up to `stream`   as iqa_series_tiles (K = n_images - 1 comparisons of n tiles)
+ *   k, bottom_idx [K * k], bottom_val [K * k] (MAY BE NULL)   k = 0: no bottom-k list (bottom_idx may then be NULL)
+ *   below_idx [K * capacity], below_counts [K]                 below_counts NULL: no threshold list
+ * Either list may be left out, not both (IQA_ERR_NULL). */
+#define IQA_FIND_LISI 0
+#define IQA_FIND_AUGLISI 1
+int iqa_series_find(const float* const* img_ptrs_host, int n_images, int mode,
+                    int N, int N_T, float C1, float C2, float C, float D,
+                    float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                    float* lisi_num, float* auglisi_num, float* out2,
+                    void* workspace, size_t workspace_bytes,
+                    int index, int k, int* bottom_idx, float* bottom_val,
+                    float threshold, int* below_idx, int capacity, int* below_counts, void* stream);
+
 /* P:66 "a larger tile formed by merging smaller ones": apply Eqs. 3-4 to every g x g block
  * of an nt x nt tile matrix, giving the (nt/g) x (nt/g) matrices of tile size g*N_T.
  *   in:  lisi, auglisi, sum_x, sum_y  [nt*nt]

@@ -53,14 +53,95 @@ __device__ __forceinline__ int block_exclusive_scan(int c, int* warp_tot, int& t
     __syncthreads();                                        // previous use of warp_tot is over
     if (lane == 31) warp_tot[w] = inc;
     __syncthreads();
-    int base = 0, tot = 0;
-    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) {
-        const int t = warp_tot[i];
-        if (i < w) base += t;
-        tot += t;
+    // every warp scans the (at most 32) warp totals itself: lane l holds warp l's total
+    const int nw = (int)(blockDim.x >> 5);
+    const int t = lane < nw ? warp_tot[lane] : 0;
+    int tinc = t;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int q = __shfl_up_sync(0xffffffffu, tinc, o);
+        if (lane >= o) tinc += q;
     }
-    total = tot;
+    total = __shfl_sync(0xffffffffu, tinc, 31);
+    const int base = __shfl_sync(0xffffffffu, tinc - t, w);
     return base + inc - c;
+}
+
+// The kCandPerThread = 16 consecutive values [i0, i0 + 16) of a matrix of n values; positions >= n read as `fill`.
+// Four 128-bit loads when the run is whole and 16-byte aligned (a warp then touches 2 KiB with 4 instructions instead of 16).
+__device__ __forceinline__ void load_run16(const float* __restrict__ v, int i0, int n, float fill, float (&f)[kCandPerThread]) {
+    if (i0 + kCandPerThread <= n && (((uintptr_t)(v + i0)) & 15u) == 0) {
+        const float4* q = reinterpret_cast<const float4*>(v + i0);
+#pragma unroll
+        for (int j = 0; j < kCandPerThread / 4; ++j) {
+            const float4 a = __ldg(q + j);
+            f[4 * j] = a.x; f[4 * j + 1] = a.y; f[4 * j + 2] = a.z; f[4 * j + 3] = a.w;
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < kCandPerThread; ++j) f[j] = i0 + j < n ? v[i0 + j] : fill;
+    }
+}
+
+// ---- 64-bit (order key, tile index) pairs: unique, and their unsigned order is the (value, index) order -------------
+__device__ __forceinline__ unsigned long long key64(uint32_t u, int idx) { return ((unsigned long long)u << 32) | (uint32_t)idx; }
+__device__ __forceinline__ unsigned long long umin64(unsigned long long a, unsigned long long b) { return a < b ? a : b; }
+__device__ __forceinline__ unsigned long long umax64(unsigned long long a, unsigned long long b) { return a < b ? b : a; }
+// One key per lane -> ascending by lane (bitonic network over shuffles, 15 compare-exchange steps).
+__device__ __forceinline__ unsigned long long warp_sort32(unsigned long long x, int lane) {
+#pragma unroll
+    for (int size = 2; size <= 32; size <<= 1)
+#pragma unroll
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            const unsigned long long y = __shfl_xor_sync(0xffffffffu, x, stride);
+            const bool keep_min = ((lane & stride) == 0) == ((lane & size) == 0);
+            x = keep_min ? umin64(x, y) : umax64(x, y);
+        }
+    return x;
+}
+// x: this warp's ascending list (one key per lane); other_rev: lane i holds element 31 - i of another ascending list.
+// Returns the 32 smallest of the 64 keys, ascending by lane (bitonic merge).
+__device__ __forceinline__ unsigned long long warp_merge_low32(unsigned long long x, unsigned long long other_rev, int lane) {
+    x = umin64(x, other_rev);
+#pragma unroll
+    for (int stride = 16; stride > 0; stride >>= 1) {
+        const unsigned long long y = __shfl_xor_sync(0xffffffffu, x, stride);
+        x = (lane & stride) == 0 ? umin64(x, y) : umax64(x, y);
+    }
+    return x;
+}
+// Ascending bitonic sort of keys[0, P) in shared memory, P a power of two: by the first warp alone when P <= 64 (no CTA
+// barrier per step), by the whole CTA otherwise.  Ends with a CTA barrier.
+__device__ __forceinline__ void sort_keys_shared(unsigned long long* keys, int P) {
+    const int tid = threadIdx.x;
+    if (P <= 64) {
+        if (tid < 32) {
+            for (int size = 2; size <= P; size <<= 1)
+                for (int stride = size >> 1; stride > 0; stride >>= 1) {
+                    for (int i = tid; i < P / 2; i += 32) {
+                        const int lo = 2 * i - (i & (stride - 1));
+                        const int hi = lo + stride;
+                        const bool up = (lo & size) == 0;
+                        const unsigned long long a = keys[lo], b = keys[hi];
+                        if ((a > b) == up) { keys[lo] = b; keys[hi] = a; }
+                    }
+                    __syncwarp();
+                }
+        }
+        __syncthreads();
+        return;
+    }
+    for (int size = 2; size <= P; size <<= 1)
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            for (int i = tid; i < P / 2; i += (int)blockDim.x) {
+                const int lo = 2 * i - (i & (stride - 1));  // index with the `stride` bit clear
+                const int hi = lo + stride;
+                const bool up = (lo & size) == 0;
+                const unsigned long long a = keys[lo], b = keys[hi];
+                if ((a > b) == up) { keys[lo] = b; keys[hi] = a; }
+            }
+            __syncthreads();
+        }
 }
 
 // Work layout of both kernels: a SUPER-CHUNK is 16 blockDim.x consecutive tiles (16384 for 1024 threads); thread t
@@ -81,9 +162,11 @@ below_kernel(const float* __restrict__ values, int n, float threshold, int* __re
     for (int c0 = 0; c0 < n; c0 += kCandChunk) {
         const int i0 = c0 + threadIdx.x * kCandPerThread;
         uint32_t flags = 0;
+        float f[kCandPerThread];
+        load_run16(v, i0, n, __int_as_float(0x7f800000), f);             // +Inf is never below a threshold
 #pragma unroll
         for (int j = 0; j < kCandPerThread; ++j)
-            if (i0 + j < n && v[i0 + j] < threshold) flags |= 1u << j;
+            if (f[j] < threshold) flags |= 1u << j;
         int total;
         int pos = base + block_exclusive_scan(__popc(flags), warp_tot, total);
         for (uint32_t f = flags; f; f &= f - 1) {
@@ -98,11 +181,13 @@ below_kernel(const float* __restrict__ values, int n, float threshold, int* __re
 // values [n_maps][n]; indices [n_maps][k], vals [n_maps][k] (nullable).  Entries beyond
 // min(k, n) are filled with index -1 and value +Inf.  k <= kMaxBottomK.
 __global__ void __launch_bounds__(kCandThreads)
-bottom_k_kernel(const float* __restrict__ values, int n, int k, int* __restrict__ indices, float* __restrict__ vals) {
+bottom_k_kernel(const float* __restrict__ values, int n, int k, int* __restrict__ indices, float* __restrict__ vals,
+                float threshold, int* __restrict__ below_idx, int capacity, int* __restrict__ below_counts) {
     __shared__ int hist[256];
     __shared__ int warp_tot[kCandThreads / 32];
     __shared__ uint32_t s_prefix, s_and[kCandThreads / 32], s_or[kCandThreads / 32];
     __shared__ int s_rank;
+    __shared__ unsigned long long s_tau;
     __shared__ unsigned long long keys[kMaxBottomK];
     pdl_prologue();
     const float* v = values + (size_t)blockIdx.x * n;
@@ -111,12 +196,129 @@ bottom_k_kernel(const float* __restrict__ values, int n, int k, int* __restrict_
     const int kCandChunk = (int)blockDim.x * kCandPerThread;
     const bool resident = n <= kCandChunk;                  // the whole matrix sits in registers: read once
     uint32_t u[kCandPerThread];                             // order keys of this thread's tiles of a super-chunk
+    uint32_t below_flags = 0;                               // resident matrices with below_counts: tiles < threshold
     auto load_keys = [&](int c0) {
         const int i0 = c0 + tid * kCandPerThread;
+        float f[kCandPerThread];
+        load_run16(v, i0, n, __int_as_float(0x7fc00000), f);             // NaN: order key 0xffffffff, never below
 #pragma unroll
-        for (int j = 0; j < kCandPerThread; ++j) u[j] = i0 + j < n ? order_key(v[i0 + j]) : 0xffffffffu;
+        for (int j = 0; j < kCandPerThread; ++j) {
+            u[j] = order_key(f[j]);
+            if (below_counts && f[j] < threshold) below_flags |= 1u << j;
+        }
     };
     if (resident) load_keys(0);
+
+    // ---- the threshold list of the same matrix (iqa_series_find: one launch, one read of the matrix), as below_kernel ----
+    if (below_counts && resident) {
+        int total;
+        int pos = block_exclusive_scan(__popc(below_flags), warp_tot, total);
+        int* out = below_idx + (size_t)blockIdx.x * capacity;
+        for (uint32_t fl = below_flags; fl; fl &= fl - 1) {
+            if (pos < capacity) out[pos] = tid * kCandPerThread + (__ffs(fl) - 1);
+            ++pos;
+        }
+        if (tid == 0) below_counts[blockIdx.x] = total;
+    }
+
+    // ---- small k (<= 32) of a resident matrix: no radix passes.  A threshold tau with at least kk tiles <= tau is the
+    //      kk-th smallest of >= kk GROUP minima: the minima of the warps' 512-tile runs when at least kk warps hold
+    //      tiles (one shuffle reduction per warp, one rank count in warp 0), else the minima of the threads' 16-tile
+    //      runs (every warp sorts its 32 thread minima, a tree of bitonic merges keeps the 32 smallest of the CTA:
+    //      exact, and then all tiles <= tau belong to kk threads: at most 16 kk <= 512 of them).  The tiles <= tau are
+    //      gathered (any order: the (key, index) pairs are unique) and sorted.  Warp minima bound nothing from above:
+    //      should more than kMaxBottomK tiles pass (spatially sorted matrices), the radix select below takes over. ----
+    if (resident && kk <= 32) {
+        const int lane = tid & 31, w = tid >> 5, nw = (int)(blockDim.x >> 5);
+        const int i0 = tid * kCandPerThread;
+        unsigned long long m = ~0ull;                       // threads past the matrix hold no tile
+        {
+            uint32_t best = 0xffffffffu; int bj = -1;       // first minimum of the run: lowest index among equals
+#pragma unroll
+            for (int j = 0; j < kCandPerThread; ++j)
+                if (i0 + j < n && (bj < 0 || u[j] < best)) { best = u[j]; bj = j; }
+            if (bj >= 0) m = key64(best, i0 + bj);
+        }
+        const int data_warps = (n + 32 * kCandPerThread - 1) / (32 * kCandPerThread);
+        if (tid == 0) { s_rank = 0; s_tau = ~0ull; }
+        if (data_warps >= kk) {
+            unsigned long long x = m;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) x = umin64(x, __shfl_xor_sync(0xffffffffu, x, o));
+            if (lane == 0) keys[w] = x;
+            __syncthreads();
+            if (w == 0) {
+                x = lane < nw ? keys[lane] : ~0ull;
+                int r = 0;                                  // keys smaller than this lane's (real keys are unique)
+#pragma unroll
+                for (int l = 0; l < 32; ++l) r += __shfl_sync(0xffffffffu, x, l) < x ? 1 : 0;
+                if (r == kk - 1 && x != ~0ull) s_tau = x;
+            }
+        } else {
+            unsigned long long x = warp_sort32(m, lane);
+            for (int r = 1; r < nw; r <<= 1) {              // nw is a power of two
+                if ((w & (2 * r - 1)) == r) keys[w * 32 + lane] = x;
+                __syncthreads();
+                if ((w & (2 * r - 1)) == 0) x = warp_merge_low32(x, keys[(w + r) * 32 + 31 - lane], lane);
+            }
+            if (w == 0) {
+                const unsigned long long t = __shfl_sync(0xffffffffu, x, kk - 1);
+                if (lane == 0) s_tau = t;                   // ~0ull when fewer than kk threads hold tiles: every tile passes
+            }
+        }
+        __syncthreads();                                    // s_tau is set; the lists in keys[] have been read
+        const unsigned long long tau = s_tau;
+        const uint32_t tau_hi = (uint32_t)(tau >> 32), tau_lo = (uint32_t)tau;
+        uint32_t sel = 0;
+#pragma unroll
+        for (int j = 0; j < kCandPerThread; ++j)
+            if (i0 + j < n && (u[j] < tau_hi || (u[j] == tau_hi && (uint32_t)(i0 + j) <= tau_lo))) sel |= 1u << j;
+        if (sel) {
+            int pos = atomicAdd(&s_rank, __popc(sel));
+#pragma unroll
+            for (int j = 0; j < kCandPerThread; ++j)
+                if (sel & (1u << j)) {
+                    if (pos < kMaxBottomK) keys[pos] = key64(u[j], i0 + j);
+                    ++pos;
+                }
+        }
+        __syncthreads();
+        const int total = s_rank;                           // >= kk
+        if (total <= kMaxBottomK) {
+            int* out_i = indices + (size_t)blockIdx.x * k;
+            float* out_v = vals ? vals + (size_t)blockIdx.x * k : nullptr;
+            for (int i = kk + tid; i < k; i += (int)blockDim.x) {
+                out_i[i] = -1;
+                if (out_v) out_v[i] = __int_as_float(0x7f800000);
+            }
+            if (total <= 32) {                              // one key per lane of warp 0: its rank is its place
+                if (w == 0) {
+                    const unsigned long long x = lane < total ? keys[lane] : ~0ull;
+                    int r = 0;
+#pragma unroll
+                    for (int l = 0; l < 32; ++l) r += __shfl_sync(0xffffffffu, x, l) < x ? 1 : 0;
+                    if (lane < total && r < kk) {
+                        const int idx = (int)(uint32_t)x;
+                        out_i[r] = idx;
+                        if (out_v) out_v[r] = v[idx];
+                    }
+                }
+                return;
+            }
+            int P = 64;
+            while (P < total) P <<= 1;
+            for (int i = total + tid; i < P; i += (int)blockDim.x) keys[i] = ~0ull;
+            __syncthreads();
+            sort_keys_shared(keys, P);
+            for (int i = tid; i < kk; i += (int)blockDim.x) {
+                const int idx = (int)(uint32_t)keys[i];
+                out_i[i] = idx;
+                if (out_v) out_v[i] = v[idx];
+            }
+            return;
+        }
+        __syncthreads();                                    // (uniform) too many tiles passed: radix select
+    }
 
     // ---- the bits all keys share: similarity values cluster (augLISI ~ 0.99x), so their leading bits are equal;
     //      a digit on which every key agrees would send all the atomics of a pass to ONE histogram bucket ----
@@ -272,8 +474,12 @@ bottom_k_cluster_kernel(const float* __restrict__ values, int n, int k, int* __r
     const int tid = threadIdx.x;
     const int i0 = (r * kCandThreads + tid) * kCandPerThread;               // first tile of this thread
     uint32_t u[kCandPerThread];
+    {
+        float f[kCandPerThread];
+        load_run16(v, i0, n, __int_as_float(0x7fc00000), f);
 #pragma unroll
-    for (int j = 0; j < kCandPerThread; ++j) u[j] = i0 + j < n ? order_key(v[i0 + j]) : 0xffffffffu;
+        for (int j = 0; j < kCandPerThread; ++j) u[j] = order_key(f[j]);
+    }
 
     // ---- bits all keys of the matrix share ----
     uint32_t k_and = 0xffffffffu, k_or = 0u;
@@ -415,9 +621,11 @@ below_cluster_kernel(const float* __restrict__ values, int n, float threshold, i
     int* out = indices + map * (size_t)capacity;
     const int i0 = (r * kCandThreads + (int)threadIdx.x) * kCandPerThread;
     uint32_t flags = 0;
+    float f[kCandPerThread];
+    load_run16(v, i0, n, __int_as_float(0x7f800000), f);
 #pragma unroll
     for (int j = 0; j < kCandPerThread; ++j)
-        if (i0 + j < n && v[i0 + j] < threshold) flags |= 1u << j;
+        if (f[j] < threshold) flags |= 1u << j;
     int total;
     int pos = block_exclusive_scan(__popc(flags), warp_tot, total);
     if (threadIdx.x == 0) cta_total = total;

@@ -810,7 +810,7 @@ const char* iqa_status_string(int status) {
     }
 }
 
-const char* iqa_version(void) { return "0.6.0"; }
+const char* iqa_version(void) { return "0.7.0"; }
 
 int iqa_debug_knob(const char* name, int value) {
     if (!name) return -1;
@@ -1031,9 +1031,42 @@ int iqa_tiles_bottom_k(const float* values, int n_tiles, int n_maps, int k,
         ? launch_cluster(bottom_k_cluster_kernel, (unsigned)n_maps * (unsigned)cs, (unsigned)kCandThreads, 0,
                          (cudaStream_t)stream, (unsigned)cs, values, n_tiles, k, indices, vals)
         : launch(bottom_k_kernel, (unsigned)n_maps, (unsigned)cand_threads(n_tiles), 0, (cudaStream_t)stream, values,
-                 n_tiles, k, indices, vals);
+                 n_tiles, k, indices, vals, 0.0f, (int*)nullptr, 0, (int*)nullptr);
     if (e != cudaSuccess) return IQA_ERR_CUDA;
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+}
+
+int iqa_series_find(const float* const* img_ptrs_host, int n_images, int mode,
+                    int N, int N_T, float C1, float C2, float C, float D,
+                    float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                    float* lisi_num, float* auglisi_num, float* out2,
+                    void* workspace, size_t workspace_bytes,
+                    int index, int k, int* bottom_idx, float* bottom_val,
+                    float threshold, int* below_idx, int capacity, int* below_counts, void* stream) {
+    // every argument of the candidate step is checked before the series is enqueued
+    if (index != IQA_FIND_LISI && index != IQA_FIND_AUGLISI) return IQA_ERR_SHAPE;
+    if (k < 0 || k > kMaxBottomK || capacity < 0) return IQA_ERR_SHAPE;
+    if (k == 0 && !below_counts) return IQA_ERR_NULL;
+    if (k > 0 && !bottom_idx) return IQA_ERR_NULL;
+    if (below_counts && capacity > 0 && !below_idx) return IQA_ERR_NULL;
+    if (below_counts && threshold != threshold) return IQA_ERR_PARAM;
+    if (const int rc = iqa_series_tiles(img_ptrs_host, n_images, mode, N, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
+                                        lisi_num, auglisi_num, out2, workspace, workspace_bytes, stream))
+        return rc;
+    const float* values = index == IQA_FIND_LISI ? lisi : auglisi;
+    const int n = (N / N_T) * (N / N_T), K = n_images - 1;
+    // both lists of a matrix that one CTA keeps in registers: ONE launch, the matrix is read once
+    if (k > 0 && below_counts && n <= cand_threads(n) * kCandPerThread) {
+        if (launch(bottom_k_kernel, (unsigned)K, (unsigned)cand_threads(n), 0, (cudaStream_t)stream, values, n, k,
+                   bottom_idx, bottom_val, threshold, below_idx, capacity, below_counts) != cudaSuccess)
+            return IQA_ERR_CUDA;
+        return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
+    }
+    if (k > 0)
+        if (const int rc = iqa_tiles_bottom_k(values, n, K, k, bottom_idx, bottom_val, stream)) return rc;
+    if (below_counts)
+        if (const int rc = iqa_tiles_below(values, n, K, threshold, below_idx, capacity, below_counts, stream)) return rc;
+    return IQA_OK;
 }
 
 int iqa_merge_tiles_batch(const float* lisi, const float* auglisi,

@@ -179,6 +179,21 @@ def test_series_and_candidate_validation():
     assert B.iqa_tiles_below(FAKE, 16, 1, 0.5, FAKE, -1, FAKE) == B.IQA_ERR_SHAPE
     assert B.iqa_tiles_below(FAKE, 16, 1, math.nan, FAKE, 16, FAKE) == B.IQA_ERR_PARAM
 
+    def find(imgs=tbl, M=3, N=256, N_T=16, index=B.IQA_FIND_AUGLISI, k=4, bi=FAKE, thr=0.5, li=FAKE, cap=8, cnt=FAKE):
+        return B.iqa_series_find(imgs, M, B.IQA_SERIES_REFERENCE, N, N_T, 1e-6, 1e-6, 1e-6, 5e-7, FAKE, FAKE, FAKE, FAKE,
+                                 None, None, None, None, 0, index, k, bi, None, thr, li, cap, cnt, None)
+
+    # the candidate arguments are checked BEFORE the series is enqueued, then the series' own validation applies
+    assert find(index=2) == B.IQA_ERR_SHAPE
+    assert find(k=-1) == B.IQA_ERR_SHAPE and find(k=1025) == B.IQA_ERR_SHAPE and find(cap=-1) == B.IQA_ERR_SHAPE
+    assert find(k=0, cnt=None) == B.IQA_ERR_NULL               # neither list asked for
+    assert find(bi=None) == B.IQA_ERR_NULL
+    assert find(li=None) == B.IQA_ERR_NULL
+    assert find(thr=math.nan) == B.IQA_ERR_PARAM
+    assert find(imgs=bad) == B.IQA_ERR_NULL
+    assert find(N=100) == B.IQA_ERR_SHAPE
+    assert find(N_T=128) == B.IQA_ERR_WORKSPACE
+
 
 def test_2d_validation():
     a = (1e-6, 1e-6, 1e-6, 5e-7)

@@ -86,6 +86,36 @@ def test_bottom_k_all_equal_and_sorted_inputs(B):
         _check_bottom_k(B, maps, k)
 
 
+@pytest.mark.parametrize("nt,n_maps,k", [(128, 3, 32), (128, 2, 17), (127, 2, 32), (5, 3, 7), (100, 2, 1), (64, 4, 16),
+                                         (90, 2, 31), (23, 5, 32)])
+def test_bottom_k_small_k_path(B, nt, n_maps, k):
+    """k <= 32 on a matrix of at most 16384 tiles takes the threshold-by-thread-minima path (no radix passes): random
+    values with ties, map bases that are not 16-byte aligned (odd nt), and the adversarial layouts of that path -- all
+    the lowest values inside ONE thread's run of 16 tiles, sorted and reversed matrices, all-equal matrices, NaN."""
+    rng = np.random.default_rng(7 * nt + k)
+    maps = np.round(rng.random((n_maps, nt, nt)), 3).astype(np.float32)
+    maps[0].ravel()[:: 11] = -0.0
+    if nt * nt >= 48:
+        maps[-1].ravel()[32:48] = np.linspace(-2.0, -1.0, 16, dtype=np.float32)     # the lowest 16 in one thread's run
+    _check_bottom_k(B, maps, k)
+    n = nt * nt
+    ramp = np.arange(n, dtype=np.float32)
+    special = np.stack([ramp.reshape(nt, nt), ramp[::-1].reshape(nt, nt).copy(),
+                        np.full((nt, nt), 0.5, np.float32), (ramp % 3).reshape(nt, nt)])
+    _check_bottom_k(B, special, k)
+    withnan = maps.copy()
+    withnan[0].ravel()[1::4] = np.nan                      # NaN sorts last (never produced by the kernels: C2, C > 0)
+    import torch
+    idx, _ = B.tiles_bottom_k(_dev(withnan), k)
+    torch.cuda.synchronize()
+    got = idx.cpu().numpy()[0]
+    flat = withnan[0].ravel()
+    order = np.lexsort((np.arange(n), np.where(np.isnan(flat), np.inf, flat + 0.0)))
+    finite = order[~np.isnan(flat[order])]
+    kk = min(k, finite.size)
+    assert np.array_equal(got[:kk], finite[:kk])
+
+
 @pytest.mark.parametrize("thr", [-1.0, 0.0, 0.25, 0.5, 0.99, 2.0])
 def test_below_threshold_random(B, thr):
     rng = np.random.default_rng(3)
@@ -112,28 +142,70 @@ def test_candidates_on_oracle_matrices_of_config1(B):
             _check_below(B, maps, thr)
 
 
-def test_find_transients_end_to_end(B):
-    """Series -> bottom-k on the device: the switched-off transients of a config-[0] series are among the
-    flagged tiles of each comparison, and the flagged tiles are exactly the bottom-k of the device matrix."""
+@pytest.mark.parametrize("mode,index", [("reference", "auglisi"), ("consecutive", "lisi")])
+def test_find_transients_end_to_end(B, mode, index):
+    """iqa_series_find: series -> bottom-k and threshold list inside ONE call.  The lists are exactly the oracle's
+    selection on the device matrix of each comparison, the matrices are those of iqa_series_tiles, and the switched-off
+    transients of a config-[0] series are among the flagged tiles."""
     import torch
     import oracle
     from paper_2501_10653_b200 import synth
     cfg = synth.CONFIGS[0]
     imgs, meta = synth.make_series(cfg, 4)
     dev = [torch.from_numpy(a).cuda() for a in imgs]
-    out = B.find_transients(dev, "reference", cfg.N_T, cfg.C1, cfg.C2, cfg.C, cfg.D, k=12)
+    plain = B.series_tiles(dev, mode, cfg.N_T, cfg.C1, cfg.C2, cfg.C, cfg.D)
+    thr = float(np.quantile(plain[index].cpu().numpy(), 0.02))
+    out = B.find_transients(dev, mode, cfg.N_T, cfg.C1, cfg.C2, cfg.C, cfg.D, k=12, index=index, threshold=thr,
+                            capacity=20)
     torch.cuda.synchronize()
+    for nm in ("lisi", "auglisi", "X", "Y", "whole"):
+        assert torch.equal(out[nm], plain[nm]), nm
     cand = out["candidates"].cpu().numpy()
-    mats = out["auglisi"].cpu().numpy()
+    mats = out[index].cpu().numpy()
+    below, counts = out["below"].cpu().numpy(), out["below_counts"].cpu().numpy()
     nt = cfg.N // cfg.N_T
     src, ch = meta["sources"], meta["changed"]
     for c in range(3):
         ei, ev = oracle.bottom_k(mats[c], 12)            # selection is exact on the same fp32 matrix
         assert np.array_equal(cand[c], ei)
         assert np.array_equal(out["candidate_values"][c].cpu().numpy(), ev)
-        off = [i for i, s in zip(ch, meta["state_y"][c + 1]) if s and src["amp_x"][i] > 10 * cfg.noise_sigma]
-        tiles = {int(src["cy"][i]) // cfg.N_T * nt + int(src["cx"][i]) // cfg.N_T for i in off}
-        assert tiles <= set(cand[c].tolist()), (c, tiles, cand[c])
+        eb = oracle.below_threshold(mats[c], thr)
+        assert counts[c] == eb.size
+        w = min(eb.size, 20)
+        assert np.array_equal(below[c, :w], eb[:w]) and np.all(below[c, w:] == -1)
+        if mode == "reference" and index == "auglisi":
+            off = [i for i, s in zip(ch, meta["state_y"][c + 1]) if s and src["amp_x"][i] > 10 * cfg.noise_sigma]
+            tiles = {int(src["cy"][i]) // cfg.N_T * nt + int(src["cx"][i]) // cfg.N_T for i in off}
+            assert tiles <= set(cand[c].tolist()), (c, tiles, cand[c])
+    only_k = B.find_transients(dev, mode, cfg.N_T, cfg.C1, cfg.C2, cfg.C, cfg.D, k=5, index=index)
+    assert "below" not in only_k and torch.equal(only_k["candidates"], out["candidates"][:, :5])
+
+
+@pytest.mark.parametrize("N,N_T,k", [(2048, 16, 16), (2048, 16, 40), (2048, 8, 16), (1024, 64, 32)])
+def test_series_find_lists_match_oracle_selection(B, N, N_T, k):
+    """iqa_series_find on 16384-tile matrices (both lists from ONE launch of the candidate kernel, small-k and radix
+    paths), on 65536-tile matrices (cluster kernels, two launches) and on 256-tile matrices: the lists are the
+    oracle's selection on the device matrices, which are those of iqa_series_tiles."""
+    import torch
+    import oracle
+    g = torch.Generator(device="cuda").manual_seed(N + N_T + k)
+    imgs = [torch.rand((N, N), generator=g, device="cuda") - 0.3 for _ in range(3)]
+    imgs[2][: N // 2] = imgs[1][: N // 2]                      # half of the tiles of comparison 1 are identical: ties at 1.0
+    kw = dict(C1=1e-3, C2=1e-3, C=1e-3, D=5e-4)
+    plain = B.series_tiles(imgs, "consecutive", N_T, **kw)
+    mats = plain["auglisi"].cpu().numpy()
+    thr = float(np.quantile(mats[0], 0.003))
+    out = B.find_transients(imgs, "consecutive", N_T, k=k, threshold=thr, capacity=64, **kw)
+    torch.cuda.synchronize()
+    assert torch.equal(out["auglisi"], plain["auglisi"]) and torch.equal(out["whole"], plain["whole"])
+    for c in range(2):
+        ei, ev = oracle.bottom_k(mats[c], k)
+        assert np.array_equal(out["candidates"][c].cpu().numpy(), ei), c
+        assert np.array_equal(out["candidate_values"][c].cpu().numpy(), ev), c
+        eb = oracle.below_threshold(mats[c], thr)
+        assert int(out["below_counts"][c]) == eb.size
+        w = min(eb.size, 64)
+        assert np.array_equal(out["below"][c].cpu().numpy()[:w], eb[:w])
 
 
 def test_candidate_error_codes(B):
