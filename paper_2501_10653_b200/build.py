@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "iqa_tiles.cu")]
-HEADERS = [os.path.join(CSRC, "iqa_kernels.cuh"), os.path.join(CSRC, "iqa_aggregate.cuh"),
+HEADERS = [os.path.join(CSRC, "iqa_kernels.cuh"), os.path.join(CSRC, "iqa_aggregate.cuh"), os.path.join(CSRC, "iqa_generic_vec.cuh"),
            os.path.join(CSRC, "iqa_any.cuh"), os.path.join(CSRC, "iqa_tma.cuh"), os.path.join(CSRC, "iqa_candidates.cuh"),
            os.path.join(_ROOT, "include", "iqa_tiles.h")]
 LIB = os.path.join(_HERE, "libiqa_tiles.so")

@@ -135,33 +135,47 @@ __device__ __forceinline__ void terms_wide2(float s0, float s1, float d0, float 
     aY = add2(aY, pack2(y0, y1));
 }
 
+// Pixel4<T>: four horizontally adjacent pixels of type T.  terms() takes them as the kWords 32-bit words they occupy
+// (registers: the generic kernels load them from global memory), row() reads them from shared memory.
 template <typename T> struct Pixel4;
 
 template <> struct Pixel4<float> {
-    static constexpr int kBytes = 16;
+    static constexpr int kBytes = 16, kWords = 4;
+    template <int MODE>
+    static __device__ __forceinline__ void terms(const uint32_t* x, const uint32_t* y, float C1, Acc16& a) {
+        pixel_terms2<MODE>(__uint_as_float(x[0]), __uint_as_float(x[1]), __uint_as_float(y[0]), __uint_as_float(y[1]), C1,
+                           a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
+        pixel_terms2<MODE>(__uint_as_float(x[2]), __uint_as_float(x[3]), __uint_as_float(y[2]), __uint_as_float(y[3]), C1,
+                           a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+    }
     template <int MODE>
     static __device__ __forceinline__ void row(const unsigned char* xs, const unsigned char* ys, float C1, Acc16& a) {
-        const float4 vx = *reinterpret_cast<const float4*>(xs);
-        const float4 vy = *reinterpret_cast<const float4*>(ys);
-        pixel_terms2<MODE>(vx.x, vx.y, vy.x, vy.y, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
-        pixel_terms2<MODE>(vx.z, vx.w, vy.z, vy.w, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+        const uint4 vx = *reinterpret_cast<const uint4*>(xs);
+        const uint4 vy = *reinterpret_cast<const uint4*>(ys);
+        const uint32_t wx[4] = {vx.x, vx.y, vx.z, vx.w}, wy[4] = {vy.x, vy.y, vy.z, vy.w};
+        terms<MODE>(wx, wy, C1, a);
     }
 };
 
 template <> struct Pixel4<__half> {
-    static constexpr int kBytes = 8;
+    static constexpr int kBytes = 8, kWords = 2;
+    template <int MODE>
+    static __device__ __forceinline__ void terms(const uint32_t* x, const uint32_t* y, float C1, Acc16& a) {
+        // the clamp (P:27) on two pixels at once in fp16 (max(NaN, 0) = 0, as in fp32), then the exact conversion
+        const __half2 zero = __float2half2_rn(0.0f);
+        const float2 x01 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&x[0]), zero));
+        const float2 x23 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&x[1]), zero));
+        const float2 y01 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&y[0]), zero));
+        const float2 y23 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&y[1]), zero));
+        pixel_terms2<MODE, false>(x01.x, x01.y, y01.x, y01.y, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
+        pixel_terms2<MODE, false>(x23.x, x23.y, y23.x, y23.y, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+    }
     template <int MODE>
     static __device__ __forceinline__ void row(const unsigned char* xs, const unsigned char* ys, float C1, Acc16& a) {
         const uint2 qx = *reinterpret_cast<const uint2*>(xs);
         const uint2 qy = *reinterpret_cast<const uint2*>(ys);
-        // the clamp (P:27) on two pixels at once in fp16 (max(NaN, 0) = 0, as in fp32), then the exact conversion
-        const __half2 zero = __float2half2_rn(0.0f);
-        const float2 x01 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&qx.x), zero));
-        const float2 x23 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&qx.y), zero));
-        const float2 y01 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&qy.x), zero));
-        const float2 y23 = __half22float2(__hmax2(*reinterpret_cast<const __half2*>(&qy.y), zero));
-        pixel_terms2<MODE, false>(x01.x, x01.y, y01.x, y01.y, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
-        pixel_terms2<MODE, false>(x23.x, x23.y, y23.x, y23.y, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+        const uint32_t wx[2] = {qx.x, qx.y}, wy[2] = {qy.x, qy.y};
+        terms<MODE>(wx, wy, C1, a);
     }
 };
 
@@ -175,16 +189,21 @@ __device__ __forceinline__ void s16x2_to_float(uint32_t w, float& lo, float& hi)
     unpack2(f, lo, hi);
 }
 template <> struct Pixel4<short> {
-    static constexpr int kBytes = 8;
+    static constexpr int kBytes = 8, kWords = 2;
+    template <int MODE>
+    static __device__ __forceinline__ void terms(const uint32_t* x, const uint32_t* y, float C1, Acc16& a) {
+        float x0, x1, x2, x3, y0, y1, y2, y3;
+        s16x2_to_float(x[0], x0, x1); s16x2_to_float(x[1], x2, x3);
+        s16x2_to_float(y[0], y0, y1); s16x2_to_float(y[1], y2, y3);
+        pixel_terms2<MODE, false>(x0, x1, y0, y1, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
+        pixel_terms2<MODE, false>(x2, x3, y2, y3, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+    }
     template <int MODE>
     static __device__ __forceinline__ void row(const unsigned char* xs, const unsigned char* ys, float C1, Acc16& a) {
         const uint2 qx = *reinterpret_cast<const uint2*>(xs);
         const uint2 qy = *reinterpret_cast<const uint2*>(ys);
-        float x0, x1, x2, x3, y0, y1, y2, y3;
-        s16x2_to_float(qx.x, x0, x1); s16x2_to_float(qx.y, x2, x3);
-        s16x2_to_float(qy.x, y0, y1); s16x2_to_float(qy.y, y2, y3);
-        pixel_terms2<MODE, false>(x0, x1, y0, y1, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
-        pixel_terms2<MODE, false>(x2, x3, y2, y3, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+        const uint32_t wx[2] = {qx.x, qx.y}, wy[2] = {qy.x, qy.y};
+        terms<MODE>(wx, wy, C1, a);
     }
 };
 
@@ -197,21 +216,25 @@ __device__ __forceinline__ void u8x4_to_float(uint32_t w, float& f0, float& f1, 
                        __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7653))), m), f2, f3);
 }
 template <> struct Pixel4<unsigned char> {
-    static constexpr int kBytes = 4;
+    static constexpr int kBytes = 4, kWords = 1;
+    template <int MODE>
+    static __device__ __forceinline__ void terms(const uint32_t* x, const uint32_t* y, float C1, Acc16& a) {
+        float x0, x1, x2, x3, y0, y1, y2, y3;
+        u8x4_to_float(x[0], x0, x1, x2, x3);
+        u8x4_to_float(y[0], y0, y1, y2, y3);
+        pixel_terms2<MODE, false>(x0, x1, y0, y1, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);      // unsigned: nothing to clamp
+        pixel_terms2<MODE, false>(x2, x3, y2, y3, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+    }
     template <int MODE>
     static __device__ __forceinline__ void row(const unsigned char* xs, const unsigned char* ys, float C1, Acc16& a) {
         const uint32_t qx = *reinterpret_cast<const uint32_t*>(xs);
         const uint32_t qy = *reinterpret_cast<const uint32_t*>(ys);
-        float x0, x1, x2, x3, y0, y1, y2, y3;
-        u8x4_to_float(qx, x0, x1, x2, x3);
-        u8x4_to_float(qy, y0, y1, y2, y3);
-        pixel_terms2<MODE, false>(x0, x1, y0, y1, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);      // unsigned: nothing to clamp
-        pixel_terms2<MODE, false>(x2, x3, y2, y3, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+        terms<MODE>(&qx, &qy, C1, a);
     }
 };
 
 template <> struct Pixel4<double> {
-    static constexpr int kBytes = 32;
+    static constexpr int kBytes = 32, kWords = 8;
     static __device__ __forceinline__ void one(double xv, double yv, float& s, float& d, float& xc, float& yc) {
         const double xd = xv > 0.0 ? xv : 0.0;      // P:27; NaN -> 0
         const double yd = yv > 0.0 ? yv : 0.0;
@@ -221,19 +244,27 @@ template <> struct Pixel4<double> {
         yc = (float)yd;
     }
     template <int MODE>
-    static __device__ __forceinline__ void row(const unsigned char* xs, const unsigned char* ys, float C1, Acc16& a) {
-        const double2 x01 = *reinterpret_cast<const double2*>(xs), x23 = *reinterpret_cast<const double2*>(xs + 16);
-        const double2 y01 = *reinterpret_cast<const double2*>(ys), y23 = *reinterpret_cast<const double2*>(ys + 16);
+    static __device__ __forceinline__ void terms(const uint32_t* x, const uint32_t* y, float C1, Acc16& a) {
         float s0, s1, d0, d1, cx0, cx1, cy0, cy1;
-        one(x01.x, y01.x, s0, d0, cx0, cy0); one(x01.y, y01.y, s1, d1, cx1, cy1);
+        one(__hiloint2double((int)x[1], (int)x[0]), __hiloint2double((int)y[1], (int)y[0]), s0, d0, cx0, cy0);
+        one(__hiloint2double((int)x[3], (int)x[2]), __hiloint2double((int)y[3], (int)y[2]), s1, d1, cx1, cy1);
         terms_wide2<MODE>(s0, s1, d0, d1, cx0, cx1, cy0, cy1, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
-        one(x23.x, y23.x, s0, d0, cx0, cy0); one(x23.y, y23.y, s1, d1, cx1, cy1);
+        one(__hiloint2double((int)x[5], (int)x[4]), __hiloint2double((int)y[5], (int)y[4]), s0, d0, cx0, cy0);
+        one(__hiloint2double((int)x[7], (int)x[6]), __hiloint2double((int)y[7], (int)y[6]), s1, d1, cx1, cy1);
         terms_wide2<MODE>(s0, s1, d0, d1, cx0, cx1, cy0, cy1, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+    }
+    template <int MODE>
+    static __device__ __forceinline__ void row(const unsigned char* xs, const unsigned char* ys, float C1, Acc16& a) {
+        const uint4 xa = *reinterpret_cast<const uint4*>(xs), xb = *reinterpret_cast<const uint4*>(xs + 16);
+        const uint4 ya = *reinterpret_cast<const uint4*>(ys), yb = *reinterpret_cast<const uint4*>(ys + 16);
+        const uint32_t wx[8] = {xa.x, xa.y, xa.z, xa.w, xb.x, xb.y, xb.z, xb.w};
+        const uint32_t wy[8] = {ya.x, ya.y, ya.z, ya.w, yb.x, yb.y, yb.z, yb.w};
+        terms<MODE>(wx, wy, C1, a);
     }
 };
 
 template <> struct Pixel4<int> {
-    static constexpr int kBytes = 16;
+    static constexpr int kBytes = 16, kWords = 4;
     // after the clamp x, y are in [0, 2^31): x + y and |x - y| are exact as unsigned 32-bit integers, and one
     // integer -> fp32 conversion rounds exactly like the fp64 route of the oracle's definition
     static __device__ __forceinline__ void one(int xv, int yv, float& s, float& d, float& xc, float& yc) {
@@ -244,14 +275,19 @@ template <> struct Pixel4<int> {
         yc = __uint2float_rn(yu);
     }
     template <int MODE>
-    static __device__ __forceinline__ void row(const unsigned char* xs, const unsigned char* ys, float C1, Acc16& a) {
-        const int4 vx = *reinterpret_cast<const int4*>(xs);
-        const int4 vy = *reinterpret_cast<const int4*>(ys);
+    static __device__ __forceinline__ void terms(const uint32_t* x, const uint32_t* y, float C1, Acc16& a) {
         float s0, s1, d0, d1, cx0, cx1, cy0, cy1;
-        one(vx.x, vy.x, s0, d0, cx0, cy0); one(vx.y, vy.y, s1, d1, cx1, cy1);
+        one((int)x[0], (int)y[0], s0, d0, cx0, cy0); one((int)x[1], (int)y[1], s1, d1, cx1, cy1);
         terms_wide2<MODE>(s0, s1, d0, d1, cx0, cx1, cy0, cy1, C1, a.L[0], a.A[0], a.A[1], a.X[0], a.Y[0]);
-        one(vx.z, vy.z, s0, d0, cx0, cy0); one(vx.w, vy.w, s1, d1, cx1, cy1);
+        one((int)x[2], (int)y[2], s0, d0, cx0, cy0); one((int)x[3], (int)y[3], s1, d1, cx1, cy1);
         terms_wide2<MODE>(s0, s1, d0, d1, cx0, cx1, cy0, cy1, C1, a.L[1], a.A[2], a.A[3], a.X[1], a.Y[1]);
+    }
+    template <int MODE>
+    static __device__ __forceinline__ void row(const unsigned char* xs, const unsigned char* ys, float C1, Acc16& a) {
+        const uint4 vx = *reinterpret_cast<const uint4*>(xs);
+        const uint4 vy = *reinterpret_cast<const uint4*>(ys);
+        const uint32_t wx[4] = {vx.x, vx.y, vx.z, vx.w}, wy[4] = {vy.x, vy.y, vy.z, vy.w};
+        terms<MODE>(wx, wy, C1, a);
     }
 };
 

@@ -21,6 +21,7 @@
 #include "iqa_aggregate.cuh"
 #include "iqa_any.cuh"
 #include "iqa_candidates.cuh"
+#include "iqa_generic_vec.cuh"
 #include "iqa_kernels.cuh"
 #include "iqa_tma.cuh"
 
@@ -30,7 +31,6 @@ using namespace iqa;
 
 constexpr int kMaxN = 1 << 20;   // 2^40 pixels; keeps every grid and tile index inside int
 constexpr int kMaxDevices = 64;
-constexpr int kGenericBatch = 32;   // pairs per chunk of the pair-by-pair paths
 
 bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
@@ -48,11 +48,12 @@ bool pos_normal(float v) { return std::isfinite(v) && v >= FLT_MIN; }
 //   IQA_NO_PDL           1: launch without programmatic dependent launch
 //   IQA_CAND_NO_CLUSTER  1: candidate kernels never use the cluster twins
 //   IQA_ANY_NO_WIDE      1: any_kernel never lets a lane own eight columns
+//   IQA_GENERIC_NO_VEC   1: the generic path always takes the scalar-load kernels
 enum Knob { kKnobForceGeneric, kKnobForceAny, kKnobTmaConfig, kKnobTmaMaxCtas, kKnobNoPdl, kKnobCandNoCluster, kKnobNoWide,
-            kNumKnobs };
+            kKnobGenericNoVec, kNumKnobs };
 const char* const kKnobNames[kNumKnobs] = {"IQA_FORCE_GENERIC", "IQA_FORCE_ANY", "IQA_TMA_CONFIG", "IQA_TMA_MAX_CTAS",
-                                           "IQA_NO_PDL", "IQA_CAND_NO_CLUSTER", "IQA_ANY_NO_WIDE"};
-const int kKnobDefaults[kNumKnobs] = {0, 0, -1, 0, 0, 0, 0};
+                                           "IQA_NO_PDL", "IQA_CAND_NO_CLUSTER", "IQA_ANY_NO_WIDE", "IQA_GENERIC_NO_VEC"};
+const int kKnobDefaults[kNumKnobs] = {0, 0, -1, 0, 0, 0, 0, 0};
 struct Knobs {
     std::atomic<int> v[kNumKnobs];
     Knobs() {
@@ -582,8 +583,14 @@ int fire(const std::vector<AnyLaunch>& q, cudaStream_t st) {
 }
 
 // ---- generic kernels (pair by pair) ---------------------------------------------------------------------------
+// vec: x and y have the same alignment row by row -> the warp-per-piece kernel with 128-bit loads (iqa_generic_vec.cuh)
 template <int MODE, typename T>
-cudaError_t launch_generic_one(const GenericParams& g, long long n, int N_T, int pieces, cudaStream_t st) {
+cudaError_t launch_generic_one(const GenericParams& g, long long n, int N_T, int pieces, bool vec, cudaStream_t st) {
+    if (vec) {
+        const long long units = n * pieces;
+        return launch(generic_vec_kernel<MODE, T>, (unsigned)((units + kWarpsPerCta - 1) / kWarpsPerCta), kCtaThreads, 0, st,
+                      g, units);
+    }
     if ((long long)N_T * N_T <= kWarpTilePixels)          // small tiles: one warp per tile (pieces == 1 here)
         return launch(generic_warp_kernel<MODE, T>, (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta), kCtaThreads, 0, st, g, n);
     return launch(generic_kernel<MODE, T>, (unsigned)(n * pieces), kCtaThreads, 0, st, g);
@@ -593,7 +600,10 @@ int launch_generic(int mode, const void* const* xs, const void* const* ys, int n
     const int nt = ceil_div(g2.W, N_T);
     const long long n = (long long)nt * ceil_div(g2.H, N_T);
     if (n * pl.pieces > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    const int es = esize_of(g2.ptype);
     for (int i = 0; i < n_pairs; ++i) {
+        const bool vec = !knob(kKnobGenericNoVec) && (((uintptr_t)xs[i] ^ (uintptr_t)ys[i]) & 15u) == 0 &&
+                         (((g2.pitch_x - g2.pitch_y) * es) & 15) == 0;
         GenericParams g{};
         TileParams& p = g.tp;
         p.x = (const float*)xs[i]; p.y = (const float*)ys[i]; p.N = g2.W; p.H = g2.H; p.nt = nt;
@@ -606,15 +616,15 @@ int launch_generic(int mode, const void* const* xs, const void* const* ys, int n
         g.N_T = N_T; g.pieces = pl.pieces;
         cudaError_t e;
         switch (g2.ptype) {
-            case IQA_PIXEL_F64: e = launch_generic_one<kModeFused, double>(g, n, N_T, pl.pieces, st); break;
-            case IQA_PIXEL_F16: e = launch_generic_one<kModeFused, __half>(g, n, N_T, pl.pieces, st); break;
-            case IQA_PIXEL_I16: e = launch_generic_one<kModeFused, short>(g, n, N_T, pl.pieces, st); break;
-            case IQA_PIXEL_I32: e = launch_generic_one<kModeFused, int>(g, n, N_T, pl.pieces, st); break;
-            case IQA_PIXEL_U8: e = launch_generic_one<kModeFused, unsigned char>(g, n, N_T, pl.pieces, st); break;
+            case IQA_PIXEL_F64: e = launch_generic_one<kModeFused, double>(g, n, N_T, pl.pieces, vec, st); break;
+            case IQA_PIXEL_F16: e = launch_generic_one<kModeFused, __half>(g, n, N_T, pl.pieces, vec, st); break;
+            case IQA_PIXEL_I16: e = launch_generic_one<kModeFused, short>(g, n, N_T, pl.pieces, vec, st); break;
+            case IQA_PIXEL_I32: e = launch_generic_one<kModeFused, int>(g, n, N_T, pl.pieces, vec, st); break;
+            case IQA_PIXEL_U8: e = launch_generic_one<kModeFused, unsigned char>(g, n, N_T, pl.pieces, vec, st); break;
             default:
-                e = mode == kModeLisi  ? launch_generic_one<kModeLisi, float>(g, n, N_T, pl.pieces, st)
-                    : mode == kModeAug ? launch_generic_one<kModeAug, float>(g, n, N_T, pl.pieces, st)
-                                       : launch_generic_one<kModeFused, float>(g, n, N_T, pl.pieces, st);
+                e = mode == kModeLisi  ? launch_generic_one<kModeLisi, float>(g, n, N_T, pl.pieces, vec, st)
+                    : mode == kModeAug ? launch_generic_one<kModeAug, float>(g, n, N_T, pl.pieces, vec, st)
+                                       : launch_generic_one<kModeFused, float>(g, n, N_T, pl.pieces, vec, st);
         }
         if (e != cudaSuccess) return IQA_ERR_CUDA;
     }

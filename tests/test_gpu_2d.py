@@ -327,6 +327,29 @@ def test_any_kernel_pixel_types(B, U, dtype, H, W, N_T):
         _check_typed(B, U, x, y, xd, yd, N_T, k, f"any {dtype} {H}x{W} N_T={N_T} narrow lanes")
 
 
+@pytest.mark.parametrize("dtype", ["float32", "float64", "float16", "int16", "int32", "uint8"])
+@pytest.mark.parametrize("H,W,N_T", [(257, 301, 64), (200, 333, 32), (130, 515, 150), (90, 77, 7), (64, 1001, 300),
+                                     (300, 63, 16), (65, 129, 2), (40, 50, 3), (1, 5, 8), (100, 3, 64)])
+def test_generic_vector_kernels(B, U, dtype, H, W, N_T):
+    """Row pitches that are not multiples of 16 bytes (no tensor map), x and y aligned alike: the generic kernels with
+    128-bit loads (iqa_generic_vec.cuh) -- a CTA per tile piece (split tiles included) or a warp per small tile,
+    every base offset inside a 16-byte line, every pixel type -- and the scalar-load kernels on the same inputs
+    (IQA_GENERIC_NO_VEC) against oracle.tiles_2d_any.  The halo of the windows holds NaN / large values."""
+    import torch
+    rng = np.random.default_rng(H * 5 + W + N_T)
+    x, y, k = _typed_pair(rng, H, W, dtype)
+    per16 = 16 // x.dtype.itemsize
+    pitch = W + (1 if (W + 1) % per16 else 2)                       # never a multiple of 16 bytes
+    assert pitch % per16 != 0 or N_T < 4
+    for off in sorted({0, 1, per16 - 1, per16 + 1}):
+        xd, yd = _typed_window(x, pitch, off), _typed_window(y, pitch + per16, off)   # equal pitches modulo 16 bytes
+        got, _ = _check_typed(B, U, x, y, xd, yd, N_T, k, f"generic vec {dtype} {H}x{W} N_T={N_T} off={off}", plan="generic")
+    with B.knob("IQA_GENERIC_NO_VEC", 1):
+        sc, _ = _check_typed(B, U, x, y, xd, yd, N_T, k, f"generic scalar {dtype} {H}x{W} N_T={N_T}", plan="generic")
+    for n in got:                                                    # same arithmetic, another summation order
+        assert torch.all((got[n] - sc[n]).abs() <= 4e-6 * sc[n].abs() + 1e-30), n
+
+
 def test_any_kernel_matches_tma_kernel_on_power_of_two_tiles(B, U):
     """IQA_FORCE_ANY sends a power-of-two shape through any_kernel: the same per-pixel arithmetic in another
     summation order, so the two kernels agree to a few ulps (and both with the oracle)."""
