@@ -673,6 +673,40 @@ def measure_read_ceiling():
             "what": "hbm_read_ceiling: TMA loads into shared-memory rings, nothing computed, best of the sweep"}
 
 
+FLOOR_SRC = os.path.join(ROOT, "launch_floor.cu")
+FLOOR_EXE = os.path.join(ROOT, "launch_floor")
+
+
+def build_launch_floor(force: bool = False) -> str:
+    """Compile the launch-floor probe (launch_floor.cu, beside this file: a measurement aid, not part of the library)."""
+    import subprocess
+    from paper_2501_10653_b200 import build
+    if not force and os.path.exists(FLOOR_EXE) and os.path.getmtime(FLOOR_EXE) >= os.path.getmtime(FLOOR_SRC):
+        return FLOOR_EXE
+    subprocess.run([build._nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17",
+                    "-o", FLOOR_EXE, FLOOR_SRC], check=True)
+    return FLOOR_EXE
+
+
+def measure_launch_floor():
+    """Cost of one dependent kernel launch in a CUDA graph on this GPU, and of a last-CTA-finishes tail (fence, ticket,
+    re-read of the partials): what the single-pair latencies have to be read against."""
+    import subprocess
+    try:
+        out = subprocess.run([build_launch_floor()], capture_output=True, text=True, timeout=120).stdout
+    except Exception as exc:           # a diagnostic: never let it take the bench line down
+        return {"error": repr(exc)[:300]}
+    res = {}
+    for ln in out.splitlines():
+        f = ln.replace(":", "").replace(",", "").split()
+        if len(f) >= 8 and f[0].startswith("pdl=") and f[1].startswith("grid="):
+            res[f"{f[0]}_{f[1]}"] = {"null_us": float(f[3]), "ticket_us": float(f[6])}
+    res["what"] = ("launch_floor: us per kernel, 64 kernels back to back in one CUDA graph (best of 20 replays): an empty "
+                   "kernel, and one whose last CTA (integer ticket after a fence) re-reads a 32-byte partial of every "
+                   "CTA and reduces them")
+    return res
+
+
 def run_ours(args):
     import torch
     if not torch.cuda.is_available():
@@ -698,6 +732,12 @@ def run_ours(args):
             raise SystemExit(f"--paths: unknown row(s) {sorted(names)}; known: {[r[0] for r in PATH_ROWS]}")
         res = measure_paths(torch, binding, args.steps, args.warmup, device, not args.no_graph, rows=rows)
         print(json.dumps({"metric": METRIC, "unit": UNIT, "library_version": binding.iqa_version(), "paths": res}))
+        return
+    if args.series_only:
+        # only the time-series / candidate rows of the config [3] sky (ncu captures of the series and candidate kernels)
+        res = measure_series(torch, binding, synth.CONFIGS[3], args.series_images, max(3, min(args.steps, 10)), 3, device,
+                             not args.no_graph)
+        print(json.dumps({"metric": METRIC, "unit": UNIT, "library_version": binding.iqa_version(), "series": res}))
         return
     idx, pairs, pairs_e2e = WORKLOADS[args.workload]
     if args.pairs:
@@ -770,6 +810,7 @@ def run_ours(args):
     if extras:
         # read-only ceiling of the kernel's own access pattern, and the time-series modes at N = 8192
         also["read_ceiling"] = measure_read_ceiling()
+        also["launch_floor"] = measure_launch_floor()
         cs = synth.CONFIGS[3] if args.workload in ("cfg1", "cfg3") else cfg
         guarded(f"series_{cs.name}_M{args.series_images}",
                 lambda: measure_series(torch, binding, cs, args.series_images, max(3, min(K, 10)), 3, device, use_graph))
@@ -845,6 +886,8 @@ def main():
     ap.add_argument("--series-images", type=int, default=9, help="snapshots of the time-series measurement in `also`")
     ap.add_argument("--nt", type=int, default=0, help="override the workload's tile side N_T (a point of the config [2] sweep)")
     ap.add_argument("--paths", default="", help="comma-separated rows of PATH_ROWS: time only those kernel paths and print them")
+    ap.add_argument("--series-only", action="store_true",
+                    help="time only the time-series rows (N = 8192, N_T = 64) with their candidate lists and print them")
     ap.add_argument("--sweep", action="store_true", help="also time BASELINE.json config [2] (N=2048, N_T = 8..512)")
     args = ap.parse_args()
     args.warmup = max(3, args.warmup)
