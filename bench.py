@@ -556,6 +556,54 @@ def measure_paths(torch, binding, steps, warmup, device, use_graph, rows=PATH_RO
     return out
 
 
+SERIES_ANY_ROWS = [("f32_NT48", "float32", 48), ("f64_NT64", "float64", 64), ("i32_NT64", "int32", 64), ("i16_NT64", "int16", 64)]
+
+
+def measure_series_any(torch, binding, steps, warmup, device, use_graph, M=9, N=8192, rows=SERIES_ANY_ROWS):
+    """Time series of shapes / pixel types tma_kernel does not take (SURVEY.md 8(f)-2 + 8(f)-4): M snapshots through
+    iqa_series_tiles_2d_typed, i.e. K = M - 1 pair computations in one any_kernel launch whose item order puts the
+    comparisons of one image location on neighbouring CTAs (an image shared by two comparisons comes from DRAM once,
+    from L2 afterwards).  `pair_major` = the same call with that order switched off (IQA_SERIES_PAIR_MAJOR)."""
+    out = {}
+    k = PATH_CONSTS
+    K = M - 1
+    for name, dtype, N_T in rows:
+        dt = getattr(torch, dtype)
+        es = torch.empty((), dtype=dt).element_size()
+        xs, ys = make_path_inputs(torch, (name, dtype, N, N, N, 0, N_T), (M + 1) // 2, device)
+        imgs = (xs + ys)[:M]
+        ntx = -(-N // N_T)
+        n = ntx * ntx
+        o = [torch.empty((K, n), dtype=torch.float32, device=device) for _ in range(4)]
+        out2 = torch.empty((K, 2), dtype=torch.float32, device=device)
+        wsb = K * binding.iqa_workspace_bytes_2d(N, N, N_T)
+        ws = torch.empty(wsb, dtype=torch.uint8, device=device) if wsb else None
+        table, _ = binding._ptr_table(imgs)
+        ptype = binding._pixel_types()[dt]
+        row = {"pixel": dtype, "N": N, "N_T": N_T, "images": M, "plan": binding.plan_name(imgs[0], N_T)}
+        for mode_name, mode in binding.SERIES_MODES.items():
+            def step():
+                rc = binding.iqa_series_tiles_2d_typed(table, M, mode, ptype, N, N, N, N_T, *k, *o, None, None, out2, ws, wsb,
+                                                       torch.cuda.current_stream().cuda_stream)
+                if rc:
+                    raise binding.IqaError(rc, "iqa_series_tiles_2d_typed")
+            res = {}
+            for label, knob in (("us_per_comparison", 0), ("us_per_comparison_pair_major", 1)):
+                with binding.knob("IQA_SERIES_PAIR_MAJOR", knob):
+                    fn = graph_of(torch, step) if use_graph else step
+                    for _ in range(warmup):
+                        fn()
+                    res[label] = time_region(torch, fn, steps) * 1e3 / (steps * K)
+            series_b = es * N * N * M + 16 * n * K
+            res["dram_GBps_series_bytes"] = series_b / K / (res["us_per_comparison"] * 1e-6) / 1e9
+            res["pairwise_equivalent_GBps"] = (2 * es * N * N + 16 * n) / (res["us_per_comparison"] * 1e-6) / 1e9
+            row[mode_name] = res
+        out[name] = row
+        del xs, ys, imgs, o, ws
+        torch.cuda.empty_cache()
+    return out
+
+
 def series_bytes(N: int, N_T: int, M: int) -> int:
     """Algorithmic bytes of one iqa_series_tiles call: every image read once + 16 B per tile and comparison."""
     return 4 * N * N * M + 16 * (N // N_T) ** 2 * (M - 1)
@@ -737,7 +785,9 @@ def run_ours(args):
         # only the time-series / candidate rows of the config [3] sky (ncu captures of the series and candidate kernels)
         res = measure_series(torch, binding, synth.CONFIGS[3], args.series_images, max(3, min(args.steps, 10)), 3, device,
                              not args.no_graph)
-        print(json.dumps({"metric": METRIC, "unit": UNIT, "library_version": binding.iqa_version(), "series": res}))
+        res_any = measure_series_any(torch, binding, max(3, min(args.steps, 10)), 3, device, not args.no_graph)
+        print(json.dumps({"metric": METRIC, "unit": UNIT, "library_version": binding.iqa_version(), "series": res,
+                          "series_any": res_any}))
         return
     idx, pairs, pairs_e2e = WORKLOADS[args.workload]
     if args.pairs:
@@ -811,6 +861,7 @@ def run_ours(args):
         # read-only ceiling of the kernel's own access pattern, and the time-series modes at N = 8192
         also["read_ceiling"] = measure_read_ceiling()
         also["launch_floor"] = measure_launch_floor()
+        guarded("series_any", lambda: measure_series_any(torch, binding, max(3, min(K, 5)), 3, device, use_graph))
         cs = synth.CONFIGS[3] if args.workload in ("cfg1", "cfg3") else cfg
         guarded(f"series_{cs.name}_M{args.series_images}",
                 lambda: measure_series(torch, binding, cs, args.series_images, max(3, min(K, 10)), 3, device, use_graph))

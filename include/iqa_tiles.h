@@ -231,7 +231,10 @@ int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_
  * For 16-byte aligned images and a power-of-two N_T >= 8 one persistent TMA-fed kernel keeps the
  * x block of every comparison in shared memory, so each image is read from HBM ONCE:
  * 4 (K+1)/K bytes per pixel and comparison instead of the 8 of K independent pair calls.  Other
- * shapes are computed pair by pair (same results, 8 bytes). */
+ * tile sides and pixel types (the _typed entry points) run the K pair computations in ONE launch of
+ * the general TMA kernel whose item order puts the comparisons of one image location on neighbouring
+ * CTAs: every image still comes from HBM once, its second reader finds it in L2.  Row pitches no
+ * tensor map can describe are computed pair by pair (same results, 8 bytes). */
 #define IQA_SERIES_REFERENCE 0
 #define IQA_SERIES_CONSECUTIVE 1
 

@@ -59,6 +59,7 @@ struct AnyParams {
     int pad_mask;          // 16 / sizeof(T) - 1: box columns start at multiples of 16 bytes
     int const_s;           // the items' column offset s is the same for every item (s = shift)
     int n_pairs;
+    int pair_minor;        // item order: 0 = pair-major (batches), 1 = the pairs of one item location next to each other (series)
     int W, H, N_T;
     int ntx, nty, n_tiles;
     int kx, ky;            // whole tiles per item across / down (1, 1 when tiles are split)
@@ -316,6 +317,33 @@ __device__ __forceinline__ float4 acc_cols(const Acc16& a) {
                        (y0 + y1) + (y2 + y3));
 }
 
+// Position of a persistent CTA in its item sequence b, b + G, ...: three digits advanced by the decoded stride.
+//   pair-major (batches of independent pairs)  item = (pair, uy, ux), ux fastest
+//   pair-minor (the comparisons of a series)   item = (uy, ux, pair), pair fastest: the K comparisons of one item
+//     location run on neighbouring CTAs at the same time, so an image that two comparisons share -- I_k+1 is the y of
+//     comparison k and the x of comparison k+1, I_0 the x of every comparison in reference mode -- comes from DRAM once
+//     and from L2 afterwards
+struct AnyCursor {
+    int d0, d1, d2;
+    __device__ __forceinline__ void advance(const AnyCursor& s, int r0, int r1) {
+        d0 += s.d0;
+        const int c0 = d0 >= r0;
+        d0 -= c0 ? r0 : 0;
+        d1 += s.d1 + c0;
+        const int c1 = d1 >= r1;
+        d1 -= c1 ? r1 : 0;
+        d2 += s.d2 + c1;
+    }
+};
+__device__ __forceinline__ AnyCursor any_decode(int q, int r0, int r1) {
+    AnyCursor c;
+    const int t = q / r0;
+    c.d0 = q - t * r0;
+    c.d2 = t / r1;
+    c.d1 = t - c.d2 * r1;
+    return c;
+}
+
 template <int MODE, typename T>
 __global__ void __launch_bounds__(kTmaThreads, 2)
 any_kernel(const __grid_constant__ AnyParams p) {
@@ -350,21 +378,25 @@ any_kernel(const __grid_constant__ AnyParams p) {
     const int w = threadIdx.x >> 5;
     const int units_x = p.units_x, units_y = p.units_y;
     const int b = p.box_rows;
-    const ItemCursor stride = decode_item((int)gridDim.x, units_x, units_y);
+    const bool pm = p.pair_minor != 0;
+    const int r0 = pm ? p.n_pairs : units_x, r1 = pm ? units_x : units_y, r2 = pm ? units_y : p.n_pairs;
+    const AnyCursor stride = any_decode((int)gridDim.x, r0, r1);
+#define IQA_ANY_PAIR(c) (pm ? (c).d0 : (c).d2)
+#define IQA_ANY_UX(c) (pm ? (c).d1 : (c).d0)
+#define IQA_ANY_UY(c) (pm ? (c).d2 : (c).d1)
 
     if (w == kWarpsPerCta) {
         // ================= producer: one elected lane issues every TMA load =================
         if (lane != 0) return;
         const uint32_t box_bytes = (uint32_t)(b * p.row_bytes);
         RingPos r{0, 0, n_slots, 0u};
-        for (ItemCursor c = decode_item((int)blockIdx.x, units_x, units_y); c.pair < p.n_pairs;
-             c.advance(stride, units_x, units_y)) {
-            const AnyItem it = any_item(p, c.ux, c.uy);
+        for (AnyCursor c = any_decode((int)blockIdx.x, r0, r1); c.d2 < r2; c.advance(stride, r0, r1)) {
+            const AnyItem it = any_item(p, IQA_ANY_UX(c), IQA_ANY_UY(c));
             const int n_boxes = it.rv == p.ph ? p.boxes_per_item : (it.rv + b - 1) / b;
             for (int s = 0; s < n_boxes; ++s) {
                 const AnyBox bx = any_box(s, b, it.rv);
                 for (int j = 0; j < 2; ++j) {
-                    const int img = 2 * c.pair + j;
+                    const int img = 2 * IQA_ANY_PAIR(c) + j;
                     mbar_wait(empty_u32 + 8u * r.slot, r.phase ^ 1u);
                     mbar_expect_tx(full_u32 + 8u * r.slot, box_bytes);
                     tma_load_box(boxes_u32 + (uint32_t)r.slot * slot_bytes, p.maps + img, it.bc0, it.r0 + bx.o,
@@ -391,9 +423,8 @@ any_kernel(const __grid_constant__ AnyParams p) {
         const uint64_t pol = policy_evict_last();
         const int t_lane = lane / gsz;                // this lane's tile of the first round (the only one when gsz > 1)
         const int jy_lane = t_lane / p.kx, jx_lane = t_lane - jy_lane * p.kx;
-        for (ItemCursor c = decode_item((int)blockIdx.x, units_x, units_y); c.pair < p.n_pairs;
-             c.advance(stride, units_x, units_y)) {
-            const AnyItem it = any_item(p, c.ux, c.uy);
+        for (AnyCursor c = any_decode((int)blockIdx.x, r0, r1); c.d2 < r2; c.advance(stride, r0, r1)) {
+            const AnyItem it = any_item(p, IQA_ANY_UX(c), IQA_ANY_UY(c));
             mbar_wait(pfull_u32 + 8u * buf, phase);
             for (int t0 = 0; t0 < n_it; t0 += groups) {
                 const int t = t0 + t_lane;
@@ -433,7 +464,7 @@ any_kernel(const __grid_constant__ AnyParams p) {
                 }
                 const int tx = it.tx0 + jx, ty = it.ty0 + jy;
                 if (active && m == 0 && (split || (tx < p.ntx && ty < p.nty))) {
-                    const size_t tile = (size_t)c.pair * p.n_tiles + (size_t)ty * p.ntx + tx;
+                    const size_t tile = (size_t)IQA_ANY_PAIR(c) * p.n_tiles + (size_t)ty * p.ntx + tx;
                     if (!split) finalise_tile(p, tile, s, pol);
                     else p.ws[(tile * p.py + it.iy) * p.px + it.ix] = s;
                 }
@@ -486,11 +517,10 @@ any_kernel(const __grid_constant__ AnyParams p) {
     uint32_t part_phase = 0u;
     RingPos cy{0, 0, n_slots, 0u};
     Acc16 acc;
-    for (ItemCursor c = decode_item((int)blockIdx.x, units_x, units_y); c.pair < p.n_pairs;
-         c.advance(stride, units_x, units_y)) {
+    for (AnyCursor c = any_decode((int)blockIdx.x, r0, r1); c.d2 < r2; c.advance(stride, r0, r1)) {
         int rv = p.ph;
         if (!fixed) {
-            const AnyItem it = any_item(p, c.ux, c.uy);
+            const AnyItem it = any_item(p, IQA_ANY_UX(c), IQA_ANY_UY(c));
             rv = it.rv;
             lane_columns(it.s, it.cv);
         }
@@ -556,5 +586,9 @@ any_kernel(const __grid_constant__ AnyParams p) {
         if (++buf == kAnyPartBufs) { buf = 0; part_phase ^= 1u; }
     }
 }
+
+#undef IQA_ANY_PAIR
+#undef IQA_ANY_UX
+#undef IQA_ANY_UY
 
 }  // namespace iqa

@@ -49,11 +49,13 @@ bool pos_normal(float v) { return std::isfinite(v) && v >= FLT_MIN; }
 //   IQA_CAND_NO_CLUSTER  1: candidate kernels never use the cluster twins
 //   IQA_ANY_NO_WIDE      1: any_kernel never lets a lane own eight columns
 //   IQA_GENERIC_NO_VEC   1: the generic path always takes the scalar-load kernels
+//   IQA_SERIES_PAIR_MAJOR 1: any_kernel runs the comparisons of a series in pair-major item order (no L2 sharing)
 enum Knob { kKnobForceGeneric, kKnobForceAny, kKnobTmaConfig, kKnobTmaMaxCtas, kKnobNoPdl, kKnobCandNoCluster, kKnobNoWide,
-            kKnobGenericNoVec, kNumKnobs };
+            kKnobGenericNoVec, kKnobSeriesPairMajor, kNumKnobs };
 const char* const kKnobNames[kNumKnobs] = {"IQA_FORCE_GENERIC", "IQA_FORCE_ANY", "IQA_TMA_CONFIG", "IQA_TMA_MAX_CTAS",
-                                           "IQA_NO_PDL", "IQA_CAND_NO_CLUSTER", "IQA_ANY_NO_WIDE", "IQA_GENERIC_NO_VEC"};
-const int kKnobDefaults[kNumKnobs] = {0, 0, -1, 0, 0, 0, 0, 0};
+                                           "IQA_NO_PDL", "IQA_CAND_NO_CLUSTER", "IQA_ANY_NO_WIDE", "IQA_GENERIC_NO_VEC",
+                                           "IQA_SERIES_PAIR_MAJOR"};
+const int kKnobDefaults[kNumKnobs] = {0, 0, -1, 0, 0, 0, 0, 0, 0};
 struct Knobs {
     std::atomic<int> v[kNumKnobs];
     Knobs() {
@@ -524,8 +526,9 @@ int fire(const std::vector<TmaLaunch>& q, cudaStream_t st) {
 // ---- any_kernel: encode, then launch ---------------------------------------------------------------------------
 struct AnyLaunch { AnyParams p; AnyFn fn; unsigned grid; size_t smem; };
 
+// pair_minor: the pairs are the comparisons of a time series (they share images): item order of AnyCursor.
 bool prepare_any(std::vector<AnyLaunch>& q, int mode, const void* const* xs, const void* const* ys, int n_pairs,
-                 const Geom& g, int N_T, const Consts& k, const Outputs& out, float4* ws, const Plan& pl) {
+                 const Geom& g, int N_T, const Consts& k, const Outputs& out, float4* ws, const Plan& pl, bool pair_minor) {
     const Geometry* geo = geometry();
     if (!geo) return false;
     const AnyGeom& a = pl.any;
@@ -554,6 +557,7 @@ bool prepare_any(std::vector<AnyLaunch>& q, int mode, const void* const* xs, con
         p.shift = (int)(((uintptr_t)xs[0] & 15u) / (unsigned)esize_of(g.ptype));
         p.pad_mask = 16 / esize_of(g.ptype) - 1;
         p.const_s = a.const_s;
+        p.pair_minor = pair_minor && np > 1 && !knob(kKnobSeriesPairMajor) ? 1 : 0;
         p.n_pairs = np; p.W = g.W; p.H = g.H; p.N_T = N_T; p.ntx = ntx; p.nty = nty; p.n_tiles = (int)n;
         p.kx = a.kx; p.ky = a.ky; p.px = a.px; p.py = a.py; p.pw = a.pw; p.ph = a.ph;
         p.units_x = a.units_x; p.units_y = a.units_y; p.box_rows = a.box_rows; p.row_bytes = a.row_bytes;
@@ -638,7 +642,7 @@ bool finalise_is_small(int pieces, long long n) { return pieces <= 32 && n >= 64
 // S1-S4 for n_pairs pairs (xs[i], ys[i]) with the plan's kernel; `out` / `ws` point at pair 0.  The plan is
 // downgraded to the generic kernels (before anything is launched) when a tensor map cannot be encoded.
 int launch_pairs(int mode, const void* const* xs, const void* const* ys, int n_pairs, const Geom& g, int N_T,
-                 const Consts& k, const Outputs& out, float4* ws, Plan& pl, cudaStream_t st) {
+                 const Consts& k, const Outputs& out, float4* ws, Plan& pl, cudaStream_t st, bool series_order = false) {
     if (pl.kind == kPlanTma) {
         std::vector<TmaLaunch> q;
         q.reserve((size_t)ceil_div(n_pairs, kMaxImages / 2));
@@ -649,7 +653,7 @@ int launch_pairs(int mode, const void* const* xs, const void* const* ys, int n_p
     } else if (pl.kind == kPlanAny) {
         std::vector<AnyLaunch> q;
         q.reserve((size_t)ceil_div(n_pairs, kAnyMaxImages / 2));
-        if (prepare_any(q, mode, xs, ys, n_pairs, g, N_T, k, out, ws, pl)) return fire(q, st);
+        if (prepare_any(q, mode, xs, ys, n_pairs, g, N_T, k, out, ws, pl, series_order)) return fire(q, st);
         generic_plan(pl, N_T);
     }
     return launch_generic(mode, xs, ys, n_pairs, g, N_T, k, out, ws, pl, st);
@@ -797,7 +801,7 @@ int run_series(const void* const* imgs, int n_images, int series, const Geom& g,
         xs[i] = series == kReference ? imgs[0] : imgs[i];
         ys[i] = imgs[i + 1];
     }
-    if (const int rc = launch_pairs(kModeFused, xs.data(), ys.data(), K, g, N_T, k, out, ws, pl, st)) return rc;
+    if (const int rc = launch_pairs(kModeFused, xs.data(), ys.data(), K, g, N_T, k, out, ws, pl, st, true)) return rc;
     return finish_comparisons(out, out2, K, n, k, ws, pl, st);
 }
 

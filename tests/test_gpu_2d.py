@@ -406,6 +406,39 @@ def test_typed_batch_and_series(B, U, dtype, N_T):
             U.assert_parity(got, ref, k["C"], f"typed series {dtype} {mode} {c}")
 
 
+@pytest.mark.parametrize("dtype,N_T", [("float32", 48), ("float32", 150), ("int32", 64), ("float64", 20)])
+def test_typed_series_item_order(B, U, dtype, N_T):
+    """A typed / odd-N_T series is ONE any_kernel launch per 32 comparisons in pair-minor item order (the comparisons of an
+    image location on neighbouring CTAs, shared images from L2).  The order is scheduling only: bit-identical to the
+    pair-major order, for 35 comparisons (two launches), split tiles included; first, 32nd and last comparison against
+    the oracle in both modes."""
+    import torch
+    import oracle
+    rng = np.random.default_rng(N_T + 1)
+    H, W, M = 190, 330, 36
+    per16 = 16 // np.dtype(dtype).itemsize
+    pitch = -(-W // per16) * per16
+    imgs, k = [], None
+    for _ in range(M):
+        a, _, k = _typed_pair(rng, H, W, dtype)
+        imgs.append(a)
+    dev = [_typed_window(a, pitch, 0) for a in imgs]
+    assert B.plan_name(dev[0], N_T) == "tma_any"
+    for mode in ("reference", "consecutive"):
+        so = B.series_tiles_2d(dev, mode, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+        with B.knob("IQA_SERIES_PAIR_MAJOR", 1):
+            pm = B.series_tiles_2d(dev, mode, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+        torch.cuda.synchronize()
+        for n in so:
+            assert torch.equal(so[n], pm[n]), (mode, n)
+        idx = oracle.comparison_indices(M, mode)
+        for c in (0, 31, 32, M - 2):
+            ix, iy = idx[c]
+            ref = oracle.tiles_2d_any(imgs[ix], imgs[iy], N_T, **k)
+            got = {n: so[n][c].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+            U.assert_parity(got, ref, k["C"], f"series order {dtype} N_T={N_T} {mode} {c}")
+
+
 def test_paper_named_entry_points_with_odd_tile_sides(B, U):
     """iqa_lisi_tiles / iqa_auglisi_tiles / iqa_fused_tiles with N_T = 48 and 100 (N % N_T == 0): the three modes of
     any_kernel; the standalone results equal the fused ones bit for bit."""
