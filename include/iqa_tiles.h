@@ -320,6 +320,16 @@ int iqa_series_find(const float* const* img_ptrs_host, int n_images, int mode,
                     int index, int k, int* bottom_idx, float* bottom_val,
                     float threshold, int* below_idx, int capacity, int* below_counts, void* stream);
 
+/* iqa_series_find_2d_typed: the same for H x W images with a row pitch, edge tiles and any supported pixel type
+ * (arguments as iqa_series_tiles_2d_typed, then the candidate arguments of iqa_series_find); n = ceil(H / N_T) * ceil(W / N_T). */
+int iqa_series_find_2d_typed(const void* const* img_ptrs_host, int n_images, int mode, int pixel_type,
+                             int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
+                             float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                             float* lisi_num, float* auglisi_num, float* out2,
+                             void* workspace, size_t workspace_bytes,
+                             int index, int k, int* bottom_idx, float* bottom_val,
+                             float threshold, int* below_idx, int capacity, int* below_counts, void* stream);
+
 /* P:66 "a larger tile formed by merging smaller ones": apply Eqs. 3-4 to every g x g block
  * of an nt x nt tile matrix, giving the (nt/g) x (nt/g) matrices of tile size g*N_T.
  *   in:  lisi, auglisi, sum_x, sum_y  [nt*nt]

@@ -26,7 +26,7 @@ EXPORTS = ("iqa_status_string", "iqa_version", "iqa_debug_knob", "iqa_workspace_
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
            "iqa_query_plan", "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_tiles_2d_typed",
            "iqa_fused_batch_2d", "iqa_fused_batch_2d_typed", "iqa_series_tiles_2d", "iqa_series_tiles_2d_typed",
-           "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_series_find", "iqa_tiles_below", "iqa_tiles_bottom_k",
+           "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_series_find", "iqa_series_find_2d_typed", "iqa_tiles_below", "iqa_tiles_bottom_k",
            "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_merge_tiles_batch",
            "iqa_pyramid_levels", "iqa_pyramid_tiles", "iqa_pyramid",
            "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
@@ -86,6 +86,9 @@ def _load() -> ctypes.CDLL:
     lib.iqa_series_find.restype = i
     lib.iqa_series_find.argtypes = [vp, i, i, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, vp, sz,
                                     i, i, vp, vp, f, vp, i, vp, vp]
+    lib.iqa_series_find_2d_typed.restype = i
+    lib.iqa_series_find_2d_typed.argtypes = [vp, i, i, i, i, i, ctypes.c_longlong, i, f, f, f, f,
+                                             vp, vp, vp, vp, vp, vp, vp, vp, sz, i, i, vp, vp, f, vp, i, vp, vp]
     lib.iqa_query_plan.restype = i
     lib.iqa_query_plan.argtypes = [vp, i, i, i, ctypes.c_longlong, i, i]
     lib.iqa_debug_knob.restype = i
@@ -362,6 +365,19 @@ def iqa_series_find(img_ptrs_host, n_images, mode, N, N_T, C1, C2, C, D, lisi, a
                                _ptr(lisi_num), _ptr(auglisi_num), _ptr(out2), _ptr(workspace), int(workspace_bytes),
                                int(index), int(k), _ptr(bottom_idx), _ptr(bottom_val), float(threshold),
                                _ptr(below_idx), int(capacity), _ptr(below_counts), _stream(stream))
+
+
+def iqa_series_find_2d_typed(img_ptrs_host, n_images, mode, pixel_type, H, W, pitch, N_T, C1, C2, C, D,
+                             lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num, out2, workspace, workspace_bytes,
+                             index, k, bottom_idx, bottom_val, threshold, below_idx, capacity, below_counts,
+                             stream=None) -> int:
+    it, _ = _ptr_table(img_ptrs_host)
+    return lib.iqa_series_find_2d_typed(it, int(n_images), int(mode), int(pixel_type), int(H), int(W), int(pitch), int(N_T),
+                                        C1, C2, C, D, _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
+                                        _ptr(lisi_num), _ptr(auglisi_num), _ptr(out2), _ptr(workspace),
+                                        int(workspace_bytes), int(index), int(k), _ptr(bottom_idx), _ptr(bottom_val),
+                                        float(threshold), _ptr(below_idx), int(capacity), _ptr(below_counts),
+                                        _stream(stream))
 
 
 def iqa_tiles_below(values, n_tiles, n_maps, threshold, indices, capacity, counts, stream=None) -> int:
@@ -690,6 +706,43 @@ def find_transients(images, mode, N_T, C1, C2, C, D, k: int = 16, index: str = "
                              out.get("below_counts"), _current_stream(dev))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_series_find")
+    return out
+
+
+def find_transients_2d(images, mode, N_T, C1, C2, C, D, k: int = 16, index: str = "auglisi", threshold=None,
+                       capacity=None) -> dict:
+    """``find_transients`` for H x W images of any supported pixel type with a common row pitch and edge tiles
+    (``iqa_series_find_2d_typed``): the series outputs as (K, nty, ntx) tensors plus the candidate lists, tile index
+    t = ty * ntx + tx."""
+    import torch
+    if index not in ("auglisi", "lisi"):
+        raise ValueError("index must be 'auglisi' or 'lisi'")
+    if mode not in SERIES_MODES:
+        raise ValueError(f"mode must be one of {tuple(SERIES_MODES)}")
+    if len(images) < 2 or N_T <= 0:
+        raise IqaError(IQA_ERR_SHAPE, "find_transients_2d")
+    H, W, pitch, ptype = _check_2d_list(images)
+    K, nty, ntx, dev = len(images) - 1, -(-H // N_T), -(-W // N_T), images[0].device
+    out = {nm: torch.empty((K, nty, ntx), dtype=torch.float32, device=dev) for nm in ("lisi", "auglisi", "X", "Y")}
+    out["whole"] = torch.empty((K, 2), dtype=torch.float32, device=dev)
+    out["candidates"] = torch.empty((K, k), dtype=torch.int32, device=dev)
+    out["candidate_values"] = torch.empty((K, k), dtype=torch.float32, device=dev)
+    cap = 0
+    if threshold is not None:
+        cap = nty * ntx if capacity is None else int(capacity)
+        out["below"] = torch.full((K, cap), -1, dtype=torch.int32, device=dev)
+        out["below_counts"] = torch.empty(K, dtype=torch.int32, device=dev)
+    nbytes = K * iqa_workspace_bytes_2d(H, W, N_T)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev) if nbytes else None
+    with _device_of(images[0]):
+        rc = iqa_series_find_2d_typed(images, len(images), SERIES_MODES[mode], ptype, H, W, pitch, N_T, C1, C2, C, D,
+                                      out["lisi"], out["auglisi"], out["X"], out["Y"], None, None, out["whole"], ws,
+                                      nbytes, IQA_FIND_AUGLISI if index == "auglisi" else IQA_FIND_LISI, k,
+                                      out["candidates"], out["candidate_values"],
+                                      0.0 if threshold is None else float(threshold), out.get("below"), cap,
+                                      out.get("below_counts"), _current_stream(dev))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_series_find_2d_typed")
     return out
 
 

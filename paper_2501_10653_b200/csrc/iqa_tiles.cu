@@ -1050,25 +1050,20 @@ int iqa_tiles_bottom_k(const float* values, int n_tiles, int n_maps, int k,
     return cudaGetLastError() == cudaSuccess ? IQA_OK : IQA_ERR_CUDA;
 }
 
-int iqa_series_find(const float* const* img_ptrs_host, int n_images, int mode,
-                    int N, int N_T, float C1, float C2, float C, float D,
-                    float* lisi, float* auglisi, float* sum_x, float* sum_y,
-                    float* lisi_num, float* auglisi_num, float* out2,
-                    void* workspace, size_t workspace_bytes,
-                    int index, int k, int* bottom_idx, float* bottom_val,
-                    float threshold, int* below_idx, int capacity, int* below_counts, void* stream) {
-    // every argument of the candidate step is checked before the series is enqueued
+namespace {
+int check_find_args(int index, int k, const int* bottom_idx, float threshold, const int* below_idx, int capacity,
+                    const int* below_counts) {
     if (index != IQA_FIND_LISI && index != IQA_FIND_AUGLISI) return IQA_ERR_SHAPE;
     if (k < 0 || k > kMaxBottomK || capacity < 0) return IQA_ERR_SHAPE;
     if (k == 0 && !below_counts) return IQA_ERR_NULL;
     if (k > 0 && !bottom_idx) return IQA_ERR_NULL;
     if (below_counts && capacity > 0 && !below_idx) return IQA_ERR_NULL;
     if (below_counts && threshold != threshold) return IQA_ERR_PARAM;
-    if (const int rc = iqa_series_tiles(img_ptrs_host, n_images, mode, N, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
-                                        lisi_num, auglisi_num, out2, workspace, workspace_bytes, stream))
-        return rc;
-    const float* values = index == IQA_FIND_LISI ? lisi : auglisi;
-    const int n = (N / N_T) * (N / N_T), K = n_images - 1;
+    return IQA_OK;
+}
+// The candidate lists of K matrices of n tiles behind the series kernels of the same call.
+int launch_find(const float* values, int n, int K, int k, int* bottom_idx, float* bottom_val, float threshold,
+                int* below_idx, int capacity, int* below_counts, void* stream) {
     // both lists of a matrix that one CTA keeps in registers: ONE launch, the matrix is read once
     if (k > 0 && below_counts && n <= cand_threads(n) * kCandPerThread) {
         if (launch(bottom_k_kernel, (unsigned)K, (unsigned)cand_threads(n), 0, (cudaStream_t)stream, values, n, k,
@@ -1081,6 +1076,39 @@ int iqa_series_find(const float* const* img_ptrs_host, int n_images, int mode,
     if (below_counts)
         if (const int rc = iqa_tiles_below(values, n, K, threshold, below_idx, capacity, below_counts, stream)) return rc;
     return IQA_OK;
+}
+}  // namespace
+
+int iqa_series_find(const float* const* img_ptrs_host, int n_images, int mode,
+                    int N, int N_T, float C1, float C2, float C, float D,
+                    float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                    float* lisi_num, float* auglisi_num, float* out2,
+                    void* workspace, size_t workspace_bytes,
+                    int index, int k, int* bottom_idx, float* bottom_val,
+                    float threshold, int* below_idx, int capacity, int* below_counts, void* stream) {
+    // every argument of the candidate step is checked before the series is enqueued
+    if (const int rc = check_find_args(index, k, bottom_idx, threshold, below_idx, capacity, below_counts)) return rc;
+    if (const int rc = iqa_series_tiles(img_ptrs_host, n_images, mode, N, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
+                                        lisi_num, auglisi_num, out2, workspace, workspace_bytes, stream))
+        return rc;
+    return launch_find(index == IQA_FIND_LISI ? lisi : auglisi, (N / N_T) * (N / N_T), n_images - 1, k, bottom_idx,
+                       bottom_val, threshold, below_idx, capacity, below_counts, stream);
+}
+
+int iqa_series_find_2d_typed(const void* const* img_ptrs_host, int n_images, int mode, int pixel_type,
+                             int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
+                             float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                             float* lisi_num, float* auglisi_num, float* out2,
+                             void* workspace, size_t workspace_bytes,
+                             int index, int k, int* bottom_idx, float* bottom_val,
+                             float threshold, int* below_idx, int capacity, int* below_counts, void* stream) {
+    if (const int rc = check_find_args(index, k, bottom_idx, threshold, below_idx, capacity, below_counts)) return rc;
+    if (const int rc = iqa_series_tiles_2d_typed(img_ptrs_host, n_images, mode, pixel_type, H, W, pitch, N_T, C1, C2, C, D,
+                                                 lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num, out2, workspace,
+                                                 workspace_bytes, stream))
+        return rc;
+    return launch_find(index == IQA_FIND_LISI ? lisi : auglisi, ceil_div(H, N_T) * ceil_div(W, N_T), n_images - 1, k,
+                       bottom_idx, bottom_val, threshold, below_idx, capacity, below_counts, stream);
 }
 
 int iqa_merge_tiles_batch(const float* lisi, const float* auglisi,

@@ -193,6 +193,12 @@ def test_series_and_candidate_validation():
     assert find(imgs=bad) == B.IQA_ERR_NULL
     assert find(N=100) == B.IQA_ERR_SHAPE
     assert find(N_T=128) == B.IQA_ERR_WORKSPACE
+    tb = B.iqa_series_find_2d_typed(tbl, 3, B.IQA_SERIES_REFERENCE, B.IQA_PIXEL_I16, 64, 80, 80, 8, 1e-6, 1e-6, 1e-6, 5e-7,
+                                    FAKE, FAKE, FAKE, FAKE, None, None, None, None, 0, 5, 4, FAKE, None, 0.5, FAKE, 8, FAKE)
+    assert tb == B.IQA_ERR_SHAPE                                # index 5: rejected before anything else
+    tb = B.iqa_series_find_2d_typed(tbl, 3, B.IQA_SERIES_REFERENCE, 9, 64, 80, 80, 8, 1e-6, 1e-6, 1e-6, 5e-7,
+                                    FAKE, FAKE, FAKE, FAKE, None, None, None, None, 0, 1, 4, FAKE, None, 0.5, FAKE, 8, FAKE)
+    assert tb == B.IQA_ERR_SHAPE                                # unknown pixel type: the series' own validation
 
 
 def test_2d_validation():

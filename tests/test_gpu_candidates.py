@@ -208,6 +208,42 @@ def test_series_find_lists_match_oracle_selection(B, N, N_T, k):
         assert np.array_equal(out["below"][c].cpu().numpy()[:w], eb[:w])
 
 
+@pytest.mark.parametrize("dtype,N_T", [("int16", 64), ("float32", 48), ("uint8", 20)])
+def test_series_find_2d_typed(B, dtype, N_T):
+    """iqa_series_find_2d_typed on H x W windows of other pixel types (any_kernel in series item order, then the candidate
+    kernel): matrices equal to iqa_series_tiles_2d_typed, lists equal to the oracle's selection on them."""
+    import torch
+    import oracle
+    rng = np.random.default_rng(N_T)
+    H, W, M = 700, 1000, 5
+    dt = np.dtype(dtype)
+    per16 = 16 // dt.itemsize
+    pitch = -(-W // per16) * per16
+    base = rng.integers(0, 200, (H, W)) if dt.kind in "iu" else rng.normal(0.05, 0.2, (H, W))
+    dev = []
+    for m in range(M):
+        a = base.copy()
+        a[100 * m:100 * m + 40, 150 * m:150 * m + 40] = 0          # a source switched off somewhere else in every snapshot
+        buf = torch.zeros((H, pitch), dtype=getattr(torch, dtype), device="cuda")
+        buf[:, :W].copy_(torch.from_numpy(a.astype(dt)))
+        dev.append(buf[:, :W])
+    kw = dict(C1=1e-3, C2=1e-3, C=1e-3, D=5e-4)
+    plain = B.series_tiles_2d(dev, "consecutive", N_T, **kw)
+    mats = plain["auglisi"].cpu().numpy()
+    thr = float(np.quantile(mats[0], 0.05))
+    out = B.find_transients_2d(dev, "consecutive", N_T, k=9, threshold=thr, capacity=30, **kw)
+    torch.cuda.synchronize()
+    assert torch.equal(out["auglisi"], plain["auglisi"]) and torch.equal(out["whole"], plain["whole"])
+    for c in range(M - 1):
+        ei, ev = oracle.bottom_k(mats[c], 9)
+        assert np.array_equal(out["candidates"][c].cpu().numpy(), ei), c
+        assert np.array_equal(out["candidate_values"][c].cpu().numpy(), ev), c
+        eb = oracle.below_threshold(mats[c], thr)
+        assert int(out["below_counts"][c]) == eb.size
+        w = min(eb.size, 30)
+        assert np.array_equal(out["below"][c].cpu().numpy()[:w], eb[:w])
+
+
 def test_candidate_error_codes(B):
     import torch
     v = torch.zeros((4, 4), dtype=torch.float32, device="cuda")
