@@ -32,7 +32,10 @@ template <typename T> struct VecGeom {
     static constexpr int kAL = 16 / kES;                  // elements per 16 bytes
     static constexpr int kSlotE = kAL < 4 ? 4 : kAL;      // elements per slot (fp64: two 16-byte groups)
     static constexpr int kVecs = kSlotE / kAL;            // 16-byte loads per slot and image
-    static constexpr int kInFlight = kVecs == 1 ? kVecInFlight : 2;   // slots a thread loads before it computes
+    // slots a thread loads before it computes: 4 (fp32 / int32), 6 for 1- and 2-byte pixels (measured: int16 3.7 -> 4.1 TB/s,
+    // fp32 loses with 6), 2 for fp64 (two groups per slot).  A software pipeline (next round's loads in flight while this
+    // round is computed) needs more than the 80 registers that three CTAs per SM leave and was slower in every variant.
+    static constexpr int kInFlight = kVecs == 2 ? 2 : kES <= 2 ? 6 : kVecInFlight;
 };
 
 // Zero the elements of one 16-byte group whose tile column c_first + e is outside [0, cols_t).
@@ -85,11 +88,11 @@ __device__ __forceinline__ float4 vec_tile_sums(const T* __restrict__ x, const T
     uintptr_t ty = (uintptr_t)(y + row0 * (size_t)pitch_y + col0) + (uintptr_t)((long long)r * pby);
     const long long sx = (long long)dr * pbx, sy = (long long)dr * pby;
     const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
-    for (int k0 = tid; k0 < n_slots; k0 += group * G::kInFlight) {
-        uint4 vx[G::kInFlight][G::kVecs], vy[G::kInFlight][G::kVecs];
-        int cl[G::kInFlight];
+    constexpr int U = G::kInFlight, V = G::kVecs;
+    // one round = U slots of this thread: issue their loads (advancing the thread's (row, slot) position) ...
+    auto load_round = [&](int k0, uint4 (&vx)[U][V], uint4 (&vy)[U][V], int (&cl)[U]) {
 #pragma unroll
-        for (int u = 0; u < G::kInFlight; ++u) {
+        for (int u = 0; u < U; ++u) {
             const bool live = k0 + u * group < n_slots;
             const int a = (int)(tx & 15u) / G::kES;
             const int c_lo = q * G::kSlotE - a;                       // tile column of the slot's first element
@@ -97,7 +100,7 @@ __device__ __forceinline__ float4 vec_tile_sums(const T* __restrict__ x, const T
             const uint4* px = reinterpret_cast<const uint4*>((tx & ~(uintptr_t)15u) + (uintptr_t)(q * (G::kSlotE * G::kES)));
             const uint4* py = reinterpret_cast<const uint4*>((ty & ~(uintptr_t)15u) + (uintptr_t)(q * (G::kSlotE * G::kES)));
 #pragma unroll
-            for (int v = 0; v < G::kVecs; ++v) {
+            for (int v = 0; v < V; ++v) {
                 const int cf = c_lo + v * G::kAL;
                 const bool any = live && cf < cols_t && cf + G::kAL > 0;
                 vx[u][v] = any ? __ldg(px + v) : zero;
@@ -106,16 +109,25 @@ __device__ __forceinline__ float4 vec_tile_sums(const T* __restrict__ x, const T
             q += dq; tx += sx; ty += sy;
             if (q >= qmax) { q -= qmax; tx += pbx; ty += pby; }
         }
+    };
+    // ... and, a round later, mask them and add their terms
+    auto compute_round = [&](uint4 (&vx)[U][V], uint4 (&vy)[U][V], const int (&cl)[U]) {
 #pragma unroll
-        for (int u = 0; u < G::kInFlight; ++u) {
+        for (int u = 0; u < U; ++u) {
 #pragma unroll
-            for (int v = 0; v < G::kVecs; ++v) mask_group<T>(vx[u][v], vy[u][v], cl[u] + v * G::kAL, cols_t);
+            for (int v = 0; v < V; ++v) mask_group<T>(vx[u][v], vy[u][v], cl[u] + v * G::kAL, cols_t);
             const uint32_t* wx = reinterpret_cast<const uint32_t*>(&vx[u][0]);
             const uint32_t* wy = reinterpret_cast<const uint32_t*>(&vy[u][0]);
             constexpr int kW = Pixel4<T>::kWords;
 #pragma unroll
             for (int c = 0; c < G::kSlotE / 4; ++c) Pixel4<T>::template terms<MODE>(wx + c * kW, wy + c * kW, C1, acc);
         }
+    };
+    for (int k0 = tid; k0 < n_slots; k0 += group * U) {
+        uint4 vx[U][V], vy[U][V];
+        int cl[U];
+        load_round(k0, vx, vy, cl);
+        compute_round(vx, vy, cl);
     }
     return acc_cols(acc);
 }
