@@ -85,3 +85,55 @@ def test_random_series_cases(B, U, case):
         exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], K["C2"], K["C"])
         w = got["whole"][c].cpu().numpy()
         assert abs(w[0] - exp[0]) <= 1e-5 * abs(exp[0]) and abs(w[1] - exp[1]) <= 1e-5 * abs(exp[1]) + 1e-6
+
+
+@pytest.mark.parametrize("case", range(24))
+def test_random_typed_series_find_cases(B, U, case):
+    """iqa_series_find_2d_typed on random windows: every pixel type, tile sides of any kind, row pitches with and
+    without a tensor map (any_kernel in series item order / tma_kernel series modes / generic kernels pair by pair),
+    then the candidate lists -- matrices against the oracle, lists against the oracle's selection on the device matrices."""
+    import torch
+    import oracle
+    rng = np.random.default_rng(3000 + case)
+    H, W = int(rng.integers(8, 400)), int(rng.integers(8, 500))
+    N_T = int(rng.choice([8, 16, 64, 128, 4, 7, 20, 48, 100, 150]))
+    M = int(rng.integers(2, 6))
+    dtype = np.dtype(["float32", "float64", "float16", "int16", "int32", "uint8"][case % 6])
+    per16 = 16 // dtype.itemsize
+    pitch = W + int(rng.integers(0, 9))
+    if rng.random() < 0.7:
+        pitch = -(-pitch // per16) * per16
+    off = int(rng.integers(0, per16)) if rng.random() < 0.4 else 0
+    mode = ["reference", "consecutive"][(case // 6) % 2]
+    if dtype.kind in "iu":
+        lo = 0 if dtype == np.uint8 else -50
+        imgs = [rng.integers(lo, 250, (H, W)).astype(dtype) for _ in range(M)]
+        k = dict(C1=1e-3, C2=1e-3, C=1e-3, D=5e-4)
+    else:
+        imgs = [rng.normal(0.05, 0.2, (H, W)).astype(dtype) for _ in range(M)]
+        k = K
+    for j in range(1, M):
+        m = rng.random((H, W)) < 0.5
+        imgs[j][m] = imgs[j - 1][m]
+    dev = [_window(a, pitch, off) for a in imgs]
+    nty, ntx = -(-H // N_T), -(-W // N_T)
+    kk = int(rng.integers(1, 40))
+    index = ["auglisi", "lisi"][case % 2]
+    plain = B.series_tiles_2d(dev, mode, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    thr = float(np.quantile(plain[index].cpu().numpy(), 0.3))
+    out = B.find_transients_2d(dev, mode, N_T, k["C1"], k["C2"], k["C"], k["D"], k=kk, index=index, threshold=thr)
+    torch.cuda.synchronize()
+    what = f"find case {case}: {H}x{W} N_T={N_T} M={M} {mode} {dtype} pitch={pitch} off={off} k={kk}"
+    for c, (ix, iy) in enumerate(oracle.comparison_indices(M, mode)):
+        ref = oracle.tiles_2d_any(imgs[ix], imgs[iy], N_T, **k)
+        g = {n: plain[n][c].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+        U.assert_parity(g, ref, k["C"], what + f" cmp {c}")
+        assert torch.equal(out[index][c], plain[index][c]), what
+        mat = out[index][c].cpu().numpy()
+        ei, ev = oracle.bottom_k(mat, kk)
+        n_real = ei.size
+        assert np.array_equal(out["candidates"][c].cpu().numpy()[:n_real], ei), what
+        assert np.array_equal(out["candidate_values"][c].cpu().numpy()[:n_real], ev), what
+        eb = oracle.below_threshold(mat, thr)
+        assert int(out["below_counts"][c]) == eb.size, what
+        assert np.array_equal(out["below"][c].cpu().numpy()[:eb.size], eb), what
