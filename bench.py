@@ -479,6 +479,7 @@ PATH_ROWS = [
     ("f32_NT48", "float32", 8192, 8192, 8192, 0, 48), ("f32_NT100", "float32", 8192, 8192, 8192, 0, 100),
     ("f32_NT50", "float32", 8192, 8192, 8192, 0, 50), ("f32_NT64_base4B", "float32", 8192, 8188, 8192, 1, 64),
     ("f32_NT100_base4B", "float32", 8192, 8188, 8192, 3, 100), ("f32_NT300_split", "float32", 8192, 8192, 8192, 0, 300),
+    ("f32_NT130_split", "float32", 8192, 8192, 8192, 0, 130), ("i16_NT200_split", "int16", 8192, 8192, 8192, 0, 200),
     ("f16_NT64", "float16", 8192, 8192, 8192, 0, 64), ("i16_NT64", "int16", 8192, 8192, 8192, 0, 64),
     ("u8_NT64", "uint8", 8192, 8192, 8192, 0, 64), ("f64_NT64", "float64", 8192, 8192, 8192, 0, 64),
     ("i32_NT64", "int32", 8192, 8192, 8192, 0, 64), ("f16_NT100", "float16", 8192, 8192, 8192, 0, 100),

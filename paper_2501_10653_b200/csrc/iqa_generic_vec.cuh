@@ -161,8 +161,9 @@ generic_vec_kernel(const GenericParams g, long long n_units) {
     const int ty = (int)(tile / p.nt), tx = (int)(tile % p.nt);
     const int rows_t = min(N_T, p.H - ty * N_T);             // edge tiles hold only the pixels that exist
     const int cols_t = min(N_T, p.N - tx * N_T);
-    const int r_begin = piece * kGenericRows;
-    const int r_end = min(rows_t, r_begin + kGenericRows);
+    const int rpp = (N_T + g.pieces - 1) / g.pieces;          // rows per piece: ceil(N_T / 64) pieces of equal height
+    const int r_begin = piece * rpp;
+    const int r_end = min(rows_t, r_begin + rpp);
     float4 v = vec_tile_sums<MODE, T>(reinterpret_cast<const T*>(p.x), reinterpret_cast<const T*>(p.y), p.pitch_x,
                                       p.pitch_y, (size_t)ty * N_T + r_begin, r_end - r_begin, (size_t)tx * N_T, cols_t,
                                       p.C1, lane, 32);

@@ -185,7 +185,7 @@ constexpr int kWarpInFlight = 8;         // generic_warp_kernel: pixel pairs a l
 struct GenericParams {
     TileParams tp;
     int N_T;
-    int pieces;               // ceil(N_T / kGenericRows)
+    int pieces;               // ceil(N_T / kGenericRows) pieces of ceil(N_T / pieces) rows
 };
 
 template <int MODE, typename T = float>
@@ -201,8 +201,9 @@ generic_kernel(const GenericParams g) {
     const int ty = tile / p.nt, tx = tile % p.nt;
     const int rows_t = min(N_T, p.H - ty * N_T);             // edge tiles hold only the pixels that exist
     const int cols_t = min(N_T, p.N - tx * N_T);
-    const int r_begin = piece * kGenericRows;
-    const int r_end = min(rows_t, r_begin + kGenericRows);
+    const int rpp = (N_T + g.pieces - 1) / g.pieces;          // rows per piece: ceil(N_T / 64) pieces of equal height
+    const int r_begin = piece * rpp;
+    const int r_end = min(rows_t, r_begin + rpp);
     const long long npix = r_end > r_begin ? (long long)(r_end - r_begin) * cols_t : 0;
     const size_t row0 = (size_t)ty * N_T + r_begin, col0 = (size_t)tx * N_T;
 

@@ -268,14 +268,25 @@ def _typed_window(a, pitch, off):
 def _check_typed(B, U, x, y, xd, yd, N_T, k, what, plan="tma_any"):
     import torch
     import oracle
+    ref = oracle.tiles_2d_any(x, y, N_T, **k)
+
+    def run(tag):
+        got = B.fused_tiles_2d(xd, yd, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+        torch.cuda.synchronize()
+        g = {n: v.cpu().numpy().astype(np.float64) for n, v in got.items()}
+        U.assert_parity(g, ref, k["C"], what + tag)
+        return got
+
+    if plan == "tma_any" and B.plan_name(xd, N_T) == "generic":
+        # the plan sends shapes that fill few lanes of any_kernel to the 128-bit generic kernel: check that path as
+        # the library takes it, then any_kernel itself on the same shape (IQA_FORCE_ANY)
+        run(" (default plan: generic)")
+        with B.knob("IQA_FORCE_ANY", 1):
+            assert B.plan_name(xd, N_T) == "tma_any", what
+            return run(" (forced any_kernel)"), ref
     if plan is not None:
         assert B.plan_name(xd, N_T) == plan, (what, B.plan_name(xd, N_T))
-    got = B.fused_tiles_2d(xd, yd, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
-    torch.cuda.synchronize()
-    g = {n: v.cpu().numpy().astype(np.float64) for n, v in got.items()}
-    ref = oracle.tiles_2d_any(x, y, N_T, **k)
-    U.assert_parity(g, ref, k["C"], what)
-    return got, ref
+    return run(""), ref
 
 
 ANY_SHAPES = [
@@ -423,11 +434,12 @@ def test_typed_series_item_order(B, U, dtype, N_T):
         a, _, k = _typed_pair(rng, H, W, dtype)
         imgs.append(a)
     dev = [_typed_window(a, pitch, 0) for a in imgs]
-    assert B.plan_name(dev[0], N_T) == "tma_any"
     for mode in ("reference", "consecutive"):
-        so = B.series_tiles_2d(dev, mode, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
-        with B.knob("IQA_SERIES_PAIR_MAJOR", 1):
-            pm = B.series_tiles_2d(dev, mode, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+        with B.knob("IQA_FORCE_ANY", 1):                 # (the plan would send the split N_T = 150 to the generic kernel)
+            assert B.plan_name(dev[0], N_T) == "tma_any"
+            so = B.series_tiles_2d(dev, mode, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+            with B.knob("IQA_SERIES_PAIR_MAJOR", 1):
+                pm = B.series_tiles_2d(dev, mode, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
         torch.cuda.synchronize()
         for n in so:
             assert torch.equal(so[n], pm[n]), (mode, n)
@@ -447,12 +459,14 @@ def test_paper_named_entry_points_with_odd_tile_sides(B, U):
     for N, N_T in ((960, 48), (1200, 100), (1000, 250)):
         x, y, k = _typed_pair(rng, N, N, "float32")
         xd, yd = U.to_dev(x), U.to_dev(y)
-        assert B.plan_name(xd, N_T) == "tma_any"
-        f, _, _ = U.check_pair(x, y, N_T, k, f"square any N_T={N_T}", xd=xd, yd=yd)
-        fo = B.fused_tiles(xd, yd, N_T, **k)
-        li = B.lisi_tiles(xd, yd, N_T, k["C1"], k["C2"], k["D"])
-        au = B.auglisi_tiles(xd, yd, N_T, k["C"])
-        assert torch.equal(li, fo["lisi"]) and torch.equal(au, fo["auglisi"])
+        for force in (0, 1):                             # the library's plan (N_T = 250: generic kernel), then any_kernel
+            with B.knob("IQA_FORCE_ANY", force):
+                assert B.plan_name(xd, N_T) == ("generic" if N_T == 250 and not force else "tma_any")
+                f, _, _ = U.check_pair(x, y, N_T, k, f"square any N_T={N_T} force={force}", xd=xd, yd=yd)
+                fo = B.fused_tiles(xd, yd, N_T, **k)
+                li = B.lisi_tiles(xd, yd, N_T, k["C1"], k["C2"], k["D"])
+                au = B.auglisi_tiles(xd, yd, N_T, k["C"])
+                assert torch.equal(li, fo["lisi"]) and torch.equal(au, fo["auglisi"])
 
 
 def test_unaligned_bases(B, U):
