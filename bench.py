@@ -605,6 +605,33 @@ def measure_series_any(torch, binding, steps, warmup, device, use_graph, M=9, N=
     return out
 
 
+PLAN_SWEEP_NT = (66, 70, 113, 120, 130, 150, 170, 200, 230, 260, 330, 400)
+
+
+def measure_plan_sweep(torch, binding, steps, warmup, device, use_graph):
+    """The sweep behind the plan-by-lane-fill rule: for tile sides where any_kernel leaves lanes idle, the
+    library's own plan against any_kernel forced (IQA_FORCE_ANY) and the 128-bit generic kernel forced (IQA_FORCE_GENERIC);
+    2 pairs of 8192 x 8192 per step, GB/s on each row's own algorithmic bytes."""
+    rows = [(f"{dt}_NT{nt}", dt, 8192, 8192, 8192, 0, nt) for dt in ("float32", "int16", "float64", "uint8")
+            for nt in PLAN_SWEEP_NT]
+    rows += [("float32_NT64_off1", "float32", 8192, 8188, 8192, 1, 64), ("float32_NT32_off1", "float32", 8192, 8188, 8192, 1, 32),
+             ("int16_NT64_off1", "int16", 8192, 8184, 8192, 1, 64), ("float32_NT16_off1", "float32", 8192, 8188, 8192, 1, 16)]
+    out = {}
+    for r in rows:
+        res = {}
+        for label, kn in (("plan", None), ("any", "IQA_FORCE_ANY"), ("generic", "IQA_FORCE_GENERIC")):
+            if kn is None:
+                m = measure_paths(torch, binding, steps, warmup, device, use_graph, rows=[r], pairs=2)
+            else:
+                with binding.knob(kn, 1):
+                    m = measure_paths(torch, binding, steps, warmup, device, use_graph, rows=[r], pairs=2)
+            res[label] = {"kernel": m[r[0]]["plan"], "GBps": round(m[r[0]]["GBps"])}
+        best = max(res["any"]["GBps"], res["generic"]["GBps"])
+        res["plan_below_best_pct"] = round(100.0 * (1.0 - res["plan"]["GBps"] / best), 1)
+        out[r[0]] = res
+    return out
+
+
 def series_bytes(N: int, N_T: int, M: int) -> int:
     """Algorithmic bytes of one iqa_series_tiles call: every image read once + 16 B per tile and comparison."""
     return 4 * N * N * M + 16 * (N // N_T) ** 2 * (M - 1)
@@ -782,6 +809,10 @@ def run_ours(args):
         res = measure_paths(torch, binding, args.steps, args.warmup, device, not args.no_graph, rows=rows)
         print(json.dumps({"metric": METRIC, "unit": UNIT, "library_version": binding.iqa_version(), "paths": res}))
         return
+    if args.plan_sweep:
+        res = measure_plan_sweep(torch, binding, max(3, min(args.steps, 10)), 3, device, not args.no_graph)
+        print(json.dumps({"metric": METRIC, "unit": UNIT, "library_version": binding.iqa_version(), "plan_sweep": res}))
+        return
     if args.series_only:
         # only the time-series / candidate rows of the config [3] sky (ncu captures of the series and candidate kernels)
         res = measure_series(torch, binding, synth.CONFIGS[3], args.series_images, max(3, min(args.steps, 10)), 3, device,
@@ -938,6 +969,8 @@ def main():
     ap.add_argument("--series-images", type=int, default=9, help="snapshots of the time-series measurement in `also`")
     ap.add_argument("--nt", type=int, default=0, help="override the workload's tile side N_T (a point of the config [2] sweep)")
     ap.add_argument("--paths", default="", help="comma-separated rows of PATH_ROWS: time only those kernel paths and print them")
+    ap.add_argument("--plan-sweep", action="store_true",
+                    help="any_kernel against the generic kernel over tile sides that leave lanes idle (the plan rule's evidence)")
     ap.add_argument("--series-only", action="store_true",
                     help="time only the time-series rows (N = 8192, N_T = 64) with their candidate lists and print them")
     ap.add_argument("--sweep", action="store_true", help="also time BASELINE.json config [2] (N=2048, N_T = 8..512)")
