@@ -557,34 +557,37 @@ def measure_paths(torch, binding, steps, warmup, device, use_graph, rows=PATH_RO
     return out
 
 
-SERIES_ANY_ROWS = [("f32_NT48", "float32", 48), ("f64_NT64", "float64", 64), ("i32_NT64", "int32", 64), ("i16_NT64", "int16", 64)]
+# (row name, pixel dtype, N_T, width W, row pitch in elements)
+SERIES_ANY_ROWS = [("f32_NT48", "float32", 48, 8192, 8192), ("f64_NT64", "float64", 64, 8192, 8192),
+                   ("i32_NT64", "int32", 64, 8192, 8192), ("i16_NT64", "int16", 64, 8192, 8192),
+                   ("generic_f32_NT64_pitch8190", "float32", 64, 8190, 8190)]
 
 
 def measure_series_any(torch, binding, steps, warmup, device, use_graph, M=9, N=8192, rows=SERIES_ANY_ROWS):
     """Time series of shapes / pixel types tma_kernel does not take (SURVEY.md 8(f)-2 + 8(f)-4): M snapshots through
-    iqa_series_tiles_2d_typed, i.e. K = M - 1 pair computations in one any_kernel launch whose item order puts the
+    iqa_series_tiles_2d_typed, i.e. K = M - 1 pair computations in one any_kernel (or 128-bit generic kernel) launch whose item order puts the
     comparisons of one image location on neighbouring CTAs (an image shared by two comparisons comes from DRAM once,
     from L2 afterwards).  `pair_major` = the same call with that order switched off (IQA_SERIES_PAIR_MAJOR)."""
     out = {}
     k = PATH_CONSTS
     K = M - 1
-    for name, dtype, N_T in rows:
+    for name, dtype, N_T, W, pitch in rows:
         dt = getattr(torch, dtype)
         es = torch.empty((), dtype=dt).element_size()
-        xs, ys = make_path_inputs(torch, (name, dtype, N, N, N, 0, N_T), (M + 1) // 2, device)
+        xs, ys = make_path_inputs(torch, (name, dtype, N, W, pitch, 0, N_T), (M + 1) // 2, device)
         imgs = (xs + ys)[:M]
-        ntx = -(-N // N_T)
-        n = ntx * ntx
+        n = -(-N // N_T) * -(-W // N_T)
         o = [torch.empty((K, n), dtype=torch.float32, device=device) for _ in range(4)]
         out2 = torch.empty((K, 2), dtype=torch.float32, device=device)
-        wsb = K * binding.iqa_workspace_bytes_2d(N, N, N_T)
+        wsb = K * binding.iqa_workspace_bytes_2d(N, W, N_T)
         ws = torch.empty(wsb, dtype=torch.uint8, device=device) if wsb else None
         table, _ = binding._ptr_table(imgs)
         ptype = binding._pixel_types()[dt]
-        row = {"pixel": dtype, "N": N, "N_T": N_T, "images": M, "plan": binding.plan_name(imgs[0], N_T)}
+        row = {"pixel": dtype, "H": N, "W": W, "pitch": pitch, "N_T": N_T, "images": M,
+               "plan": binding.plan_name(imgs[0], N_T, series=True)}
         for mode_name, mode in binding.SERIES_MODES.items():
             def step():
-                rc = binding.iqa_series_tiles_2d_typed(table, M, mode, ptype, N, N, N, N_T, *k, *o, None, None, out2, ws, wsb,
+                rc = binding.iqa_series_tiles_2d_typed(table, M, mode, ptype, N, W, pitch, N_T, *k, *o, None, None, out2, ws, wsb,
                                                        torch.cuda.current_stream().cuda_stream)
                 if rc:
                     raise binding.IqaError(rc, "iqa_series_tiles_2d_typed")
@@ -595,9 +598,9 @@ def measure_series_any(torch, binding, steps, warmup, device, use_graph, M=9, N=
                     for _ in range(warmup):
                         fn()
                     res[label] = time_region(torch, fn, steps) * 1e3 / (steps * K)
-            series_b = es * N * N * M + 16 * n * K
+            series_b = es * N * W * M + 16 * n * K
             res["dram_GBps_series_bytes"] = series_b / K / (res["us_per_comparison"] * 1e-6) / 1e9
-            res["pairwise_equivalent_GBps"] = (2 * es * N * N + 16 * n) / (res["us_per_comparison"] * 1e-6) / 1e9
+            res["pairwise_equivalent_GBps"] = (2 * es * N * W + 16 * n) / (res["us_per_comparison"] * 1e-6) / 1e9
             row[mode_name] = res
         out[name] = row
         del xs, ys, imgs, o, ws

@@ -142,35 +142,52 @@ __device__ __forceinline__ float4 warp_sum4(float4 v) {
     return v;
 }
 
-// One WARP per (tile, piece of up to kGenericRows rows), eight units per CTA: the units are independent streams
+// The pairs of one launch: image pointers in the kernel parameters (a batch of independent pairs, or the comparisons of
+// a time series, which share images).
+constexpr int kVecMaxPairs = 32;
+struct VecBatch {
+    const void* x[kVecMaxPairs];
+    const void* y[kVecMaxPairs];
+    int n_pairs;
+    int pair_minor;      // unit order: 0 = pair-major; 1 = the pairs of one tile piece next to each other (series: an image
+                         // shared by two comparisons comes from DRAM once and from L2 afterwards, as in any_kernel)
+};
+
+// One WARP per (pair, tile, piece of ceil(N_T / pieces) rows), eight units per CTA: the units are independent streams
 // (no CTA barrier, no serial tail per tile), so the loads of up to 24 warps per SM overlap.  (A CTA per tile -- the
 // mapping of the scalar generic_kernel -- was measured at 3.7 TB/s here: a 64 x 64 tile is 32 KiB, and a CTA that
 // loads, reduces and exits leaves the SM waiting on one DRAM latency per tile.)  pieces == 1: the warp finalises its
-// tile; otherwise the partial goes to the workspace [tile][piece] and finalise_*_kernel finishes.
+// tile; otherwise the partial goes to the workspace [pair][tile][piece] and finalise_*_kernel finishes.
+// g.tp.x / g.tp.y are unused (the images are b.x / b.y); the output arrays and the workspace start at pair 0 of the launch.
 template <int MODE, typename T>
 __global__ void __launch_bounds__(kCtaThreads, 3)
-generic_vec_kernel(const GenericParams g, long long n_units) {
+generic_vec_kernel(const GenericParams g, const __grid_constant__ VecBatch b, long long units_per_pair) {
     pdl_prologue();
     const TileParams& p = g.tp;
     const int N_T = g.N_T;
     const long long unit = (long long)blockIdx.x * kWarpsPerCta + (threadIdx.x >> 5);
-    if (unit >= n_units) return;
+    if (unit >= units_per_pair * b.n_pairs) return;
     const int lane = threadIdx.x & 31;
-    const long long tile = unit / g.pieces;
-    const int piece = (int)(unit - tile * g.pieces);
+    int pair;
+    long long v_unit;                                        // (tile, piece) inside the pair
+    if (b.pair_minor) { v_unit = unit / b.n_pairs; pair = (int)(unit - v_unit * b.n_pairs); }
+    else { pair = (int)(unit / units_per_pair); v_unit = unit - pair * units_per_pair; }
+    const long long tile = v_unit / g.pieces;
+    const int piece = (int)(v_unit - tile * g.pieces);
     const int ty = (int)(tile / p.nt), tx = (int)(tile % p.nt);
     const int rows_t = min(N_T, p.H - ty * N_T);             // edge tiles hold only the pixels that exist
     const int cols_t = min(N_T, p.N - tx * N_T);
     const int rpp = (N_T + g.pieces - 1) / g.pieces;          // rows per piece: ceil(N_T / 64) pieces of equal height
     const int r_begin = piece * rpp;
     const int r_end = min(rows_t, r_begin + rpp);
-    float4 v = vec_tile_sums<MODE, T>(reinterpret_cast<const T*>(p.x), reinterpret_cast<const T*>(p.y), p.pitch_x,
+    float4 v = vec_tile_sums<MODE, T>(reinterpret_cast<const T*>(b.x[pair]), reinterpret_cast<const T*>(b.y[pair]), p.pitch_x,
                                       p.pitch_y, (size_t)ty * N_T + r_begin, r_end - r_begin, (size_t)tx * N_T, cols_t,
                                       p.C1, lane, 32);
     v = warp_sum4(v);
     if (lane == 0) {
-        if (p.ws == nullptr) finalise_tile(p, (size_t)tile, v);
-        else p.ws[(size_t)tile * g.pieces + piece] = v;
+        const size_t t = (size_t)pair * (size_t)(units_per_pair / g.pieces) + (size_t)tile;
+        if (p.ws == nullptr) finalise_tile(p, t, v);
+        else p.ws[t * g.pieces + piece] = v;
     }
 }
 

@@ -15,6 +15,7 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <type_traits>
 #include <utility>
 #include <vector>
 
@@ -608,27 +609,46 @@ int fire(const std::vector<AnyLaunch>& q, cudaStream_t st) {
 }
 
 // ---- generic kernels (pair by pair) ---------------------------------------------------------------------------
-// vec: x and y have the same alignment row by row -> the warp-per-piece kernel with 128-bit loads (iqa_generic_vec.cuh)
+// The scalar-load generic kernels, one pair per launch.
 template <int MODE, typename T>
-cudaError_t launch_generic_one(const GenericParams& g, long long n, int N_T, int pieces, bool vec, cudaStream_t st) {
-    if (vec) {
-        const long long units = n * pieces;
-        return launch(generic_vec_kernel<MODE, T>, (unsigned)((units + kWarpsPerCta - 1) / kWarpsPerCta), kCtaThreads, 0, st,
-                      g, units);
-    }
+cudaError_t launch_generic_one(const GenericParams& g, long long n, int N_T, int pieces, cudaStream_t st) {
     if ((long long)N_T * N_T <= kWarpTilePixels)          // small tiles: one warp per tile (pieces == 1 here)
         return launch(generic_warp_kernel<MODE, T>, (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta), kCtaThreads, 0, st, g, n);
     return launch(generic_kernel<MODE, T>, (unsigned)(n * pieces), kCtaThreads, 0, st, g);
 }
+// The warp-per-piece kernel with 128-bit loads (iqa_generic_vec.cuh): up to kVecMaxPairs pairs per launch.
+template <int MODE, typename T>
+cudaError_t launch_generic_vec(const GenericParams& g, const VecBatch& b, long long n, int pieces, cudaStream_t st) {
+    const long long upp = n * pieces, units = upp * b.n_pairs;
+    return launch(generic_vec_kernel<MODE, T>, (unsigned)((units + kWarpsPerCta - 1) / kWarpsPerCta), kCtaThreads, 0, st, g, b,
+                  upp);
+}
+template <typename F32, typename Other>
+cudaError_t by_pixel_type(int ptype, int mode, F32&& f32, Other&& other) {
+    switch (ptype) {
+        case IQA_PIXEL_F64: return other((double*)nullptr);
+        case IQA_PIXEL_F16: return other((__half*)nullptr);
+        case IQA_PIXEL_I16: return other((short*)nullptr);
+        case IQA_PIXEL_I32: return other((int*)nullptr);
+        case IQA_PIXEL_U8: return other((unsigned char*)nullptr);
+        default: return f32(mode);
+    }
+}
+
+// series_order: the pairs are the comparisons of a time series (pair-minor unit order in the 128-bit kernel).
 int launch_generic(int mode, const void* const* xs, const void* const* ys, int n_pairs, const Geom& g2, int N_T,
-                   const Consts& k, const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st) {
+                   const Consts& k, const Outputs& out, float4* ws, const Plan& pl, cudaStream_t st, bool series_order) {
     const int nt = ceil_div(g2.W, N_T);
     const long long n = (long long)nt * ceil_div(g2.H, N_T);
     if (n * pl.pieces > 0x7fffffffLL) return IQA_ERR_SHAPE;
     const int es = esize_of(g2.ptype);
-    for (int i = 0; i < n_pairs; ++i) {
-        const bool vec = !knob(kKnobGenericNoVec) && (((uintptr_t)xs[i] ^ (uintptr_t)ys[i]) & 15u) == 0 &&
-                         (((g2.pitch_x - g2.pitch_y) * es) & 15) == 0;
+    // x and y aligned alike row by row (every pair): the kernel with 128-bit loads, kVecMaxPairs pairs per launch
+    bool vec = !knob(kKnobGenericNoVec) && (((g2.pitch_x - g2.pitch_y) * es) & 15) == 0;
+    for (int i = 0; i < n_pairs && vec; ++i) vec = (((uintptr_t)xs[i] ^ (uintptr_t)ys[i]) & 15u) == 0;
+    const int per_launch = vec ? kVecMaxPairs : 1;
+    if (n * pl.pieces * per_launch > 0x7fffffffLL) return IQA_ERR_SHAPE;
+    for (int i = 0; i < n_pairs; i += per_launch) {
+        const int np = n_pairs - i < per_launch ? n_pairs - i : per_launch;
         GenericParams g{};
         TileParams& p = g.tp;
         p.x = (const float*)xs[i]; p.y = (const float*)ys[i]; p.N = g2.W; p.H = g2.H; p.nt = nt;
@@ -640,16 +660,24 @@ int launch_generic(int mode, const void* const* xs, const void* const* ys, int n
         p.ws = (ws && pl.pieces > 1) ? ws + (size_t)i * (size_t)n * pl.pieces : nullptr;
         g.N_T = N_T; g.pieces = pl.pieces;
         cudaError_t e;
-        switch (g2.ptype) {
-            case IQA_PIXEL_F64: e = launch_generic_one<kModeFused, double>(g, n, N_T, pl.pieces, vec, st); break;
-            case IQA_PIXEL_F16: e = launch_generic_one<kModeFused, __half>(g, n, N_T, pl.pieces, vec, st); break;
-            case IQA_PIXEL_I16: e = launch_generic_one<kModeFused, short>(g, n, N_T, pl.pieces, vec, st); break;
-            case IQA_PIXEL_I32: e = launch_generic_one<kModeFused, int>(g, n, N_T, pl.pieces, vec, st); break;
-            case IQA_PIXEL_U8: e = launch_generic_one<kModeFused, unsigned char>(g, n, N_T, pl.pieces, vec, st); break;
-            default:
-                e = mode == kModeLisi  ? launch_generic_one<kModeLisi, float>(g, n, N_T, pl.pieces, vec, st)
-                    : mode == kModeAug ? launch_generic_one<kModeAug, float>(g, n, N_T, pl.pieces, vec, st)
-                                       : launch_generic_one<kModeFused, float>(g, n, N_T, pl.pieces, vec, st);
+        if (vec) {
+            VecBatch b{};
+            for (int j = 0; j < np; ++j) { b.x[j] = xs[i + j]; b.y[j] = ys[i + j]; }
+            b.n_pairs = np;
+            b.pair_minor = series_order && np > 1 && !knob(kKnobSeriesPairMajor) ? 1 : 0;
+            e = by_pixel_type(g2.ptype, mode,
+                [&](int m) { return m == kModeLisi  ? launch_generic_vec<kModeLisi, float>(g, b, n, pl.pieces, st)
+                                    : m == kModeAug ? launch_generic_vec<kModeAug, float>(g, b, n, pl.pieces, st)
+                                                    : launch_generic_vec<kModeFused, float>(g, b, n, pl.pieces, st); },
+                [&](auto* t) { using T = std::remove_pointer_t<decltype(t)>;
+                               return launch_generic_vec<kModeFused, T>(g, b, n, pl.pieces, st); });
+        } else {
+            e = by_pixel_type(g2.ptype, mode,
+                [&](int m) { return m == kModeLisi  ? launch_generic_one<kModeLisi, float>(g, n, N_T, pl.pieces, st)
+                                    : m == kModeAug ? launch_generic_one<kModeAug, float>(g, n, N_T, pl.pieces, st)
+                                                    : launch_generic_one<kModeFused, float>(g, n, N_T, pl.pieces, st); },
+                [&](auto* t) { using T = std::remove_pointer_t<decltype(t)>;
+                               return launch_generic_one<kModeFused, T>(g, n, N_T, pl.pieces, st); });
         }
         if (e != cudaSuccess) return IQA_ERR_CUDA;
     }
@@ -677,7 +705,7 @@ int launch_pairs(int mode, const void* const* xs, const void* const* ys, int n_p
         if (prepare_any(q, mode, xs, ys, n_pairs, g, N_T, k, out, ws, pl, series_order)) return fire(q, st);
         generic_plan(pl, N_T);
     }
-    return launch_generic(mode, xs, ys, n_pairs, g, N_T, k, out, ws, pl, st);
+    return launch_generic(mode, xs, ys, n_pairs, g, N_T, k, out, ws, pl, st, series_order);
 }
 
 // After S1-S4 of n_cmp comparisons: the second pass of split tiles, then Eqs. 3-4 per comparison.
