@@ -426,8 +426,8 @@ Plan make_plan(const Geom& g, int N_T, Align al, bool series) {
     // any_kernel binds lanes to box columns, and an item is whole tiles or ONE piece of a tile: a 64-column tile behind a
     // shifted base fills 17 of 32 lanes, a 130-column tile two pieces of 20 lanes.  The warp-per-piece kernel with 128-bit
     // loads (iqa_generic_vec.cuh: every lane busy whatever the width; x and y are aligned alike here) is faster there.
-    // Thresholds measured at N = 8192: whole tiles at <= 0.56 lane fill; split tiles below 0.7 (4-byte
-    // pixels) / 0.6 (fp64) / always (1- and 2-byte pixels: split pieces run four columns per lane).
+    // Thresholds measured at N = 8192: whole tiles at <= 0.56 lane fill; split tiles below 0.8 (4- and
+    // 8-byte pixels) / always (1- and 2-byte pixels: split pieces run four columns per lane).
     if ((long long)N_T * N_T > kWarpTilePixels && !knob(kKnobForceAny)) {
         const AnyGeom& a = pl.any;
         const bool split = a.px * a.py > 1;
@@ -437,7 +437,7 @@ Plan make_plan(const Geom& g, int N_T, Align al, bool series) {
         const double whole = es == 1 ? 0.5 : 0.56;       // whole tiles: N_T = 64 behind a shift, N_T = 65 .. 71 (uint8: 64 only)
         const double limit = es <= 2 ? (split ? 2.0 : whole)
                            : series  ? (split ? 0.5 : -1.0)
-                                     : (!split ? whole : es == 8 ? 0.6 : 0.7);
+                                     : (!split ? whole : 0.8);
         const bool narrow_image = !split && a.kx >= ceil_div(g.W, N_T);       // the image, not the mapping, limits the fill
         if (!narrow_image && (split ? fill < limit : fill <= limit)) {
             generic_plan(pl, N_T);

@@ -286,11 +286,11 @@ def test_typed_batch_series_validation_and_knobs():
     # plan rule of any_kernel (no GPU needed): shapes that would fill few of its lanes go to the 128-bit generic kernel
     F32, U8 = B.IQA_PIXEL_F32, B.IQA_PIXEL_U8
     q = lambda ptr, pt, nt: B.iqa_query_plan(ptr, pt, 4096, 4096, 4096, nt)
-    assert q(FAKE, F32, 100) == B.IQA_PLAN_TMA_ANY and q(FAKE, F32, 200) == B.IQA_PLAN_TMA_ANY
-    assert q(FAKE, F32, 120) == B.IQA_PLAN_GENERIC and q(FAKE, F32, 150) == B.IQA_PLAN_GENERIC       # split, fill < 0.7
+    assert q(FAKE, F32, 100) == B.IQA_PLAN_TMA_ANY and q(FAKE, F32, 330) == B.IQA_PLAN_TMA_ANY
+    assert q(FAKE, F32, 120) == B.IQA_PLAN_GENERIC and q(FAKE, F32, 200) == B.IQA_PLAN_GENERIC       # split, fill < 0.8
     assert q(FAKE + 4, F32, 64) == B.IQA_PLAN_GENERIC and q(FAKE + 4, F32, 100) == B.IQA_PLAN_TMA_ANY
     assert q(FAKE, I16, 200) == B.IQA_PLAN_GENERIC and q(FAKE, I16, 64) == B.IQA_PLAN_TMA_ANY        # 2-byte split tiles
-    assert q(FAKE, F64, 170) == B.IQA_PLAN_TMA_ANY and q(FAKE, F64, 120) == B.IQA_PLAN_GENERIC
+    assert q(FAKE, F64, 330) == B.IQA_PLAN_TMA_ANY and q(FAKE, F64, 170) == B.IQA_PLAN_GENERIC
     assert q(FAKE, U8, 16) == B.IQA_PLAN_TMA_ANY                                                   # small tiles stay
     with B.knob("IQA_FORCE_ANY", 1):
         assert q(FAKE, F32, 120) == B.IQA_PLAN_TMA_ANY

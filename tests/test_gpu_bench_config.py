@@ -166,7 +166,7 @@ def test_bench_path_rows_at_full_size(B, U, row):
     xs, ys = bench.make_path_inputs(torch, row, pairs, "cuda")
     # (a 64-column tile behind a base 4 bytes off fills 17 of 32 lanes of any_kernel: the plan takes the generic kernel)
     #  and split tiles that would fill few lanes take it too)
-    by_lane_fill = ("f32_NT64_base4B", "f32_NT130_split", "i16_NT200_split")
+    by_lane_fill = ("f32_NT64_base4B", "f32_NT130_split", "i16_NT200_split", "f32_NT300_split")
     expect = "generic" if name.startswith("generic") or name in by_lane_fill else "tma_any"
     assert B.plan_name(xs[0], N_T) == expect, (name, B.plan_name(xs[0], N_T))
     C1, C2, C, D = bench.PATH_CONSTS

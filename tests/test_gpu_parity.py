@@ -392,7 +392,7 @@ def test_every_baseline_configuration_takes_the_tma_kernel(B):
     assert B.plan_name(x[:, :513], 64).startswith("tma")            # pitched window, W % 4 != 0
     assert B.plan_name(x[:, 1:514], 100) == "tma_any"               # base 4-byte aligned only: any_kernel shifts columns
     assert B.plan_name(x[:, 1:514], 64) == "generic"                # ... unless that leaves half of its lanes idle
-    assert B.plan_name(x, 130) == "generic" and B.plan_name(x, 200) == "tma_any"   # split tiles: by lane fill
+    assert B.plan_name(x, 130) == "generic" and B.plan_name(x, 110) == "tma_any"   # split tiles: by lane fill
     assert B.plan_name(x, 100) == "tma_any"                         # tile side not a power of two
     assert B.plan_name(x[:, :515], 2) == "generic"                  # N_T < 4
     y = torch.empty((300, 517), dtype=torch.float32, device="cuda")
