@@ -451,6 +451,50 @@ def test_typed_series_item_order(B, U, dtype, N_T):
             U.assert_parity(got, ref, k["C"], f"series order {dtype} N_T={N_T} {mode} {c}")
 
 
+@pytest.mark.parametrize("dtype,N_T", [("float32", 50), ("float32", 125), ("int16", 64), ("float64", 7)])
+def test_generic_vector_kernel_batches_and_series(B, U, dtype, N_T):
+    """The 128-bit generic kernel takes 32 pairs per launch: a batch of 40 pairs on a pitch no tensor map can describe
+    (two launches; split tiles at N_T = 125: workspace [pair][tile][piece]) equals the pairs one by one bit for bit and the
+    oracle; a series of 36 snapshots in pair-minor unit order equals the pair-major order bit for bit."""
+    import torch
+    import oracle
+    rng = np.random.default_rng(N_T + 17)
+    H, W = 250, 251
+    per16 = 16 // np.dtype(dtype).itemsize
+    pitch = W + (1 if (W + 1) % per16 else 2)
+    imgs, k = [], None
+    for _ in range(6):
+        a, _, k = _typed_pair(rng, H, W, dtype)
+        imgs.append(a)
+    dev = [_typed_window(a, pitch, 0) for a in imgs]
+    assert B.plan_name(dev[0], N_T) == "generic"
+    order = [(i % 6, (i * 5 + 1) % 6) for i in range(40)]
+    out = B.fused_batch_2d([dev[i] for i, _ in order], [dev[j] for _, j in order], N_T, k["C1"], k["C2"], k["C"], k["D"],
+                           numerators=True)
+    torch.cuda.synchronize()
+    for p_, (i, j) in enumerate(order):
+        if p_ in (0, 31, 32, 39):
+            one = B.fused_tiles_2d(dev[i], dev[j], N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+            for n in one:
+                assert torch.equal(one[n], out[n][p_]), (p_, n)
+            ref = oracle.tiles_2d_any(imgs[i], imgs[j], N_T, **k)
+            got = {n: out[n][p_].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+            U.assert_parity(got, ref, k["C"], f"generic batch {dtype} N_T={N_T} pair {p_}")
+    series = [dev[i % 6] for i in range(36)]
+    for mode in ("reference", "consecutive"):
+        so = B.series_tiles_2d(series, mode, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+        with B.knob("IQA_SERIES_PAIR_MAJOR", 1):
+            pm = B.series_tiles_2d(series, mode, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+        torch.cuda.synchronize()
+        for n in so:
+            assert torch.equal(so[n], pm[n]), (mode, n)
+        for c, (ix, iy) in enumerate(oracle.comparison_indices(36, mode)):
+            if c in (0, 33, 34):
+                ref = oracle.tiles_2d_any(imgs[ix % 6], imgs[iy % 6], N_T, **k)
+                got = {n: so[n][c].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+                U.assert_parity(got, ref, k["C"], f"generic series {dtype} N_T={N_T} {mode} {c}")
+
+
 def test_paper_named_entry_points_with_odd_tile_sides(B, U):
     """iqa_lisi_tiles / iqa_auglisi_tiles / iqa_fused_tiles with N_T = 48 and 100 (N % N_T == 0): the three modes of
     any_kernel; the standalone results equal the fused ones bit for bit."""
