@@ -49,11 +49,14 @@
  *     never leave work behind.  IQA_ERR_CUDA from a failing launch or copy is the one exception: earlier
  *     launches of the same call may already be enqueued and the outputs are then undefined.
  *   * Any N_T that divides N is accepted.  Images whose row pitch is a multiple of 16 bytes (N % 4 == 0
- *     for the square fp32 entry points) take a persistent TMA-fed kernel whatever the alignment of
- *     their base: tma_kernel for power-of-two N_T >= 8, any_kernel for every other N_T >= 4 and for
- *     the other pixel types.  Other pitches and N_T < 4 take a generic (slower, still CUDA) kernel.
- *     Results are deterministic: fixed reduction order,
- *     no floating-point atomics; two calls on the same inputs are bit-identical.
+ *     for the square fp32 entry points) and whose bases sit at the same offset inside their 16-byte
+ *     lines take a persistent TMA-fed kernel: tma_kernel for fp32 with a power-of-two N_T >= 8 and
+ *     16-byte aligned bases, any_kernel for every other N_T >= 4, the other pixel types and shifted
+ *     bases -- except the shapes that would leave most of any_kernel's lanes idle (split tiles of
+ *     113 .. ~200 columns, a 64-column tile behind a shifted base), which, like every other pitch and
+ *     N_T < 4, take the generic kernel (128-bit loads when x and y are aligned alike, scalar loads
+ *     otherwise; still CUDA).  iqa_query_plan tells which.  Results are deterministic: fixed reduction
+ *     order, no floating-point atomics; two calls on the same inputs are bit-identical.
  * ============================================================================= */
 #ifndef IQA_TILES_H
 #define IQA_TILES_H
