@@ -1,11 +1,14 @@
 """-m gpu seeded fuzz: random shapes, pitches, alignments, tile sizes, pixel types and series lengths through
 the C ABI against the oracle (the same tolerance as everywhere else).  Every case is reproducible from its index."""
+import os
+
 import numpy as np
 import pytest
 
 pytestmark = pytest.mark.gpu
 
 K = dict(C1=1e-6, C2=1e-6, C=1e-6, D=5e-7)
+EXTRA = int(os.environ.get("IQA_FUZZ_EXTRA", "0"))      # soak runs: IQA_FUZZ_EXTRA=600 adds that many cases to every test
 
 
 @pytest.fixture(scope="module")
@@ -30,7 +33,7 @@ def _window(a, pitch, off):
     return view
 
 
-@pytest.mark.parametrize("case", range(48))
+@pytest.mark.parametrize("case", range(48 + EXTRA))
 def test_random_2d_cases(B, U, case):
     import torch
     import oracle
@@ -61,7 +64,7 @@ def test_random_2d_cases(B, U, case):
     U.assert_parity(g, ref, k["C"], f"case {case}: {H}x{W} N_T={N_T} pitch={pitch} off={off} {dtype}")
 
 
-@pytest.mark.parametrize("case", range(16))
+@pytest.mark.parametrize("case", range(16 + EXTRA))
 def test_random_series_cases(B, U, case):
     import torch
     import oracle
@@ -87,7 +90,7 @@ def test_random_series_cases(B, U, case):
         assert abs(w[0] - exp[0]) <= 1e-5 * abs(exp[0]) and abs(w[1] - exp[1]) <= 1e-5 * abs(exp[1]) + 1e-6
 
 
-@pytest.mark.parametrize("case", range(24))
+@pytest.mark.parametrize("case", range(24 + EXTRA))
 def test_random_typed_series_find_cases(B, U, case):
     """iqa_series_find_2d_typed on random windows: every pixel type, tile sides of any kind, row pitches with and
     without a tensor map (any_kernel in series item order / tma_kernel series modes / generic kernels pair by pair),
