@@ -6,8 +6,8 @@
 // S1-S4 of SURVEY.md 8(a): clamp, Eq. 1 / Eq. 2 terms, per-tile sums, Eqs. 1-2.
 //
 // Row r of a tile starts a(r) elements past a 16-byte boundary, and a(r) changes from row to row when the pitch is
-// odd.  A SLOT is one 16-byte-aligned group of kSlotE = max(4, 16 / sizeof(T)) elements of one tile row; a row of
-// cols_t pixels needs at most qmax = ceil((16 / sizeof(T) - 1 + cols_t) / kSlotE) slots.  The lanes of a warp (one
+// odd.  A SLOT is one or two 16-byte-aligned groups (kSlotE elements: 4 fp32 / int32, 4 fp64, 16 fp16 / int16, 32 uint8) of
+// one tile row; a row of cols_t pixels needs at most qmax = ceil((16 / sizeof(T) - 1 + cols_t) / kSlotE) slots.  The lanes of a warp (one
 // warp per tile piece) stride over the rows x qmax slots of their piece, so every lane is
 // busy whatever the tile width; each thread issues the loads of kVecInFlight slots of both images before the first
 // term is computed.  Elements of a slot outside the tile's columns are zeroed in the raw words (a (0, 0) pixel pair
@@ -30,12 +30,14 @@ constexpr int kVecInFlight = 4;      // slots (32 bytes of each image, 64 for fp
 template <typename T> struct VecGeom {
     static constexpr int kES = (int)sizeof(T);
     static constexpr int kAL = 16 / kES;                  // elements per 16 bytes
-    static constexpr int kSlotE = kAL < 4 ? 4 : kAL;      // elements per slot (fp64: two 16-byte groups)
+    // elements per slot: one 16-byte group (4-byte pixels), two groups for fp64 (4 pixels) and for 1- and 2-byte pixels
+    // (32 / 16 pixels: the slot's addressing and masks are paid per slot -- int16 N_T = 200 4.2 -> 4.6 TB/s)
+    static constexpr int kSlotE = kES == 4 ? kAL : 2 * kAL;
     static constexpr int kVecs = kSlotE / kAL;            // 16-byte loads per slot and image
-    // slots a thread loads before it computes: 4 (fp32 / int32), 6 for 1- and 2-byte pixels (measured: int16 3.7 -> 4.1 TB/s,
-    // fp32 loses with 6), 2 for fp64 (two groups per slot).  A software pipeline (next round's loads in flight while this
-    // round is computed) needs more than the 80 registers that three CTAs per SM leave and was slower in every variant.
-    static constexpr int kInFlight = kVecs == 2 ? 2 : kES <= 2 ? 6 : kVecInFlight;
+    // slots a thread loads before it computes: 4 (fp32 / int32), 2 for the two-group slots (measured; three lose on narrow
+    // tiles).  A software pipeline (next round's loads in flight while this round is computed) needs more than the 80
+    // registers that three CTAs per SM leave and was slower in every variant.
+    static constexpr int kInFlight = kVecs == 2 ? 2 : kVecInFlight;
 };
 
 // Zero the elements of one 16-byte group whose tile column c_first + e is outside [0, cols_t).
