@@ -74,7 +74,8 @@ typedef enum {
     IQA_ERR_PARAM = 3,
     IQA_ERR_ALIGN = 4,
     IQA_ERR_WORKSPACE = 5,
-    IQA_ERR_CUDA = 6
+    IQA_ERR_CUDA = 6,
+    IQA_ERR_STATIC_LIMIT = 7      /* iqa_fused_tiles_static only: the shape needs more than IQA_STATIC_WORKSPACE_BYTES */
 } iqa_status;
 
 /* Static, never-freed description of a status code ("unknown status" for other values). */
@@ -113,6 +114,44 @@ int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
                     float* sum_x, float* sum_y,
                     float* lisi_num, float* auglisi_num,
                     void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- the same call for programs that may not allocate device memory ---------------------------
+ * iqa_fused_tiles wants a workspace for tiles wider than 64 pixels, and somebody has to cudaMalloc it.
+ * Some users of this library cannot: a plug-in inside a telescope pipeline or an inference server whose
+ * host program hands out ALL device memory at start-up and gives a plug-in nothing but the pointers of its
+ * input and output buffers; a per-snapshot loop that must never hit the device-wide synchronisation that
+ * cudaMalloc / cudaFree imply; a binding from a language that has no CUDA allocator at hand.  For them
+ * iqa_fused_tiles_static is iqa_fused_tiles with the workspace argument removed: the partial sums of split
+ * tiles go to a fixed array of IQA_STATIC_WORKSPACE_BYTES that is part of the library image itself (a
+ * file-scope __device__ array in iqa_tiles.cu).  Same kernels, same order of summation: the outputs are
+ * bit-identical to iqa_fused_tiles on the same inputs.
+ *
+ *   cost      every GPU on which this process uses the library keeps those IQA_STATIC_WORKSPACE_BYTES (1 MiB)
+ *             reserved from the moment the library's code is loaded onto it until the process ends, whether
+ *             or not this entry point is ever called.
+ *   limit     shapes with iqa_workspace_bytes(N, N_T) > IQA_STATIC_WORKSPACE_BYTES are refused with
+ *             IQA_ERR_STATIC_LIMIT before anything is enqueued (1 MiB covers every BASELINE.json
+ *             configuration up to N = 16384, N_T = 128; N = 32768, N_T = 128 would need 4 MiB: use
+ *             iqa_fused_tiles with a workspace of your own there).  Shapes that need no workspace
+ *             (N_T <= 64, ...) never touch the array.
+ *   set-up    the FIRST call on each device that needs the array looks up its device address (one
+ *             cudaGetSymbolAddress with that device current, cached per device afterwards; a failure is
+ *             IQA_ERR_CUDA).  Make that first call during start-up, outside any stream capture.
+ *   no allocation   the call itself never calls cudaMalloc, cudaFree, or a library routine that does.
+ *   sharing   ALL calls on a device use the SAME array, and it keeps whatever the last call left in it.
+ *             Nothing in it has to start at zero -- every slot the second pass reads was written by the
+ *             first pass of the same call -- so no clearing is done or needed.  But two calls that may
+ *             run on the GPU at the same time (different streams, or different host threads on
+ *             different streams) RACE on it and both results are then garbage: keep the calls of one
+ *             device on one stream, or order them with events.  Calls on different devices do not interact.
+ * Arguments and every other error as iqa_fused_tiles (lisi_num, auglisi_num MAY BE NULL). */
+#define IQA_STATIC_WORKSPACE_BYTES 1048576
+int iqa_fused_tiles_static(const float* x, const float* y, int N, int N_T,
+                           float C1, float C2, float C, float D,
+                           float* lisi, float* auglisi,
+                           float* sum_x, float* sum_y,
+                           float* lisi_num, float* auglisi_num,
+                           void* stream);
 
 /* Diagnostic: which kernel a call on this image would take (host-side decision only, nothing is enqueued).
  *   x, pixel_type, H, W, pitch, N_T as for iqa_fused_tiles_2d_typed; series != 0: as for the time-series entry points.

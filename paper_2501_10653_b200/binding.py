@@ -21,9 +21,11 @@ import os
 from . import build as _build
 
 IQA_OK, IQA_ERR_NULL, IQA_ERR_SHAPE, IQA_ERR_PARAM, IQA_ERR_ALIGN, IQA_ERR_WORKSPACE, IQA_ERR_CUDA = range(7)
+IQA_ERR_STATIC_LIMIT = 7
+IQA_STATIC_WORKSPACE_BYTES = 1 << 20     # include/iqa_tiles.h; tests/test_zz_no_alloc.py checks the two agree
 
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_debug_knob", "iqa_workspace_bytes", "iqa_lisi_tiles",
-           "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_batch_workspace_bytes", "iqa_fused_batch",
+           "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_fused_tiles_static", "iqa_batch_workspace_bytes", "iqa_fused_batch",
            "iqa_query_plan", "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_tiles_2d_typed",
            "iqa_fused_batch_2d", "iqa_fused_batch_2d_typed", "iqa_series_tiles_2d", "iqa_series_tiles_2d_typed",
            "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_series_find", "iqa_series_find_2d_typed", "iqa_tiles_below", "iqa_tiles_bottom_k",
@@ -75,6 +77,8 @@ def _load() -> ctypes.CDLL:
     lib.iqa_auglisi_tiles.argtypes = [vp, vp, i, i, f, vp, vp, sz, vp]
     lib.iqa_fused_tiles.restype = i
     lib.iqa_fused_tiles.argtypes = [vp, vp, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_fused_tiles_static.restype = i
+    lib.iqa_fused_tiles_static.argtypes = [vp, vp, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, vp]
     lib.iqa_batch_workspace_bytes.restype = sz
     lib.iqa_batch_workspace_bytes.argtypes = [i, i, i]
     lib.iqa_fused_batch.restype = i
@@ -211,6 +215,13 @@ def iqa_fused_tiles(x, y, N, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
                                _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
                                _ptr(lisi_num), _ptr(auglisi_num),
                                _ptr(workspace), int(workspace_bytes), _stream(stream))
+
+
+def iqa_fused_tiles_static(x, y, N, N_T, C1, C2, C, D, lisi, auglisi, sum_x, sum_y,
+                           lisi_num=None, auglisi_num=None, stream=None) -> int:
+    return lib.iqa_fused_tiles_static(_ptr(x), _ptr(y), int(N), int(N_T), C1, C2, C, D,
+                                      _ptr(lisi), _ptr(auglisi), _ptr(sum_x), _ptr(sum_y),
+                                      _ptr(lisi_num), _ptr(auglisi_num), _stream(stream))
 
 
 def iqa_batch_workspace_bytes(n_pairs: int, N: int, N_T: int) -> int:
@@ -468,6 +479,21 @@ def fused_tiles(x, y, N_T, C1, C2, C, D, numerators: bool = False, workspace=Non
                              out.get("L"), out.get("A"), workspace, wsb, _current_stream(x.device))
     if rc != IQA_OK:
         raise IqaError(rc, "iqa_fused_tiles")
+    return out
+
+
+def fused_tiles_static(x, y, N_T, C1, C2, C, D, out: dict) -> dict:
+    """``fused_tiles`` for callers that may not allocate device memory: nothing is allocated here or in the
+    library.  ``out`` holds the caller's own (nt, nt) float32 CUDA tensors ``lisi``, ``auglisi``, ``X``, ``Y`` and
+    optionally ``L``, ``A``; the split-tile partial sums go to the library's built-in 1 MiB array
+    (``IQA_STATIC_WORKSPACE_BYTES``; larger shapes raise ``IqaError`` with ``IQA_ERR_STATIC_LIMIT``).  All calls on
+    a device share that array: keep them on one stream (overlapping calls race).  See include/iqa_tiles.h."""
+    N = _check_images(x, y)
+    with _device_of(x.device):
+        rc = iqa_fused_tiles_static(x, y, N, N_T, C1, C2, C, D, out["lisi"], out["auglisi"], out["X"], out["Y"],
+                                    out.get("L"), out.get("A"), _current_stream(x.device))
+    if rc != IQA_OK:
+        raise IqaError(rc, "iqa_fused_tiles_static")
     return out
 
 

@@ -15,6 +15,7 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <type_traits>
 #include <utility>
 #include <vector>
@@ -858,6 +859,36 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace
 
+// ---- built-in workspace of iqa_fused_tiles_static ------------------------------------------------------------
+// For callers that cannot allocate device memory (include/iqa_tiles.h explains who): the partial sums of split
+// tiles land here instead of in a caller-supplied workspace.  The array is part of the library's device image, so
+// every GPU that loads this library holds these IQA_STATIC_WORKSPACE_BYTES until the process exits.  One array per
+// device, shared by every call on that device and never cleared (nothing in it has to start at zero: the second pass
+// reads only slots the first pass of the same call wrote); calls that overlap on the GPU race on it.
+static __device__ __align__(256) unsigned char g_static_workspace[IQA_STATIC_WORKSPACE_BYTES];
+
+namespace {
+
+// In host code `g_static_workspace` is only the host-side handle of the symbol: handing it to a kernel would pass a
+// host address.  Its device address differs from GPU to GPU and comes from cudaGetSymbolAddress, asked once per
+// device with that device current and then kept.  Allocates nothing.
+int static_workspace(void** ws) {
+    static std::mutex mu;
+    static void* addr[kMaxDevices] = {};
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return IQA_ERR_CUDA;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_static_workspace) != cudaSuccess || !p) return IQA_ERR_CUDA;
+        addr[dev] = p;
+    }
+    *ws = addr[dev];
+    return IQA_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 const char* iqa_status_string(int status) {
@@ -869,6 +900,7 @@ const char* iqa_status_string(int status) {
         case IQA_ERR_ALIGN: return "pointer alignment: images to their element size, workspace 16-byte";
         case IQA_ERR_WORKSPACE: return "workspace missing or smaller than iqa_workspace_bytes / iqa_batch_workspace_bytes";
         case IQA_ERR_CUDA: return "CUDA launch or copy failed";
+        case IQA_ERR_STATIC_LIMIT: return "iqa_fused_tiles_static: this shape needs more than IQA_STATIC_WORKSPACE_BYTES of workspace; call iqa_fused_tiles with a workspace of your own";
         default: return "unknown status";
     }
 }
@@ -921,6 +953,28 @@ int iqa_fused_tiles(const float* x, const float* y, int N, int N_T,
     const void* ys[1] = {y};
     return run_batch(kModeFused, xs, ys, 1, square_geom(N), N_T, true, C1, C2, C, D, o, nullptr, workspace,
                      workspace_bytes, stream);
+}
+
+// iqa_fused_tiles without a workspace argument and without any allocation: split-tile partial sums go to
+// g_static_workspace (above).  Everything is validated, and a shape beyond the array refused, BEFORE the first CUDA call;
+// the first call on a device that needs the array looks its address up (do that outside stream capture).
+int iqa_fused_tiles_static(const float* x, const float* y, int N, int N_T,
+                           float C1, float C2, float C, float D,
+                           float* lisi, float* auglisi, float* sum_x, float* sum_y,
+                           float* lisi_num, float* auglisi_num, void* stream) {
+    const Outputs o{lisi, auglisi, sum_x, sum_y, lisi_num, auglisi_num};
+    if (!x || !y) return IQA_ERR_NULL;
+    if (const int s = validate_common(kModeFused, 1, square_geom(N), N_T, true, C1, C2, C, D, o, nullptr)) return s;
+    if (((uintptr_t)x | (uintptr_t)y) & 3u) return IQA_ERR_ALIGN;
+    const size_t need = workspace_bytes_for(1, N, N_T);
+    if (need > (size_t)IQA_STATIC_WORKSPACE_BYTES) return IQA_ERR_STATIC_LIMIT;
+    void* ws = nullptr;
+    if (need > 0)
+        if (const int s = static_workspace(&ws)) return s;
+    const void* xs[1] = {x};
+    const void* ys[1] = {y};
+    return run_batch(kModeFused, xs, ys, 1, square_geom(N), N_T, true, C1, C2, C, D, o, nullptr, ws,
+                     need > 0 ? (size_t)IQA_STATIC_WORKSPACE_BYTES : 0, stream);
 }
 
 int iqa_query_plan(const void* x, int pixel_type, int H, int W, long long pitch, int N_T, int series) {
