@@ -156,8 +156,9 @@ int iqa_fused_tiles_static(const float* x, const float* y, int N, int N_T,
 /* Diagnostic: which kernel a call on this image would take (host-side decision only, nothing is enqueued).
  *   x, pixel_type, H, W, pitch, N_T as for iqa_fused_tiles_2d_typed; series != 0: as for the time-series entry points.
  * Returns IQA_PLAN_GENERIC, IQA_PLAN_TMA_ANY (any_kernel: any N_T >= 4, any pixel type; the time-series entry points
- * run it pair by pair), or IQA_PLAN_TMA + c (tma_kernel, c = its ring / box configuration, 0..4); -1 for bad
- * arguments.  bench.py reports it, and the GPU tests assert that every BASELINE.json configuration takes tma_kernel
+ * run it as one launch per 32 comparisons in pair-minor order; `series` is answered for a series of three or more
+ * images -- a two-image series is planned like the pair it is), or IQA_PLAN_TMA + c (tma_kernel, c = its ring / box
+ * configuration, 0..4); -1 for bad arguments.  bench.py reports it, and the GPU tests assert that every BASELINE.json configuration takes tma_kernel
  * -- a silent fall-back would cost bandwidth, not parity. */
 #define IQA_PLAN_GENERIC 0
 #define IQA_PLAN_TMA_ANY 2
@@ -185,8 +186,10 @@ int iqa_debug_knob(const char* name, int value);
  *   outputs         [nty * ntx], nty = ceil(H / N_T), ntx = ceil(W / N_T), t = ty * ntx + tx
  *   workspace       >= iqa_workspace_bytes_2d(H, W, N_T) bytes (may be NULL when 0)
  * Eqs. 3-4 over the result: iqa_aggregate with n_tiles = nty * ntx.  Pitches that are multiples of 4 take a
- * TMA-fed kernel (the TMA unit zero-fills what lies outside the image; the base needs 4-byte alignment only);
- * other pitches and N_T < 4 take the generic kernel. */
+ * TMA-fed kernel (the TMA unit zero-fills what lies outside the image; the base needs 4-byte alignment only)
+ * unless the shape would fill too few of that kernel's lanes (the lane-fill thresholds of the preamble: split tiles
+ * of 113 .. ~200 columns, a 64-column tile behind a shifted base); those shapes, other pitches and N_T < 4 take the
+ * generic kernel.  iqa_query_plan tells which. */
 size_t iqa_workspace_bytes_2d(int H, int W, int N_T);
 int iqa_fused_tiles_2d(const float* x, const float* y, int H, int W, long long pitch_x, long long pitch_y, int N_T,
                        float C1, float C2, float C, float D,
@@ -226,8 +229,11 @@ int iqa_series_tiles_2d(const float* const* img_ptrs_host, int n_images, int mod
                         void* workspace, size_t workspace_bytes, void* stream);
 
 /* The same two entry points for images of `pixel_type` pixels (pitch in ELEMENTS of that type).  Batches run in
- * one any_kernel launch per 32 pairs; a typed time series is computed pair by pair (2 sizeof(pixel) bytes per pixel
- * and comparison -- only fp32 images with a power-of-two N_T have the read-once series kernel). */
+ * one any_kernel launch per 32 pairs.  A typed time series is ONE any_kernel launch per 32 comparisons in pair-minor
+ * item order: the comparisons of one image location run on neighbouring CTAs, so each snapshot comes from HBM once
+ * and its second reader finds it in L2 (only fp32 images with a power-of-two N_T have the kernel that keeps the
+ * shared image in shared memory).  Shapes below the lane-fill thresholds, and pitches no tensor map can describe,
+ * take the generic kernels instead; iqa_query_plan is the source of truth for which kernel a call takes. */
 int iqa_fused_batch_2d_typed(const void* const* x_ptrs_host, const void* const* y_ptrs_host, int n_pairs, int pixel_type,
                              int H, int W, long long pitch, int N_T, float C1, float C2, float C, float D,
                              float* lisi, float* auglisi, float* sum_x, float* sum_y,
@@ -254,7 +260,9 @@ size_t iqa_batch_workspace_bytes(int n_pairs, int N, int N_T);
  *   out2                 [n_pairs * 2] device, MAY BE NULL: out2[2p] = LISI, out2[2p+1] = augLISI of pair p
  *   workspace            >= iqa_batch_workspace_bytes(n_pairs, N, N_T) bytes (may be NULL when 0)
  * n_pairs * n must stay below 2^31.  Results are bit-identical to n_pairs calls of
- * iqa_fused_tiles + iqa_aggregate. */
+ * iqa_fused_tiles + iqa_aggregate: the kernel is chosen per run of consecutive pairs whose x and y
+ * sit at the same offset inside their 16-byte lines, as it would be for each pair alone, so one
+ * shifted pair costs the aligned pairs of its batch nothing (it only splits the batch into more launches). */
 int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,
                     int N, int N_T, float C1, float C2, float C, float D,
                     float* lisi, float* auglisi, float* sum_x, float* sum_y,

@@ -191,14 +191,26 @@ bool encode_image_map(CUtensorMap* map, const void* img, int ptype, int H, int W
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// Per-device launch geometry, filled on first use (benign race: every thread computes the same values).
-struct Geometry { std::atomic<int> ready{0}; int sms; int tma_ctas[kNumTmaConfigs]; };
+// Per-device launch geometry, filled on first use under a mutex (`ready` is the lock-free fast path afterwards).
+// any_occ: resident CTAs per SM of any_kernel instantiation i at a given dynamic shared-memory size -- asked of the
+// runtime once per (device, instantiation, size) instead of on every call (the single-pair path is host-latency bound).
+constexpr int kAnyOccSlots = 4;
+struct AnyOcc { std::atomic<size_t> smem{0}; std::atomic<int> occ{0}; };
+struct Geometry {
+    std::atomic<int> ready{0};
+    int sms;
+    int tma_ctas[kNumTmaConfigs];
+    AnyOcc any_occ[kNumAnyFns][kAnyOccSlots];
+};
 Geometry g_geo[kMaxDevices];
+std::mutex g_geo_mutex;
 
 const Geometry* geometry() {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
     Geometry& g = g_geo[dev];
+    if (g.ready.load(std::memory_order_acquire)) return &g;
+    std::lock_guard<std::mutex> lock(g_geo_mutex);
     if (g.ready.load(std::memory_order_acquire)) return &g;
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return nullptr;
@@ -221,6 +233,31 @@ const Geometry* geometry() {
     g.sms = sms;
     g.ready.store(1, std::memory_order_release);
     return &g;
+}
+
+// Resident CTAs per SM of any_kernel instantiation `fi` with `smem` bytes of dynamic shared memory on the current
+// device (0: unknown).  A handful of sizes occur per instantiation (one per ring geometry); they are kept in a small
+// table that threads fill under the mutex; a full table just asks the runtime again.
+int any_occupancy(int fi, size_t smem) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return 0;
+    AnyOcc* slots = g_geo[dev].any_occ[fi];
+    for (int i = 0; i < kAnyOccSlots; ++i) {
+        const int occ = slots[i].occ.load(std::memory_order_acquire);
+        if (occ == 0) break;
+        if (slots[i].smem.load(std::memory_order_relaxed) == smem) return occ;
+    }
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, any_fn_at(fi), kTmaThreads, smem) != cudaSuccess || occ <= 0)
+        return 0;
+    std::lock_guard<std::mutex> lock(g_geo_mutex);
+    for (int i = 0; i < kAnyOccSlots; ++i)
+        if (slots[i].occ.load(std::memory_order_relaxed) == 0) {
+            slots[i].smem.store(smem, std::memory_order_relaxed);
+            slots[i].occ.store(occ, std::memory_order_release);
+            break;
+        }
+    return occ;
 }
 
 // Launch with the programmatic-stream-serialisation attribute (PDL): the kernel may become
@@ -397,7 +434,8 @@ Align align_of(const void* const* a, int na, const void* const* b, int nb) {
 
 // A tensor map can describe the images when every row pitch is a multiple of 16 bytes; the boxes of x and y share
 // their column grid when all bases have the same offset inside a 16-byte line (al.lo16 >= 0).
-Plan make_plan(const Geom& g, int N_T, Align al, bool series) {
+// series: the call is a time series (tma_kernel's series ring; any_kernel's pair-minor order); n_cmp: its comparisons.
+Plan make_plan(const Geom& g, int N_T, Align al, bool series, int n_cmp = 2) {
     Plan pl{};
     generic_plan(pl, N_T);
     const int es = esize_of(g.ptype);
@@ -436,8 +474,9 @@ Plan make_plan(const Geom& g, int N_T, Align al, bool series) {
         // (the comparisons of a series share images through L2 in any_kernel's pair-minor order, worth 1.2-1.35x for 4- and
         //  8-byte pixels: the generic kernel, which runs them pair by pair, has to win by more)
         const double whole = es == 1 ? 0.5 : 0.56;       // whole tiles: N_T = 64 behind a shift, N_T = 65 .. 71 (uint8: 64 only)
+        const bool sharing = series && n_cmp > 1;        // a series of two images is one pair: nothing to share
         const double limit = es <= 2 ? (split ? 2.0 : whole)
-                           : series  ? (split ? 0.5 : -1.0)
+                           : sharing ? (split ? 0.5 : -1.0)
                                      : (!split ? whole : 0.8);
         const bool narrow_image = !split && a.kx >= ceil_div(g.W, N_T);       // the image, not the mapping, limits the fill
         if (!narrow_image && (split ? fill < limit : fill <= limit)) {
@@ -558,8 +597,8 @@ bool prepare_any(std::vector<AnyLaunch>& q, int mode, const void* const* xs, con
     AnyFn fn = any_fn_at(any_fn_index(mode, g.ptype));
     const size_t smem = any_smem_bytes(a.n_slots, a.slot_bytes);
     if (smem > kAnyMaxSmem) return false;
-    int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kTmaThreads, smem) != cudaSuccess || occ <= 0) return false;
+    int occ = any_occupancy(any_fn_index(mode, g.ptype), smem);
+    if (occ <= 0) return false;
     if (occ > 2) occ = 2;
     const int ntx = ceil_div(g.W, N_T), nty = ceil_div(g.H, N_T);
     const long long n = (long long)ntx * nty;
@@ -791,19 +830,37 @@ int run_batch(int mode, const void* const* xs, const void* const* ys, int n_pair
     if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
     if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
 
-    Plan pl = make_plan(g, N_T, align_of(xs, n_pairs, ys, n_pairs), false);
     cudaStream_t st = (cudaStream_t)stream;
     float4* ws = need > 0 ? (float4*)workspace : nullptr;
     out = out.for_mode(mode);
     const Consts k{C1, C2, C, D};
-    if (const int rc = launch_pairs(mode, xs, ys, n_pairs, g, N_T, k, out, ws, pl, st)) return rc;
-    return finish_comparisons(out, out2, n_pairs, n, k, ws, pl, st);
+    // One plan per RUN of consecutive pairs of the same alignment class (the offset of x and y inside their 16-byte
+    // lines, -1 when the two differ), each run planned exactly like a call of its own: one pair behind a shifted base
+    // does not drag the aligned pairs of its batch onto the generic kernels, and every pair is summed in the order the
+    // single-pair call would use.  A uniform batch -- the usual case -- is one run.
+    const size_t ws_per_pair = (size_t)n * max_pieces(N_T);          // float4 slots; >= n * pieces of any plan
+    // (a mixed batch must not fail half way: the one shape check a later run could still trip over is made up front)
+    if (align_of(xs, n_pairs, ys, n_pairs).lo16 < 0 && (long long)ws_per_pair * kVecMaxPairs > 0x7fffffffLL)
+        return IQA_ERR_SHAPE;
+    for (int first = 0; first < n_pairs;) {
+        const Align al = align_of(xs + first, 1, ys + first, 1);
+        int np = 1;
+        while (first + np < n_pairs && align_of(xs + first + np, 1, ys + first + np, 1).lo16 == al.lo16) ++np;
+        Plan pl = make_plan(g, N_T, al, false);
+        const Outputs o = out.offset((size_t)first * (size_t)n);
+        float4* w = ws ? ws + (size_t)first * ws_per_pair : nullptr;
+        if (const int rc = launch_pairs(mode, xs + first, ys + first, np, g, N_T, k, o, w, pl, st)) return rc;
+        if (const int rc = finish_comparisons(o, out2 ? out2 + 2 * (size_t)first : nullptr, np, n, k, w, pl, st)) return rc;
+        first += np;
+    }
+    return IQA_OK;
 }
 
 // Time series: imgs = HOST array of n_images device pointers; K = n_images - 1
 // comparisons, (I_0, I_k+1) or (I_k, I_k+1).  fp32 images with a power-of-two N_T take tma_kernel, which
 // keeps the x box of every comparison in shared memory (each image is read from HBM once);
-// everything else is computed pair by pair with the kernels of the pair entry points.
+// everything else runs the K pair computations with the kernels of the pair entry points in series order
+// (any_kernel / the 128-bit generic kernel: one launch per 32 comparisons, pair-minor, shared images from L2).
 int run_series(const void* const* imgs, int n_images, int series, const Geom& g, int N_T, bool square,
                float C1, float C2, float C, float D, Outputs out, float* out2,
                void* workspace, size_t workspace_bytes, void* stream) {
@@ -822,7 +879,7 @@ int run_series(const void* const* imgs, int n_images, int series, const Geom& g,
     if (need > 0 && (!workspace || workspace_bytes < need)) return IQA_ERR_WORKSPACE;
     if (need > 0 && ((uintptr_t)workspace & 15u)) return IQA_ERR_ALIGN;
 
-    Plan pl = make_plan(g, N_T, align_of(imgs, n_images, imgs, 0), true);
+    Plan pl = make_plan(g, N_T, align_of(imgs, n_images, imgs, 0), true, K);
     cudaStream_t st = (cudaStream_t)stream;
     float4* ws = need > 0 ? (float4*)workspace : nullptr;
     const Consts k{C1, C2, C, D};
@@ -983,7 +1040,7 @@ int iqa_query_plan(const void* x, int pixel_type, int H, int W, long long pitch,
     const Geom g{H, W, pitch, pitch, pixel_type};
     const Plan pl = make_plan(g, N_T, align_of(&x, 1, &x, 0), series != 0);
     if (pl.kind == kPlanTma) return IQA_PLAN_TMA + pl.tma_cfg;
-    // the time-series entry points run any_kernel pair by pair (8 bytes per pixel and comparison)
+    // (a series runs any_kernel as one launch per 32 comparisons in pair-minor item order)
     return pl.kind == kPlanAny ? IQA_PLAN_TMA_ANY : IQA_PLAN_GENERIC;
 }
 

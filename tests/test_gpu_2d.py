@@ -451,6 +451,30 @@ def test_typed_series_item_order(B, U, dtype, N_T):
             U.assert_parity(got, ref, k["C"], f"series order {dtype} N_T={N_T} {mode} {c}")
 
 
+def test_series_of_two_images_is_planned_like_the_pair_it_is(B, U):
+    """A series of two snapshots shares nothing through L2, so its plan is the pair's plan: N_T = 150 (split tiles filling
+    0.59 of any_kernel's lanes) takes the 128-bit generic kernel in both calls and the results agree bit for bit; three
+    snapshots keep any_kernel's pair-minor order."""
+    import torch
+    rng = np.random.default_rng(77)
+    H, W, N_T = 600, 600, 150
+    a, b, k = _typed_pair(rng, H, W, np.float32)
+    c, _, _ = _typed_pair(rng, H, W, np.float32)
+    da, db, dc = (_typed_window(v, W, 0) for v in (a, b, c))
+    assert B.plan_name(da, N_T) == "generic" and B.plan_name(da, N_T, series=True) == "tma_any"
+    two = B.series_tiles_2d([da, db], "consecutive", N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    pair = B.fused_tiles_2d(da, db, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    for n in pair:
+        assert torch.equal(two[n][0], pair[n]), n
+    three = B.series_tiles_2d([da, db, dc], "consecutive", N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    import oracle
+    for cmp_i, (u, v) in enumerate([(a, b), (b, c)]):
+        ref = oracle.tiles_2d_any(u, v, N_T, **k)
+        for res, what in ((three, "three"),) + (((two, "two"),) if cmp_i == 0 else ()):
+            got = {n: res[n][cmp_i].cpu().numpy().astype(np.float64) for n in ("lisi", "auglisi", "X", "Y", "L", "A")}
+            U.assert_parity(got, ref, k["C"], f"{what}-image series, comparison {cmp_i}")
+
+
 @pytest.mark.parametrize("dtype,N_T", [("float32", 50), ("float32", 125), ("int16", 64), ("float64", 7)])
 def test_generic_vector_kernel_batches_and_series(B, U, dtype, N_T):
     """The 128-bit generic kernel takes 32 pairs per launch: a batch of 40 pairs on a pitch no tensor map can describe

@@ -299,6 +299,30 @@ def test_fused_batch_unaligned_pair_takes_generic_kernel(U, B):
         U.assert_parity(got, ref, K6["C"], f"unaligned batch pair {i}")
 
 
+@pytest.mark.parametrize("N,N_T", [(512, 64), (512, 128)])
+def test_fused_batch_of_mixed_alignment_is_planned_per_run(U, B, N, N_T):
+    """One pair behind a base 4 bytes off in a 4-pair batch: every pair gets the kernel it would get alone (bit-identical
+    to the single calls, which for the aligned pairs means tma_kernel and not the generic fall-back), Eqs. 3-4 included."""
+    P = 4
+    hosts = [_rand_pair(N, seed=40 + s) for s in range(P)]
+    buf = torch.empty(N * N + 3, dtype=torch.float32, device="cuda")
+    x2 = buf[1:1 + N * N].view(N, N)
+    x2.copy_(torch.from_numpy(hosts[2][0]))
+    xs = [U.to_dev(hosts[0][0]), U.to_dev(hosts[1][0]), x2, U.to_dev(hosts[3][0])]
+    ys = [U.to_dev(h[1]) for h in hosts]
+    assert B.plan_name(xs[0], N_T).startswith("tma:") and not B.plan_name(x2, N_T).startswith("tma:")
+    out = B.fused_batch(xs, ys, N_T, numerators=True, **K6)
+    for i in range(P):
+        single = B.fused_tiles(xs[i], ys[i], N_T, numerators=True, **K6)
+        whole = B.aggregate(single["lisi"], single["auglisi"], single["X"], single["Y"], K6["C2"], K6["C"])
+        for nm in ("lisi", "auglisi", "X", "Y", "L", "A"):
+            assert torch.equal(out[nm][i], single[nm]), (i, nm)
+        assert torch.equal(out["whole"][i], whole), i
+        ref = U.run_oracle(hosts[i][0], hosts[i][1], N_T, K6)
+        got = {nm: out[nm][i].cpu().numpy().astype(np.float64) for nm in ("lisi", "auglisi", "X", "Y", "L", "A")}
+        U.assert_parity(got, ref, K6["C"], f"mixed batch pair {i}")
+
+
 def test_aggregate_equals_whole_image_and_merge(U, B):
     """P6: Eqs. 3-4 over the tiles == the index of the whole image; g x g merge == tiles at g*N_T."""
     cfg = synth.CONFIGS[1]
