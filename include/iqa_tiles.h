@@ -165,8 +165,10 @@ int iqa_fused_tiles_static(const float* x, const float* y, int N, int N_T,
 #define IQA_PLAN_TMA 16
 int iqa_query_plan(const void* x, int pixel_type, int H, int W, long long pitch, int N_T, int series);
 
-/* Test and tuning hook: sets one of the library's process-wide knobs and returns its previous value (-1: unknown
- * name).  The knobs take their initial value from the environment variable of the same name, read once:
+/* Test and tuning hook, NOT part of the stable ABI (names and meanings may change with any release): sets one of the
+ * library's process-wide knobs and returns its previous value (-1: unknown name).  The library never reads the
+ * environment; only a build with -DIQA_TESTING takes the knobs' initial values from the environment variables of
+ * the same names:
  *   IQA_FORCE_GENERIC 1: generic kernels only        IQA_FORCE_ANY 1: any_kernel instead of tma_kernel
  *   IQA_TMA_CONFIG 0..4: tma_kernel ring / box configuration (-1: default)
  *   IQA_TMA_MAX_CTAS n: cap of the persistent grid (0: none)     IQA_NO_PDL 1: no programmatic dependent launch

@@ -131,30 +131,14 @@ __device__ __forceinline__ void pixel_terms_any(const T* __restrict__ x, const T
 // Per-tile results are stored with an L2 evict-last policy: they are a few MiB, they are read again right away
 // (finalise / aggregate / merge / candidate kernels), and keeping them in L2 keeps their write-back out of the
 // DRAM read stream of the images.
-// IQA_STORE_VARIANT (compile-time, experiments only): 0 = evict-last (the library), 1 = plain stores,
-// 2 = evict-first policy, 3 = st.global.cs, 4 = no stores at all (wrong results: the cost of the output path).
-#ifndef IQA_STORE_VARIANT
-#define IQA_STORE_VARIANT 0
-#endif
+// (plain stores, an evict-first policy and st.global.cs were measured against this: profiles/r02_store_variants.md)
 __device__ __forceinline__ uint64_t policy_evict_last() {
     uint64_t pol;
-#if IQA_STORE_VARIANT == 2
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-#else
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-#endif
     return pol;
 }
 __device__ __forceinline__ void store_result(float* dst, float v, uint64_t pol) {
-#if IQA_STORE_VARIANT == 1
-    *dst = v;
-#elif IQA_STORE_VARIANT == 3
-    __stcs(dst, v);
-#elif IQA_STORE_VARIANT == 4
-    if (v == 1.2345e-33f) *dst = v;
-#else
     asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(dst), "f"(v), "l"(pol) : "memory");
-#endif
 }
 
 template <class Params>

@@ -42,7 +42,10 @@ bool pos_finite(float v) { return std::isfinite(v) && v > 0.0f; }
 // C1 feeds rcp.approx.ftz (|x - y| + C1 with x == y): a subnormal C1 would be flushed to zero there
 bool pos_normal(float v) { return std::isfinite(v) && v >= FLT_MIN; }
 
-// ---- test / tuning knobs (iqa_debug_knob): read from the environment ONCE, then plain atomics -------------------
+// ---- test / tuning knobs (iqa_debug_knob): plain atomics, set by iqa_debug_knob only --------------------------------
+// The shipping library does NOT read the environment: a stray IQA_FORCE_GENERIC=1 in a user's shell must not cost
+// 40 % of the bandwidth silently.  A build with -DIQA_TESTING takes the initial values from the environment
+// variables of the same names (read once), which is handy under ncu.
 //   IQA_FORCE_GENERIC    1: every call takes the generic kernels
 //   IQA_FORCE_ANY        1: fp32 power-of-two shapes take the general TMA kernel (iqa_any.cuh) instead of tma_kernel
 //   IQA_TMA_CONFIG       0..4: ring / box configuration of tma_kernel (-1: default)
@@ -62,8 +65,12 @@ struct Knobs {
     std::atomic<int> v[kNumKnobs];
     Knobs() {
         for (int i = 0; i < kNumKnobs; ++i) {
+#ifdef IQA_TESTING
             const char* s = std::getenv(kKnobNames[i]);
             v[i].store((s && *s) ? std::atoi(s) : kKnobDefaults[i], std::memory_order_relaxed);
+#else
+            v[i].store(kKnobDefaults[i], std::memory_order_relaxed);
+#endif
         }
     }
 };
@@ -962,7 +969,7 @@ const char* iqa_status_string(int status) {
     }
 }
 
-const char* iqa_version(void) { return "0.7.0"; }
+const char* iqa_version(void) { return "0.8.0"; }
 
 int iqa_debug_knob(const char* name, int value) {
     if (!name) return -1;

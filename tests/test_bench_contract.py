@@ -22,6 +22,31 @@ def test_reference_arm_prints_one_contract_line():
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
     assert d["cpu_baseline"]["value"] == d["value"] and d["e2e"]["value"] == d["value"]
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0
+    # `config` is the GPU arm's, key for key (the driver compares the two); the reference arm's own bounded sample is
+    # described in cpu_baseline.sample
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2501_10653_b200 import synth
+    idx, pairs, _ = bench.WORKLOADS["cfg0"]
+    assert d["config"] == bench.workload_config(synth.CONFIGS[idx], pairs, bench.l2_note(synth.CONFIGS[idx], pairs))
+    assert "pair(s)" in d["cpu_baseline"]["sample"]
+
+
+def test_traffic_table_is_machine_written_and_parses():
+    """roofline.traffic comes from profiles/ncu_traffic.csv (rows copied out of .ncu-rep files by `bench.py
+    --traffic-extract`), keyed by workload, batch size and library version."""
+    import csv
+    sys.path.insert(0, ROOT)
+    import bench
+    path = os.path.join(ROOT, bench.NCU_TRAFFIC_FILE)
+    assert os.path.exists(path)
+    rows = list(csv.DictReader(open(path, newline="")))
+    assert rows and list(rows[0].keys()) == bench.TRAFFIC_COLUMNS
+    for r in rows:
+        total, src = bench.ncu_traffic(r["workload"], int(r["pairs_per_launch"]), r["library_version"])
+        assert total == float(r["dram__bytes_read.sum"]) + float(r["dram__bytes_write.sum"]) and r["report"] in src
+        assert bench.ncu_traffic(r["workload"], int(r["pairs_per_launch"]), "0.0.0")[0] is None     # another version
+    assert bench.ncu_traffic("no_such_workload", 1, "0.0.0")[0] is None
 
 
 def test_reference_arm_other_ranks_print_nothing():

@@ -248,11 +248,15 @@ def test_standalone_entry_points_match_fused(U, B):
     x, y, _ = synth.make_pair(cfg)
     xd, yd = U.to_dev(x), U.to_dev(y)
     k = U.consts(cfg)
-    for N_T in (16, 64, 256):
+    for N_T in (16, 64, 256):        # tma_kernel<lisi> / <auglisi>: several tiles per item, whole tiles, split tiles
         f = B.fused_tiles(xd, yd, N_T, **k)
         li = B.lisi_tiles(xd, yd, N_T, k["C1"], k["C2"], k["D"])
         au = B.auglisi_tiles(xd, yd, N_T, k["C"])
         assert torch.equal(li, f["lisi"]) and torch.equal(au, f["auglisi"])
+        # and against the oracle directly on the same data, not only through the fused call
+        ref = U.run_oracle(x, y, N_T, k)
+        got = {"lisi": li.cpu().numpy().astype(np.float64), "auglisi": au.cpu().numpy().astype(np.float64)}
+        U.assert_parity(got, ref, k["C"], f"standalone entry points, N_T={N_T}")
 
 
 @pytest.mark.parametrize("N,N_T,P", [(256, 16, 5), (2048, 64, 3), (1024, 8, 2), (1024, 256, 3), (392, 8, 4),

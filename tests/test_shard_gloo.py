@@ -2,6 +2,7 @@
 data-path collective; timing is the max over ranks."""
 import os
 import socket
+import sys
 
 import pytest
 
@@ -152,3 +153,27 @@ def test_two_ranks_share_one_pair_by_bands():
     lisi = t0[0] / (max(t0[2], t0[3]) + c2)                    # Eq. 3 from the summed partials
     aug = (t0[1] - (n - 1) * c) / (t0[2] + t0[3] + c)          # Eq. 4
     assert abs(lisi - exp[0]) <= 1e-12 * abs(exp[0]) and abs(aug - exp[1]) <= 1e-12 * abs(exp[1])
+
+
+def test_bench_gpus_n_starts_its_own_ranks():
+    """`python bench.py --gpus 2` without WORLD_SIZE re-executes itself under torch.distributed.run with two ranks
+    (the form the driver's 1-GPU command has).  --rank-map stops before CUDA: every rank joins a gloo group and reports
+    its band of ONE config-[4] pair (--shard bands) and its seeds (replicas); the bands are shard.band_rows' partition."""
+    import json
+    import subprocess
+    from paper_2501_10653_b200 import shard, synth
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items()
+           if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--rank-map", "--workload", "cfg4",
+                        "--shard", "bands"], capture_output=True, text=True, env=env, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    d = json.loads(lines[0])
+    cfg = synth.CONFIGS[4]
+    assert d["n_gpus"] == 2 and [x["rank"] for x in d["ranks"]] == [0, 1]
+    assert [tuple(x["band_rows"]) for x in d["ranks"]] == [shard.band_rows(cfg.N, cfg.N_T, k, 2) for k in range(2)]
+    assert d["ranks"][0]["band_rows"][0] == 0 and d["ranks"][1]["band_rows"][1] == cfg.N
+    assert d["ranks"][0]["band_rows"][1] == d["ranks"][1]["band_rows"][0]
+    assert d["ranks"][0]["seeds"][1] < d["ranks"][1]["seeds"][0]           # replicas: no rank repeats another's pairs
