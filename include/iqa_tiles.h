@@ -165,6 +165,13 @@ int iqa_fused_tiles_static(const float* x, const float* y, int N, int N_T,
 #define IQA_PLAN_TMA 16
 int iqa_query_plan(const void* x, int pixel_type, int H, int W, long long pitch, int N_T, int series);
 
+/* The same for a call of a given size.  One rule of the plan depends on how much work the call holds: the generic
+ * kernel (one warp per piece of a tile) only beats any_kernel's idle lanes when the whole call has several pieces per
+ * SM, so SMALL jobs -- one or two pairs of a 1024^2 or 2048^2 image with tiles of 113 .. 400 columns -- keep any_kernel
+ * (up to 3x faster there).  iqa_query_plan answers for a job large enough to fill the GPU; iqa_query_plan_n answers for
+ * n_cmp pairs (or comparisons of a series; 0 = large job) on the CURRENT device (without a device: the large-job answer). */
+int iqa_query_plan_n(const void* x, int pixel_type, int H, int W, long long pitch, int N_T, int series, int n_cmp);
+
 /* Test and tuning hook, NOT part of the stable ABI (names and meanings may change with any release): sets one of the
  * library's process-wide knobs and returns its previous value (-1: unknown name).  The library never reads the
  * environment; only a build with -DIQA_TESTING takes the knobs' initial values from the environment variables of
@@ -174,6 +181,7 @@ int iqa_query_plan(const void* x, int pixel_type, int H, int W, long long pitch,
  *   IQA_TMA_MAX_CTAS n: cap of the persistent grid (0: none)     IQA_NO_PDL 1: no programmatic dependent launch
  *   IQA_CAND_NO_CLUSTER 1: candidate kernels without thread-block clusters
  *   IQA_ANY_NO_WIDE 1: any_kernel lanes own four columns even when eight would fit
+ *   IQA_PLAN_LARGE_JOB 1: plan every call as a large job (the small-job rule of iqa_query_plan_n off)
  * They select among kernels that all satisfy the same parity bar (tests/test_gpu_parity.py runs every one). */
 int iqa_debug_knob(const char* name, int value);
 
@@ -262,7 +270,10 @@ size_t iqa_batch_workspace_bytes(int n_pairs, int N, int N_T);
  *   out2                 [n_pairs * 2] device, MAY BE NULL: out2[2p] = LISI, out2[2p+1] = augLISI of pair p
  *   workspace            >= iqa_batch_workspace_bytes(n_pairs, N, N_T) bytes (may be NULL when 0)
  * n_pairs * n must stay below 2^31.  Results are bit-identical to n_pairs calls of
- * iqa_fused_tiles + iqa_aggregate: the kernel is chosen per run of consecutive pairs whose x and y
+ * iqa_fused_tiles + iqa_aggregate whenever the batch and the single call take the same kernel (always for the
+ * power-of-two tile sides of tma_kernel and for whole-tile any_kernel shapes; the one size-dependent rule, for split
+ * tiles of 113 .. 400 columns on small images, is described at iqa_query_plan_n): the kernel is chosen per run of
+ * consecutive pairs whose x and y
  * sit at the same offset inside their 16-byte lines, as it would be for each pair alone, so one
  * shifted pair costs the aligned pairs of its batch nothing (it only splits the batch into more launches). */
 int iqa_fused_batch(const float* const* x_ptrs_host, const float* const* y_ptrs_host, int n_pairs,
@@ -442,6 +453,23 @@ int iqa_fused_host_async(const float* x_host, const float* y_host, int N, int N_
                          float* lisi_host, float* auglisi_host,
                          float* sum_x_host, float* sum_y_host, float* out2_host,
                          void* dev_scratch, size_t dev_scratch_bytes, void* stream);
+
+/* The host entry points for images of `pixel_type` pixels as a FITS file stores them ("allowing input of FITS
+ * images": BITPIX 16 / 8 / 32 / -64, fp16 from a GPU imager).  The raw pixels are uploaded and computed on as they are
+ * (the typed kernels of iqa_fused_tiles_2d_typed): a 16-bit plane costs half the PCIe bytes of its fp32 conversion, and
+ * the host path is PCIe-bound.  Arguments as iqa_fused_host(_async); x_host, y_host [N*N] of the pixel type;
+ * dev_scratch >= iqa_host_scratch_bytes_typed(N, N_T, pixel_type) bytes, 256-B aligned.  Unknown pixel_type: IQA_ERR_SHAPE. */
+size_t iqa_host_scratch_bytes_typed(int N, int N_T, int pixel_type);
+int iqa_fused_host_typed(const void* x_host, const void* y_host, int pixel_type, int N, int N_T,
+                         float C1, float C2, float C, float D,
+                         float* lisi_host, float* auglisi_host,
+                         float* sum_x_host, float* sum_y_host, float* out2_host,
+                         void* dev_scratch, size_t dev_scratch_bytes, void* stream);
+int iqa_fused_host_typed_async(const void* x_host, const void* y_host, int pixel_type, int N, int N_T,
+                               float C1, float C2, float C, float D,
+                               float* lisi_host, float* auglisi_host,
+                               float* sum_x_host, float* sum_y_host, float* out2_host,
+                               void* dev_scratch, size_t dev_scratch_bytes, void* stream);
 
 #ifdef __cplusplus
 }

@@ -26,12 +26,13 @@ IQA_STATIC_WORKSPACE_BYTES = 1 << 20     # include/iqa_tiles.h; tests/test_zz_no
 
 EXPORTS = ("iqa_status_string", "iqa_version", "iqa_debug_knob", "iqa_workspace_bytes", "iqa_lisi_tiles",
            "iqa_auglisi_tiles", "iqa_fused_tiles", "iqa_fused_tiles_static", "iqa_batch_workspace_bytes", "iqa_fused_batch",
-           "iqa_query_plan", "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_tiles_2d_typed",
+           "iqa_query_plan", "iqa_query_plan_n", "iqa_workspace_bytes_2d", "iqa_fused_tiles_2d", "iqa_fused_tiles_2d_typed",
            "iqa_fused_batch_2d", "iqa_fused_batch_2d_typed", "iqa_series_tiles_2d", "iqa_series_tiles_2d_typed",
            "iqa_series_workspace_bytes", "iqa_series_tiles", "iqa_series_find", "iqa_series_find_2d_typed", "iqa_tiles_below", "iqa_tiles_bottom_k",
            "iqa_aggregate", "iqa_aggregate_partial", "iqa_aggregate_finish", "iqa_merge_tiles", "iqa_merge_tiles_batch",
            "iqa_pyramid_levels", "iqa_pyramid_tiles", "iqa_pyramid",
-           "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async")
+           "iqa_host_scratch_bytes", "iqa_fused_host", "iqa_fused_host_async",
+           "iqa_host_scratch_bytes_typed", "iqa_fused_host_typed", "iqa_fused_host_typed_async")
 
 IQA_SERIES_REFERENCE, IQA_SERIES_CONSECUTIVE = 0, 1
 IQA_PIXEL_F32, IQA_PIXEL_F64, IQA_PIXEL_F16, IQA_PIXEL_I16, IQA_PIXEL_I32, IQA_PIXEL_U8 = range(6)
@@ -95,6 +96,8 @@ def _load() -> ctypes.CDLL:
                                              vp, vp, vp, vp, vp, vp, vp, vp, sz, i, i, vp, vp, f, vp, i, vp, vp]
     lib.iqa_query_plan.restype = i
     lib.iqa_query_plan.argtypes = [vp, i, i, i, ctypes.c_longlong, i, i]
+    lib.iqa_query_plan_n.restype = i
+    lib.iqa_query_plan_n.argtypes = [vp, i, i, i, ctypes.c_longlong, i, i, i]
     lib.iqa_debug_knob.restype = i
     lib.iqa_debug_knob.argtypes = [ctypes.c_char_p, i]
     lib.iqa_fused_batch_2d_typed.restype = i
@@ -141,6 +144,12 @@ def _load() -> ctypes.CDLL:
     lib.iqa_fused_host.argtypes = [vp, vp, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.iqa_fused_host_async.restype = i
     lib.iqa_fused_host_async.argtypes = [vp, vp, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_host_scratch_bytes_typed.restype = sz
+    lib.iqa_host_scratch_bytes_typed.argtypes = [i, i, i]
+    lib.iqa_fused_host_typed.restype = i
+    lib.iqa_fused_host_typed.argtypes = [vp, vp, i, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.iqa_fused_host_typed_async.restype = i
+    lib.iqa_fused_host_typed_async.argtypes = [vp, vp, i, i, i, f, f, f, f, vp, vp, vp, vp, vp, vp, sz, vp]
     return lib
 
 
@@ -282,10 +291,15 @@ def _pixel_types():
             torch.int16: IQA_PIXEL_I16, torch.int32: IQA_PIXEL_I32, torch.uint8: IQA_PIXEL_U8}
 
 
-def plan_name(x, N_T, series=False) -> str:
+def iqa_query_plan_n(x, pixel_type, H, W, pitch, N_T, series=0, n_cmp=0) -> int:
+    return lib.iqa_query_plan_n(_ptr(x), int(pixel_type), int(H), int(W), int(pitch), int(N_T), int(series), int(n_cmp))
+
+
+def plan_name(x, N_T, series=False, n=0) -> str:
     """Which kernel a call on the CUDA tensor ``x`` would take: 'tma:c<k>' (tma_kernel), 'tma_any' (any_kernel)
-    or 'generic'."""
-    p = iqa_query_plan(x, _pixel_types()[x.dtype], x.shape[0], x.shape[1], x.stride(0), N_T, 1 if series else 0)
+    or 'generic'.  ``n``: pairs / comparisons of the call (0: a job large enough to fill the GPU)."""
+    with _device_of(x.device):
+        p = iqa_query_plan_n(x, _pixel_types()[x.dtype], x.shape[0], x.shape[1], x.stride(0), N_T, 1 if series else 0, n)
     return f"tma:c{p - IQA_PLAN_TMA}" if p >= IQA_PLAN_TMA else {0: "generic", 2: "tma_any"}.get(p, "invalid")
 
 
@@ -434,6 +448,24 @@ def iqa_fused_host_async(x_host, y_host, N, N_T, C1, C2, C, D, lisi_host, auglis
     return lib.iqa_fused_host_async(_ptr(x_host), _ptr(y_host), int(N), int(N_T), C1, C2, C, D,
                                     _ptr(lisi_host), _ptr(auglisi_host), _ptr(sum_x_host), _ptr(sum_y_host),
                                     _ptr(out2_host), _ptr(dev_scratch), int(dev_scratch_bytes), _stream(stream))
+
+
+def iqa_host_scratch_bytes_typed(N: int, N_T: int, pixel_type: int) -> int:
+    return int(lib.iqa_host_scratch_bytes_typed(int(N), int(N_T), int(pixel_type)))
+
+
+def iqa_fused_host_typed(x_host, y_host, pixel_type, N, N_T, C1, C2, C, D, lisi_host, auglisi_host,
+                         sum_x_host, sum_y_host, out2_host, dev_scratch, dev_scratch_bytes, stream=None) -> int:
+    return lib.iqa_fused_host_typed(_ptr(x_host), _ptr(y_host), int(pixel_type), int(N), int(N_T), C1, C2, C, D,
+                                    _ptr(lisi_host), _ptr(auglisi_host), _ptr(sum_x_host), _ptr(sum_y_host),
+                                    _ptr(out2_host), _ptr(dev_scratch), int(dev_scratch_bytes), _stream(stream))
+
+
+def iqa_fused_host_typed_async(x_host, y_host, pixel_type, N, N_T, C1, C2, C, D, lisi_host, auglisi_host,
+                               sum_x_host, sum_y_host, out2_host, dev_scratch, dev_scratch_bytes, stream=None) -> int:
+    return lib.iqa_fused_host_typed_async(_ptr(x_host), _ptr(y_host), int(pixel_type), int(N), int(N_T), C1, C2, C, D,
+                                          _ptr(lisi_host), _ptr(auglisi_host), _ptr(sum_x_host), _ptr(sum_y_host),
+                                          _ptr(out2_host), _ptr(dev_scratch), int(dev_scratch_bytes), _stream(stream))
 
 
 # ----------------------------------------------------------------------------- convenience
@@ -917,12 +949,15 @@ def pyramid(tiles: dict, C2, C) -> list:
 class HostRunner:
     """Reusable state for ``iqa_fused_host``: the device scratch and pinned result buffers."""
 
-    def __init__(self, N: int, N_T: int, device="cuda:0"):
+    def __init__(self, N: int, N_T: int, device="cuda:0", pixel_type: int = IQA_PIXEL_F32):
         import torch
         self.N, self.N_T = int(N), int(N_T)
         self.nt = self.N // self.N_T
         self.device = torch.device(device)
-        self.scratch_bytes = iqa_host_scratch_bytes(N, N_T)
+        self.pixel_type = int(pixel_type)        # IQA_PIXEL_*: the host images are uploaded and computed on as they are
+        self.esize = {IQA_PIXEL_F32: 4, IQA_PIXEL_F64: 8, IQA_PIXEL_F16: 2, IQA_PIXEL_I16: 2, IQA_PIXEL_I32: 4,
+                      IQA_PIXEL_U8: 1}.get(self.pixel_type, 0)
+        self.scratch_bytes = iqa_host_scratch_bytes_typed(N, N_T, self.pixel_type)
         if self.scratch_bytes == 0:
             raise IqaError(IQA_ERR_SHAPE, "HostRunner")
         self.scratch = torch.empty(self.scratch_bytes, dtype=torch.uint8, device=self.device)
@@ -932,7 +967,7 @@ class HostRunner:
 
     @property
     def h2d_bytes(self) -> int:
-        return 2 * 4 * self.N * self.N
+        return 2 * self.esize * self.N * self.N
 
     @property
     def d2h_bytes(self) -> int:
@@ -940,9 +975,10 @@ class HostRunner:
 
     def __call__(self, x_host, y_host, C1, C2, C, D):
         with _device_of(self.device):
-            rc = iqa_fused_host(x_host, y_host, self.N, self.N_T, C1, C2, C, D,
-                                self.out["lisi"], self.out["auglisi"], self.out["X"], self.out["Y"],
-                                self.out2, self.scratch, self.scratch_bytes, _current_stream(self.device))
+            args = (self.N, self.N_T, C1, C2, C, D, self.out["lisi"], self.out["auglisi"], self.out["X"], self.out["Y"],
+                    self.out2, self.scratch, self.scratch_bytes, _current_stream(self.device))
+            rc = (iqa_fused_host(x_host, y_host, *args) if self.pixel_type == IQA_PIXEL_F32
+                  else iqa_fused_host_typed(x_host, y_host, self.pixel_type, *args))
         if rc != IQA_OK:
             raise IqaError(rc, "iqa_fused_host")
         return self.out, self.out2
@@ -954,9 +990,9 @@ class HostPipeline:
     the slot whose pinned outputs will hold the result; ``wait(slot)`` / ``drain()`` synchronise.  The upload
     of pair i+1 overlaps the kernels, downloads and launch gaps of pair i."""
 
-    def __init__(self, N: int, N_T: int, device="cuda:0", depth: int = 2):
+    def __init__(self, N: int, N_T: int, device="cuda:0", depth: int = 2, pixel_type: int = IQA_PIXEL_F32):
         import torch
-        self.runners = [HostRunner(N, N_T, device) for _ in range(depth)]
+        self.runners = [HostRunner(N, N_T, device, pixel_type) for _ in range(depth)]
         self.streams = [torch.cuda.Stream(device=self.runners[0].device) for _ in range(depth)]
         self.next = 0
 
@@ -966,8 +1002,10 @@ class HostPipeline:
         r, st = self.runners[slot], self.streams[slot]
         st.synchronize()                         # the slot's previous pair is complete: its buffers are free
         with _device_of(r.device):
-            rc = iqa_fused_host_async(x_host, y_host, r.N, r.N_T, C1, C2, C, D, r.out["lisi"], r.out["auglisi"],
-                                      r.out["X"], r.out["Y"], r.out2, r.scratch, r.scratch_bytes, st)
+            args = (r.N, r.N_T, C1, C2, C, D, r.out["lisi"], r.out["auglisi"], r.out["X"], r.out["Y"], r.out2, r.scratch,
+                    r.scratch_bytes, st)
+            rc = (iqa_fused_host_async(x_host, y_host, *args) if r.pixel_type == IQA_PIXEL_F32
+                  else iqa_fused_host_typed_async(x_host, y_host, r.pixel_type, *args))
         if rc != IQA_OK:
             raise IqaError(rc, "iqa_fused_host_async")
         return slot
@@ -982,8 +1020,14 @@ class HostPipeline:
 
 
 def fused_host(x_host, y_host, N_T, C1, C2, C, D, device="cuda:0"):
-    """One-shot host call (allocates scratch each time; use HostRunner in loops)."""
+    """One-shot host call (allocates scratch each time; use HostRunner in loops).  x_host, y_host: square numpy arrays
+    or CPU tensors of one supported pixel type (float32, float64, float16, int16, int32, uint8)."""
     N = int(x_host.shape[0])
-    r = HostRunner(N, N_T, device)
+    names = {"float32": IQA_PIXEL_F32, "float64": IQA_PIXEL_F64, "float16": IQA_PIXEL_F16, "int16": IQA_PIXEL_I16,
+             "int32": IQA_PIXEL_I32, "uint8": IQA_PIXEL_U8}
+    dt = str(x_host.dtype).replace("torch.", "")
+    if dt not in names or str(y_host.dtype).replace("torch.", "") != dt:
+        raise TypeError("x_host and y_host must share one supported pixel type")
+    r = HostRunner(N, N_T, device, names[dt])
     out, out2 = r(x_host, y_host, C1, C2, C, D)
     return {k: v.clone() for k, v in out.items()}, out2.clone()

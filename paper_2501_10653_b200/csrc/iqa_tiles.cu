@@ -55,12 +55,13 @@ bool pos_normal(float v) { return std::isfinite(v) && v >= FLT_MIN; }
 //   IQA_ANY_NO_WIDE      1: any_kernel never lets a lane own eight columns
 //   IQA_GENERIC_NO_VEC   1: the generic path always takes the scalar-load kernels
 //   IQA_SERIES_PAIR_MAJOR 1: any_kernel runs the comparisons of a series in pair-major item order (no L2 sharing)
+//   IQA_PLAN_LARGE_JOB   1: every call is planned as if it had enough work to fill the GPU (no small-job rule in make_plan)
 enum Knob { kKnobForceGeneric, kKnobForceAny, kKnobTmaConfig, kKnobTmaMaxCtas, kKnobNoPdl, kKnobCandNoCluster, kKnobNoWide,
-            kKnobGenericNoVec, kKnobSeriesPairMajor, kNumKnobs };
+            kKnobGenericNoVec, kKnobSeriesPairMajor, kKnobPlanLargeJob, kNumKnobs };
 const char* const kKnobNames[kNumKnobs] = {"IQA_FORCE_GENERIC", "IQA_FORCE_ANY", "IQA_TMA_CONFIG", "IQA_TMA_MAX_CTAS",
                                            "IQA_NO_PDL", "IQA_CAND_NO_CLUSTER", "IQA_ANY_NO_WIDE", "IQA_GENERIC_NO_VEC",
-                                           "IQA_SERIES_PAIR_MAJOR"};
-const int kKnobDefaults[kNumKnobs] = {0, 0, -1, 0, 0, 0, 0, 0, 0};
+                                           "IQA_SERIES_PAIR_MAJOR", "IQA_PLAN_LARGE_JOB"};
+const int kKnobDefaults[kNumKnobs] = {0, 0, -1, 0, 0, 0, 0, 0, 0, 0};
 struct Knobs {
     std::atomic<int> v[kNumKnobs];
     Knobs() {
@@ -439,10 +440,25 @@ Align align_of(const void* const* a, int na, const void* const* b, int nb) {
     return Align{lo};
 }
 
+// The 128-bit generic kernel runs one WARP per piece of a tile (<= 64 rows) and keeps a few 16-byte loads per lane in
+// flight: it only beats any_kernel's idle lanes when there are enough pieces to give every SM several warps.  Below that
+// (one or two pairs of a 1024^2 / 2048^2 image with tiles of 113 .. 400 columns) any_kernel, whose TMA ring keeps tens of
+// KiB in flight per SM whatever the item count, is up to 3x faster.  Measured crossovers (pieces of the whole call per
+// SM; sweeps at N = 1024 / 2048 with 2, 4 and 32 pairs): ~4.5 for 4-byte pixels, ~12 for fp64, ~4 for 1- and 2-byte pixels.
+// Without a device (a CPU-only box asking iqa_query_plan) the rule is off.
+bool small_job(const Geom& g, int N_T, int es, long long n_cmp) {
+    if (knob(kKnobPlanLargeJob)) return false;
+    const Geometry* geo = geometry();
+    if (!geo) return false;
+    const long long units = (long long)ceil_div(g.W, N_T) * ceil_div(g.H, N_T) * ceil_div(N_T, kGenericRows) * n_cmp;
+    const long long per_sm_x2 = es == 8 ? 24 : es == 4 ? 9 : 8;          // twice the crossover
+    return 2 * units < per_sm_x2 * geo->sms;
+}
+
 // A tensor map can describe the images when every row pitch is a multiple of 16 bytes; the boxes of x and y share
 // their column grid when all bases have the same offset inside a 16-byte line (al.lo16 >= 0).
 // series: the call is a time series (tma_kernel's series ring; any_kernel's pair-minor order); n_cmp: its comparisons.
-Plan make_plan(const Geom& g, int N_T, Align al, bool series, int n_cmp = 2) {
+Plan make_plan(const Geom& g, int N_T, Align al, bool series, int n_cmp) {
     Plan pl{};
     generic_plan(pl, N_T);
     const int es = esize_of(g.ptype);
@@ -486,7 +502,7 @@ Plan make_plan(const Geom& g, int N_T, Align al, bool series, int n_cmp = 2) {
                            : sharing ? (split ? 0.5 : -1.0)
                                      : (!split ? whole : 0.8);
         const bool narrow_image = !split && a.kx >= ceil_div(g.W, N_T);       // the image, not the mapping, limits the fill
-        if (!narrow_image && (split ? fill < limit : fill <= limit)) {
+        if (!narrow_image && (split ? fill < limit : fill <= limit) && !small_job(g, N_T, es, n_cmp)) {
             generic_plan(pl, N_T);
             return pl;
         }
@@ -853,7 +869,7 @@ int run_batch(int mode, const void* const* xs, const void* const* ys, int n_pair
         const Align al = align_of(xs + first, 1, ys + first, 1);
         int np = 1;
         while (first + np < n_pairs && align_of(xs + first + np, 1, ys + first + np, 1).lo16 == al.lo16) ++np;
-        Plan pl = make_plan(g, N_T, al, false);
+        Plan pl = make_plan(g, N_T, al, false, n_pairs);          // (the job's size is the call's, not the run's)
         const Outputs o = out.offset((size_t)first * (size_t)n);
         float4* w = ws ? ws + (size_t)first * ws_per_pair : nullptr;
         if (const int rc = launch_pairs(mode, xs + first, ys + first, np, g, N_T, k, o, w, pl, st)) return rc;
@@ -1042,10 +1058,14 @@ int iqa_fused_tiles_static(const float* x, const float* y, int N, int N_T,
 }
 
 int iqa_query_plan(const void* x, int pixel_type, int H, int W, long long pitch, int N_T, int series) {
+    return iqa_query_plan_n(x, pixel_type, H, W, pitch, N_T, series, 0);
+}
+
+int iqa_query_plan_n(const void* x, int pixel_type, int H, int W, long long pitch, int N_T, int series, int n_cmp) {
     const int es = esize_of(pixel_type);
-    if (!x || es == 0 || H <= 0 || W <= 0 || N_T <= 0 || pitch < W || ((uintptr_t)x & (uintptr_t)(es - 1))) return -1;
+    if (!x || es == 0 || H <= 0 || W <= 0 || N_T <= 0 || n_cmp < 0 || pitch < W || ((uintptr_t)x & (uintptr_t)(es - 1))) return -1;
     const Geom g{H, W, pitch, pitch, pixel_type};
-    const Plan pl = make_plan(g, N_T, align_of(&x, 1, &x, 0), series != 0);
+    const Plan pl = make_plan(g, N_T, align_of(&x, 1, &x, 0), series != 0, n_cmp > 0 ? n_cmp : 1 << 30);
     if (pl.kind == kPlanTma) return IQA_PLAN_TMA + pl.tma_cfg;
     // (a series runs any_kernel as one launch per 32 comparisons in pair-minor item order)
     return pl.kind == kPlanAny ? IQA_PLAN_TMA_ANY : IQA_PLAN_GENERIC;
@@ -1353,34 +1373,37 @@ int iqa_merge_tiles(const float* lisi, const float* auglisi,
                                  sum_y_out, stream);
 }
 
-size_t iqa_host_scratch_bytes(int N, int N_T) {
-    if (status_of_shape(N, N_T) != IQA_OK) return 0;
-    const size_t img = align_up((size_t)N * (size_t)N * sizeof(float), 256);
+size_t iqa_host_scratch_bytes(int N, int N_T) { return iqa_host_scratch_bytes_typed(N, N_T, IQA_PIXEL_F32); }
+
+size_t iqa_host_scratch_bytes_typed(int N, int N_T, int pixel_type) {
+    if (status_of_shape(N, N_T) != IQA_OK || esize_of(pixel_type) == 0) return 0;
+    const size_t img = align_up((size_t)N * (size_t)N * (size_t)esize_of(pixel_type), 256);
     const size_t n = (size_t)(N / N_T) * (size_t)(N / N_T);
     const size_t per_tile = align_up(n * sizeof(float), 256);
     return 2 * img + 4 * per_tile + 256 + align_up(workspace_bytes_for(1, N, N_T), 256);
 }
 
 namespace {
-int fused_host_impl(const float* x_host, const float* y_host, int N, int N_T,
+int fused_host_impl(const void* x_host, const void* y_host, int ptype, int N, int N_T,
                     float C1, float C2, float C, float D,
                     float* lisi_host, float* auglisi_host,
                     float* sum_x_host, float* sum_y_host, float* out2_host,
                     void* dev_scratch, size_t dev_scratch_bytes, void* stream, bool synchronise) {
     if (!x_host || !y_host || !dev_scratch) return IQA_ERR_NULL;
+    if (esize_of(ptype) == 0) return IQA_ERR_SHAPE;
     if (const int s = status_of_shape(N, N_T)) return s;
     if (!pos_normal(C1) || !pos_finite(C2) || !pos_finite(C) || !std::isfinite(D)) return IQA_ERR_PARAM;
-    if (dev_scratch_bytes < iqa_host_scratch_bytes(N, N_T)) return IQA_ERR_WORKSPACE;
+    if (dev_scratch_bytes < iqa_host_scratch_bytes_typed(N, N_T, ptype)) return IQA_ERR_WORKSPACE;
     if ((uintptr_t)dev_scratch & 255u) return IQA_ERR_ALIGN;
 
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t img_bytes = (size_t)N * (size_t)N * sizeof(float);
+    const size_t img_bytes = (size_t)N * (size_t)N * (size_t)esize_of(ptype);
     const size_t img = align_up(img_bytes, 256);
     const size_t n = (size_t)(N / N_T) * (size_t)(N / N_T);
     const size_t per_tile = align_up(n * sizeof(float), 256);
     char* base = (char*)dev_scratch;
-    float* xd = (float*)base;
-    float* yd = (float*)(base + img);
+    void* xd = base;
+    void* yd = base + img;
     float* d_lisi = (float*)(base + 2 * img);
     float* d_aug = (float*)(base + 2 * img + per_tile);
     float* d_sx = (float*)(base + 2 * img + 2 * per_tile);
@@ -1391,10 +1414,14 @@ int fused_host_impl(const float* x_host, const float* y_host, int N, int N_T,
 
     if (cudaMemcpyAsync(xd, x_host, img_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return IQA_ERR_CUDA;
     if (cudaMemcpyAsync(yd, y_host, img_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return IQA_ERR_CUDA;
-    const float* xs[1] = {xd};
-    const float* ys[1] = {yd};
-    const int rc = iqa_fused_batch(xs, ys, 1, N, N_T, C1, C2, C, D, d_lisi, d_aug, d_sx, d_sy, nullptr, nullptr,
-                                   d_out2, ws_bytes ? ws : nullptr, ws_bytes, stream);
+    // (the uploaded pixels are computed on as they are: no conversion pass, 2 sizeof(pixel) bytes per pixel pair over PCIe)
+    const void* xs[1] = {xd};
+    const void* ys[1] = {yd};
+    const Outputs o{d_lisi, d_aug, d_sx, d_sy, nullptr, nullptr};
+    Geom g = square_geom(N);
+    g.ptype = ptype;
+    const int rc = run_batch(kModeFused, xs, ys, 1, g, N_T, true, C1, C2, C, D, o, d_out2, ws_bytes ? ws : nullptr, ws_bytes,
+                             stream);
     if (rc != IQA_OK) return rc;
     const size_t nb = n * sizeof(float);
     cudaError_t e = cudaSuccess;
@@ -1413,8 +1440,8 @@ int iqa_fused_host(const float* x_host, const float* y_host, int N, int N_T,
                    float* lisi_host, float* auglisi_host,
                    float* sum_x_host, float* sum_y_host, float* out2_host,
                    void* dev_scratch, size_t dev_scratch_bytes, void* stream) {
-    return fused_host_impl(x_host, y_host, N, N_T, C1, C2, C, D, lisi_host, auglisi_host, sum_x_host, sum_y_host,
-                           out2_host, dev_scratch, dev_scratch_bytes, stream, true);
+    return fused_host_impl(x_host, y_host, IQA_PIXEL_F32, N, N_T, C1, C2, C, D, lisi_host, auglisi_host, sum_x_host,
+                           sum_y_host, out2_host, dev_scratch, dev_scratch_bytes, stream, true);
 }
 
 int iqa_fused_host_async(const float* x_host, const float* y_host, int N, int N_T,
@@ -1422,8 +1449,26 @@ int iqa_fused_host_async(const float* x_host, const float* y_host, int N, int N_
                          float* lisi_host, float* auglisi_host,
                          float* sum_x_host, float* sum_y_host, float* out2_host,
                          void* dev_scratch, size_t dev_scratch_bytes, void* stream) {
-    return fused_host_impl(x_host, y_host, N, N_T, C1, C2, C, D, lisi_host, auglisi_host, sum_x_host, sum_y_host,
-                           out2_host, dev_scratch, dev_scratch_bytes, stream, false);
+    return fused_host_impl(x_host, y_host, IQA_PIXEL_F32, N, N_T, C1, C2, C, D, lisi_host, auglisi_host, sum_x_host,
+                           sum_y_host, out2_host, dev_scratch, dev_scratch_bytes, stream, false);
+}
+
+int iqa_fused_host_typed(const void* x_host, const void* y_host, int pixel_type, int N, int N_T,
+                         float C1, float C2, float C, float D,
+                         float* lisi_host, float* auglisi_host,
+                         float* sum_x_host, float* sum_y_host, float* out2_host,
+                         void* dev_scratch, size_t dev_scratch_bytes, void* stream) {
+    return fused_host_impl(x_host, y_host, pixel_type, N, N_T, C1, C2, C, D, lisi_host, auglisi_host, sum_x_host,
+                           sum_y_host, out2_host, dev_scratch, dev_scratch_bytes, stream, true);
+}
+
+int iqa_fused_host_typed_async(const void* x_host, const void* y_host, int pixel_type, int N, int N_T,
+                               float C1, float C2, float C, float D,
+                               float* lisi_host, float* auglisi_host,
+                               float* sum_x_host, float* sum_y_host, float* out2_host,
+                               void* dev_scratch, size_t dev_scratch_bytes, void* stream) {
+    return fused_host_impl(x_host, y_host, pixel_type, N, N_T, C1, C2, C, D, lisi_host, auglisi_host, sum_x_host,
+                           sum_y_host, out2_host, dev_scratch, dev_scratch_bytes, stream, false);
 }
 
 }  // extern "C"

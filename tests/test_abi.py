@@ -122,6 +122,23 @@ def test_standalone_and_aggregate_validation():
                             0x1010, 1 << 30) == B.IQA_ERR_ALIGN
 
 
+def test_typed_host_validation():
+    args = (1e-6, 1e-6, 1e-6, 5e-7, None, None, None, None, None)
+    I16 = B.IQA_PIXEL_I16
+    assert B.iqa_host_scratch_bytes_typed(256, 16, I16) >= 2 * 256 * 256 * 2 + 4 * 256 * 4 + 8
+    assert B.iqa_host_scratch_bytes_typed(256, 16, I16) < B.iqa_host_scratch_bytes(256, 16)
+    assert B.iqa_host_scratch_bytes_typed(256, 16, B.IQA_PIXEL_F32) == B.iqa_host_scratch_bytes(256, 16)
+    assert B.iqa_host_scratch_bytes_typed(256, 16, 99) == 0 and B.iqa_host_scratch_bytes_typed(256, 24, I16) == 0
+    for fn in (B.iqa_fused_host_typed, B.iqa_fused_host_typed_async):
+        assert fn(None, FAKE, I16, 256, 16, *args, FAKE, 1 << 30) == B.IQA_ERR_NULL
+        assert fn(FAKE, FAKE, I16, 256, 16, *args, None, 1 << 30) == B.IQA_ERR_NULL
+        assert fn(FAKE, FAKE, 99, 256, 16, *args, FAKE, 1 << 30) == B.IQA_ERR_SHAPE
+        assert fn(FAKE, FAKE, I16, 256, 24, *args, FAKE, 1 << 30) == B.IQA_ERR_SHAPE
+        assert fn(FAKE, FAKE, I16, 256, 16, 0.0, *args[1:], FAKE, 1 << 30) == B.IQA_ERR_PARAM
+        assert fn(FAKE, FAKE, I16, 256, 16, *args, FAKE, 16) == B.IQA_ERR_WORKSPACE
+        assert fn(FAKE, FAKE, I16, 256, 16, *args, 0x1010, 1 << 30) == B.IQA_ERR_ALIGN
+
+
 def test_batch_validation():
     tbl = (ctypes.c_void_p * 3)(FAKE, FAKE, FAKE)
     bad = (ctypes.c_void_p * 3)(FAKE, 0, FAKE)

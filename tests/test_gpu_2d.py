@@ -451,6 +451,67 @@ def test_typed_series_item_order(B, U, dtype, N_T):
             U.assert_parity(got, ref, k["C"], f"series order {dtype} N_T={N_T} {mode} {c}")
 
 
+@pytest.mark.parametrize("dtype,N,N_T", [(np.int16, 512, 64), (np.uint8, 500, 100), (np.float16, 384, 48), (np.int32, 256, 128),
+                                         (np.float64, 256, 16)])
+def test_typed_host_entry_points(B, U, dtype, N, N_T):
+    """iqa_fused_host_typed / _async (FITS planes as stored): raw pixels uploaded and computed on as they are; the
+    four per-tile arrays and Eqs. 3-4 against the oracle, through the blocking call and through a two-stream pipeline."""
+    import torch
+    import oracle
+    rng = np.random.default_rng(int(N_T) + 5)
+    pairs = [_typed_pair(rng, N, N, dtype) for _ in range(3)]
+    k = pairs[0][2]
+    names = ("lisi", "auglisi", "X", "Y")
+
+    def check(out, out2, x, y, what):
+        ref = oracle.tiles_2d_any(x, y, N_T, **k)
+        U.assert_parity({n: out[n].numpy().astype(np.float64) for n in names}, {**{n: ref[n] for n in names}, "A": ref["A"]},
+                        k["C"], what)
+        exp = oracle.aggregate(ref["lisi"], ref["auglisi"], ref["X"], ref["Y"], k["C2"], k["C"])
+        assert abs(out2[0].item() - exp[0]) <= 1e-5 * abs(exp[0]) and abs(out2[1].item() - exp[1]) <= 1e-5 * abs(exp[1]) + 1e-7
+
+    out, out2 = B.fused_host(pairs[0][0], pairs[0][1], N_T, **k)                     # pageable numpy input, blocking call
+    check(out, out2, pairs[0][0], pairs[0][1], f"fused_host {np.dtype(dtype).name}")
+    ptype = B._pixel_types()[torch.from_numpy(pairs[0][0]).dtype]
+    pipe = B.HostPipeline(N, N_T, "cuda:0", depth=2, pixel_type=ptype)
+    assert pipe.runners[0].h2d_bytes == 2 * np.dtype(dtype).itemsize * N * N
+    pinned = [(torch.from_numpy(x).pin_memory(), torch.from_numpy(y).pin_memory()) for x, y, _ in pairs]
+    for (xp, yp), (x, y, _) in zip(pinned, pairs):
+        slot = pipe.submit(xp, yp, k["C1"], k["C2"], k["C"], k["D"])
+        o, o2 = pipe.wait(slot)
+        check(o, o2, x, y, f"host pipeline {np.dtype(dtype).name}")
+    pipe.drain()
+
+
+def test_small_jobs_keep_any_kernel(B, U):
+    """The generic kernel runs one warp per piece of a tile, so it needs several pieces per SM to beat any_kernel's idle
+    lanes: one pair of a 600 x 600 image with 150-pixel tiles is 16 tiles x 3 pieces = 48 warps for 148 SMs and stays on
+    any_kernel (iqa_query_plan_n), a batch of 64 such pairs (3072 pieces) takes the generic kernel.  Both against the oracle."""
+    import torch
+    import oracle
+    rng = np.random.default_rng(78)
+    H, W, N_T = 600, 600, 150
+    a, b, k = _typed_pair(rng, H, W, np.float32)
+    da, db = _typed_window(a, W, 0), _typed_window(b, W, 0)
+    ref = oracle.tiles_2d_any(a, b, N_T, **k)
+    names = ("lisi", "auglisi", "X", "Y", "L", "A")
+    with B.knob("IQA_PLAN_LARGE_JOB", 0):
+        assert B.plan_name(da, N_T) == "generic"                       # a job that fills the GPU
+        assert B.plan_name(da, N_T, n=1) == "tma_any" and B.plan_name(da, N_T, n=64) == "generic"
+        one = B.fused_tiles_2d(da, db, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+        many = B.fused_batch_2d([da] * 64, [db] * 64, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    with B.knob("IQA_FORCE_ANY", 1):
+        forced_any = B.fused_tiles_2d(da, db, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    with B.knob("IQA_FORCE_GENERIC", 1):
+        forced_gen = B.fused_tiles_2d(da, db, N_T, k["C1"], k["C2"], k["C"], k["D"], numerators=True)
+    for n in names:
+        assert torch.equal(one[n], forced_any[n]), n                   # the single pair took any_kernel ...
+        assert torch.equal(many[n][63], forced_gen[n]), n              # ... the batch the generic kernel
+    for res, what in ((one, "one pair"), ({n: many[n][0] for n in names}, "batch of 64")):
+        got = {n: res[n].cpu().numpy().astype(np.float64) for n in names}
+        U.assert_parity(got, ref, k["C"], f"small-job rule, {what}")
+
+
 def test_series_of_two_images_is_planned_like_the_pair_it_is(B, U):
     """A series of two snapshots shares nothing through L2, so its plan is the pair's plan: N_T = 150 (split tiles filling
     0.59 of any_kernel's lanes) takes the 128-bit generic kernel in both calls and the results agree bit for bit; three
